@@ -1,0 +1,756 @@
+/*
+ * hot_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, double-precision CPU statement of what the hot path of 2HOT (Warren, SC'13,
+ * arXiv:1310.4502; text in PAPER.md) computes: keys -> sort -> bucket oct-tree -> moments ->
+ * per-sink-group walk with an opening criterion -> Plummer-softened particle-particle and
+ * Cartesian-multipole particle-cell sums, plus the definition it approximates (direct sum, and
+ * the direct Ewald sum for periodic boxes).
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may
+ * load this file.  It shares no code, header, table or constant generator with the CUDA library
+ * under paper_1310_4502_b200/csrc, and neither includes the other.
+ *
+ * Every function cites the passage it follows.  The paper prints almost none of the hot-path
+ * mechanics (it defers to WS93, ref [67]); the readings taken are those of SURVEY.md 8(c) and
+ * are listed in DESIGN.md "Readings".  Pins (tests/test_oracle_*.py): two-body closed form,
+ * antisymmetry / momentum, uniform-sphere and Plummer-sphere analytic fields, theta->0 tree ==
+ * direct sum, finite differences of the Green's function tensors, the (b/r)^(p+1) order law
+ * of Fig 6, coverage invariant, tree invariants, brute-force Z-order, and for the
+ * periodic part: Ewald constants, lattice symmetry values, tree+images+far-field vs direct Ewald.
+ *
+ * PARITY UNPINNED against the paper itself (the paper prints no worked force value, key, or
+ * list count): key bit order, NLEAF/NCRIT, the integer-geometry MAC, the far-field coefficient
+ * route.  They are pinned only by the mathematics above.
+ *
+ * Build: gcc -O2 -std=c11 -fopenmp -ffp-contract=off -shared -fPIC hot_oracle.c -lm
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_MAXLEVEL 21
+#define ORC_NMOM 35 /* multi-indices (a,b,c), a+b+c <= 4 */
+
+typedef struct {
+    int64_t n;
+    double lo[3], size;
+    int periodic, nleaf, ncrit;
+    /* particles */
+    uint64_t *key;  /* [n] body keys, caller's order */
+    uint64_t *skey; /* [n] sorted keys */
+    uint32_t *perm; /* [n] sorted position -> caller's index */
+    double *x;      /* [n][3] positions in key order */
+    double *m;      /* [n] masses in key order */
+    /* cells, ascending numeric key (level-major, Morton within a level) */
+    int64_t ncells, capcells;
+    uint64_t *ckey;
+    int32_t *clevel;
+    int64_t *cfirst, *ccount;
+    uint8_t *cmask;
+    int64_t *cchild;  /* index of first child, -1 for a leaf */
+    int64_t *cparent; /* -1 for the root */
+    /* sink groups in particle order */
+    int64_t ngroups;
+    int64_t *gcell;
+    /* moments about the centre of mass, eq (6): mom[c][k] = sum m d^alpha_k; com[c][3]; bmax[c] */
+    double *mom, *com, *bmax;
+    /* periodic far field (C-9 step 2), built on demand */
+    int far_ready;
+    double far_coef[165]; /* coefficient of x^a y^b z^c of psi_sm, a+b+c<=8 (odd ones zero) */
+    double far_S[165];    /* global raw moments about the box centre */
+} orc_t;
+
+/* ------------------------------------------------------------------------------------------
+ * multi-index tables: alpha_k = (a,b,c) ordered by degree, then lexicographic x>y>z:
+ * degree 0: 000; degree 1: 100 010 001; degree 2: 200 110 101 020 011 002; ...
+ * ---------------------------------------------------------------------------------------- */
+static int MI_A[ORC_NMOM], MI_B[ORC_NMOM], MI_C[ORC_NMOM], MI_READY = 0;
+static void mi_init(void) {
+    if (MI_READY) return;
+    int k = 0;
+    for (int d = 0; d <= 4; ++d)
+        for (int a = d; a >= 0; --a)
+            for (int b = d - a; b >= 0; --b) {
+                MI_A[k] = a; MI_B[k] = b; MI_C[k] = d - a - b; ++k;
+            }
+    MI_READY = 1;
+}
+static double factorial(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
+
+/* ------------------------------------------------------------------------------------------
+ * C-2 keys ("mapping of spatial co-ordinates to integer keys described in WS93";
+ * north_star: 63-bit Morton + placeholder bit).  The scaling to [0,1) is done in float with one
+ * subtract and one multiply (no contraction: -ffp-contract=off), because that sequence is part
+ * of the key's definition.  Returns 0, or -1 if a coordinate is outside.
+ * ---------------------------------------------------------------------------------------- */
+static int key_coords(const float *p, const float lo[3], float inv, uint32_t ic[3]) {
+    for (int k = 0; k < 3; ++k) {
+        volatile float d = p[k] - lo[k];
+        volatile float t = d * inv;
+        if (!(t >= 0.0f) || !(t < 1.0f)) return -1;
+        float s = floorf(t * 2097152.0f);
+        int64_t i = (int64_t)s;
+        if (i < 0) i = 0;
+        if (i > 2097151) i = 2097151;
+        ic[k] = (uint32_t)i;
+    }
+    return 0;
+}
+static uint64_t morton_from_coords(const uint32_t ic[3]) {
+    uint64_t mkey = 0;
+    for (int b = 0; b < ORC_MAXLEVEL; ++b) {
+        mkey |= (uint64_t)((ic[0] >> b) & 1u) << (3 * b + 2);
+        mkey |= (uint64_t)((ic[1] >> b) & 1u) << (3 * b + 1);
+        mkey |= (uint64_t)((ic[2] >> b) & 1u) << (3 * b);
+    }
+    return mkey | (1ull << 63);
+}
+int orc_keys(const float *pos, int64_t n, const float lo[3], float size, uint64_t *key) {
+    float inv = 1.0f / size;
+    for (int64_t i = 0; i < n; ++i) {
+        uint32_t ic[3];
+        if (key_coords(pos + 3 * i, lo, inv, ic)) return -1;
+        key[i] = morton_from_coords(ic);
+    }
+    return 0;
+}
+/* integer corner of a cell key at a given level (C-2 step 4): key = 1<<3l | morton>>(63-3l) */
+static void key_corner(uint64_t key, int level, int64_t o[3]) {
+    uint64_t mort = key & ((1ull << (3 * level)) - 1ull); /* strip placeholder */
+    uint32_t ic[3] = {0, 0, 0};
+    for (int b = 0; b < level; ++b) {
+        ic[0] |= (uint32_t)((mort >> (3 * b + 2)) & 1ull) << b;
+        ic[1] |= (uint32_t)((mort >> (3 * b + 1)) & 1ull) << b;
+        ic[2] |= (uint32_t)((mort >> (3 * b)) & 1ull) << b;
+    }
+    for (int k = 0; k < 3; ++k) o[k] = (int64_t)ic[k] << (ORC_MAXLEVEL - level);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-3 stable sort of (key, index): bottom-up merge sort, ties keep ascending original index.
+ * ---------------------------------------------------------------------------------------- */
+static void stable_sort_keys(const uint64_t *key, int64_t n, uint64_t *skey, uint32_t *perm) {
+    uint64_t *ka = malloc(sizeof(uint64_t) * (size_t)n), *kb = malloc(sizeof(uint64_t) * (size_t)n);
+    uint32_t *pa = malloc(sizeof(uint32_t) * (size_t)n), *pb = malloc(sizeof(uint32_t) * (size_t)n);
+    for (int64_t i = 0; i < n; ++i) { ka[i] = key[i]; pa[i] = (uint32_t)i; }
+    for (int64_t w = 1; w < n; w *= 2) {
+        for (int64_t s = 0; s < n; s += 2 * w) {
+            int64_t mid = s + w < n ? s + w : n, end = s + 2 * w < n ? s + 2 * w : n;
+            int64_t i = s, j = mid, o = s;
+            while (i < mid && j < end) {
+                if (ka[j] < ka[i]) { kb[o] = ka[j]; pb[o++] = pa[j++]; } /* strict: left wins ties */
+                else { kb[o] = ka[i]; pb[o++] = pa[i++]; }
+            }
+            while (i < mid) { kb[o] = ka[i]; pb[o++] = pa[i++]; }
+            while (j < end) { kb[o] = ka[j]; pb[o++] = pa[j++]; }
+        }
+        uint64_t *tk = ka; ka = kb; kb = tk;
+        uint32_t *tp = pa; pa = pb; pb = tp;
+    }
+    memcpy(skey, ka, sizeof(uint64_t) * (size_t)n);
+    memcpy(perm, pa, sizeof(uint32_t) * (size_t)n);
+    free(ka); free(kb); free(pa); free(pb);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-4 tree: the unique bucket oct-tree of the sorted keys.  Breadth-first with a queue, so the
+ * cells come out in ascending numeric key order.  A cell is a leaf iff count <= NLEAF or it is
+ * at level 21; otherwise its non-empty octants are its children.
+ * ---------------------------------------------------------------------------------------- */
+static void cells_reserve(orc_t *t, int64_t want) {
+    if (want <= t->capcells) return;
+    int64_t cap = t->capcells ? t->capcells : 1024;
+    while (cap < want) cap *= 2;
+    t->ckey = realloc(t->ckey, sizeof(uint64_t) * (size_t)cap);
+    t->clevel = realloc(t->clevel, sizeof(int32_t) * (size_t)cap);
+    t->cfirst = realloc(t->cfirst, sizeof(int64_t) * (size_t)cap);
+    t->ccount = realloc(t->ccount, sizeof(int64_t) * (size_t)cap);
+    t->cmask = realloc(t->cmask, (size_t)cap);
+    t->cchild = realloc(t->cchild, sizeof(int64_t) * (size_t)cap);
+    t->cparent = realloc(t->cparent, sizeof(int64_t) * (size_t)cap);
+    t->capcells = cap;
+}
+static void build_tree(orc_t *t) {
+    cells_reserve(t, 1);
+    t->ncells = 1;
+    t->ckey[0] = 1; t->clevel[0] = 0; t->cfirst[0] = 0; t->ccount[0] = t->n;
+    t->cmask[0] = 0; t->cchild[0] = -1; t->cparent[0] = -1;
+    for (int64_t c = 0; c < t->ncells; ++c) { /* the array is the queue */
+        int level = t->clevel[c];
+        if (t->ccount[c] <= t->nleaf || level == ORC_MAXLEVEL) continue; /* leaf */
+        int64_t first = t->cfirst[c], end = first + t->ccount[c];
+        int shift = 60 - 3 * level; /* next 3 key bits below this cell's prefix */
+        int64_t i = first;
+        t->cchild[c] = t->ncells;
+        while (i < end) {
+            int oct = (int)((t->skey[i] >> shift) & 7ull);
+            int64_t j = i;
+            while (j < end && (int)((t->skey[j] >> shift) & 7ull) == oct) ++j;
+            cells_reserve(t, t->ncells + 1);
+            int64_t d = t->ncells++;
+            t->ckey[d] = (t->ckey[c] << 3) | (uint64_t)oct;
+            t->clevel[d] = level + 1; t->cfirst[d] = i; t->ccount[d] = j - i;
+            t->cmask[d] = 0; t->cchild[d] = -1; t->cparent[d] = c;
+            t->cmask[c] |= (uint8_t)(1u << oct);
+            i = j;
+        }
+    }
+}
+/* sink groups: count <= NCRIT (or level 21) and (root or parent count > NCRIT) */
+static void build_groups(orc_t *t) {
+    int64_t ng = 0;
+    int64_t *tmp = malloc(sizeof(int64_t) * (size_t)t->ncells);
+    for (int64_t c = 0; c < t->ncells; ++c) {
+        int small = t->ccount[c] <= t->ncrit || t->clevel[c] == ORC_MAXLEVEL;
+        int top = t->cparent[c] < 0 || t->ccount[t->cparent[c]] > t->ncrit;
+        if (small && top) tmp[ng++] = c;
+    }
+    /* order by first particle (insertion into a position table: groups partition [0,n)) */
+    int64_t *at = malloc(sizeof(int64_t) * (size_t)t->n);
+    for (int64_t i = 0; i < t->n; ++i) at[i] = -1;
+    for (int64_t g = 0; g < ng; ++g) at[t->cfirst[tmp[g]]] = tmp[g];
+    t->gcell = malloc(sizeof(int64_t) * (size_t)(ng ? ng : 1));
+    t->ngroups = 0;
+    for (int64_t i = 0; i < t->n; ++i) if (at[i] >= 0) t->gcell[t->ngroups++] = at[i];
+    free(at); free(tmp);
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-5 upward pass, eq (6): raw moments about the centre of mass, directly from the
+ * cell's particle range.  mom[k] = sum_j m_j dx^a dy^b dz^c for alpha_k = (a,b,c), |alpha| <= 4.
+ * ---------------------------------------------------------------------------------------- */
+static void build_moments(orc_t *t) {
+    mi_init();
+    t->mom = calloc((size_t)t->ncells * ORC_NMOM, sizeof(double));
+    t->com = calloc((size_t)t->ncells * 3, sizeof(double));
+    t->bmax = calloc((size_t)t->ncells, sizeof(double));
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t c = 0; c < t->ncells; ++c) {
+        int64_t f = t->cfirst[c], e = f + t->ccount[c];
+        double M0 = 0, z[3] = {0, 0, 0};
+        for (int64_t j = f; j < e; ++j) {
+            M0 += t->m[j];
+            for (int k = 0; k < 3; ++k) z[k] += t->m[j] * t->x[3 * j + k];
+        }
+        for (int k = 0; k < 3; ++k) z[k] /= M0;
+        double *mo = t->mom + (size_t)c * ORC_NMOM, bm = 0;
+        for (int64_t j = f; j < e; ++j) {
+            double d[3];
+            for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - z[k];
+            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+            if (r > bm) bm = r;
+            for (int k = 0; k < ORC_NMOM; ++k)
+                mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
+        }
+        for (int k = 0; k < 3; ++k) t->com[3 * c + k] = z[k];
+        t->bmax[c] = bm;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * create / destroy
+ * ---------------------------------------------------------------------------------------- */
+void orc_destroy(orc_t *t) {
+    if (!t) return;
+    free(t->key); free(t->skey); free(t->perm); free(t->x); free(t->m);
+    free(t->ckey); free(t->clevel); free(t->cfirst); free(t->ccount); free(t->cmask);
+    free(t->cchild); free(t->cparent); free(t->gcell); free(t->mom); free(t->com); free(t->bmax);
+    free(t);
+}
+orc_t *orc_create(const float *pos, const float *mass, int64_t n, const float lo[3], float size,
+                  int periodic, int nleaf, int ncrit, int with_moments, int *status) {
+    *status = 0;
+    if (n < 1 || !(size > 0) || nleaf < 1 || ncrit < nleaf) { *status = -1; return NULL; }
+    orc_t *t = calloc(1, sizeof(orc_t));
+    t->n = n; t->size = size; t->periodic = periodic; t->nleaf = nleaf; t->ncrit = ncrit;
+    for (int k = 0; k < 3; ++k) t->lo[k] = lo[k];
+    t->key = malloc(sizeof(uint64_t) * (size_t)n);
+    t->skey = malloc(sizeof(uint64_t) * (size_t)n);
+    t->perm = malloc(sizeof(uint32_t) * (size_t)n);
+    t->x = malloc(sizeof(double) * 3 * (size_t)n);
+    t->m = malloc(sizeof(double) * (size_t)n);
+    if (orc_keys(pos, n, lo, size, t->key)) { *status = -2; orc_destroy(t); return NULL; }
+    stable_sort_keys(t->key, n, t->skey, t->perm);
+    for (int64_t i = 0; i < n; ++i) {
+        for (int k = 0; k < 3; ++k) t->x[3 * i + k] = (double)pos[3 * (int64_t)t->perm[i] + k];
+        t->m[i] = (double)mass[t->perm[i]];
+    }
+    build_tree(t);
+    build_groups(t);
+    if (with_moments) build_moments(t);
+    return t;
+}
+
+/* plain getters for the parity tests */
+int64_t orc_n(const orc_t *t) { return t->n; }
+int64_t orc_ncells(const orc_t *t) { return t->ncells; }
+int64_t orc_ngroups(const orc_t *t) { return t->ngroups; }
+void orc_get_keys(const orc_t *t, uint64_t *key, uint64_t *skey, uint32_t *perm) {
+    if (key) memcpy(key, t->key, sizeof(uint64_t) * (size_t)t->n);
+    if (skey) memcpy(skey, t->skey, sizeof(uint64_t) * (size_t)t->n);
+    if (perm) memcpy(perm, t->perm, sizeof(uint32_t) * (size_t)t->n);
+}
+void orc_get_cells(const orc_t *t, uint64_t *key, int32_t *level, int64_t *first, int64_t *count,
+                   uint8_t *mask, int64_t *child, int64_t *parent) {
+    size_t nc = (size_t)t->ncells;
+    if (key) memcpy(key, t->ckey, 8 * nc);
+    if (level) memcpy(level, t->clevel, 4 * nc);
+    if (first) memcpy(first, t->cfirst, 8 * nc);
+    if (count) memcpy(count, t->ccount, 8 * nc);
+    if (mask) memcpy(mask, t->cmask, nc);
+    if (child) memcpy(child, t->cchild, 8 * nc);
+    if (parent) memcpy(parent, t->cparent, 8 * nc);
+}
+void orc_get_groups(const orc_t *t, int64_t *gcell) {
+    memcpy(gcell, t->gcell, sizeof(int64_t) * (size_t)t->ngroups);
+}
+void orc_get_moments(const orc_t *t, double *mom, double *com, double *bmax) {
+    size_t nc = (size_t)t->ncells;
+    if (mom) memcpy(mom, t->mom, 8 * nc * ORC_NMOM);
+    if (com) memcpy(com, t->com, 8 * nc * 3);
+    if (bmax) memcpy(bmax, t->bmax, 8 * nc);
+}
+/* per sorted particle: index of the leaf cell that holds it (cell membership) */
+void orc_get_leaf_of(const orc_t *t, int64_t *leaf) {
+    for (int64_t c = 0; c < t->ncells; ++c)
+        if (t->cchild[c] < 0)
+            for (int64_t j = t->cfirst[c]; j < t->cfirst[c] + t->ccount[c]; ++j) leaf[j] = c;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-6 Green's function tensors.  g(R) = (|R|^2 + eps^2)^(-1/2) (Plummer).
+ * d^alpha g is obtained from the chain rule exactly as it reads: each derivative either hits
+ * the power of u = |R|^2+eps^2 (factor R_i, next D_k) or an R_j already brought down (delta_ij).
+ * D_k = (-1)^k (2k-1)!! u^(-(2k+1)/2).  The recursion enumerates every pairing of the index
+ * list once: the first remaining index is either unpaired (factor R) or paired with a later one.
+ * ---------------------------------------------------------------------------------------- */
+static double dg_rec(const int *idx, int nidx, int npairs, int ntot, const double R[3],
+                     const double *D) {
+    if (nidx == 0) return D[ntot - npairs];
+    double s = R[idx[0]] * dg_rec(idx + 1, nidx - 1, npairs, ntot, R, D);
+    int rest[8];
+    for (int j = 1; j < nidx; ++j) {
+        if (idx[j] != idx[0]) continue; /* delta_{i0,ij} */
+        int q = 0;
+        for (int k = 1; k < nidx; ++k) if (k != j) rest[q++] = idx[k];
+        s += dg_rec(rest, nidx - 2, npairs + 1, ntot, R, D);
+    }
+    return s;
+}
+static double dg(int a, int b, int c, const double R[3], const double *D) {
+    int idx[8], n = 0;
+    for (int i = 0; i < a; ++i) idx[n++] = 0;
+    for (int i = 0; i < b; ++i) idx[n++] = 1;
+    for (int i = 0; i < c; ++i) idx[n++] = 2;
+    return dg_rec(idx, n, 0, n, R, D);
+}
+static void make_D(double u, double *D, int kmax) {
+    double dfact = 1; /* (2k-1)!! */
+    for (int k = 0; k <= kmax; ++k) {
+        if (k > 0) dfact *= (2 * k - 1);
+        D[k] = ((k & 1) ? -1.0 : 1.0) * dfact * pow(u, -0.5 * (2 * k + 1));
+    }
+}
+/* exported for the finite-difference pin */
+double orc_dg(int a, int b, int c, const double R[3], double eps) {
+    double D[8]; make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + eps * eps, D, a + b + c);
+    return dg(a, b, c, R, D);
+}
+
+/* eq (5) with Delta = 0 (cell-body), Green's function g, truncated at `order`:
+ *   phi(x) = - sum_{|alpha|<=p} ((-1)^|alpha| / alpha!) d^alpha g(R) M_alpha,   R = x - z
+ *   a_k(x) = - d_k phi = + sum ... d^(alpha+e_k) g(R) M_alpha
+ * (the multi-index form of the n-fold outer product / tensor inner product of eq (5); the minus
+ * sign makes phi the potential of attracting masses, G = 1).  The dipole vanishes about the
+ * centre of mass; order 0 -> n=0; order 2 -> n=0,2; order 3 -> n<=3; order 4 -> n<=4.        */
+static void cell_on_sink(const double *mo, const double z[3], int order, const double x[3],
+                         double eps2, double acc[3], double *pot) {
+    double R[3] = {x[0] - z[0], x[1] - z[1], x[2] - z[2]}, D[8];
+    make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + eps2, D, order + 1);
+    for (int k = 0; k < ORC_NMOM; ++k) {
+        int a = MI_A[k], b = MI_B[k], c = MI_C[k], n = a + b + c;
+        if (n > order) break;
+        if (n == 1) continue; /* dipole about the centre of mass is zero by construction */
+        double w = ((n & 1) ? -1.0 : 1.0) / (factorial(a) * factorial(b) * factorial(c)) * mo[k];
+        *pot -= w * dg(a, b, c, R, D);
+        acc[0] += w * dg(a + 1, b, c, R, D);
+        acc[1] += w * dg(a, b + 1, c, R, D);
+        acc[2] += w * dg(a, b, c + 1, R, D);
+    }
+}
+/* C-1 summand (eq (2) right-hand side, Plummer-softened): source (y,m) on sink x */
+static void body_on_sink(const double y[3], double m, const double x[3], double eps2,
+                         double acc[3], double *pot) {
+    double d[3] = {y[0] - x[0], y[1] - x[1], y[2] - x[2]};
+    double u = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
+    double ri = 1.0 / sqrt(u), ri3 = ri / u;
+    for (int k = 0; k < 3; ++k) acc[k] += m * d[k] * ri3;
+    *pot -= m * ri;
+}
+/* exported single interactions (pins O-1, O-7, O-8, O-9) */
+void orc_cell_on_sink(const double *mom35, const double z[3], int order, const double x[3],
+                      double eps, double acc[3], double *pot) {
+    mi_init();
+    acc[0] = acc[1] = acc[2] = 0; *pot = 0;
+    cell_on_sink(mom35, z, order, x, eps * eps, acc, pot);
+}
+/* moments of an arbitrary particle set about its centre of mass (same definition as C-5) */
+void orc_moments_of(const double *y, const double *m, int64_t n, double *mom35, double z[3]) {
+    mi_init();
+    double M0 = 0; z[0] = z[1] = z[2] = 0;
+    for (int64_t j = 0; j < n; ++j) { M0 += m[j]; for (int k = 0; k < 3; ++k) z[k] += m[j] * y[3 * j + k]; }
+    for (int k = 0; k < 3; ++k) z[k] /= M0;
+    for (int k = 0; k < ORC_NMOM; ++k) mom35[k] = 0;
+    for (int64_t j = 0; j < n; ++j) {
+        double d[3] = {y[3 * j] - z[0], y[3 * j + 1] - z[1], y[3 * j + 2] - z[2]};
+        for (int k = 0; k < ORC_NMOM; ++k)
+            mom35[k] += m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-1 direct sum over all sources for the listed sinks (caller's indices).  Self term skipped.
+ * ---------------------------------------------------------------------------------------- */
+void orc_direct(const float *pos, const float *mass, int64_t n, double eps, const int64_t *sinks,
+                int64_t ns, double *acc, double *pot) {
+    double eps2 = eps * eps;
+#pragma omp parallel for schedule(static)
+    for (int64_t s = 0; s < ns; ++s) {
+        int64_t i = sinks ? sinks[s] : s;
+        double x[3] = {pos[3 * i], pos[3 * i + 1], pos[3 * i + 2]}, a[3] = {0, 0, 0}, p = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double y[3] = {pos[3 * j], pos[3 * j + 1], pos[3 * j + 2]};
+            body_on_sink(y, (double)mass[j], x, eps2, a, &p);
+        }
+        acc[3 * s] = a[0]; acc[3 * s + 1] = a[1]; acc[3 * s + 2] = a[2]; pot[s] = p;
+    }
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-7 walk with the integer-geometry minimum-distance MAC.  Cells and groups are cubes on the
+ * 2^21 grid; the source may be shifted by an image vector (units of 2^21).  Accept iff
+ * (double)(sC*sC) < theta2 * (double)d2  with d2 the squared gap between the cubes.
+ * ---------------------------------------------------------------------------------------- */
+typedef struct {
+    const orc_t *t; double theta2; int64_t go[3], gs; int64_t sh[3];
+    int64_t npc, npp, covered;       /* counts */
+    int64_t *pc, *pp; int64_t cap;   /* optional lists: accepted cells / rejected leaves */
+    int64_t nleafrej;
+    /* evaluation */
+    int eval, order; double eps2; double shx[3];
+    int64_t gfirst, gcount; double *acc, *pot; /* [gcount][3], [gcount], group-local */
+} walk_t;
+
+static int mac_accept(const walk_t *w, int64_t c) {
+    const orc_t *t = w->t;
+    int level = t->clevel[c];
+    int64_t o[3], s = (int64_t)1 << (ORC_MAXLEVEL - level);
+    key_corner(t->ckey[c], level, o);
+    uint64_t d2 = 0;
+    for (int k = 0; k < 3; ++k) {
+        int64_t oc = o[k] + w->sh[k];
+        int64_t g1 = oc - (w->go[k] + w->gs), g2 = w->go[k] - (oc + s);
+        int64_t g = g1 > g2 ? g1 : g2;
+        if (g < 0) g = 0;
+        d2 += (uint64_t)(g * g);
+    }
+    return (double)((uint64_t)(s * s)) < w->theta2 * (double)d2;
+}
+static void walk_rec(walk_t *w, int64_t c) {
+    const orc_t *t = w->t;
+    if (mac_accept(w, c)) {
+        if (w->pc && w->npc < w->cap) w->pc[w->npc] = c;
+        w->npc++; w->covered += t->ccount[c];
+        if (w->eval)
+            for (int64_t i = 0; i < w->gcount; ++i) {
+                double z[3] = {t->com[3 * c] + w->shx[0], t->com[3 * c + 1] + w->shx[1], t->com[3 * c + 2] + w->shx[2]};
+                cell_on_sink(t->mom + (size_t)c * ORC_NMOM, z, w->order, t->x + 3 * (w->gfirst + i),
+                             w->eps2, w->acc + 3 * i, w->pot + i);
+            }
+    } else if (t->cchild[c] < 0) {
+        if (w->pp && w->nleafrej < w->cap) w->pp[w->nleafrej] = c;
+        w->nleafrej++; w->npp += t->ccount[c];
+        if (w->eval)
+            for (int64_t i = 0; i < w->gcount; ++i)
+                for (int64_t j = t->cfirst[c]; j < t->cfirst[c] + t->ccount[c]; ++j) {
+                    if (j == w->gfirst + i && w->sh[0] == 0 && w->sh[1] == 0 && w->sh[2] == 0) continue;
+                    double y[3] = {t->x[3 * j] + w->shx[0], t->x[3 * j + 1] + w->shx[1], t->x[3 * j + 2] + w->shx[2]};
+                    body_on_sink(y, t->m[j], t->x + 3 * (w->gfirst + i), w->eps2, w->acc + 3 * i, w->pot + i);
+                }
+    } else {
+        int nch = 0; for (int b = 0; b < 8; ++b) nch += (t->cmask[c] >> b) & 1;
+        for (int k = 0; k < nch; ++k) walk_rec(w, t->cchild[c] + k);
+    }
+}
+static void walk_setup(walk_t *w, const orc_t *t, double theta, int64_t g) {
+    memset(w, 0, sizeof(*w));
+    w->t = t; w->theta2 = theta * theta;
+    int64_t gc = t->gcell[g];
+    key_corner(t->ckey[gc], t->clevel[gc], w->go);
+    w->gs = (int64_t)1 << (ORC_MAXLEVEL - t->clevel[gc]);
+    w->gfirst = t->cfirst[gc]; w->gcount = t->ccount[gc];
+}
+static int image_range(const orc_t *t) { return t->periodic ? 2 : 0; } /* ws = 2 */
+
+/* list counts per group, summed over the (2ws+1)^3 images when periodic; covered = sum of
+ * count(C) over accepted cells + L_pp, which must equal n * (number of images) */
+void orc_walk_counts(const orc_t *t, double theta, const int64_t *groups, int64_t ng,
+                     int64_t *Lpc, int64_t *Lpp, int64_t *covered) {
+    int ws = image_range(t);
+#pragma omp parallel for schedule(dynamic, 8)
+    for (int64_t q = 0; q < ng; ++q) {
+        int64_t g = groups ? groups[q] : q;
+        int64_t npc = 0, npp = 0, cov = 0;
+        for (int ix = -ws; ix <= ws; ++ix) for (int iy = -ws; iy <= ws; ++iy) for (int iz = -ws; iz <= ws; ++iz) {
+            walk_t w; walk_setup(&w, t, theta, g);
+            w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
+            walk_rec(&w, 0);
+            npc += w.npc; npp += w.npp; cov += w.covered;
+        }
+        Lpc[q] = npc; Lpp[q] = npp; if (covered) covered[q] = cov;
+    }
+}
+/* the lists themselves for one group and one image (tiny N): accepted cell indices and rejected
+ * leaf cell indices, in walk order; returns their numbers through npc / nleaf */
+void orc_walk_lists(const orc_t *t, double theta, int64_t g, const int img[3], int64_t cap,
+                    int64_t *pc, int64_t *npc, int64_t *leaves, int64_t *nleaf) {
+    walk_t w; walk_setup(&w, t, theta, g);
+    for (int k = 0; k < 3; ++k) w.sh[k] = (int64_t)img[k] << ORC_MAXLEVEL;
+    w.pc = pc; w.pp = leaves; w.cap = cap;
+    walk_rec(&w, 0);
+    *npc = w.npc; *nleaf = w.nleafrej;
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-9 periodic pieces.  psi(r): Green's function of a unit point mass in the unit box plus a
+ * uniform neutralising background, zero box mean (Ewald form of ref [25]):
+ *   psi(r) = sum_n erfc(alpha|r-n|)/|r-n| + (1/pi) sum_{h!=0} exp(-pi^2 h^2/alpha^2)/h^2 cos(2 pi h.r) - pi/alpha^2
+ * alpha = 2, |n_k| <= 4, |h|^2 <= 49.  Positions in units of the box.
+ * ---------------------------------------------------------------------------------------- */
+#define EW_ALPHA 2.0
+#define EW_NR 4
+#define EW_H2 49
+void orc_ewald_psi(const double r[3], double *psi, double grad[3]) {
+    const double al = EW_ALPHA, PI = 3.14159265358979323846;
+    double p = -PI / (al * al), g[3] = {0, 0, 0};
+    for (int nx = -EW_NR; nx <= EW_NR; ++nx) for (int ny = -EW_NR; ny <= EW_NR; ++ny) for (int nz = -EW_NR; nz <= EW_NR; ++nz) {
+        double d[3] = {r[0] - nx, r[1] - ny, r[2] - nz};
+        double dd = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (dd == 0) continue; /* caller handles the singular term */
+        p += erfc(al * dd) / dd;
+        double f = (erfc(al * dd) + 2 * al * dd / sqrt(PI) * exp(-al * al * dd * dd)) / (dd * dd * dd);
+        for (int k = 0; k < 3; ++k) g[k] -= f * d[k];
+    }
+    int hm = 7;
+    for (int hx = -hm; hx <= hm; ++hx) for (int hy = -hm; hy <= hm; ++hy) for (int hz = -hm; hz <= hm; ++hz) {
+        int h2 = hx * hx + hy * hy + hz * hz;
+        if (h2 == 0 || h2 > EW_H2) continue;
+        double ph = 2 * PI * (hx * r[0] + hy * r[1] + hz * r[2]);
+        double e = exp(-PI * PI * h2 / (al * al)) / h2;
+        p += e / PI * cos(ph);
+        double s = -2 * e * sin(ph);
+        g[0] += s * hx; g[1] += s * hy; g[2] += s * hz;
+    }
+    *psi = p; if (grad) { grad[0] = g[0]; grad[1] = g[1]; grad[2] = g[2]; }
+}
+/* psi_sm(r) = psi(r) - sum_{|n|_inf<=2} 1/|r-n| : analytic for |r_k| < 3 (C-9 step 2) */
+static double psi_smooth(const double r[3]) {
+    double p; orc_ewald_psi(r, &p, NULL);
+    for (int nx = -2; nx <= 2; ++nx) for (int ny = -2; ny <= 2; ++ny) for (int nz = -2; nz <= 2; ++nz) {
+        double d[3] = {r[0] - nx, r[1] - ny, r[2] - nz};
+        double dd = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (dd == 0) { /* at r = 0 psi() left the whole n=0 term out; erfc(al r)/r - 1/r -> -2 al/sqrt(pi) */
+            p -= 2 * EW_ALPHA / sqrt(3.14159265358979323846);
+            continue;
+        }
+        p -= 1.0 / dd;
+    }
+    return p;
+}
+double orc_psi_smooth(const double r[3]) { return psi_smooth(r); }
+
+double orc_ewald_xi(void);
+/* direct Ewald sum (the ladder's bottom rung), C-9 "Definition": minimum image
+ * softened with Plummer, all other images and the background through psi.  Units: box = size. */
+void orc_ewald_direct(const float *pos, const float *mass, int64_t n, double size, double eps,
+                      const int64_t *sinks, int64_t ns, double *acc, double *pot) {
+    double xi = orc_ewald_xi(); /* lim_{r->0} psi(r) - 1/r */
+    double eps1 = eps / size;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t s = 0; s < ns; ++s) {
+        int64_t i = sinks ? sinks[s] : s;
+        double a[3] = {0, 0, 0}, p = 0;
+        for (int64_t j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double r[3], rt[3];
+            for (int k = 0; k < 3; ++k) {
+                r[k] = ((double)pos[3 * i + k] - (double)pos[3 * j + k]) / size;
+                rt[k] = r[k] - floor(r[k] + 0.5);
+            }
+            double psi, g[3]; orc_ewald_psi(rt, &psi, g); /* psi is periodic: use the minimum image */
+            double d2 = rt[0] * rt[0] + rt[1] * rt[1] + rt[2] * rt[2];
+            double mj = (double)mass[j];
+            if (d2 > 0) {
+                double d1 = sqrt(d2), u = d2 + eps1 * eps1;
+                p -= mj * (psi - 1.0 / d1 + 1.0 / sqrt(u));
+                for (int k = 0; k < 3; ++k) a[k] += mj * (g[k] + rt[k] / (d1 * d2) - rt[k] / (u * sqrt(u)));
+            } else { /* coincident distinct bodies: psi() left the singular n=0 term out, whose
+                        regular part erfc(a r)/r - 1/r -> -2a/sqrt(pi) must be put back */
+                p -= mj * (psi - 2 * EW_ALPHA / sqrt(3.14159265358979323846) + 1.0 / eps1);
+                for (int k = 0; k < 3; ++k) a[k] += mj * g[k];
+            }
+        }
+        p -= (double)mass[i] * xi;
+        for (int k = 0; k < 3; ++k) acc[3 * s + k] = a[k] / (size * size);
+        pot[s] = p / size;
+    }
+}
+double orc_ewald_xi(void) {
+    double r0[3] = {0, 0, 0}, p; orc_ewald_psi(r0, &p, NULL);
+    return p - 2 * EW_ALPHA / sqrt(3.14159265358979323846);
+}
+
+/* far-field table (C-9 step 2; "sums the infinite series of each relevant
+ * combination of powers of the co-ordinates ... pre-computed coefficients ... used in a local
+ * expansion about the center of the volume", p = 8, ws = 2).  The coefficients are the Taylor
+ * coefficients of psi_sm about r = 0 through total degree 8:  c_alpha = d^alpha psi_sm(0)/alpha!.
+ * psi_sm = [erfc(al r)/r - 1/r]                      (A: = -erf(al r)/r, a power series in r^2)
+ *        + sum_{n!=0} erfc(al|r-n|)/|r-n|            (B: radial function, tensor by the chain rule)
+ *        + (1/pi) sum_h w_h cos(2 pi h.r)            (C: power series of the cosine)
+ *        - pi/al^2                                   (D)
+ *        - sum_{0<|n|_inf<=2} 1/|r-n|                (E: the 124 explicit cubes, eps = 0)
+ * For a radial f(d) the chain-rule recursion dg_rec applies with D_k = (1/d d/dd)^k f:
+ * for f = erfc(al d)/d, D_k = (-1)^k B_k, B_0 = f, B_k = ((2k-1) B_(k-1) + (2 al^2)^k e^(-al^2 d^2)/(al sqrt(pi)))/d^2.
+ * far_coef is indexed over all (a,b,c), a+b+c<=8, degree-major; odd ones are zero by symmetry. */
+static int far_index(int a, int b, int c) { /* position of (a,b,c) in degree-major order */
+    int d = a + b + c, k = 0;
+    for (int dd = 0; dd < d; ++dd) k += (dd + 1) * (dd + 2) / 2;
+    for (int aa = d; aa > a; --aa) k += d - aa + 1;
+    return k + (d - a - b);
+}
+static void far_build_table(orc_t *t) {
+    const double al = EW_ALPHA, PI = 3.14159265358979323846;
+    for (int k = 0; k < 165; ++k) t->far_coef[k] = 0;
+    for (int deg = 0; deg <= 8; deg += 2)
+        for (int a = deg; a >= 0; a -= 2) for (int b = deg - a; b >= 0; b -= 2) {
+            int c = deg - a - b, m = deg / 2;
+            double afac = factorial(a) * factorial(b) * factorial(c), co = 0;
+            /* A */
+            co += -(2 * al / sqrt(PI)) * ((m & 1) ? -1.0 : 1.0) * pow(al, 2 * m) / (factorial(m) * (2 * m + 1))
+                  * factorial(m) / (factorial(a / 2) * factorial(b / 2) * factorial(c / 2));
+            /* B and E */
+            for (int nx = -EW_NR; nx <= EW_NR; ++nx) for (int ny = -EW_NR; ny <= EW_NR; ++ny) for (int nz = -EW_NR; nz <= EW_NR; ++nz) {
+                if (!nx && !ny && !nz) continue;
+                double R[3] = {-(double)nx, -(double)ny, -(double)nz};
+                double d2 = R[0] * R[0] + R[1] * R[1] + R[2] * R[2], d = sqrt(d2), D[10];
+                double B = erfc(al * d) / d, ex = exp(-al * al * d2) / (al * sqrt(PI));
+                D[0] = B;
+                for (int k = 1; k <= deg; ++k) { B = ((2 * k - 1) * B + pow(2 * al * al, k) * ex) / d2; D[k] = (k & 1) ? -B : B; }
+                co += dg(a, b, c, R, D) / afac;
+                if (abs(nx) <= 2 && abs(ny) <= 2 && abs(nz) <= 2) { make_D(d2, D, deg); co -= dg(a, b, c, R, D) / afac; }
+            }
+            /* C */
+            for (int hx = -7; hx <= 7; ++hx) for (int hy = -7; hy <= 7; ++hy) for (int hz = -7; hz <= 7; ++hz) {
+                int h2 = hx * hx + hy * hy + hz * hz;
+                if (h2 == 0 || h2 > EW_H2) continue;
+                double w = exp(-PI * PI * h2 / (al * al)) / h2 / PI;
+                co += w * ((m & 1) ? -1.0 : 1.0) * pow(2 * PI, 2 * m) * pow(hx, a) * pow(hy, b) * pow(hz, c) / afac;
+            }
+            /* D */
+            if (deg == 0) co -= PI / (al * al);
+            t->far_coef[far_index(a, b, c)] = co;
+        }
+}
+static void far_prepare(orc_t *t) {
+    if (t->far_ready) return;
+    far_build_table(t);
+    /* global raw moments about the box centre, box units: S_abc = sum m (x-c)^a (y-c)^b (z-c)^c */
+    for (int k = 0; k < 165; ++k) t->far_S[k] = 0;
+    for (int64_t j = 0; j < t->n; ++j) {
+        double d[3];
+        for (int k = 0; k < 3; ++k) d[k] = (t->x[3 * j + k] - (t->lo[k] + 0.5 * t->size)) / t->size;
+        for (int deg = 0, q = 0; deg <= 8; ++deg)
+            for (int a = deg; a >= 0; --a) for (int b = deg - a; b >= 0; --b, ++q)
+                t->far_S[q] += t->m[j] * pow(d[0], a) * pow(d[1], b) * pow(d[2], deg - a - b);
+    }
+    t->far_ready = 1;
+}
+void orc_far_table(orc_t *t, double *coef165) { far_prepare(t); memcpy(coef165, t->far_coef, sizeof(double) * 165); }
+/* sum_j m_j psi_sm(x - x_j) and its gradient at x, by the binomial expansion of every monomial
+ * (x - x_j)^alpha = sum_beta C(alpha,beta) (x-c)^(alpha-beta) (-(x_j-c))^beta  (C-9 step 2) */
+static double binom(int n, int k) { return factorial(n) / (factorial(k) * factorial(n - k)); }
+static void far_on_sink(const orc_t *t, const double x[3], double *val, double grad[3]) {
+    double d[3];
+    for (int k = 0; k < 3; ++k) d[k] = (x[k] - (t->lo[k] + 0.5 * t->size)) / t->size;
+    double v = 0, g[3] = {0, 0, 0};
+    for (int deg = 0, q = 0; deg <= 8; ++deg)
+        for (int a = deg; a >= 0; --a) for (int b = deg - a; b >= 0; --b, ++q) {
+            int c = deg - a - b; double co = t->far_coef[q];
+            if (co == 0) continue;
+            for (int i = 0; i <= a; ++i) for (int j = 0; j <= b; ++j) for (int k = 0; k <= c; ++k) {
+                double S = t->far_S[far_index(i, j, k)];
+                double w = co * binom(a, i) * binom(b, j) * binom(c, k) * (((i + j + k) & 1) ? -1.0 : 1.0) * S;
+                int pa = a - i, pb = b - j, pc = c - k;
+                v += w * pow(d[0], pa) * pow(d[1], pb) * pow(d[2], pc);
+                if (pa) g[0] += w * pa * pow(d[0], pa - 1) * pow(d[1], pb) * pow(d[2], pc);
+                if (pb) g[1] += w * pb * pow(d[0], pa) * pow(d[1], pb - 1) * pow(d[2], pc);
+                if (pc) g[2] += w * pc * pow(d[0], pa) * pow(d[1], pb) * pow(d[2], pc - 1);
+            }
+        }
+    *val = v; grad[0] = g[0]; grad[1] = g[1]; grad[2] = g[2];
+}
+
+/* ------------------------------------------------------------------------------------------
+ * C-8 tree evaluation for the listed groups (all if groups == NULL).  Results go to acc[n][3],
+ * pot[n] in the CALLER's particle order; entries of particles outside the listed groups are left
+ * untouched.  Periodic: 125 explicit images (Plummer g on every explicit term) + far field
+ * (a = +grad, phi = -value; the j = i term stays in, C-9 step 3).
+ * ---------------------------------------------------------------------------------------- */
+void orc_tree_forces(orc_t *t, double theta, double eps, int order, const int64_t *groups,
+                     int64_t ng, double *acc, double *pot, int64_t *Lpc, int64_t *Lpp) {
+    mi_init();
+    int ws = image_range(t);
+    if (t->periodic) far_prepare(t);
+    if (!groups) ng = t->ngroups;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t q = 0; q < ng; ++q) {
+        int64_t g = groups ? groups[q] : q;
+        walk_t w; walk_setup(&w, t, theta, g);
+        int64_t nG = w.gcount, npc = 0, npp = 0;
+        double *a = calloc((size_t)nG * 3, sizeof(double)), *p = calloc((size_t)nG, sizeof(double));
+        for (int ix = -ws; ix <= ws; ++ix) for (int iy = -ws; iy <= ws; ++iy) for (int iz = -ws; iz <= ws; ++iz) {
+            walk_setup(&w, t, theta, g);
+            w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
+            w.shx[0] = ix * t->size; w.shx[1] = iy * t->size; w.shx[2] = iz * t->size;
+            w.eval = 1; w.order = order; w.eps2 = eps * eps; w.acc = a; w.pot = p;
+            walk_rec(&w, 0);
+            npc += w.npc; npp += w.npp;
+        }
+        if (Lpc) Lpc[q] = npc;
+        if (Lpp) Lpp[q] = npp;
+        for (int64_t i = 0; i < nG; ++i) {
+            int64_t s = w.gfirst + i, o = (int64_t)t->perm[s];
+            if (t->periodic) {
+                double v, gr[3]; far_on_sink(t, t->x + 3 * s, &v, gr);
+                p[i] -= v / t->size;
+                for (int k = 0; k < 3; ++k) a[3 * i + k] += gr[k] / (t->size * t->size);
+            }
+            for (int k = 0; k < 3; ++k) acc[3 * o + k] = a[3 * i + k];
+            pot[o] = p[i];
+        }
+        free(a); free(p);
+    }
+}
+int orc_num_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
