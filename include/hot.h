@@ -1,0 +1,128 @@
+/*
+ * hot.h -- C ABI of the B200-native hot path of 2HOT's hashed oct-tree method
+ * (Warren, "2HOT: An Improved Parallel Hashed Oct-Tree N-Body Algorithm for Cosmological
+ * Simulation", SC'13, arXiv:1310.4502; the text is PAPER.md, cited as PAPER.md:<line>).
+ *
+ * What the library computes (one GPU, every stage a CUDA kernel for sm_100a):
+ *   hot_build : integer keys from coordinates ("mapping of spatial co-ordinates to
+ *               integer keys described in WS93"), on-node radix sort, bodies into
+ *               key order, the hashed oct-tree of the sorted keys and the sink
+ *               cells of the m x n blocking.
+ *   hot_forces: moments of eq (6), the source/sink traversal with a multipole
+ *               acceptance criterion and the Plummer-softened
+ *                particle-particle and Cartesian-multipole particle-cell
+ *               interactions of eq (5) giving the right-hand side of eq (2)
+ *               (PAPER.md:57): acc_i = -grad phi(x_i), phi_i, G = 1, self term excluded.
+ *               Periodic boxes: 124 boundary cubes + local expansion, p = 8, ws = 2.
+ *   hot_stats : sizes, interaction counts and per-stage device times of the last calls.
+ *
+ * The readings of everything the paper leaves open (key bit order, bucket sizes, the
+ * opening criterion, the far-field route) are listed in DESIGN.md "Readings".
+ *
+ * Conventions
+ *   - "device" pointers are CUDA device pointers of the current device (e.g. torch data_ptr());
+ *     "host" pointers are ordinary host memory.  The library never keeps a caller pointer.
+ *   - One implicit context per process.  Not thread-safe.
+ *   - Every call returns HOT_OK (0) or a negative hot_status; hot_last_error() gives the text.
+ *     No exceptions, no abort, no printing.  After a failed hot_build there is no build.
+ *   - Work is enqueued on the stream given to hot_set_stream (default: the legacy stream 0).
+ *     hot_build synchronises that stream (it needs the cell count to size the tree);
+ *     hot_forces synchronises it once at the end to read the error flag.
+ */
+#ifndef HOT_H_
+#define HOT_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    HOT_OK = 0,
+    HOT_EINVAL = -1,  /* bad argument: NULL, n out of range, size <= 0, theta, eps, order */
+    HOT_ERANGE = -2,  /* a particle lies outside [lo, lo+size)^3 (open AND periodic mode) */
+    HOT_ENOMEM = -3,  /* device or host allocation failed */
+    HOT_ECUDA = -4,   /* a CUDA call or kernel failed; text in hot_last_error() */
+    HOT_EORDER = -5,  /* hot_forces / export before a successful hot_build */
+    HOT_EINTERNAL = -6 /* traversal scratch exhausted or an internal invariant failed */
+} hot_status;
+
+/* Root cube of the tree and, when periodic, the period. size > 0. */
+typedef struct {
+    float lo[3];
+    float size;
+} hot_box;
+
+/* Filled by hot_stats (host struct).  Times are device milliseconds of the LAST call that ran
+ * the stage, measured with CUDA events on the library's stream. */
+typedef struct {
+    int64_t n, n_cells, n_leaves, n_groups;
+    int32_t max_level, nleaf, ncrit, periodic;
+    int64_t hash_capacity;
+    int32_t hash_max_probe, order; /* order of the last hot_forces */
+    /* sum over sink groups G of n_G * L_pp(G) and n_G * L_pc(G); L_pp counts the group's own
+     * particles too (the self slot), images included when periodic */
+    uint64_t pp_interactions, pc_interactions;
+    uint64_t cells_visited;     /* MAC tests of the last walk */
+    uint64_t walk_spills;       /* traversal-stack spills to the global arena */
+    float ms_keygen, ms_sort, ms_gather, ms_tree, ms_moments, ms_walk_eval, ms_farfield;
+    float ms_build_total, ms_forces_total;
+    int64_t bytes_allocated;
+} hot_stats_t;
+
+/* Bucket sizes of the tree: a cell with more than nleaf bodies is split (down
+ * to level 21); sink groups are the cells with at most ncrit bodies whose parent has more.
+ * 1 <= nleaf <= ncrit <= 256, nleaf <= 32.  Takes effect at the next hot_build.
+ * Defaults: nleaf = 16, ncrit = 64. */
+int hot_set_params(int nleaf, int ncrit);
+
+/* pos : device, [n][3] fp32 row-major x,y,z; borrowed.   mass: device, [n] fp32 > 0; borrowed.
+ * n   : 1 <= n <= 2^27 (and < 2^27 coincident bodies in one finest-level cell).
+ * periodic: 0 open, 1 periodic with period box.size.  In both modes every particle must satisfy
+ *           0 <= fl32((x-lo)*fl32(1/size)) < 1 per axis, else HOT_ERANGE (the caller wraps).
+ * Builds keys, the stable key-sorted permutation, key-ordered bodies, cells, hash table and
+ * sink groups; replaces any previous build. */
+int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int periodic);
+
+/* theta: opening angle, 0 <= theta < 1 (0: every interaction is particle-particle).
+ * eps  : Plummer softening length >= 0 (0 with coincident distinct bodies gives inf/NaN).
+ * order: 0 (monopole), 2 (through quadrupole) or 4 (through hexadecapole, octupole included).
+ * acc  : device, [n][3] fp32, caller's particle order; overwritten.
+ * pot  : device, [n] fp32 or NULL; overwritten.
+ * May be called repeatedly on one build with different theta / eps / order. */
+int hot_forces(double theta, double eps, int order, float* acc, float* pot);
+
+int hot_stats(hot_stats_t* out);
+
+/* Same path with HOST buffers: copies pos/mass to the device, hot_build, hot_forces, copies acc
+ * (and pot unless NULL) back; returns after the results are in host memory. */
+int hot_step_host(const float* pos, const float* mass, int64_t n, hot_box box, int periodic,
+                  double theta, double eps, int order, float* acc, float* pot);
+
+int hot_set_stream(void* cuda_stream); /* cudaStream_t; NULL = legacy default stream */
+void hot_free(void);                   /* releases everything the library owns */
+const char* hot_last_error(void);
+
+/* ---- introspection for the parity tests: HOST output arrays, caller-allocated -------------- */
+/* sorted keys and the permutation: key_sorted[i] = key of caller's particle perm[i]; [n] each */
+int hot_export_keys(uint64_t* key_sorted, uint32_t* perm);
+/* cells in ascending numeric key order; any pointer may be NULL.  cap = array length;
+ * *ncells is always set; HOT_EINVAL if cap is too small.
+ * child = index of the first child or -1 for a leaf; parent = -1 for the root. */
+int hot_export_cells(uint64_t* key, uint32_t* first, uint32_t* count, uint8_t* mask,
+                     int32_t* child, int32_t* parent, int64_t cap, int64_t* ncells);
+/* sink groups in particle order: cell index, and the list counts of the last hot_forces
+ * (zeros before the first): L_pc = accepted cells, L_pp = particles of rejected leaves. */
+int hot_export_groups(int32_t* cell, uint64_t* lpc, uint64_t* lpp, int64_t cap, int64_t* ngroups);
+/* moments of the last hot_forces: com [ncells][3] double, m0 [ncells], m2 [ncells][6]
+ * (xx xy xz yy yz zz), m3 [ncells][10], m4 [ncells][15] (degree-major, x>y>z); NULL to skip;
+ * m3/m4 only when the last order was 4 (else HOT_EINVAL if requested). */
+int hot_export_moments(double* com, float* m0, float* m2, float* m3, float* m4, int64_t cap);
+/* hash table: cell index of each key, -1 if absent.  keys, idx: host, [nkeys]. */
+int hot_lookup_keys(const uint64_t* keys, int64_t nkeys, int32_t* idx);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOT_H_ */

@@ -1,0 +1,198 @@
+"""ctypes marshalling for include/hot.h.  Same names as the C entry points."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIBPATH = os.path.join(_HERE, "libhot.so")
+_lib = None
+
+STATUS = {0: "HOT_OK", -1: "HOT_EINVAL", -2: "HOT_ERANGE", -3: "HOT_ENOMEM", -4: "HOT_ECUDA",
+          -5: "HOT_EORDER", -6: "HOT_EINTERNAL"}
+
+
+class HotError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"{STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class hot_box(C.Structure):
+    _fields_ = [("lo", C.c_float * 3), ("size", C.c_float)]
+
+
+class hot_stats_t(C.Structure):
+    _fields_ = [("n", C.c_int64), ("n_cells", C.c_int64), ("n_leaves", C.c_int64), ("n_groups", C.c_int64),
+                ("max_level", C.c_int32), ("nleaf", C.c_int32), ("ncrit", C.c_int32), ("periodic", C.c_int32),
+                ("hash_capacity", C.c_int64), ("hash_max_probe", C.c_int32), ("order", C.c_int32),
+                ("pp_interactions", C.c_uint64), ("pc_interactions", C.c_uint64),
+                ("cells_visited", C.c_uint64), ("walk_spills", C.c_uint64),
+                ("ms_keygen", C.c_float), ("ms_sort", C.c_float), ("ms_gather", C.c_float), ("ms_tree", C.c_float),
+                ("ms_moments", C.c_float), ("ms_walk_eval", C.c_float), ("ms_farfield", C.c_float),
+                ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float), ("bytes_allocated", C.c_int64)]
+
+
+def library_path() -> str:
+    return _LIBPATH
+
+
+def _load():
+    """Load libhot.so; fail loudly if it was not built (no fallback of any kind)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIBPATH):
+            raise ImportError(f"{_LIBPATH} is missing: run `python -m paper_1310_4502_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        lib = C.CDLL(_LIBPATH)
+        lib.hot_last_error.restype = C.c_char_p
+        lib.hot_build.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, hot_box, C.c_int]
+        lib.hot_forces.argtypes = [C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+        lib.hot_stats.argtypes = [C.POINTER(hot_stats_t)]
+        lib.hot_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, hot_box, C.c_int, C.c_double,
+                                      C.c_double, C.c_int, C.c_void_p, C.c_void_p]
+        lib.hot_set_stream.argtypes = [C.c_void_p]
+        lib.hot_set_params.argtypes = [C.c_int, C.c_int]
+        lib.hot_free.restype = None
+        lib.hot_export_keys.argtypes = [C.c_void_p, C.c_void_p]
+        lib.hot_export_cells.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
+        lib.hot_export_groups.argtypes = [C.c_void_p] * 3 + [C.c_int64, C.POINTER(C.c_int64)]
+        lib.hot_export_moments.argtypes = [C.c_void_p] * 5 + [C.c_int64]
+        lib.hot_lookup_keys.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
+        _lib = lib
+    return _lib
+
+
+def _check(rc: int):
+    if rc != 0:
+        raise HotError(rc, _load().hot_last_error().decode())
+
+
+def _box(lo, size) -> hot_box:
+    b = hot_box()
+    b.lo[0], b.lo[1], b.lo[2] = float(lo[0]), float(lo[1]), float(lo[2])
+    b.size = float(size)
+    return b
+
+
+def hot_last_error() -> str:
+    return _load().hot_last_error().decode()
+
+
+def hot_set_stream(stream=None):
+    """Pass a torch.cuda.Stream (or None for the legacy default stream)."""
+    ptr = None if stream is None else C.c_void_p(stream.cuda_stream)
+    _check(_load().hot_set_stream(ptr))
+
+
+def hot_set_params(nleaf: int = 16, ncrit: int = 64):
+    _check(_load().hot_set_params(int(nleaf), int(ncrit)))
+
+
+def hot_free():
+    _load().hot_free()
+
+
+_n_built = 0
+_dev = None
+
+
+def hot_build(pos, mass, lo, size, periodic=False):
+    """pos [n,3] / mass [n]: contiguous CUDA float32 tensors (borrowed for the call)."""
+    import torch
+
+    global _n_built, _dev
+    if not (pos.is_cuda and mass.is_cuda and pos.dtype == torch.float32 and mass.dtype == torch.float32):
+        raise TypeError("hot_build wants CUDA float32 tensors")
+    if not (pos.is_contiguous() and mass.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3
+            and mass.numel() == pos.shape[0]):
+        raise TypeError("hot_build wants contiguous pos [n,3] and mass [n]")
+    n = pos.shape[0]
+    _n_built, _dev = 0, pos.device
+    _check(_load().hot_build(pos.data_ptr(), mass.data_ptr(), n, _box(lo, size), int(bool(periodic))))
+    _n_built = n
+
+
+def hot_forces(theta, eps, order, acc=None, pot=None, want_pot=True):
+    """Returns (acc [n,3], pot [n] or None) as CUDA float32 tensors in the caller's particle order."""
+    import torch
+
+    n = _n_built
+    if acc is None:
+        acc = torch.empty((max(n, 1), 3), dtype=torch.float32, device=_dev or "cuda")
+    if pot is None and want_pot:
+        pot = torch.empty(max(n, 1), dtype=torch.float32, device=_dev or "cuda")
+    _check(_load().hot_forces(float(theta), float(eps), int(order), acc.data_ptr(),
+                              pot.data_ptr() if pot is not None else None))
+    return acc, pot
+
+
+def hot_stats() -> dict:
+    s = hot_stats_t()
+    _check(_load().hot_stats(C.byref(s)))
+    return {k: getattr(s, k) for k, _ in hot_stats_t._fields_}
+
+
+def hot_step_host(pos, mass, lo, size, periodic, theta, eps, order, acc=None, pot=None):
+    """HOST numpy float32 arrays in, HOST arrays out; copies are inside the call."""
+    pos = np.ascontiguousarray(pos, dtype=np.float32)
+    mass = np.ascontiguousarray(mass, dtype=np.float32)
+    n = pos.shape[0]
+    if acc is None:
+        acc = np.empty((n, 3), np.float32)
+    if pot is None:
+        pot = np.empty(n, np.float32)
+    _check(_load().hot_step_host(pos.ctypes.data, mass.ctypes.data, n, _box(lo, size), int(bool(periodic)),
+                                 float(theta), float(eps), int(order), acc.ctypes.data, pot.ctypes.data))
+    return acc, pot
+
+
+def hot_export_keys():
+    n = hot_stats()["n"]
+    key = np.empty(n, np.uint64)
+    perm = np.empty(n, np.uint32)
+    _check(_load().hot_export_keys(key.ctypes.data, perm.ctypes.data))
+    return key, perm
+
+
+def hot_export_cells() -> dict:
+    nc = hot_stats()["n_cells"]
+    out = dict(key=np.empty(nc, np.uint64), first=np.empty(nc, np.uint32), count=np.empty(nc, np.uint32),
+               mask=np.empty(nc, np.uint8), child=np.empty(nc, np.int32), parent=np.empty(nc, np.int32))
+    got = C.c_int64()
+    _check(_load().hot_export_cells(out["key"].ctypes.data, out["first"].ctypes.data, out["count"].ctypes.data,
+                                    out["mask"].ctypes.data, out["child"].ctypes.data, out["parent"].ctypes.data,
+                                    nc, C.byref(got)))
+    return out
+
+
+def hot_export_groups() -> dict:
+    ng = hot_stats()["n_groups"]
+    out = dict(cell=np.empty(ng, np.int32), lpc=np.empty(ng, np.uint64), lpp=np.empty(ng, np.uint64))
+    got = C.c_int64()
+    _check(_load().hot_export_groups(out["cell"].ctypes.data, out["lpc"].ctypes.data, out["lpp"].ctypes.data,
+                                     ng, C.byref(got)))
+    return out
+
+
+def hot_export_moments(order: int) -> dict:
+    nc = hot_stats()["n_cells"]
+    out = dict(com=np.empty((nc, 3), np.float64), m0=np.empty(nc, np.float32))
+    m2 = m3 = m4 = None
+    if order >= 2:
+        out["m2"] = m2 = np.empty((nc, 6), np.float32)
+    if order >= 4:
+        out["m3"] = m3 = np.empty((nc, 10), np.float32)
+        out["m4"] = m4 = np.empty((nc, 15), np.float32)
+    p = lambda a: a.ctypes.data if a is not None else None
+    _check(_load().hot_export_moments(p(out["com"]), p(out["m0"]), p(m2), p(m3), p(m4), nc))
+    return out
+
+
+def hot_lookup_keys(keys) -> np.ndarray:
+    keys = np.ascontiguousarray(keys, dtype=np.uint64)
+    idx = np.empty(keys.shape[0], np.int32)
+    _check(_load().hot_lookup_keys(keys.ctypes.data, keys.shape[0], idx.ctypes.data))
+    return idx

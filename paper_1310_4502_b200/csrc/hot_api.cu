@@ -1,0 +1,409 @@
+// hot_api.cu -- the C ABI of include/hot.h: context, allocations, stage orchestration, exports.
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <vector>
+
+#include "hot_internal.h"
+
+namespace {
+
+struct Ctx {
+    cudaStream_t stream = nullptr;
+    Tree t;
+    bool built = false;
+    int nleaf = 16, ncrit = 64;
+    int last_order = -1;
+    char err[512] = "";
+    // scratch owned across calls
+    int* d_flags = nullptr;               // [0] build error bits, [1] hash max probe, [2] forces error bits
+    unsigned int* d_counter = nullptr;
+    unsigned long long* d_stat = nullptr; // 4 counters
+    uint32_t* d_gstack = nullptr; size_t gstack_bytes = 0; int64_t gstack_cap = 0;
+    std::vector<void*> tree_allocs;       // everything owned by the current build
+    int64_t bytes = 0;
+    hot_stats_t st{};
+    cudaEvent_t ev[8] = {};
+    bool ev_ready = false;
+    // host staging for hot_step_host
+    float *h_pos = nullptr, *h_mass = nullptr, *h_acc = nullptr, *h_pot = nullptr; int64_t h_n = 0;
+    float *hd_pos = nullptr, *hd_mass = nullptr, *hd_acc = nullptr, *hd_pot = nullptr;
+};
+Ctx g;
+
+int fail(int code, const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g.err, sizeof(g.err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+#define CUDA_TRY(expr)                                                                                   \
+    do {                                                                                                 \
+        cudaError_t e_ = (expr);                                                                         \
+        if (e_ != cudaSuccess) {                                                                         \
+            int code_ = e_ == cudaErrorMemoryAllocation ? HOT_ENOMEM : HOT_ECUDA;                        \
+            cudaGetLastError();                                                                          \
+            return fail(code_, "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(e_), __FILE__, __LINE__); \
+        }                                                                                                \
+    } while (0)
+
+template <typename T> cudaError_t tree_alloc(T** p, size_t count) {
+    void* q = nullptr;
+    size_t bytes = count * sizeof(T);
+    if (bytes == 0) bytes = sizeof(T);
+    cudaError_t e = cudaMalloc(&q, bytes);
+    if (e != cudaSuccess) return e;
+    g.tree_allocs.push_back(q);
+    g.bytes += (int64_t)bytes;
+    *p = static_cast<T*>(q);
+    return cudaSuccess;
+}
+void drop_build() {
+    for (void* p : g.tree_allocs) cudaFree(p);
+    g.tree_allocs.clear();
+    g.bytes = 0;
+    int nleaf = g.t.nleaf, ncrit = g.t.ncrit;
+    g.t = Tree();
+    g.t.nleaf = nleaf; g.t.ncrit = ncrit;
+    g.built = false;
+    g.last_order = -1;
+}
+int ensure_scratch() {
+    if (!g.d_flags) {
+        CUDA_TRY(cudaMalloc(&g.d_flags, 4 * sizeof(int)));
+        CUDA_TRY(cudaMalloc(&g.d_counter, sizeof(unsigned int)));
+        CUDA_TRY(cudaMalloc(&g.d_stat, 4 * sizeof(unsigned long long)));
+    }
+    if (!g.ev_ready) {
+        for (auto& e : g.ev) CUDA_TRY(cudaEventCreate(&e));
+        g.ev_ready = true;
+    }
+    return HOT_OK;
+}
+float ms_between(cudaEvent_t a, cudaEvent_t b) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, a, b) != cudaSuccess) { cudaGetLastError(); ms = 0; }
+    return ms;
+}
+
+} // namespace
+
+extern "C" {
+
+const char* hot_last_error(void) { return g.err; }
+
+int hot_set_stream(void* s) {
+    g.stream = static_cast<cudaStream_t>(s);
+    return HOT_OK;
+}
+
+int hot_set_params(int nleaf, int ncrit) {
+    if (nleaf < 1 || nleaf > HOT_MAX_NLEAF || ncrit < nleaf || ncrit > HOT_MAX_NCRIT)
+        return fail(HOT_EINVAL, "hot_set_params: need 1 <= nleaf <= %d, nleaf <= ncrit <= %d", HOT_MAX_NLEAF, HOT_MAX_NCRIT);
+    g.nleaf = nleaf; g.ncrit = ncrit;
+    return HOT_OK;
+}
+
+void hot_free(void) {
+    drop_build();
+    cudaFree(g.d_flags); cudaFree(g.d_counter); cudaFree(g.d_stat); cudaFree(g.d_gstack);
+    g.d_flags = nullptr; g.d_counter = nullptr; g.d_stat = nullptr; g.d_gstack = nullptr; g.gstack_bytes = 0;
+    if (g.ev_ready) { for (auto& e : g.ev) cudaEventDestroy(e); g.ev_ready = false; }
+    cudaFreeHost(g.h_pos); cudaFreeHost(g.h_mass); cudaFreeHost(g.h_acc); cudaFreeHost(g.h_pot);
+    cudaFree(g.hd_pos); cudaFree(g.hd_mass); cudaFree(g.hd_acc); cudaFree(g.hd_pot);
+    g.h_pos = g.h_mass = g.h_acc = g.h_pot = nullptr; g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
+    cudaGetLastError();
+    g.st = hot_stats_t{};
+}
+
+int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int periodic) {
+    if (!pos || !mass) return fail(HOT_EINVAL, "hot_build: NULL pos or mass");
+    if (n < 1 || n > ((int64_t)1 << 27)) return fail(HOT_EINVAL, "hot_build: n = %lld outside [1, 2^27]", (long long)n);
+    if (!(box.size > 0.0f) || !(box.size < 3.0e38f)) return fail(HOT_EINVAL, "hot_build: box.size must be positive and finite");
+    if (periodic != 0 && periodic != 1) return fail(HOT_EINVAL, "hot_build: periodic must be 0 or 1");
+    int rc = ensure_scratch();
+    if (rc) return rc;
+    drop_build();
+    Tree& t = g.t;
+    t.n = n; t.periodic = periodic; t.nleaf = g.nleaf; t.ncrit = g.ncrit; t.box = box;
+    for (int k = 0; k < 3; ++k) t.lo[k] = (double)box.lo[k];
+    t.size = (double)box.size;
+    cudaStream_t st = g.stream;
+    const float inv = 1.0f / box.size; // one IEEE fp32 division on the host: part of the key's definition
+
+    struct Guard { bool ok = false; ~Guard() { if (!ok) drop_build(); } } guard;
+
+    uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
+    const int64_t nblk = tree_num_blocks(n);
+    const int rows = HOT_NLEVELS + 2;
+    CUDA_TRY(tree_alloc(&t.key[0], (size_t)n));
+    CUDA_TRY(tree_alloc(&t.key[1], (size_t)n));
+    CUDA_TRY(tree_alloc(&t.idx[0], (size_t)n));
+    CUDA_TRY(tree_alloc(&t.idx[1], (size_t)n));
+    CUDA_TRY(tree_alloc(&t.body, (size_t)n));
+    CUDA_TRY(tree_alloc(&t.plev, (size_t)n));
+    CUDA_TRY(tree_alloc(&d_hist, sort_hist_elems(n)));
+    CUDA_TRY(tree_alloc(&d_counts, (size_t)rows * (size_t)nblk));
+    CUDA_TRY(tree_alloc(&d_totals, (size_t)rows));
+    CUDA_TRY(cudaMemsetAsync(g.d_flags, 0, 4 * sizeof(int), st));
+
+    CUDA_TRY(cudaEventRecord(g.ev[0], st));
+    CUDA_TRY(launch_keygen(pos, n, box.lo[0], box.lo[1], box.lo[2], inv, t.key[0], t.idx[0], g.d_flags, st));
+    CUDA_TRY(cudaEventRecord(g.ev[1], st));
+    CUDA_TRY(launch_radix_sort(t.key, t.idx, n, d_hist, st));
+    CUDA_TRY(cudaEventRecord(g.ev[2], st));
+    CUDA_TRY(launch_gather(pos, mass, t.idx[0], n, t.body, st));
+    CUDA_TRY(cudaEventRecord(g.ev[3], st));
+    CUDA_TRY(launch_tree_levels(t.key[0], n, t.nleaf, t.ncrit, t.plev, d_counts, st));
+    CUDA_TRY(launch_tree_scan(d_counts, nblk, d_totals, st));
+    uint32_t totals[HOT_NLEVELS + 2];
+    int flags[4];
+    CUDA_TRY(cudaMemcpyAsync(totals, d_totals, sizeof(totals), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(flags, g.d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (flags[0] & 1) return fail(HOT_ERANGE, "hot_build: a particle lies outside [lo, lo+size)^3");
+    t.level_base[0] = 0;
+    t.max_level = 0;
+    for (int l = 0; l < HOT_NLEVELS; ++l) {
+        t.level_base[l + 1] = t.level_base[l] + (int64_t)totals[l];
+        if (totals[l]) t.max_level = l;
+    }
+    t.ncells = t.level_base[HOT_NLEVELS];
+    t.ngroups = (int64_t)totals[HOT_NLEVELS];
+    t.nleaves = (int64_t)totals[HOT_NLEVELS + 1];
+    if (t.ncells >= ((int64_t)1 << 31) - 1) return fail(HOT_EINTERNAL, "hot_build: %lld cells exceed the 31-bit cell index", (long long)t.ncells);
+    t.hcap = 64;
+    while (t.hcap < 2 * t.ncells) t.hcap <<= 1;
+    CUDA_TRY(tree_alloc(&t.ckey, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.cfirst, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.ccount, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.cmask, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.cchild, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.cparent, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.wcell, (size_t)t.ncells));
+    CUDA_TRY(tree_alloc(&t.group, (size_t)t.ngroups));
+    CUDA_TRY(tree_alloc(&t.glpc, (size_t)t.ngroups));
+    CUDA_TRY(tree_alloc(&t.glpp, (size_t)t.ngroups));
+    CUDA_TRY(tree_alloc(&t.hkey, (size_t)t.hcap));
+    CUDA_TRY(tree_alloc(&t.hval, (size_t)t.hcap));
+    CUDA_TRY(cudaMemsetAsync(t.hkey, 0, sizeof(uint64_t) * (size_t)t.hcap, st));
+    CUDA_TRY(cudaMemsetAsync(t.cmask, 0, sizeof(uint32_t) * (size_t)t.ncells, st));
+    CUDA_TRY(cudaMemsetAsync(t.glpc, 0, sizeof(uint64_t) * (size_t)t.ngroups, st));
+    CUDA_TRY(cudaMemsetAsync(t.glpp, 0, sizeof(uint64_t) * (size_t)t.ngroups, st));
+    TreeEmitArgs ea;
+    ea.skey = t.key[0]; ea.plev = t.plev; ea.counts = d_counts; ea.n = n; ea.nblk = nblk;
+    for (int l = 0; l <= HOT_NLEVELS; ++l) ea.level_base[l] = t.level_base[l];
+    ea.ckey = t.ckey; ea.cfirst = t.cfirst; ea.ccount = t.ccount; ea.cchild = t.cchild; ea.cparent = t.cparent;
+    ea.group = t.group; ea.hkey = t.hkey; ea.hval = t.hval; ea.hmask = t.hcap - 1; ea.maxprobe = g.d_flags + 1;
+    CUDA_TRY(launch_tree_emit(ea, st));
+    CUDA_TRY(launch_tree_link(t.ckey, t.cparent, t.cmask, t.ncells, st));
+    CUDA_TRY(launch_tree_finalize(t.ckey, t.cfirst, t.ccount, t.cmask, t.cchild, t.wcell, t.ncells, g.d_flags, st));
+    CUDA_TRY(cudaEventRecord(g.ev[4], st));
+    CUDA_TRY(cudaMemcpyAsync(flags, g.d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (flags[0] & 2) return fail(HOT_ERANGE, "hot_build: 2^27 or more coincident bodies in one finest-level cell");
+    t.hash_max_probe = flags[1];
+
+    hot_stats_t& s = g.st;
+    s = hot_stats_t{};
+    s.n = n; s.n_cells = t.ncells; s.n_leaves = t.nleaves; s.n_groups = t.ngroups; s.max_level = t.max_level;
+    s.nleaf = t.nleaf; s.ncrit = t.ncrit; s.periodic = periodic; s.hash_capacity = t.hcap; s.hash_max_probe = t.hash_max_probe;
+    s.order = -1;
+    s.ms_keygen = ms_between(g.ev[0], g.ev[1]);
+    s.ms_sort = ms_between(g.ev[1], g.ev[2]);
+    s.ms_gather = ms_between(g.ev[2], g.ev[3]);
+    s.ms_tree = ms_between(g.ev[3], g.ev[4]);
+    s.ms_build_total = ms_between(g.ev[0], g.ev[4]);
+    s.bytes_allocated = g.bytes;
+    guard.ok = true;
+    g.built = true;
+    return HOT_OK;
+}
+
+int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
+    if (!g.built) return fail(HOT_EORDER, "hot_forces: no successful hot_build");
+    if (!acc) return fail(HOT_EINVAL, "hot_forces: NULL acc");
+    if (!(theta >= 0.0) || !(theta < 1.0)) return fail(HOT_EINVAL, "hot_forces: theta must be in [0, 1)");
+    if (!(eps >= 0.0)) return fail(HOT_EINVAL, "hot_forces: eps must be >= 0");
+    if (order == 1) order = 0;
+    if (order != 0 && order != 2 && order != 4) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2 or 4");
+    Tree& t = g.t;
+    cudaStream_t st = g.stream;
+    CUDA_TRY(cudaEventRecord(g.ev[5], st));
+    // S6: moments, cached per build at the highest order asked so far
+    if (t.mom_order < order) {
+        if (!t.cellA) CUDA_TRY(tree_alloc(&t.cellA, (size_t)t.ncells));
+        if (order >= 2 && !t.cellM2) CUDA_TRY(tree_alloc(&t.cellM2, (size_t)t.ncells));
+        if (order >= 4 && !t.cellM34) CUDA_TRY(tree_alloc(&t.cellM34, (size_t)t.ncells));
+        CUDA_TRY(launch_moments(t, order, st));
+        t.mom_order = order;
+    }
+    CUDA_TRY(cudaEventRecord(g.ev[6], st));
+    const int scap = (t.ncrit + 31) / 32;
+    const int nwarps = force_grid_warps(order, t.periodic, scap);
+    const int64_t gcap = 8192; // spill arena entries per warp
+    size_t need = (size_t)nwarps * (size_t)gcap * sizeof(uint32_t) * (t.periodic ? 2 : 1);
+    if (need > g.gstack_bytes) {
+        cudaFree(g.d_gstack); g.d_gstack = nullptr; g.gstack_bytes = 0;
+        CUDA_TRY(cudaMalloc(&g.d_gstack, need));
+        g.gstack_bytes = need;
+    }
+    CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, sizeof(unsigned int), st));
+    CUDA_TRY(cudaMemsetAsync(g.d_stat, 0, 4 * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
+    ForceArgs a{};
+    a.wcell = t.wcell; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellM34 = t.cellM34;
+    a.body = t.body; a.perm = t.idx[0]; a.group = t.group; a.ngroups = t.ngroups;
+    a.theta2 = theta * theta; // formed once on the host in double (R-7)
+    a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic; a.scap = scap;
+    for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
+    a.size = t.size;
+    a.acc = acc; a.pot = pot; a.glpc = t.glpc; a.glpp = t.glpp;
+    a.counter = g.d_counter; a.stat = g.d_stat; a.gstack = g.d_gstack; a.gstack_cap = gcap; a.errflag = g.d_flags + 2;
+    CUDA_TRY(launch_forces(a, st));
+    CUDA_TRY(cudaEventRecord(g.ev[7], st));
+    int flag = 0;
+    unsigned long long stat[4];
+    CUDA_TRY(cudaMemcpyAsync(&flag, g.d_flags + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (flag) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted (flag %d)", flag);
+    hot_stats_t& s = g.st;
+    s.order = order;
+    s.cells_visited = stat[0]; s.walk_spills = stat[1]; s.pp_interactions = stat[2]; s.pc_interactions = stat[3];
+    s.ms_moments = ms_between(g.ev[5], g.ev[6]);
+    s.ms_walk_eval = ms_between(g.ev[6], g.ev[7]);
+    s.ms_farfield = 0;
+    s.ms_forces_total = ms_between(g.ev[5], g.ev[7]);
+    s.bytes_allocated = g.bytes + (int64_t)g.gstack_bytes;
+    g.last_order = order;
+    return HOT_OK;
+}
+
+int hot_stats(hot_stats_t* out) {
+    if (!out) return fail(HOT_EINVAL, "hot_stats: NULL out");
+    *out = g.st;
+    return HOT_OK;
+}
+
+int hot_step_host(const float* pos, const float* mass, int64_t n, hot_box box, int periodic, double theta, double eps,
+                  int order, float* acc, float* pot) {
+    if (!pos || !mass || !acc) return fail(HOT_EINVAL, "hot_step_host: NULL argument");
+    if (n < 1 || n > ((int64_t)1 << 27)) return fail(HOT_EINVAL, "hot_step_host: n out of range");
+    if (g.h_n < n) {
+        cudaFree(g.hd_pos); cudaFree(g.hd_mass); cudaFree(g.hd_acc); cudaFree(g.hd_pot);
+        g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
+        CUDA_TRY(cudaMalloc(&g.hd_pos, sizeof(float) * 3 * (size_t)n));
+        CUDA_TRY(cudaMalloc(&g.hd_mass, sizeof(float) * (size_t)n));
+        CUDA_TRY(cudaMalloc(&g.hd_acc, sizeof(float) * 3 * (size_t)n));
+        CUDA_TRY(cudaMalloc(&g.hd_pot, sizeof(float) * (size_t)n));
+        g.h_n = n;
+    }
+    cudaStream_t st = g.stream;
+    CUDA_TRY(cudaMemcpyAsync(g.hd_pos, pos, sizeof(float) * 3 * (size_t)n, cudaMemcpyHostToDevice, st));
+    CUDA_TRY(cudaMemcpyAsync(g.hd_mass, mass, sizeof(float) * (size_t)n, cudaMemcpyHostToDevice, st));
+    int rc = hot_build(g.hd_pos, g.hd_mass, n, box, periodic);
+    if (rc) return rc;
+    rc = hot_forces(theta, eps, order, g.hd_acc, pot ? g.hd_pot : nullptr);
+    if (rc) return rc;
+    CUDA_TRY(cudaMemcpyAsync(acc, g.hd_acc, sizeof(float) * 3 * (size_t)n, cudaMemcpyDeviceToHost, st));
+    if (pot) CUDA_TRY(cudaMemcpyAsync(pot, g.hd_pot, sizeof(float) * (size_t)n, cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    return HOT_OK;
+}
+
+// ---- introspection -----------------------------------------------------------------------------
+int hot_export_keys(uint64_t* key_sorted, uint32_t* perm) {
+    if (!g.built) return fail(HOT_EORDER, "hot_export_keys: no build");
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    if (key_sorted) CUDA_TRY(cudaMemcpy(key_sorted, g.t.key[0], sizeof(uint64_t) * (size_t)g.t.n, cudaMemcpyDeviceToHost));
+    if (perm) CUDA_TRY(cudaMemcpy(perm, g.t.idx[0], sizeof(uint32_t) * (size_t)g.t.n, cudaMemcpyDeviceToHost));
+    return HOT_OK;
+}
+int hot_export_cells(uint64_t* key, uint32_t* first, uint32_t* count, uint8_t* mask, int32_t* child, int32_t* parent,
+                     int64_t cap, int64_t* ncells) {
+    if (!g.built) return fail(HOT_EORDER, "hot_export_cells: no build");
+    const Tree& t = g.t;
+    if (ncells) *ncells = t.ncells;
+    if (cap < t.ncells) return fail(HOT_EINVAL, "hot_export_cells: cap %lld < %lld cells", (long long)cap, (long long)t.ncells);
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    size_t nc = (size_t)t.ncells;
+    if (key) CUDA_TRY(cudaMemcpy(key, t.ckey, 8 * nc, cudaMemcpyDeviceToHost));
+    if (first) CUDA_TRY(cudaMemcpy(first, t.cfirst, 4 * nc, cudaMemcpyDeviceToHost));
+    if (count) CUDA_TRY(cudaMemcpy(count, t.ccount, 4 * nc, cudaMemcpyDeviceToHost));
+    if (child) CUDA_TRY(cudaMemcpy(child, t.cchild, 4 * nc, cudaMemcpyDeviceToHost));
+    if (parent) CUDA_TRY(cudaMemcpy(parent, t.cparent, 4 * nc, cudaMemcpyDeviceToHost));
+    if (mask) {
+        std::vector<uint32_t> m(nc);
+        CUDA_TRY(cudaMemcpy(m.data(), t.cmask, 4 * nc, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < nc; ++i) mask[i] = (uint8_t)m[i];
+    }
+    return HOT_OK;
+}
+int hot_export_groups(int32_t* cell, uint64_t* lpc, uint64_t* lpp, int64_t cap, int64_t* ngroups) {
+    if (!g.built) return fail(HOT_EORDER, "hot_export_groups: no build");
+    const Tree& t = g.t;
+    if (ngroups) *ngroups = t.ngroups;
+    if (cap < t.ngroups) return fail(HOT_EINVAL, "hot_export_groups: cap too small");
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    size_t ng = (size_t)t.ngroups;
+    if (cell) {
+        std::vector<GroupRec> r(ng);
+        CUDA_TRY(cudaMemcpy(r.data(), t.group, sizeof(GroupRec) * ng, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < ng; ++i) cell[i] = (int32_t)r[i].cell;
+    }
+    if (lpc) CUDA_TRY(cudaMemcpy(lpc, t.glpc, 8 * ng, cudaMemcpyDeviceToHost));
+    if (lpp) CUDA_TRY(cudaMemcpy(lpp, t.glpp, 8 * ng, cudaMemcpyDeviceToHost));
+    return HOT_OK;
+}
+int hot_export_moments(double* com, float* m0, float* m2, float* m3, float* m4, int64_t cap) {
+    if (!g.built || g.t.mom_order < 0) return fail(HOT_EORDER, "hot_export_moments: no hot_forces yet");
+    const Tree& t = g.t;
+    if (cap < t.ncells) return fail(HOT_EINVAL, "hot_export_moments: cap too small");
+    if ((m2 && t.mom_order < 2) || ((m3 || m4) && t.mom_order < 4)) return fail(HOT_EINVAL, "hot_export_moments: order not computed");
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    size_t nc = (size_t)t.ncells;
+    if (com || m0) {
+        std::vector<CellA> a(nc);
+        CUDA_TRY(cudaMemcpy(a.data(), t.cellA, sizeof(CellA) * nc, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < nc; ++i) {
+            if (com) { com[3 * i] = a[i].zx; com[3 * i + 1] = a[i].zy; com[3 * i + 2] = a[i].zz; }
+            if (m0) m0[i] = a[i].m0;
+        }
+    }
+    if (m2) {
+        std::vector<CellM2> a(nc);
+        CUDA_TRY(cudaMemcpy(a.data(), t.cellM2, sizeof(CellM2) * nc, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < nc; ++i) {
+            float* o = m2 + 6 * i;
+            o[0] = a[i].xx; o[1] = a[i].xy; o[2] = a[i].xz; o[3] = a[i].yy; o[4] = a[i].yz; o[5] = a[i].zz;
+        }
+    }
+    if (m3 || m4) {
+        std::vector<CellM34> a(nc);
+        CUDA_TRY(cudaMemcpy(a.data(), t.cellM34, sizeof(CellM34) * nc, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < nc; ++i) {
+            if (m3) memcpy(m3 + 10 * i, a[i].v, 10 * sizeof(float));
+            if (m4) memcpy(m4 + 15 * i, a[i].v + 10, 15 * sizeof(float));
+        }
+    }
+    return HOT_OK;
+}
+int hot_lookup_keys(const uint64_t* keys, int64_t nkeys, int32_t* idx) {
+    if (!g.built) return fail(HOT_EORDER, "hot_lookup_keys: no build");
+    if (nkeys < 0 || (nkeys > 0 && (!keys || !idx))) return fail(HOT_EINVAL, "hot_lookup_keys: bad arguments");
+    if (nkeys == 0) return HOT_OK;
+    uint64_t* dk = nullptr; int32_t* di = nullptr;
+    CUDA_TRY(cudaMalloc(&dk, 8 * (size_t)nkeys));
+    cudaError_t e = cudaMalloc(&di, 4 * (size_t)nkeys);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(dk, keys, 8 * (size_t)nkeys, cudaMemcpyHostToDevice, g.stream);
+    if (e == cudaSuccess) e = launch_hash_lookup(g.t.hkey, g.t.hval, g.t.hcap - 1, dk, nkeys, di, g.stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(idx, di, 4 * (size_t)nkeys, cudaMemcpyDeviceToHost, g.stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(g.stream);
+    cudaFree(dk); cudaFree(di);
+    CUDA_TRY(e);
+    return HOT_OK;
+}
+
+} // extern "C"

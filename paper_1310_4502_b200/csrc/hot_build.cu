@@ -1,0 +1,479 @@
+// hot_build.cu -- S1 keygen, S2 radix sort, S3 gather, S4 tree + hash, S5 sink groups.
+// All stages are HBM-bound streaming kernels; see DESIGN.md "Kernels" for bytes per particle.
+#include "hot_internal.h"
+
+#define FULL 0xffffffffu
+
+// ------------------------------------------------------------------------------------------
+// S1 keys.  PAPER.md:150 defers the coordinate -> key mapping to WS93; reading (R-1):
+// t = fl32(fl32(x - lo) * fl32(1/size)), i = floor(t * 2^21), 63-bit Morton interleave with x the
+// most significant bit of each triple, placeholder bit 63.  The subtract and the multiply are
+// separate IEEE fp32 operations (no FMA contraction): they define the key.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t spread21(uint32_t v) {
+    uint64_t x = v & 0x1fffffu;
+    x = (x | x << 32) & 0x001f00000000ffffull;
+    x = (x | x << 16) & 0x001f0000ff0000ffull;
+    x = (x | x << 8) & 0x100f00f00f00f00full;
+    x = (x | x << 4) & 0x10c30c30c30c30c3ull;
+    x = (x | x << 2) & 0x1249249249249249ull;
+    return x;
+}
+__device__ __forceinline__ uint32_t compact21(uint64_t x) {
+    x &= 0x1249249249249249ull;
+    x = (x | x >> 2) & 0x10c30c30c30c30c3ull;
+    x = (x | x >> 4) & 0x100f00f00f00f00full;
+    x = (x | x >> 8) & 0x001f0000ff0000ffull;
+    x = (x | x >> 16) & 0x001f00000000ffffull;
+    x = (x | x >> 32) & 0x1fffffull;
+    return (uint32_t)x;
+}
+__device__ __forceinline__ uint32_t grid_coord(float x, float lo, float inv, bool& bad) {
+    float t = __fmul_rn(__fsub_rn(x, lo), inv);
+    if (!(t >= 0.0f) || !(t < 1.0f)) bad = true;
+    int i = (int)floorf(__fmul_rn(t, 2097152.0f));
+    i = max(0, min(2097151, i));
+    return (uint32_t)i;
+}
+__device__ __forceinline__ uint64_t body_key(float x, float y, float z, float lox, float loy, float loz,
+                                             float inv, bool& bad) {
+    uint32_t ix = grid_coord(x, lox, inv, bad), iy = grid_coord(y, loy, inv, bad), iz = grid_coord(z, loz, inv, bad);
+    return (1ull << 63) | (spread21(ix) << 2) | (spread21(iy) << 1) | spread21(iz);
+}
+// 4 bodies per thread: three 128-bit loads, two 128-bit key stores, one 128-bit index store
+__global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ pos, int64_t n, float lox, float loy,
+                                                     float loz, float inv, uint64_t* __restrict__ key,
+                                                     uint32_t* __restrict__ idx, int* __restrict__ errflag, int vec) {
+    int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; // quad index
+    int64_t i0 = q * 4;
+    if (i0 >= n) return;
+    bool bad = false;
+    if (vec && i0 + 4 <= n) {
+        const float4* p4 = reinterpret_cast<const float4*>(pos) + q * 3;
+        float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
+        uint64_t k0 = body_key(a.x, a.y, a.z, lox, loy, loz, inv, bad);
+        uint64_t k1 = body_key(a.w, b.x, b.y, lox, loy, loz, inv, bad);
+        uint64_t k2 = body_key(b.z, b.w, c.x, lox, loy, loz, inv, bad);
+        uint64_t k3 = body_key(c.y, c.z, c.w, lox, loy, loz, inv, bad);
+        ulonglong2* ko = reinterpret_cast<ulonglong2*>(key + i0);
+        ko[0] = make_ulonglong2(k0, k1);
+        ko[1] = make_ulonglong2(k2, k3);
+        *reinterpret_cast<uint4*>(idx + i0) = make_uint4((uint32_t)i0, (uint32_t)i0 + 1, (uint32_t)i0 + 2, (uint32_t)i0 + 3);
+    } else {
+        for (int64_t i = i0; i < n && i < i0 + 4; ++i) {
+            key[i] = body_key(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], lox, loy, loz, inv, bad);
+            idx[i] = (uint32_t)i;
+        }
+    }
+    if (bad) atomicOr(errflag, 1);
+}
+cudaError_t launch_keygen(const float* pos, int64_t n, float lox, float loy, float loz, float inv,
+                          uint64_t* key, uint32_t* idx, int* errflag, cudaStream_t st) {
+    int64_t quads = (n + 3) / 4;
+    int vec = (reinterpret_cast<uintptr_t>(pos) & 15u) == 0; // 128-bit loads need a 16-byte aligned base
+    keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, n, lox, loy, loz, inv, key, idx, errflag, vec);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// S2 LSD radix sort of (key, idx), 8-bit digits, 8 passes (PAPER.md:150 names an American-flag
+// radix sort for the on-node sort; a stable LSD sort gives the unique stable permutation).
+// Per pass: tile histogram -> row scan -> stable scatter.  Tile = 256 threads x 16 keys, keys
+// held warp-striped so the in-tile order is (warp, round, lane).
+// ------------------------------------------------------------------------------------------
+#define SORT_THREADS 256
+#define SORT_ITEMS 16
+#define SORT_TILE (SORT_THREADS * SORT_ITEMS)
+#define SORT_WARPS (SORT_THREADS / 32)
+
+static inline int64_t sort_blocks(int64_t n) { return (n + SORT_TILE - 1) / SORT_TILE; }
+size_t sort_hist_elems(int64_t n) { return (size_t)256 * (size_t)sort_blocks(n) + 256; }
+
+__global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(const uint64_t* __restrict__ key, int64_t n, int shift,
+                                                                 uint32_t* __restrict__ hist, int64_t nblk) {
+    __shared__ uint32_t h[256];
+    h[threadIdx.x] = 0;
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * SORT_TILE;
+    int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        int64_t i = base + w * (32 * SORT_ITEMS) + k * 32 + lane;
+        if (i < n) atomicAdd(&h[(uint32_t)(key[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = h[threadIdx.x];
+}
+// in-place exclusive scan of each row (one block per row); totals[row] = row sum
+__global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ data, int64_t rowlen, uint32_t* __restrict__ totals) {
+    __shared__ uint32_t wsum[32];
+    __shared__ uint32_t carry, ctot;
+    uint32_t* row = data + (int64_t)blockIdx.x * rowlen;
+    int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    if (threadIdx.x == 0) carry = 0;
+    __syncthreads();
+    for (int64_t base = 0; base < rowlen; base += 1024) {
+        int64_t i = base + threadIdx.x;
+        uint32_t v = i < rowlen ? row[i] : 0, x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wsum[w] = x;
+        __syncthreads();
+        if (w == 0) {
+            uint32_t s = wsum[lane], t = s;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, t, o); if (lane >= o) t += y; }
+            wsum[lane] = t - s; // exclusive warp offsets
+            if (lane == 31) ctot = t;
+        }
+        __syncthreads();
+        uint32_t c = carry;
+        if (i < rowlen) row[i] = c + wsum[w] + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) carry = c + ctot;
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) totals[blockIdx.x] = carry;
+}
+__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+                                                                    uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, int64_t n,
+                                                                    int shift, const uint32_t* __restrict__ hist,
+                                                                    const uint32_t* __restrict__ totals, int64_t nblk) {
+    __shared__ uint32_t wcount[SORT_WARPS][256];
+    __shared__ uint32_t gbase[256];
+    __shared__ uint32_t wtot[SORT_WARPS];
+    int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    // digit base = exclusive scan of the 256 row totals + this tile's offset inside the row
+    {
+        uint32_t v = totals[tid], x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wtot[w] = x;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int j = 0; j < w; ++j) off += wtot[j];
+        gbase[tid] = off + x - v + hist[(int64_t)tid * nblk + blockIdx.x];
+    }
+#pragma unroll
+    for (int j = 0; j < SORT_WARPS; ++j) wcount[j][tid] = 0;
+    __syncthreads();
+    int64_t base = (int64_t)blockIdx.x * SORT_TILE + w * (32 * SORT_ITEMS);
+    uint64_t kk[SORT_ITEMS];
+    uint32_t rk[SORT_ITEMS]; // digit | rank << 8
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        int64_t i = base + k * 32 + lane;
+        bool valid = i < n;
+        kk[k] = valid ? kin[i] : ~0ull;
+        uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
+        uint32_t m = __match_any_sync(FULL, valid ? d : 256u);
+        uint32_t r = __popc(m & ((1u << lane) - 1u));
+        uint32_t old = valid ? wcount[w][d] : 0;
+        __syncwarp();
+        if (valid && r == 0) wcount[w][d] = old + __popc(m);
+        __syncwarp();
+        rk[k] = d | ((old + r) << 8);
+    }
+    __syncthreads();
+    { // exclusive prefix over the warps of the tile, per digit
+        uint32_t run = 0;
+#pragma unroll
+        for (int j = 0; j < SORT_WARPS; ++j) { uint32_t t = wcount[j][tid]; wcount[j][tid] = run; run += t; }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        int64_t i = base + k * 32 + lane;
+        if (i < n) {
+            uint32_t d = rk[k] & 255u;
+            uint32_t p = gbase[d] + wcount[w][d] + (rk[k] >> 8);
+            kout[p] = kk[k];
+            vout[p] = vin[i];
+        }
+    }
+}
+cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st) {
+    int64_t nblk = sort_blocks(n);
+    uint32_t* totals = hist + (size_t)256 * nblk;
+    int cur = 0;
+    for (int pass = 0; pass < 8; ++pass) {
+        int shift = pass * 8;
+        sort_hist_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], n, shift, hist, nblk);
+        scan_rows_kernel<<<256, 1024, 0, st>>>(hist, nblk, totals);
+        sort_scatter_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], idx[cur], key[cur ^ 1], idx[cur ^ 1], n, shift,
+                                                                     hist, totals, nblk);
+        cur ^= 1;
+    }
+    // 8 passes: the result is back in buffer 0
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// S3 gather into key order as float4 (x,y,z,m): the "structure" the interaction kernels stage.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) gather_kernel(const float* __restrict__ pos, const float* __restrict__ mass,
+                                                     const uint32_t* __restrict__ perm, int64_t n, float4* __restrict__ body) {
+    int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    uint32_t j = perm[i];
+    body[i] = make_float4(__ldg(pos + 3 * (int64_t)j), __ldg(pos + 3 * (int64_t)j + 1), __ldg(pos + 3 * (int64_t)j + 2), __ldg(mass + j));
+}
+cudaError_t launch_gather(const float* pos, const float* mass, const uint32_t* perm, int64_t n, float4* body, cudaStream_t st) {
+    gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, mass, perm, n, body);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------
+// S4/S5 tree from the sorted keys in one sweep.
+// For sorted position i:
+//   b_i      = level at which key[i-1] and key[i] first differ (0 for i = 0, 22 if equal)
+//   Lleaf_i  = level of the leaf holding i   = min(21, 1 + max_{j in [i-NLEAF,i]} cpl(key[j], key[j+NLEAF]))
+//   Lgroup_i = level of the sink group of i  = same with NCRIT
+// (cpl = number of common leading 3-bit digits; a level-L cell holds more than W bodies iff some
+//  window of W+1 consecutive sorted keys containing i shares its first L digits.)
+// A cell (l, i) -- level l, first body i -- exists iff b_i <= l <= Lleaf_i; in level-major order its
+// index is level_base[l] + #{i' < i : b_i' <= l <= Lleaf_i'} (ascending numeric key order, C-4).
+// ------------------------------------------------------------------------------------------
+#define TREE_TILE 1024
+#define TREE_ROWS (HOT_NLEVELS + 2) // 22 level rows, row 22 = groups, row 23 = leaves
+int64_t tree_num_blocks(int64_t n) { return (n + TREE_TILE - 1) / TREE_TILE; }
+
+__device__ __forceinline__ int first_diff_level(uint64_t a, uint64_t b) { // 1..21, 22 if equal
+    uint64_t x = a ^ b;
+    if (x == 0) return 22;
+    int p = 63 - __clzll((long long)x);
+    return 21 - p / 3;
+}
+
+__global__ void __launch_bounds__(TREE_TILE) tree_levels_kernel(const uint64_t* __restrict__ skey, int64_t n, int nleaf, int ncrit,
+                                                                uint32_t* __restrict__ plev, uint32_t* __restrict__ counts, int64_t nblk) {
+    __shared__ uint64_t sk[TREE_TILE + 2 * HOT_MAX_NCRIT];
+    __shared__ signed char wa[TREE_TILE + HOT_MAX_NCRIT + 32], wb[TREE_TILE + HOT_MAX_NCRIT + 32];
+    __shared__ uint32_t cnt[TREE_ROWS];
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int64_t T0 = (int64_t)blockIdx.x * TREE_TILE;
+    const int H = ncrit; // halo on both sides
+    for (int p = tid; p < TREE_TILE + 2 * H; p += TREE_TILE) {
+        int64_t g = T0 - H + p;
+        sk[p] = (g >= 0 && g < n) ? skey[g] : 0ull;
+    }
+    if (tid < TREE_ROWS) cnt[tid] = 0;
+    __syncthreads();
+    const int64_t i = T0 + tid;
+    const bool valid = i < n;
+    int lev[2];
+#pragma unroll
+    for (int which = 0; which < 2; ++which) {
+        const int W = which ? ncrit : nleaf;
+        // w_p = cpl(key[p], key[p+W]) for global p in [T0-W, T0+TILE), -1 outside the array
+        const int L = TREE_TILE + W;
+        for (int q = tid; q < L + 32; q += TREE_TILE) {
+            int64_t g = T0 - W + q;
+            signed char v = -1;
+            if (q < L && g >= 0 && g + W < n) v = (signed char)(first_diff_level(sk[q + H - W], sk[q + H]) - 1);
+            wa[q] = v;
+        }
+        __syncthreads();
+        // sliding max over [i-W, i] (length W+1) by doubling: M_k[q] = max w[q .. q+2^k-1]
+        int K = 31 - __clz(W + 1);
+        signed char *src = wa, *dst = wb;
+        for (int k = 0; k < K; ++k) {
+            for (int q = tid; q < L; q += TREE_TILE) {
+                int q2 = q + (1 << k);
+                signed char a = src[q], b = q2 < L ? src[q2] : (signed char)-1;
+                dst[q] = a > b ? a : b;
+            }
+            __syncthreads();
+            signed char* t = src; src = dst; dst = t;
+        }
+        // position i-W is q = tid, position i is q = tid+W
+        signed char a = src[tid], b = src[tid + W - (1 << K) + 1];
+        int D = a > b ? a : b;
+        lev[which] = min(HOT_MAXLEVEL, D + 1);
+        __syncthreads();
+    }
+    int b = 0;
+    if (valid && i > 0) b = first_diff_level(sk[tid + H - 1], sk[tid + H]);
+    const int Lleaf = lev[0], Lgroup = lev[1];
+    if (valid) plev[i] = (uint32_t)b | ((uint32_t)Lleaf << 8) | ((uint32_t)Lgroup << 16);
+#pragma unroll 1
+    for (int l = 0; l < HOT_NLEVELS; ++l) {
+        uint32_t m = __ballot_sync(FULL, valid && b <= l && l <= Lleaf);
+        if (lane == 0 && m) atomicAdd(&cnt[l], (uint32_t)__popc(m));
+    }
+    {
+        uint32_t m = __ballot_sync(FULL, valid && b <= Lgroup);
+        if (lane == 0 && m) atomicAdd(&cnt[HOT_NLEVELS], (uint32_t)__popc(m));
+        m = __ballot_sync(FULL, valid && b <= Lleaf);
+        if (lane == 0 && m) atomicAdd(&cnt[HOT_NLEVELS + 1], (uint32_t)__popc(m));
+    }
+    __syncthreads();
+    if (tid < TREE_ROWS) counts[(int64_t)tid * nblk + blockIdx.x] = cnt[tid];
+}
+cudaError_t launch_tree_levels(const uint64_t* skey, int64_t n, int nleaf, int ncrit, uint32_t* plev, uint32_t* counts, cudaStream_t st) {
+    int64_t nblk = tree_num_blocks(n);
+    tree_levels_kernel<<<(unsigned)nblk, TREE_TILE, 0, st>>>(skey, n, nleaf, ncrit, plev, counts, nblk);
+    return cudaGetLastError();
+}
+cudaError_t launch_tree_scan(uint32_t* counts, int64_t nblk, uint32_t* totals, cudaStream_t st) {
+    scan_rows_kernel<<<TREE_ROWS, 1024, 0, st>>>(counts, nblk, totals);
+    return cudaGetLastError();
+}
+
+__device__ __forceinline__ uint64_t hash64(uint64_t k) {
+    k ^= k >> 33; k *= 0xff51afd7ed558ccdull; k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ull; k ^= k >> 33;
+    return k;
+}
+struct LevelBase { int64_t v[HOT_NLEVELS + 1]; };
+
+__global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __restrict__ skey, const uint32_t* __restrict__ plev,
+                                                              const uint32_t* __restrict__ counts, int64_t n, int64_t nblk, LevelBase LB,
+                                                              uint64_t* __restrict__ ckey, uint32_t* __restrict__ cfirst,
+                                                              uint32_t* __restrict__ ccount, int32_t* __restrict__ cchild,
+                                                              int32_t* __restrict__ cparent, GroupRec* __restrict__ group,
+                                                              uint64_t* __restrict__ hkey, int32_t* __restrict__ hval, int64_t hmask,
+                                                              int* __restrict__ maxprobe) {
+    __shared__ uint32_t wpre[HOT_NLEVELS + 1][32]; // per row, per warp: exclusive prefix inside the tile
+    __shared__ uint32_t boff[HOT_NLEVELS + 1];
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    const int64_t i = (int64_t)blockIdx.x * TREE_TILE + tid;
+    const bool valid = i < n;
+    uint32_t pl = valid ? plev[i] : 0xffffffu;
+    const int b = valid ? (int)(pl & 255u) : 99, Lleaf = valid ? (int)((pl >> 8) & 255u) : -1, Lgroup = valid ? (int)((pl >> 16) & 255u) : -1;
+    const uint32_t lt = (1u << lane) - 1u;
+#pragma unroll 1
+    for (int l = 0; l < HOT_NLEVELS; ++l) {
+        uint32_t m = __ballot_sync(FULL, b <= l && l <= Lleaf);
+        if (lane == 0) wpre[l][w] = __popc(m);
+    }
+    {
+        uint32_t m = __ballot_sync(FULL, valid && b <= Lgroup);
+        if (lane == 0) wpre[HOT_NLEVELS][w] = __popc(m);
+    }
+    if (tid <= HOT_NLEVELS) boff[tid] = counts[(int64_t)tid * nblk + blockIdx.x];
+    __syncthreads();
+    if (tid <= HOT_NLEVELS) {
+        uint32_t run = 0;
+        for (int j = 0; j < 32; ++j) { uint32_t t = wpre[tid][j]; wpre[tid][j] = run; run += t; }
+    }
+    __syncthreads();
+    const uint64_t mykey = valid ? skey[i] : 0;
+    int64_t prev_incl = 0;   // inclusive count at level l-1 (global rank inside the level)
+    int32_t prev_cell = -1;  // index of cell (l-1, i) if it exists
+    uint32_t gcount = 0; int32_t gcell = -1;
+#pragma unroll 1
+    for (int l = 0; l < HOT_NLEVELS; ++l) {
+        const bool exists = b <= l && l <= Lleaf;
+        uint32_t m = __ballot_sync(FULL, exists);
+        int64_t excl = (int64_t)boff[l] + wpre[l][w] + __popc(m & lt);
+        int64_t incl = excl + (exists ? 1 : 0);
+        if (exists) {
+            int32_t c = (int32_t)(LB.v[l] + excl);
+            const int sh = 63 - 3 * l;
+            uint64_t ck = mykey >> sh;
+            // end of the cell: first j > i whose key leaves the prefix (gallop + bisection)
+            int64_t lo = i, hi;
+            if (l == 0) hi = n;
+            else {
+                int64_t step = 1, p = i + 1;
+                while (p < n && (skey[p] >> sh) == ck) { lo = p; step <<= 1; p = i + step; }
+                hi = p < n ? p : n;
+                while (hi - lo > 1) {
+                    int64_t mid = (lo + hi) >> 1;
+                    if ((skey[mid] >> sh) == ck) lo = mid; else hi = mid;
+                }
+            }
+            uint32_t cnt = (uint32_t)(hi - i);
+            ckey[c] = ck; cfirst[c] = (uint32_t)i; ccount[c] = cnt;
+            cparent[c] = l == 0 ? -1 : (int32_t)(LB.v[l - 1] + prev_incl - 1);
+            if (l == Lleaf) cchild[c] = -1;
+            if (prev_cell >= 0) cchild[prev_cell] = c; // cell (l-1, i) is internal: its first child starts at i too
+            prev_cell = c;
+            if (l == Lgroup) { gcount = cnt; gcell = c; }
+            // hash insert (open addressing, linear probing)
+            uint64_t h = hash64(ck) & (uint64_t)hmask;
+            int probe = 0;
+            while (true) {
+                unsigned long long old = atomicCAS((unsigned long long*)&hkey[h], 0ull, (unsigned long long)ck);
+                if (old == 0ull) { hval[h] = c; break; }
+                h = (h + 1) & (uint64_t)hmask; ++probe;
+            }
+            if (probe > 0 && probe > *((volatile int*)maxprobe)) atomicMax(maxprobe, probe);
+        } else prev_cell = -1;
+        prev_incl = incl;
+    }
+    {
+        bool isg = valid && b <= Lgroup;
+        uint32_t m = __ballot_sync(FULL, isg);
+        if (isg) {
+            int64_t r = (int64_t)boff[HOT_NLEVELS] + wpre[HOT_NLEVELS][w] + __popc(m & lt);
+            GroupRec g; g.first = (uint32_t)i; g.count = gcount; g.cell = (uint32_t)gcell; g.pad = 0;
+            group[r] = g;
+        }
+    }
+}
+cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
+    LevelBase LB;
+    for (int l = 0; l <= HOT_NLEVELS; ++l) LB.v[l] = a.level_base[l];
+    tree_emit_kernel<<<(unsigned)a.nblk, TREE_TILE, 0, st>>>(a.skey, a.plev, a.counts, a.n, a.nblk, LB, a.ckey, a.cfirst, a.ccount,
+                                                             a.cchild, a.cparent, a.group, a.hkey, a.hval, a.hmask, a.maxprobe);
+    return cudaGetLastError();
+}
+__global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restrict__ ckey, const int32_t* __restrict__ cparent,
+                                                        uint32_t* __restrict__ cmask, int64_t ncells) {
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
+    if (c >= ncells) return;
+    atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ckey[c] & 7ull));
+}
+cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, cudaStream_t st) {
+    if (ncells > 1) tree_link_kernel<<<(unsigned)((ncells - 1 + 255) / 256), 256, 0, st>>>(ckey, cparent, cmask, ncells);
+    return cudaGetLastError();
+}
+__global__ void __launch_bounds__(256) tree_finalize_kernel(const uint64_t* __restrict__ ckey, const uint32_t* __restrict__ cfirst,
+                                                            const uint32_t* __restrict__ ccount, const uint32_t* __restrict__ cmask,
+                                                            const int32_t* __restrict__ cchild, WalkCell* __restrict__ wc,
+                                                            int64_t ncells, int* __restrict__ errflag) {
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncells) return;
+    uint64_t k = ckey[c];
+    int level = (63 - __clzll((long long)k)) / 3;
+    uint64_t mort = k & ((1ull << (3 * level)) - 1ull);
+    int up = HOT_MAXLEVEL - level;
+    uint64_t ox = (uint64_t)compact21(mort >> 2) << up, oy = (uint64_t)compact21(mort >> 1) << up, oz = (uint64_t)compact21(mort) << up;
+    bool leaf = cchild[c] < 0;
+    uint32_t cnt = leaf ? ccount[c] : (uint32_t)__popc(cmask[c]);
+    if (cnt >= (1u << 27)) { atomicOr(errflag, 2); cnt = (1u << 27) - 1; }
+    uint64_t packed = ox | (oy << 21) | (oz << 42) | (leaf ? (1ull << 63) : 0ull);
+    WalkCell r;
+    r.x = (uint32_t)packed; r.y = (uint32_t)(packed >> 32);
+    r.z = leaf ? cfirst[c] : (uint32_t)cchild[c];
+    r.w = ((uint32_t)level << 27) | cnt;
+    wc[c] = r;
+}
+cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount, const uint32_t* cmask,
+                                 const int32_t* cchild, WalkCell* wc, int64_t ncells, int* errflag, cudaStream_t st) {
+    tree_finalize_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, st>>>(ckey, cfirst, ccount, cmask, cchild, wc, ncells, errflag);
+    return cudaGetLastError();
+}
+__global__ void hash_lookup_kernel(const uint64_t* __restrict__ hkey, const int32_t* __restrict__ hval, int64_t hmask,
+                                   const uint64_t* __restrict__ keys, int64_t nkeys, int32_t* __restrict__ out) {
+    int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (q >= nkeys) return;
+    uint64_t k = keys[q];
+    int32_t r = -1;
+    if (k != 0) {
+        uint64_t h = hash64(k) & (uint64_t)hmask;
+        while (true) {
+            uint64_t s = hkey[h];
+            if (s == k) { r = hval[h]; break; }
+            if (s == 0) break;
+            h = (h + 1) & (uint64_t)hmask;
+        }
+    }
+    out[q] = r;
+}
+cudaError_t launch_hash_lookup(const uint64_t* hkey, const int32_t* hval, int64_t hmask, const uint64_t* keys, int64_t nkeys,
+                               int32_t* out, cudaStream_t st) {
+    if (nkeys > 0) hash_lookup_kernel<<<(unsigned)((nkeys + 255) / 256), 256, 0, st>>>(hkey, hval, hmask, keys, nkeys, out);
+    return cudaGetLastError();
+}

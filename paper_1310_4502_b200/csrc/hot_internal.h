@@ -1,0 +1,111 @@
+// Internal declarations shared by the translation units of libhot (CUDA, sm_100a).
+// Not part of the public boundary (include/hot.h) and never seen by the oracle.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "hot.h"
+
+#define HOT_MAXLEVEL 21
+#define HOT_NLEVELS 22        // levels 0..21
+#define HOT_MAX_NCRIT 256
+#define HOT_MAX_NLEAF 32
+
+// 16-byte record the walk reads per visited cell (S7).
+//   x: ox | oy<<21 (low 11 bits of oy)          packed 63-bit integer corner on the 2^21 grid
+//   y: oy>>11 | oz<<10 | leaf<<31
+//   z: first child (internal) or first body (leaf)
+//   w: level<<27 | count  (count = number of children, or of bodies for a leaf; < 2^27)
+struct __align__(16) WalkCell { uint32_t x, y, z, w; };
+
+// per-cell expansion data (S6), gathered when a cell is accepted
+struct __align__(16) CellA { double zx, zy, zz; float m0; float t2; };   // centre of mass, mass, trace M2
+struct __align__(16) CellM2 { float xx, xy, xz, yy, yz, zz, pad0, pad1; };
+// order 4: M3 (10) + M4 (15) + traces t3 (3), T4 (6), t4 (1) = 35 floats -> 36
+struct __align__(16) CellM34 { float v[36]; };
+
+struct GroupRec { uint32_t first, count, cell, pad; };
+
+struct Tree {
+    int64_t n = 0;
+    int periodic = 0, nleaf = 16, ncrit = 64;
+    hot_box box{};
+    double lo[3], size;
+    // bodies
+    uint64_t* key[2] = {nullptr, nullptr};   // ping-pong, key[0] holds the sorted keys after build
+    uint32_t* idx[2] = {nullptr, nullptr};   // idx[0] = perm
+    float4* body = nullptr;                  // key-ordered (x,y,z,m)
+    uint32_t* plev = nullptr;                // per body: b | Lleaf<<8 | Lgroup<<16
+    // cells
+    int64_t ncells = 0, nleaves = 0, ngroups = 0;
+    int max_level = 0;
+    int64_t level_base[HOT_NLEVELS + 1];
+    uint64_t* ckey = nullptr;
+    uint32_t *cfirst = nullptr, *ccount = nullptr, *cmask = nullptr;
+    int32_t *cchild = nullptr, *cparent = nullptr;
+    WalkCell* wcell = nullptr;
+    GroupRec* group = nullptr;
+    uint64_t *glpc = nullptr, *glpp = nullptr;
+    // hash
+    int64_t hcap = 0;
+    uint64_t* hkey = nullptr;
+    int32_t* hval = nullptr;
+    int hash_max_probe = 0;
+    // moments
+    int mom_order = -1;
+    CellA* cellA = nullptr;
+    CellM2* cellM2 = nullptr;
+    CellM34* cellM34 = nullptr;
+};
+
+// ---- build stages (hot_build.cu) ------------------------------------------------------------
+// every launcher returns the cudaError_t of its last launch; all work goes to `st`
+cudaError_t launch_keygen(const float* pos, int64_t n, float lox, float loy, float loz, float inv,
+                          uint64_t* key, uint32_t* idx, int* errflag, cudaStream_t st);
+// sorts (key,idx) pairs stably, ascending; result ends in key[0]/idx[0]; scratch: hist of sort_hist_elems(n) u32
+size_t sort_hist_elems(int64_t n);
+cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st);
+cudaError_t launch_gather(const float* pos, const float* mass, const uint32_t* perm, int64_t n,
+                          float4* body, cudaStream_t st);
+// tree pass 1: per-body levels + per-block per-level counts.  counts: [HOT_NLEVELS+1][nblk] u32
+int64_t tree_num_blocks(int64_t n);
+cudaError_t launch_tree_levels(const uint64_t* skey, int64_t n, int nleaf, int ncrit, uint32_t* plev,
+                               uint32_t* counts, cudaStream_t st);
+// exclusive scan of each row of counts over blocks; totals[row]
+cudaError_t launch_tree_scan(uint32_t* counts, int64_t nblk, uint32_t* totals, cudaStream_t st);
+struct TreeEmitArgs {
+    const uint64_t* skey; const uint32_t* plev; const uint32_t* counts; int64_t n, nblk;
+    int64_t level_base[HOT_NLEVELS + 1];
+    uint64_t* ckey; uint32_t* cfirst; uint32_t* ccount; int32_t* cchild; int32_t* cparent;
+    GroupRec* group; uint64_t* hkey; int32_t* hval; int64_t hmask; int* maxprobe;
+};
+cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st);
+cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, cudaStream_t st);
+cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount,
+                                 const uint32_t* cmask, const int32_t* cchild, WalkCell* wc,
+                                 int64_t ncells, int* errflag, cudaStream_t st);
+cudaError_t launch_hash_lookup(const uint64_t* hkey, const int32_t* hval, int64_t hmask,
+                               const uint64_t* keys, int64_t nkeys, int32_t* out, cudaStream_t st);
+
+// ---- upward pass (hot_moments.cu) -------------------------------------------------------------
+cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st);
+
+// ---- walk + interactions (hot_forces.cu) ------------------------------------------------------
+struct ForceArgs {
+    const WalkCell* wcell; const CellA* cellA; const CellM2* cellM2; const CellM34* cellM34;
+    const float4* body; const uint32_t* perm; const GroupRec* group; int64_t ngroups;
+    double theta2; float eps2; int order; int periodic;
+    int scap;                     // ceil(ncrit/32): sinks per lane the kernel must hold
+    double lo[3], size;
+    float* acc; float* pot;
+    uint64_t* glpc; uint64_t* glpp;
+    unsigned int* counter;        // dynamic group scheduler
+    unsigned long long* stat;     // [0] cells visited, [1] spills, [2] sum n*Lpp, [3] sum n*Lpc
+    uint32_t* gstack; int64_t gstack_cap; // per-warp spill arena (entries per warp)
+    int* errflag;
+};
+int force_grid_warps(int order, int periodic, int scap); // resident warps the kernel is launched with
+cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st);
+
+// ---- periodic far field (hot_periodic.cu) -----------------------------------------------------
+cudaError_t launch_farfield(const Tree& t, double* scratch, float* acc, float* pot, cudaStream_t st);
