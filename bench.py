@@ -1,0 +1,327 @@
+#!/usr/bin/env python
+"""bench.py -- the measurement contract of this repo.
+
+A *step* is one pass of the whole hot path over one batch of synthetic particles:
+hot_build (keys, sort, gather, tree, groups) + hot_forces (moments, walk, P-P / P-C kernels, scatter).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+                    [--config 0..4] [--scale S] [--theta T] [--order P] [--nleaf L] [--ncrit C]
+
+Default workload: BASELINE.json configs[2] (the N = 2^24 clustered mix the metric is quoted on),
+theta = 0.6, quadrupole order.  Prints ONE JSON line (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+# flops per interaction counted from the library's own inner loops:
+# FFMA = 2, FADD/FMUL = 1, rsqrt = 1.
+FLOPS_PP = 20
+FLOPS_PC = {0: 20, 2: 62, 4: 275}
+# FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
+# 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
+FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
+SORT_BYTES_PER_BODY = 8 * 32          # 8 passes x (8 B histogram read + 12 B read + 12 B write)
+KEYGEN_BYTES_PER_BODY = 24
+GATHER_BYTES_PER_BODY = 36
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2)
+    ap.add_argument("--scale", type=int, default=None)
+    ap.add_argument("--theta", type=float, default=None)
+    ap.add_argument("--order", type=int, default=None)
+    ap.add_argument("--nleaf", type=int, default=16)
+    ap.add_argument("--ncrit", type=int, default=64)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def workload(args, rank=0):
+    from paper_1310_4502_b200 import workloads as W
+
+    w = W.config(args.config, args.scale)
+    if rank:  # independent replicas on the other ranks: same recipe, another seed
+        gen = {0: W.uniform_cube, 1: W.plummer_sphere, 2: W.clustered_mix}.get(args.config)
+        if gen is not None:
+            w2 = gen(w.n, W.SEED0 + args.config + 1000 * rank)
+            w2.eps, w2.theta, w2.order = w.eps, w.theta, w.order
+            w = w2
+    if args.theta is not None:
+        w.theta = args.theta
+    elif args.config == 2:
+        w.theta = 0.6
+    if args.order is not None:
+        w.order = args.order
+    return w
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            f = [x.strip() for x in r.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx = float(f[1])
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": mx, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def cpu_oracle_sample(args, w_full, budget_s=12.0):
+    """The oracle as it stands, whole path, on a smaller replica of the same workload."""
+    import numpy as np
+
+    from oracle import oracle as O
+    from paper_1310_4502_b200 import workloads as W
+
+    scale = {0: 14, 1: 16, 2: 16, 3: 32, 4: 32}[args.config]
+    if args.scale is not None:
+        scale = min(scale, args.scale)
+    w = W.config(args.config, scale)
+    t0 = time.perf_counter()
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic, nleaf=args.nleaf, ncrit=args.ncrit)
+    t_build = time.perf_counter() - t0
+    counts = T.cells()["count"][T.groups()]
+    order = np.random.default_rng(0).permutation(T.ngroups)
+    done, inter, t_eval, chunk = 0, 0, 0.0, max(8, O.num_threads() * 4)
+    while done < T.ngroups and t_eval < budget_s:
+        sel = order[done:done + chunk]
+        t1 = time.perf_counter()
+        _, _, lpc, lpp = T.forces(w_full.theta, w.eps, w_full.order, groups=sel)
+        t_eval += time.perf_counter() - t1
+        inter += int((counts[sel] * (lpc + lpp)).sum())
+        done += len(sel)
+    frac = done / T.ngroups
+    t = t_eval + t_build * frac
+    return {"value": inter / t / 1e9, "unit": "Ginteractions/s", "cores": O.num_threads(), "kind": "oracle",
+            "sample": (f"{w.name}: same generator at n={w.n}; oracle keys+sort+tree+moments in full "
+                       f"({t_build:.1f} s, charged pro rata) and walk+evaluation of {done}/{T.ngroups} "
+                       f"random sink groups ({t_eval:.1f} s), theta={w_full.theta}, order={w_full.order}"),
+            "seconds": t, "interactions": inter}
+
+
+def run_reference(args):
+    """--impl reference: the oracle, timed on the host cores, same metric and config."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    w = workload(args)
+    vals = []
+    for _ in range(max(1, args.warmup > 0)):
+        cpu_oracle_sample(args, w, budget_s=2.0)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        vals.append(cpu_oracle_sample(args, w, budget_s=8.0))
+    wall = time.perf_counter() - t0
+    inter = sum(v["interactions"] for v in vals)
+    secs = sum(v["seconds"] for v in vals)
+    value = inter / secs / 1e9
+    base = vals[-1]
+    out = {"impl": "reference", "metric": "interactions_per_second", "value": value, "unit": "Ginteractions/s",
+           "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps,
+           "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": config_dict(args, w), "gpu_launches": 0,
+           "cpu_baseline": {"value": value, "unit": "Ginteractions/s", "cores": base["cores"], "kind": "oracle",
+                            "sample": base["sample"]},
+           "e2e": {"value": value, "unit": "Ginteractions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+
+
+def config_dict(args, w):
+    return {"workload": f"BASELINE.json configs[{args.config}]: {w.name}, n={w.n}, "
+                        f"{'periodic' if w.periodic else 'open'}, eps={w.eps:g}, theta={w.theta:g}, order={w.order}",
+            "n": w.n, "theta": w.theta, "eps": w.eps, "order": w.order, "nleaf": args.nleaf, "ncrit": args.ncrit,
+            "l2": "inputs (pos+mass 16 B/body) and every per-step array exceed the 126 MB L2 at n >= 2^23; "
+                  "each step rebuilds keys, tree and moments from the caller's arrays",
+            "parallelism": "replicas only (one independent problem per GPU, no collective)"}
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        run_reference(args)
+        return
+    import numpy as np
+    import torch
+
+    import paper_1310_4502_b200 as hot
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        dist.init_process_group("nccl")
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product path has no CPU fallback")
+    torch.cuda.set_device(local)
+    w = workload(args, rank)
+    hot.hot_set_params(args.nleaf, args.ncrit)
+    pos = torch.from_numpy(w.pos).cuda()
+    mass = torch.from_numpy(w.mass).cuda()
+    acc = torch.empty((w.n, 3), dtype=torch.float32, device="cuda")
+    pot = torch.empty(w.n, dtype=torch.float32, device="cuda")
+
+    def step():
+        hot.hot_build(pos, mass, w.lo, w.size, w.periodic)
+        hot.hot_forces(w.theta, w.eps, w.order, acc=acc, pot=pot)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+            torch.cuda.synchronize()
+
+    for _ in range(max(3, args.warmup)):
+        step()
+    barrier()
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage = {}
+    e0.record()
+    for _ in range(args.steps):
+        step()
+        st = hot.hot_stats()
+        for k in ("ms_keygen", "ms_sort", "ms_gather", "ms_tree", "ms_moments", "ms_walk_eval", "ms_farfield",
+                  "ms_build_total", "ms_forces_total"):
+            stage[k] = stage.get(k, 0.0) + st[k] / args.steps
+    e1.record()
+    barrier()
+    ms = e0.elapsed_time(e1) / args.steps
+    clocks = sampler.stop() if rank == 0 else None
+    st = hot.hot_stats()
+    inter = st["pp_interactions"] + st["pc_interactions"]
+    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
+    tint = torch.tensor([float(inter)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tint, op=dist.ReduceOp.SUM)
+    ms_max, inter_all = float(tms.item()), float(tint.item())
+
+    # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        hp = torch.from_numpy(w.pos).pin_memory(); hm = torch.from_numpy(w.mass).pin_memory()
+        ha = torch.empty((w.n, 3), dtype=torch.float32).pin_memory(); hq = torch.empty(w.n, dtype=torch.float32).pin_memory()
+        hot.hot_step_host(hp.numpy(), hm.numpy(), w.lo, w.size, w.periodic, w.theta, w.eps, w.order, ha.numpy(), hq.numpy())
+        barrier()
+        t0 = time.perf_counter()
+        nrep = max(1, min(args.steps, 3))
+        for _ in range(nrep):
+            hot.hot_step_host(hp.numpy(), hm.numpy(), w.lo, w.size, w.periodic, w.theta, w.eps, w.order, ha.numpy(), hq.numpy())
+        torch.cuda.synchronize()
+        te = torch.tensor([(time.perf_counter() - t0) / nrep], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(te, op=dist.ReduceOp.MAX)
+        e2e = {"value": inter_all / float(te.item()) / 1e9, "unit": "Ginteractions/s",
+               "ms_per_step": 1e3 * float(te.item()), "h2d_bytes_per_step": 16 * w.n, "d2h_bytes_per_step": 16 * w.n}
+        assert np.isfinite(ha.numpy()).all()
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+    flops = st["pp_interactions"] * FLOPS_PP + st["pc_interactions"] * FLOPS_PC[w.order]
+    kern_s = stage["ms_walk_eval"] * 1e-3
+    achieved = flops / kern_s / 1e12
+    out = {
+        "metric": "interactions_per_second", "value": inter_all / (ms_max * 1e-3) / 1e9, "unit": "Ginteractions/s",
+        "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_max,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": config_dict(args, w),
+        "force_eval_s_per_step": ms_max * 1e-3,
+        "interactions_per_step": {"pp": st["pp_interactions"], "pc": st["pc_interactions"],
+                                  "per_particle": inter / w.n},
+        "kernel_only_Ginteractions_per_s": inter / kern_s / 1e9,
+        "stages_ms": {k: round(v, 4) for k, v in stage.items()},
+        "tree": {"n_cells": st["n_cells"], "n_groups": st["n_groups"], "max_level": st["max_level"],
+                 "cells_visited": st["cells_visited"], "walk_spills": st["walk_spills"]},
+        "hbm_stages": {
+            "keygen_GBps": KEYGEN_BYTES_PER_BODY * w.n / (stage["ms_keygen"] * 1e-3) / 1e9,
+            "sort_GBps": SORT_BYTES_PER_BODY * w.n / (stage["ms_sort"] * 1e-3) / 1e9,
+            "gather_GBps": GATHER_BYTES_PER_BODY * w.n / (stage["ms_gather"] * 1e-3) / 1e9},
+        "gpu_launches": int((st["launches_build"] + st["launches_forces"]) * args.steps),
+        "clocks": clocks,
+        "roofline": {"bound": "alu", "kernel": "forces_kernel (fused walk + P-P + P-C)", "achieved": achieved,
+                     "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS, "traffic": None,
+                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+                     "flops_per_interaction": {"pp": FLOPS_PP, "pc": FLOPS_PC[w.order]},
+                     "kernel_ms": stage["ms_walk_eval"]},
+    }
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+        out["hbm_stages"]["peak_GBps"] = peaks.get("hbm_gbs")
+    except (OSError, ValueError):
+        out["hbm_stages"]["peak_GBps"] = 6650.0
+    if e2e:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline and world == 1:
+        cb = cpu_oracle_sample(args, w)
+        out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+    print(json.dumps(out))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

@@ -69,6 +69,7 @@ typedef struct {
     float ms_keygen, ms_sort, ms_gather, ms_tree, ms_moments, ms_walk_eval, ms_farfield;
     float ms_build_total, ms_forces_total;
     int64_t bytes_allocated;
+    int64_t launches_build, launches_forces; /* kernels launched by the last hot_build / hot_forces */
 } hot_stats_t;
 
 /* Bucket sizes of the tree: a cell with more than nleaf bodies is split (down

@@ -32,7 +32,8 @@ class hot_stats_t(C.Structure):
                 ("cells_visited", C.c_uint64), ("walk_spills", C.c_uint64),
                 ("ms_keygen", C.c_float), ("ms_sort", C.c_float), ("ms_gather", C.c_float), ("ms_tree", C.c_float),
                 ("ms_moments", C.c_float), ("ms_walk_eval", C.c_float), ("ms_farfield", C.c_float),
-                ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float), ("bytes_allocated", C.c_int64)]
+                ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float), ("bytes_allocated", C.c_int64),
+                ("launches_build", C.c_int64), ("launches_forces", C.c_int64)]
 
 
 def library_path() -> str:

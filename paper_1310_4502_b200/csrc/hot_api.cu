@@ -6,6 +6,8 @@
 
 #include "hot_internal.h"
 
+long long g_hot_launches = 0;
+
 namespace {
 
 struct Ctx {
@@ -125,6 +127,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     int rc = ensure_scratch();
     if (rc) return rc;
     drop_build();
+    g_hot_launches = 0;
     Tree& t = g.t;
     t.n = n; t.periodic = periodic; t.nleaf = g.nleaf; t.ncrit = g.ncrit; t.box = box;
     for (int k = 0; k < 3; ++k) t.lo[k] = (double)box.lo[k];
@@ -216,6 +219,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     s.ms_tree = ms_between(g.ev[3], g.ev[4]);
     s.ms_build_total = ms_between(g.ev[0], g.ev[4]);
     s.bytes_allocated = g.bytes;
+    s.launches_build = g_hot_launches;
     guard.ok = true;
     g.built = true;
     return HOT_OK;
@@ -230,6 +234,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (order != 0 && order != 2 && order != 4) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2 or 4");
     Tree& t = g.t;
     cudaStream_t st = g.stream;
+    g_hot_launches = 0;
     CUDA_TRY(cudaEventRecord(g.ev[5], st));
     // S6: moments, cached per build at the highest order asked so far
     if (t.mom_order < order) {
@@ -277,6 +282,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     s.ms_farfield = 0;
     s.ms_forces_total = ms_between(g.ev[5], g.ev[7]);
     s.bytes_allocated = g.bytes + (int64_t)g.gstack_bytes;
+    s.launches_forces = g_hot_launches;
     g.last_order = order;
     return HOT_OK;
 }

@@ -71,6 +71,7 @@ cudaError_t launch_keygen(const float* pos, int64_t n, float lox, float loy, flo
                           uint64_t* key, uint32_t* idx, int* errflag, cudaStream_t st) {
     int64_t quads = (n + 3) / 4;
     int vec = (reinterpret_cast<uintptr_t>(pos) & 15u) == 0; // 128-bit loads need a 16-byte aligned base
+    HOT_LAUNCHED(1);
     keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, n, lox, loy, loz, inv, key, idx, errflag, vec);
     return cudaGetLastError();
 }
@@ -198,6 +199,7 @@ cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uin
     int cur = 0;
     for (int pass = 0; pass < 8; ++pass) {
         int shift = pass * 8;
+        HOT_LAUNCHED(3);
         sort_hist_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], n, shift, hist, nblk);
         scan_rows_kernel<<<256, 1024, 0, st>>>(hist, nblk, totals);
         sort_scatter_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], idx[cur], key[cur ^ 1], idx[cur ^ 1], n, shift,
@@ -219,6 +221,7 @@ __global__ void __launch_bounds__(256) gather_kernel(const float* __restrict__ p
     body[i] = make_float4(__ldg(pos + 3 * (int64_t)j), __ldg(pos + 3 * (int64_t)j + 1), __ldg(pos + 3 * (int64_t)j + 2), __ldg(mass + j));
 }
 cudaError_t launch_gather(const float* pos, const float* mass, const uint32_t* perm, int64_t n, float4* body, cudaStream_t st) {
+    HOT_LAUNCHED(1);
     gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, mass, perm, n, body);
     return cudaGetLastError();
 }
@@ -312,10 +315,12 @@ __global__ void __launch_bounds__(TREE_TILE) tree_levels_kernel(const uint64_t* 
 }
 cudaError_t launch_tree_levels(const uint64_t* skey, int64_t n, int nleaf, int ncrit, uint32_t* plev, uint32_t* counts, cudaStream_t st) {
     int64_t nblk = tree_num_blocks(n);
+    HOT_LAUNCHED(1);
     tree_levels_kernel<<<(unsigned)nblk, TREE_TILE, 0, st>>>(skey, n, nleaf, ncrit, plev, counts, nblk);
     return cudaGetLastError();
 }
 cudaError_t launch_tree_scan(uint32_t* counts, int64_t nblk, uint32_t* totals, cudaStream_t st) {
+    HOT_LAUNCHED(1);
     scan_rows_kernel<<<TREE_ROWS, 1024, 0, st>>>(counts, nblk, totals);
     return cudaGetLastError();
 }
@@ -415,6 +420,7 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
 cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
     LevelBase LB;
     for (int l = 0; l <= HOT_NLEVELS; ++l) LB.v[l] = a.level_base[l];
+    HOT_LAUNCHED(1);
     tree_emit_kernel<<<(unsigned)a.nblk, TREE_TILE, 0, st>>>(a.skey, a.plev, a.counts, a.n, a.nblk, LB, a.ckey, a.cfirst, a.ccount,
                                                              a.cchild, a.cparent, a.group, a.hkey, a.hval, a.hmask, a.maxprobe);
     return cudaGetLastError();
@@ -426,6 +432,7 @@ __global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restri
     atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ckey[c] & 7ull));
 }
 cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, cudaStream_t st) {
+    if (ncells > 1) HOT_LAUNCHED(1);
     if (ncells > 1) tree_link_kernel<<<(unsigned)((ncells - 1 + 255) / 256), 256, 0, st>>>(ckey, cparent, cmask, ncells);
     return cudaGetLastError();
 }
@@ -452,6 +459,7 @@ __global__ void __launch_bounds__(256) tree_finalize_kernel(const uint64_t* __re
 }
 cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount, const uint32_t* cmask,
                                  const int32_t* cchild, WalkCell* wc, int64_t ncells, int* errflag, cudaStream_t st) {
+    HOT_LAUNCHED(1);
     tree_finalize_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, st>>>(ckey, cfirst, ccount, cmask, cchild, wc, ncells, errflag);
     return cudaGetLastError();
 }

@@ -454,6 +454,7 @@ template <int ORDER, bool PER, int SCAP> static cudaError_t launch_one(const For
         *occ_out = occ;
         return e;
     }
+    HOT_LAUNCHED(1);
     forces_kernel<ORDER, PER, SCAP><<<nblocks, WARPS_PER_BLOCK * 32, smem, st>>>(a);
     return cudaGetLastError();
 }

@@ -6,6 +6,9 @@
 
 #include "hot.h"
 
+extern long long g_hot_launches; // kernels launched by the library since the last reset (hot_stats)
+#define HOT_LAUNCHED(k) (g_hot_launches += (k))
+
 #define HOT_MAXLEVEL 21
 #define HOT_NLEVELS 22        // levels 0..21
 #define HOT_MAX_NCRIT 256

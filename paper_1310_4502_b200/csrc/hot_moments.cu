@@ -162,6 +162,7 @@ cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
         int64_t cb = t.level_base[l], ce = t.level_base[l + 1];
         if (ce <= cb) continue;
         unsigned nb = (unsigned)((ce - cb + 127) / 128);
+        HOT_LAUNCHED(1);
         if (order >= 4)
             moments_level_kernel<4><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellM34);
         else if (order >= 2)

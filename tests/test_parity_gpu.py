@@ -1,0 +1,239 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on the same seeded inputs.
+
+Integer artefacts (keys, permutation, cells, groups, list counts) must be bit-exact; fp32
+accelerations and potentials must agree with the oracle's double-precision tree on the same lists to
+median <= 1e-5 and 99.9th percentile <= 1e-4 relative error per particle (BASELINE.json north_star,
+reading in DESIGN.md R-11)."""
+import numpy as np
+import pytest
+
+from oracle import oracle as O
+from paper_1310_4502_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def _build(hot, w, nleaf=16, ncrit=64):
+    import torch
+
+    hot.hot_set_params(nleaf, ncrit)
+    pos = torch.from_numpy(w.pos).cuda()
+    mass = torch.from_numpy(w.mass).cuda()
+    hot.hot_build(pos, mass, w.lo, w.size, w.periodic)
+    return pos, mass
+
+
+def _rel_errors(acc, pot, oa, op):
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]
+    gp = pot.cpu().numpy().astype(np.float64)[m]
+    ea = np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)
+    ep = np.abs(gp - op[m]) / np.abs(op[m])
+    return ea, ep
+
+
+def _check_int_artefacts(hot, T):
+    key, skey, perm = T.keys()
+    gk, gp = hot.hot_export_keys()
+    assert (gk == skey).all(), "sorted keys"
+    assert (gp == perm).all(), "sort permutation"
+    st = hot.hot_stats()
+    assert st["n_cells"] == T.ncells and st["n_groups"] == T.ngroups
+    oc, gc = T.cells(), hot.hot_export_cells()
+    for k in ("key", "first", "count", "mask", "child", "parent"):
+        assert (oc[k].astype(np.int64) == gc[k].astype(np.int64)).all(), f"cells.{k}"
+    assert st["n_leaves"] == int((oc["child"] < 0).sum()) and st["max_level"] == int(oc["level"].max())
+    gg = hot.hot_export_groups()
+    assert (gg["cell"] == T.groups()).all(), "sink groups"
+    # cell membership: leaf of every sorted particle, via the hash table (key -> cell index)
+    leaf = T.leaf_of()
+    sel = np.random.default_rng(1).choice(T.n, min(T.n, 4096), replace=False)
+    lk = oc["key"][leaf[sel]]
+    assert (hot.hot_lookup_keys(lk) == leaf[sel]).all(), "membership through the hash"
+    return oc
+
+
+CASES = [  # cfg, scale, nleaf, ncrit, order, theta
+    (0, 14, 16, 64, 2, 0.5),     # BASELINE configs[0] in full
+    (0, 13, 16, 64, 4, 0.5),
+    (0, 12, 16, 64, 0, 0.5),
+    (1, 15, 16, 64, 2, 0.5),
+    (2, 16, 16, 64, 2, 0.6),
+    (2, 15, 16, 64, 4, 0.4),
+    (2, 15, 8, 128, 2, 0.8),
+    (1, 14, 4, 32, 4, 0.6),
+    (0, 11, 32, 256, 2, 0.5),
+]
+
+
+@pytest.mark.parametrize("cfg,scale,nleaf,ncrit,order,theta", CASES)
+def test_open_boundary_parity(hot, cfg, scale, nleaf, ncrit, order, theta):
+    w = W.config(cfg, scale)
+    _build(hot, w, nleaf, ncrit)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, nleaf=nleaf, ncrit=ncrit)
+    _check_int_artefacts(hot, T)
+    acc, pot = hot.hot_forces(theta, w.eps, order)
+    gg = hot.hot_export_groups()
+    rng = np.random.default_rng(2)
+    sel = np.sort(rng.choice(T.ngroups, min(T.ngroups, 192 if order < 4 else 64), replace=False))
+    oa, op, lpc, lpp = T.forces(theta, w.eps, order, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all(), "L_pc"
+    assert (gg["lpp"][sel] == lpp.astype(np.uint64)).all(), "L_pp"
+    # counts of every group (walk only, cheap) and the interaction totals of hot_stats
+    if T.ngroups <= 4096:
+        lpc_all, lpp_all, cov = T.walk_counts(theta)
+        assert (gg["lpc"] == lpc_all.astype(np.uint64)).all() and (gg["lpp"] == lpp_all.astype(np.uint64)).all()
+        ng = T.cells()["count"][T.groups()]
+        st = hot.hot_stats()
+        assert st["pp_interactions"] == int((ng * lpp_all).sum()) and st["pc_interactions"] == int((ng * lpc_all).sum())
+    ea, ep = _rel_errors(acc, pot, oa, op)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
+
+
+def test_moments_parity(hot):
+    w = W.config(2, 14)
+    _build(hot, w)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size)
+    hot.hot_forces(0.5, w.eps, 4)
+    g = hot.hot_export_moments(4)
+    mom, com, _ = T.moments()
+    size = np.ldexp(1.0, -T.cells()["level"].astype(np.int64)) * w.size  # cell side
+    assert np.abs(g["com"] - com).max() <= 1e-12 * w.size
+    assert np.abs(g["m0"] - mom[:, 0]).max() <= 1e-6 * mom[:, 0].max()
+    for name, sl, deg in (("m2", slice(4, 10), 2), ("m3", slice(10, 20), 3), ("m4", slice(20, 35), 4)):
+        scale = mom[:, 0] * size ** deg  # natural size of a degree-`deg` moment of the cell
+        err = np.abs(g[name] - mom[:, sl]).max(axis=1) / scale
+        assert err.max() <= 1e-6, (name, err.max())
+
+
+def test_error_vs_direct_sum_matches_oracle_tree(hot):
+    """|E(GPU)/E(oracle) - 1| <= 0.05 for the rms error against the direct sum (C0 in full)."""
+    w = W.config(0)
+    _build(hot, w)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size)
+    ad, pd = O.direct(w.pos, w.mass, w.eps)
+    for order in (2, 4):
+        acc, pot = hot.hot_forces(w.theta, w.eps, order)
+        oa, op, _, _ = T.forces(w.theta, w.eps, order)
+        e = lambda a: np.sqrt(((a - ad) ** 2).sum() / (ad ** 2).sum())
+        eg, eo = e(acc.cpu().numpy().astype(np.float64)), e(oa)
+        assert abs(eg / eo - 1) <= 0.05, (order, eg, eo)
+
+
+def test_theta_zero_is_all_particle_particle(hot):
+    w = W.config(2, 10)
+    _build(hot, w)
+    acc, pot = hot.hot_forces(0.0, w.eps, 2)
+    gg = hot.hot_export_groups()
+    assert (gg["lpc"] == 0).all() and (gg["lpp"] == w.n).all()
+    ad, pd = O.direct(w.pos, w.mass, w.eps)
+    ea = np.linalg.norm(acc.cpu().numpy() - ad, axis=1) / np.linalg.norm(ad, axis=1)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4
+
+
+def test_deterministic_and_reusable_build(hot):
+    import torch
+
+    w = W.config(1, 13)
+    _build(hot, w)
+    a1, p1 = hot.hot_forces(0.5, w.eps, 2)
+    a4, p4 = hot.hot_forces(0.5, w.eps, 4)
+    a2, p2 = hot.hot_forces(0.5, w.eps, 2)
+    assert torch.equal(a1, a2) and torch.equal(p1, p2)
+    assert not torch.equal(a1, a4)
+    a3, _ = hot.hot_forces(0.5, w.eps, 2, want_pot=False)
+    assert torch.equal(a1, a3)
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 5, 17, 33, 1023, 1025, 4097])
+def test_ragged_and_tiny_sizes(hot, n):
+    rng = np.random.default_rng(n)
+    pos = rng.uniform(0, 1, (n, 3)).astype(np.float32) * np.float32(0.999)
+    mass = rng.uniform(0.5, 1.5, n).astype(np.float32)
+    w = W.Workload("t", pos, mass, (0, 0, 0), 1.0, False, 1e-2, 0.5, 2)
+    _build(hot, w, 4, 8)
+    T = O.Tree(pos, mass, w.lo, w.size, nleaf=4, ncrit=8)
+    _check_int_artefacts(hot, T)
+    acc, pot = hot.hot_forces(0.5, w.eps, 2)
+    oa, op, lpc, lpp = T.forces(0.5, w.eps, 2)
+    gg = hot.hot_export_groups()
+    assert (gg["lpc"] == lpc.astype(np.uint64)).all() and (gg["lpp"] == lpp.astype(np.uint64)).all()
+    if n == 1:
+        assert (acc.cpu().numpy() == 0).all() and (pot.cpu().numpy() == 0).all()
+    else:
+        ea, ep = _rel_errors(acc, pot, oa, op)
+        assert ea.max() <= 1e-4 and ep.max() <= 1e-5
+
+
+def test_coincident_particles_and_finest_level_group(hot):
+    """Duplicated keys: a level-21 leaf above NLEAF and a sink group above NCRIT (kernels chunk)."""
+    rng = np.random.default_rng(5)
+    pos = rng.uniform(0, 1, (600, 3)).astype(np.float32) * np.float32(0.999)
+    pos[:300] = np.array([0.3, 0.6, 0.9], np.float32)  # 300 coincident bodies > 32*SCAP sinks
+    mass = np.full(600, 1 / 600, np.float32)
+    w = W.Workload("t", pos, mass, (0, 0, 0), 1.0, False, 1e-2, 0.5, 2)
+    _build(hot, w, 4, 32)
+    T = O.Tree(pos, mass, w.lo, w.size, nleaf=4, ncrit=32)
+    oc = _check_int_artefacts(hot, T)
+    assert oc["level"].max() == 21 and oc["count"][oc["level"] == 21].max() == 300
+    acc, pot = hot.hot_forces(0.5, w.eps, 2)
+    oa, op, lpc, lpp = T.forces(0.5, w.eps, 2)
+    gg = hot.hot_export_groups()
+    assert (gg["lpc"] == lpc.astype(np.uint64)).all() and (gg["lpp"] == lpp.astype(np.uint64)).all()
+    ea, ep = _rel_errors(acc, pot, oa, op)
+    assert np.quantile(ea, 0.99) <= 1e-4 and ep.max() <= 1e-5
+
+
+def test_error_codes(hot):
+    import torch
+
+    from paper_1310_4502_b200 import HotError
+
+    w = W.config(0, 10)
+    pos = torch.from_numpy(w.pos).cuda()
+    mass = torch.from_numpy(w.mass).cuda()
+    bad = pos.clone()
+    bad[7, 1] = 1.0  # on the upper face: outside [lo, lo+size)
+    with pytest.raises(HotError) as e:
+        hot.hot_build(bad, mass, w.lo, w.size, False)
+    assert e.value.code == -2
+    with pytest.raises(HotError) as e:  # a failed build leaves no build behind
+        hot.hot_forces(0.5, 1e-3, 2)
+    assert e.value.code == -5
+    with pytest.raises(HotError) as e:
+        hot.hot_build(pos, mass, w.lo, -1.0, False)
+    assert e.value.code == -1
+    hot.hot_build(pos, mass, w.lo, w.size, False)
+    for theta, eps, order in ((1.0, 1e-3, 2), (-0.1, 1e-3, 2), (0.5, -1.0, 2), (0.5, 1e-3, 3), (0.5, 1e-3, 6)):
+        with pytest.raises(HotError) as e:
+            hot.hot_forces(theta, eps, order)
+        assert e.value.code == -1
+    acc, pot = hot.hot_forces(0.5, 1e-3, 2)  # still usable after argument errors
+    assert torch.isfinite(acc).all()
+
+
+def test_host_buffer_entry_point_matches_device_path(hot):
+    w = W.config(0, 12)
+    _build(hot, w)
+    acc, pot = hot.hot_forces(w.theta, w.eps, w.order)
+    ha, hp = hot.hot_step_host(w.pos, w.mass, w.lo, w.size, w.periodic, w.theta, w.eps, w.order)
+    assert (acc.cpu().numpy() == ha).all() and (pot.cpu().numpy() == hp).all()
+
+
+def test_runs_on_a_user_stream(hot):
+    import torch
+
+    w = W.config(0, 12)
+    _build(hot, w)
+    a0, p0 = hot.hot_forces(w.theta, w.eps, 2)
+    s = torch.cuda.Stream()
+    hot.hot_set_stream(s)
+    try:
+        with torch.cuda.stream(s):
+            _build(hot, w)
+            a1, p1 = hot.hot_forces(w.theta, w.eps, 2)
+        s.synchronize()
+    finally:
+        hot.hot_set_stream(None)
+    assert torch.equal(a0, a1) and torch.equal(p0, p1)
