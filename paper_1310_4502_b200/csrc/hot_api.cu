@@ -22,8 +22,12 @@ struct Ctx {
     unsigned int* d_counter = nullptr;
     unsigned long long* d_stat = nullptr; // 4 counters
     uint32_t* d_gstack = nullptr; size_t gstack_bytes = 0; int64_t gstack_cap = 0;
-    std::vector<void*> tree_allocs;       // everything owned by the current build
+    // device buffers of the build, pooled across hot_build calls: a slot is keyed by the address of
+    // the pointer it serves and only ever grows, so a time-stepping caller pays cudaMalloc once
+    struct Slot { const void* key; void* p; size_t cap; };
+    std::vector<Slot> pool;
     int64_t bytes = 0;
+    uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
     hot_stats_t st{};
     cudaEvent_t ev[8] = {};
     bool ev_ready = false;
@@ -51,20 +55,29 @@ int fail(int code, const char* fmt, ...) {
     } while (0)
 
 template <typename T> cudaError_t tree_alloc(T** p, size_t count) {
-    void* q = nullptr;
     size_t bytes = count * sizeof(T);
     if (bytes == 0) bytes = sizeof(T);
-    cudaError_t e = cudaMalloc(&q, bytes);
-    if (e != cudaSuccess) return e;
-    g.tree_allocs.push_back(q);
-    g.bytes += (int64_t)bytes;
-    *p = static_cast<T*>(q);
+    Ctx::Slot* s = nullptr;
+    for (auto& q : g.pool) if (q.key == (const void*)p) { s = &q; break; }
+    if (!s) { g.pool.push_back({(const void*)p, nullptr, 0}); s = &g.pool.back(); }
+    if (s->cap < bytes) {
+        if (s->p) { cudaFree(s->p); g.bytes -= (int64_t)s->cap; s->p = nullptr; s->cap = 0; }
+        size_t want = bytes + bytes / 8; // headroom: cell counts drift from step to step
+        cudaError_t e = cudaMalloc(&s->p, want);
+        if (e != cudaSuccess) { cudaGetLastError(); want = bytes; e = cudaMalloc(&s->p, want); }
+        if (e != cudaSuccess) { s->p = nullptr; return e; }
+        s->cap = want;
+        g.bytes += (int64_t)want;
+    }
+    *p = static_cast<T*>(s->p);
     return cudaSuccess;
 }
-void drop_build() {
-    for (void* p : g.tree_allocs) cudaFree(p);
-    g.tree_allocs.clear();
+void release_pool() {
+    for (auto& q : g.pool) cudaFree(q.p);
+    g.pool.clear();
     g.bytes = 0;
+}
+void drop_build() { // forgets the build; its buffers stay pooled for the next one
     int nleaf = g.t.nleaf, ncrit = g.t.ncrit;
     g.t = Tree();
     g.t.nleaf = nleaf; g.t.ncrit = ncrit;
@@ -109,6 +122,7 @@ int hot_set_params(int nleaf, int ncrit) {
 
 void hot_free(void) {
     drop_build();
+    release_pool();
     cudaFree(g.d_flags); cudaFree(g.d_counter); cudaFree(g.d_stat); cudaFree(g.d_gstack);
     g.d_flags = nullptr; g.d_counter = nullptr; g.d_stat = nullptr; g.d_gstack = nullptr; g.gstack_bytes = 0;
     if (g.ev_ready) { for (auto& e : g.ev) cudaEventDestroy(e); g.ev_ready = false; }
@@ -137,7 +151,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
 
     struct Guard { bool ok = false; ~Guard() { if (!ok) drop_build(); } } guard;
 
-    uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
+    uint32_t *&d_hist = g.d_hist, *&d_counts = g.d_counts, *&d_totals = g.d_totals;
     const int64_t nblk = tree_num_blocks(n);
     const int rows = HOT_NLEVELS + 2;
     CUDA_TRY(tree_alloc(&t.key[0], (size_t)n));
@@ -175,7 +189,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     t.ncells = t.level_base[HOT_NLEVELS];
     t.ngroups = (int64_t)totals[HOT_NLEVELS];
     t.nleaves = (int64_t)totals[HOT_NLEVELS + 1];
-    if (t.ncells >= ((int64_t)1 << 31) - 1) return fail(HOT_EINTERNAL, "hot_build: %lld cells exceed the 31-bit cell index", (long long)t.ncells);
+    if (t.ncells >= ((int64_t)1 << 28)) return fail(HOT_EINTERNAL, "hot_build: %lld cells exceed the 28-bit cell index of the walk", (long long)t.ncells);
     t.hcap = 64;
     while (t.hcap < 2 * t.ncells) t.hcap <<= 1;
     CUDA_TRY(tree_alloc(&t.ckey, (size_t)t.ncells));

@@ -23,7 +23,7 @@ struct __align__(16) WalkCell { uint32_t x, y, z, w; };
 
 // per-cell expansion data (S6), gathered when a cell is accepted
 struct __align__(16) CellA { double zx, zy, zz; float m0; float t2; };   // centre of mass, mass, trace M2
-struct __align__(16) CellM2 { float xx, xy, xz, yy, yz, zz, pad0, pad1; };
+struct __align__(16) CellM2 { float xx, xy, xz, yy, yz, zz, t2, pad1; };     // t2 = trace
 // order 4: M3 (10) + M4 (15) + traces t3 (3), T4 (6), t4 (1) = 35 floats -> 36
 struct __align__(16) CellM34 { float v[36]; };
 

@@ -73,8 +73,8 @@ __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, doub
         CellM2 Q;
         Q.xx = (float)M[midx(2, 0, 0)]; Q.xy = (float)M[midx(1, 1, 0)]; Q.xz = (float)M[midx(1, 0, 1)];
         Q.yy = (float)M[midx(0, 2, 0)]; Q.yz = (float)M[midx(0, 1, 1)]; Q.zz = (float)M[midx(0, 0, 2)];
-        Q.pad0 = Q.pad1 = 0.f;
         A.t2 = Q.xx + Q.yy + Q.zz;
+        Q.t2 = A.t2; Q.pad1 = 0.f; // the trace rides in the record the P-C kernel stages with cp.async
         cellM2[c] = Q;
     }
     cellA[c] = A;
