@@ -66,8 +66,13 @@ typedef struct {
     uint64_t pp_interactions, pc_interactions;
     uint64_t cells_visited;     /* MAC tests of the last walk */
     uint64_t walk_spills;       /* traversal-stack spills to the global arena */
-    float ms_keygen, ms_sort, ms_gather, ms_tree, ms_moments, ms_walk_eval, ms_farfield;
+    float ms_keygen, ms_sort, ms_gather, ms_tree, ms_moments;
+    float ms_walk;   /* list walks: count pass + offset scan + fill pass(es) */
+    float ms_eval;   /* particle-particle / particle-cell interaction kernels (the FP32-bound stage) */
+    float ms_farfield;
     float ms_build_total, ms_forces_total;
+    int32_t list_chunks; int32_t pad0; /* group chunks the lists were walked / evaluated in (1 unless the arena is short) */
+    uint64_t list_entries;      /* accepted cells + listed bodies over all groups (4 B each, +1 B when periodic) */
     int64_t bytes_allocated;
     int64_t launches_build, launches_forces; /* kernels launched by the last hot_build / hot_forces */
 } hot_stats_t;
@@ -77,6 +82,11 @@ typedef struct {
  * 1 <= nleaf <= ncrit <= 256, nleaf <= 32.  Takes effect at the next hot_build.
  * Defaults: nleaf = 16, ncrit = 64. */
 int hot_set_params(int nleaf, int ncrit);
+
+/* Upper bound in bytes on the interaction-list arena of hot_forces (0 = default: as much as fits in
+ * ~70% of the free device memory).  When the lists of all sink groups do not fit, hot_forces walks and
+ * evaluates the groups in chunks (hot_stats list_chunks); HOT_ENOMEM if one group alone does not fit. */
+int hot_set_list_arena(int64_t max_bytes);
 
 /* pos : device, [n][3] fp32 row-major x,y,z; borrowed.   mass: device, [n] fp32 > 0; borrowed.
  * n   : 1 <= n <= 2^27 (and < 2^27 coincident bodies in one finest-level cell).

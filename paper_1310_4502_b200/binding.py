@@ -31,8 +31,10 @@ class hot_stats_t(C.Structure):
                 ("pp_interactions", C.c_uint64), ("pc_interactions", C.c_uint64),
                 ("cells_visited", C.c_uint64), ("walk_spills", C.c_uint64),
                 ("ms_keygen", C.c_float), ("ms_sort", C.c_float), ("ms_gather", C.c_float), ("ms_tree", C.c_float),
-                ("ms_moments", C.c_float), ("ms_walk_eval", C.c_float), ("ms_farfield", C.c_float),
-                ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float), ("bytes_allocated", C.c_int64),
+                ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_eval", C.c_float), ("ms_farfield", C.c_float),
+                ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float),
+                ("list_chunks", C.c_int32), ("pad0", C.c_int32), ("list_entries", C.c_uint64),
+                ("bytes_allocated", C.c_int64),
                 ("launches_build", C.c_int64), ("launches_forces", C.c_int64)]
 
 
@@ -56,6 +58,7 @@ def _load():
                                       C.c_double, C.c_int, C.c_void_p, C.c_void_p]
         lib.hot_set_stream.argtypes = [C.c_void_p]
         lib.hot_set_params.argtypes = [C.c_int, C.c_int]
+        lib.hot_set_list_arena.argtypes = [C.c_int64]
         lib.hot_free.restype = None
         lib.hot_export_keys.argtypes = [C.c_void_p, C.c_void_p]
         lib.hot_export_cells.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
@@ -86,6 +89,11 @@ def hot_set_stream(stream=None):
     """Pass a torch.cuda.Stream (or None for the legacy default stream)."""
     ptr = None if stream is None else C.c_void_p(stream.cuda_stream)
     _check(_load().hot_set_stream(ptr))
+
+
+def hot_set_list_arena(max_bytes: int = 0):
+    """Cap the interaction-list arena (0 = default); smaller caps make hot_forces work in chunks of groups."""
+    _check(_load().hot_set_list_arena(int(max_bytes)))
 
 
 def hot_set_params(nleaf: int = 16, ncrit: int = 64):

@@ -28,6 +28,13 @@ struct Ctx {
     std::vector<Slot> pool;
     int64_t bytes = 0;
     uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
+    // interaction lists (hot_forces)
+    unsigned long long* d_scan = nullptr; int64_t* d_bounds = nullptr;
+    uint32_t *d_pclist = nullptr, *d_pplist = nullptr; uint8_t *d_pcimg = nullptr, *d_ppimg = nullptr;
+    unsigned long long arena_pc = 0, arena_pp = 0; // entries the list arena holds
+    size_t arena_cap_bytes = 0;                     // 0 = as much as fits; else a cap (hot_set_list_arena)
+    std::vector<cudaEvent_t> evx;
+    bool lists_valid = false;
     hot_stats_t st{};
     cudaEvent_t ev[8] = {};
     bool ev_ready = false;
@@ -83,11 +90,12 @@ void drop_build() { // forgets the build; its buffers stay pooled for the next o
     g.t.nleaf = nleaf; g.t.ncrit = ncrit;
     g.built = false;
     g.last_order = -1;
+    g.lists_valid = false;
 }
 int ensure_scratch() {
     if (!g.d_flags) {
         CUDA_TRY(cudaMalloc(&g.d_flags, 4 * sizeof(int)));
-        CUDA_TRY(cudaMalloc(&g.d_counter, sizeof(unsigned int)));
+        CUDA_TRY(cudaMalloc(&g.d_counter, 2 * sizeof(unsigned int)));
         CUDA_TRY(cudaMalloc(&g.d_stat, 4 * sizeof(unsigned long long)));
     }
     if (!g.ev_ready) {
@@ -113,6 +121,12 @@ int hot_set_stream(void* s) {
     return HOT_OK;
 }
 
+int hot_set_list_arena(int64_t max_bytes) {
+    if (max_bytes < 0) return fail(HOT_EINVAL, "hot_set_list_arena: max_bytes must be >= 0");
+    g.arena_cap_bytes = (size_t)max_bytes;
+    return HOT_OK;
+}
+
 int hot_set_params(int nleaf, int ncrit) {
     if (nleaf < 1 || nleaf > HOT_MAX_NLEAF || ncrit < nleaf || ncrit > HOT_MAX_NCRIT)
         return fail(HOT_EINVAL, "hot_set_params: need 1 <= nleaf <= %d, nleaf <= ncrit <= %d", HOT_MAX_NLEAF, HOT_MAX_NCRIT);
@@ -126,6 +140,9 @@ void hot_free(void) {
     cudaFree(g.d_flags); cudaFree(g.d_counter); cudaFree(g.d_stat); cudaFree(g.d_gstack);
     g.d_flags = nullptr; g.d_counter = nullptr; g.d_stat = nullptr; g.d_gstack = nullptr; g.gstack_bytes = 0;
     if (g.ev_ready) { for (auto& e : g.ev) cudaEventDestroy(e); g.ev_ready = false; }
+    for (auto& e : g.evx) cudaEventDestroy(e);
+    g.evx.clear();
+    g.arena_pc = g.arena_pp = 0;
     cudaFreeHost(g.h_pos); cudaFreeHost(g.h_mass); cudaFreeHost(g.h_acc); cudaFreeHost(g.h_pot);
     cudaFree(g.hd_pos); cudaFree(g.hd_mass); cudaFree(g.hd_acc); cudaFree(g.hd_pot);
     g.h_pos = g.h_mass = g.h_acc = g.h_pot = nullptr; g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
@@ -206,8 +223,8 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(tree_alloc(&t.hval, (size_t)t.hcap));
     CUDA_TRY(cudaMemsetAsync(t.hkey, 0, sizeof(uint64_t) * (size_t)t.hcap, st));
     CUDA_TRY(cudaMemsetAsync(t.cmask, 0, sizeof(uint32_t) * (size_t)t.ncells, st));
-    CUDA_TRY(cudaMemsetAsync(t.glpc, 0, sizeof(uint64_t) * (size_t)t.ngroups, st));
-    CUDA_TRY(cudaMemsetAsync(t.glpp, 0, sizeof(uint64_t) * (size_t)t.ngroups, st));
+    CUDA_TRY(cudaMemsetAsync(t.glpc, 0, sizeof(uint32_t) * (size_t)t.ngroups, st));
+    CUDA_TRY(cudaMemsetAsync(t.glpp, 0, sizeof(uint32_t) * (size_t)t.ngroups, st));
     TreeEmitArgs ea;
     ea.skey = t.key[0]; ea.plev = t.plev; ea.counts = d_counts; ea.n = n; ea.nblk = nblk;
     for (int l = 0; l <= HOT_NLEVELS; ++l) ea.level_base[l] = t.level_base[l];
@@ -259,30 +276,106 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         t.mom_order = order;
     }
     CUDA_TRY(cudaEventRecord(g.ev[6], st));
-    const int scap = (t.ncrit + 31) / 32;
-    const int nwarps = force_grid_warps(order, t.periodic, scap);
-    const int64_t gcap = 8192; // spill arena entries per warp
+    // S7 pass 1: list lengths per group, then their exclusive scans = each group's slice of the arena
+    const int nwarps = walk_grid_warps();
+    const int64_t gcap = 4096; // spill arena entries per warp
     size_t need = (size_t)nwarps * (size_t)gcap * sizeof(uint32_t) * (t.periodic ? 2 : 1);
     if (need > g.gstack_bytes) {
         cudaFree(g.d_gstack); g.d_gstack = nullptr; g.gstack_bytes = 0;
         CUDA_TRY(cudaMalloc(&g.d_gstack, need));
         g.gstack_bytes = need;
     }
+    const int64_t ng = t.ngroups;
+    CUDA_TRY(tree_alloc(&t.pcoff, (size_t)ng + 1));
+    CUDA_TRY(tree_alloc(&t.ppoff, (size_t)ng + 1));
+    CUDA_TRY(tree_alloc(&g.d_scan, scan_scratch_elems(ng)));
     CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, sizeof(unsigned int), st));
     CUDA_TRY(cudaMemsetAsync(g.d_stat, 0, 4 * sizeof(unsigned long long), st));
     CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
+    WalkArgs wa{};
+    wa.wcell = t.wcell; wa.group = t.group; wa.g0 = 0; wa.g1 = ng;
+    wa.theta2 = theta * theta; // formed once on the host in double (R-7)
+    wa.periodic = t.periodic; wa.lpc = t.glpc; wa.lpp = t.glpp; wa.pcoff = t.pcoff; wa.ppoff = t.ppoff;
+    wa.counter = g.d_counter; wa.stat = g.d_stat; wa.gstack = g.d_gstack; wa.gstack_cap = gcap; wa.errflag = g.d_flags + 2;
+    CUDA_TRY(launch_walk(wa, false, st));
+    CUDA_TRY(launch_scan_u32_to_u64(t.glpc, ng, g.d_scan, t.pcoff, st));
+    CUDA_TRY(launch_scan_u32_to_u64(t.glpp, ng, g.d_scan, t.ppoff, st));
+    unsigned long long totpc = 0, totpp = 0;
+    int flag = 0;
+    CUDA_TRY(cudaMemcpyAsync(&totpc, t.pcoff + ng, sizeof(totpc), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(&totpp, t.ppoff + ng, sizeof(totpp), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaMemcpyAsync(&flag, g.d_flags + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CUDA_TRY(cudaStreamSynchronize(st));
+    if (flag) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted (flag %d)", flag);
+    // the list arena: everything at once if it fits in (most of) the free memory, else chunks of groups
+    const size_t esz = t.periodic ? 5 : 4; // bytes per list entry: u32 index (+ u8 image id)
+    unsigned long long cappc = totpc > 0 ? totpc : 1, cappp = totpp > 0 ? totpp : 1;
+    {
+        size_t fre = 0, tot = 0;
+        CUDA_TRY(cudaMemGetInfo(&fre, &tot));
+        const double have = 0.7 * (double)fre + (double)(g.arena_pc + g.arena_pp) * (double)esz; // what the pool already holds counts
+        const double want = (double)(cappc + cappp) * (double)esz;
+        if (g.arena_cap_bytes > 0 && want > (double)g.arena_cap_bytes) { // test hook: hot_set_list_arena
+            const double f = (double)g.arena_cap_bytes / want;
+            cappc = (unsigned long long)(cappc * f) + 1; cappp = (unsigned long long)(cappp * f) + 1;
+        } else if (want > have) {
+            const double f = have / want;
+            cappc = (unsigned long long)(cappc * f) + 1; cappp = (unsigned long long)(cappp * f) + 1;
+        }
+    }
+    std::vector<int64_t> bounds;
+    if (cappc >= totpc && cappp >= totpp) { bounds = {0, ng}; }
+    else {
+        const int maxchunks = 4096;
+        int64_t* d_bounds = nullptr; int* d_nch = nullptr;
+        CUDA_TRY(tree_alloc(&g.d_bounds, (size_t)maxchunks + 1));
+        d_bounds = g.d_bounds; d_nch = g.d_flags + 3;
+        CUDA_TRY(launch_chunk_bounds(t.pcoff, t.ppoff, ng, cappc, cappp, d_bounds, maxchunks, d_nch, st));
+        int nch = 0;
+        CUDA_TRY(cudaMemcpyAsync(&nch, d_nch, sizeof(int), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        if (nch < 1) return fail(HOT_ENOMEM, "hot_forces: the interaction lists of one sink group (or of %d chunks) do not fit the list arena "
+                                 "(%llu + %llu entries for %llu + %llu in total)", maxchunks, cappc, cappp, totpc, totpp);
+        bounds.resize((size_t)nch + 1);
+        CUDA_TRY(cudaMemcpy(bounds.data(), d_bounds, sizeof(int64_t) * ((size_t)nch + 1), cudaMemcpyDeviceToHost));
+    }
+    CUDA_TRY(tree_alloc(&g.d_pclist, (size_t)cappc));
+    CUDA_TRY(tree_alloc(&g.d_pplist, (size_t)cappp));
+    if (t.periodic) { CUDA_TRY(tree_alloc(&g.d_pcimg, (size_t)cappc)); CUDA_TRY(tree_alloc(&g.d_ppimg, (size_t)cappp)); }
+    g.arena_pc = cappc; g.arena_pp = cappp;
+    std::vector<unsigned long long> h_off; // offsets at the chunk boundaries
+    h_off.resize(2 * bounds.size());
+    if (bounds.size() == 2) { h_off = {0ull, 0ull, totpc, totpp}; }
+    else {
+        for (size_t k = 0; k < bounds.size(); ++k) {
+            CUDA_TRY(cudaMemcpy(&h_off[2 * k], t.pcoff + bounds[k], 8, cudaMemcpyDeviceToHost));
+            CUDA_TRY(cudaMemcpy(&h_off[2 * k + 1], t.ppoff + bounds[k], 8, cudaMemcpyDeviceToHost));
+        }
+    }
+    // S7 pass 2 (lists) and S8/S9/S10 (interactions), chunk by chunk
+    const size_t nchunks = bounds.size() - 1;
+    while (g.evx.size() < 3 * nchunks + 1) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); }
     ForceArgs a{};
     a.wcell = t.wcell; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellM34 = t.cellM34;
-    a.body = t.body; a.perm = t.idx[0]; a.group = t.group; a.ngroups = t.ngroups;
-    a.theta2 = theta * theta; // formed once on the host in double (R-7)
-    a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic; a.scap = scap;
+    a.body = t.body; a.perm = t.idx[0]; a.group = t.group;
+    a.pcoff = t.pcoff; a.ppoff = t.ppoff; a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
+    a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic;
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
-    a.acc = acc; a.pot = pot; a.glpc = t.glpc; a.glpp = t.glpp;
-    a.counter = g.d_counter; a.stat = g.d_stat; a.gstack = g.d_gstack; a.gstack_cap = gcap; a.errflag = g.d_flags + 2;
-    CUDA_TRY(launch_forces(a, st));
+    a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
+    wa.pclist = g.d_pclist; wa.pplist = g.d_pplist; wa.pcimg = g.d_pcimg; wa.ppimg = g.d_ppimg;
+    CUDA_TRY(cudaEventRecord(g.evx[0], st)); // end of the count pass + scans
+    for (size_t k = 0; k < nchunks; ++k) {
+        wa.g0 = a.g0 = bounds[k]; wa.g1 = a.g1 = bounds[k + 1];
+        wa.pcbase = a.pcbase = h_off[2 * k]; wa.ppbase = a.ppbase = h_off[2 * k + 1];
+        CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
+        CUDA_TRY(cudaEventRecord(g.evx[3 * k + 1], st));
+        CUDA_TRY(launch_walk(wa, true, st));
+        CUDA_TRY(cudaEventRecord(g.evx[3 * k + 2], st));
+        CUDA_TRY(launch_forces(a, st));
+        CUDA_TRY(cudaEventRecord(g.evx[3 * k + 3], st));
+    }
     CUDA_TRY(cudaEventRecord(g.ev[7], st));
-    int flag = 0;
     unsigned long long stat[4];
     CUDA_TRY(cudaMemcpyAsync(&flag, g.d_flags + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
@@ -292,12 +385,19 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     s.order = order;
     s.cells_visited = stat[0]; s.walk_spills = stat[1]; s.pp_interactions = stat[2]; s.pc_interactions = stat[3];
     s.ms_moments = ms_between(g.ev[5], g.ev[6]);
-    s.ms_walk_eval = ms_between(g.ev[6], g.ev[7]);
+    s.ms_walk = ms_between(g.ev[6], g.evx[0]);
+    s.ms_eval = 0;
+    for (size_t k = 0; k < nchunks; ++k) {
+        s.ms_walk += ms_between(g.evx[3 * k + 1], g.evx[3 * k + 2]);
+        s.ms_eval += ms_between(g.evx[3 * k + 2], g.evx[3 * k + 3]);
+    }
     s.ms_farfield = 0;
     s.ms_forces_total = ms_between(g.ev[5], g.ev[7]);
+    s.list_chunks = (int32_t)nchunks; s.list_entries = totpc + totpp;
     s.bytes_allocated = g.bytes + (int64_t)g.gstack_bytes;
     s.launches_forces = g_hot_launches;
     g.last_order = order;
+    g.lists_valid = true;
     return HOT_OK;
 }
 
@@ -373,8 +473,19 @@ int hot_export_groups(int32_t* cell, uint64_t* lpc, uint64_t* lpp, int64_t cap, 
         CUDA_TRY(cudaMemcpy(r.data(), t.group, sizeof(GroupRec) * ng, cudaMemcpyDeviceToHost));
         for (size_t i = 0; i < ng; ++i) cell[i] = (int32_t)r[i].cell;
     }
-    if (lpc) CUDA_TRY(cudaMemcpy(lpc, t.glpc, 8 * ng, cudaMemcpyDeviceToHost));
-    if (lpp) CUDA_TRY(cudaMemcpy(lpp, t.glpp, 8 * ng, cudaMemcpyDeviceToHost));
+    if (lpc || lpp) { // device holds u32 list lengths; L_pp counts the group's own bodies too (they are not in the list)
+        std::vector<uint32_t> v(ng);
+        std::vector<GroupRec> r(ng);
+        CUDA_TRY(cudaMemcpy(r.data(), t.group, sizeof(GroupRec) * ng, cudaMemcpyDeviceToHost));
+        if (lpc) {
+            CUDA_TRY(cudaMemcpy(v.data(), t.glpc, 4 * ng, cudaMemcpyDeviceToHost));
+            for (size_t i = 0; i < ng; ++i) lpc[i] = v[i];
+        }
+        if (lpp) {
+            CUDA_TRY(cudaMemcpy(v.data(), t.glpp, 4 * ng, cudaMemcpyDeviceToHost));
+            for (size_t i = 0; i < ng; ++i) lpp[i] = g.lists_valid ? (uint64_t)v[i] + r[i].count : 0;
+        }
+    }
     return HOT_OK;
 }
 int hot_export_moments(double* com, float* m0, float* m2, float* m3, float* m4, int64_t cap) {

@@ -48,7 +48,8 @@ struct Tree {
     int32_t *cchild = nullptr, *cparent = nullptr;
     WalkCell* wcell = nullptr;
     GroupRec* group = nullptr;
-    uint64_t *glpc = nullptr, *glpp = nullptr;
+    uint32_t *glpc = nullptr, *glpp = nullptr;   // list lengths of the last walk (glpp without the group's own bodies)
+    unsigned long long *pcoff = nullptr, *ppoff = nullptr; // [ngroups+1] exclusive scans of them
     // hash
     int64_t hcap = 0;
     uint64_t* hkey = nullptr;
@@ -93,21 +94,38 @@ cudaError_t launch_hash_lookup(const uint64_t* hkey, const int32_t* hval, int64_
 // ---- upward pass (hot_moments.cu) -------------------------------------------------------------
 cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st);
 
-// ---- walk + interactions (hot_forces.cu) ------------------------------------------------------
-struct ForceArgs {
-    const WalkCell* wcell; const CellA* cellA; const CellM2* cellM2; const CellM34* cellM34;
-    const float4* body; const uint32_t* perm; const GroupRec* group; int64_t ngroups;
-    double theta2; float eps2; int order; int periodic;
-    int scap;                     // ceil(ncrit/32): sinks per lane the kernel must hold
-    double lo[3], size;
-    float* acc; float* pot;
-    uint64_t* glpc; uint64_t* glpp;
-    unsigned int* counter;        // dynamic group scheduler
-    unsigned long long* stat;     // [0] cells visited, [1] spills, [2] sum n*Lpp, [3] sum n*Lpc
-    uint32_t* gstack; int64_t gstack_cap; // per-warp spill arena (entries per warp)
+// ---- walk (hot_walk.cu): emits the interaction lists of the groups [g0, g1) ---------------------------
+struct WalkArgs {
+    const WalkCell* wcell; const GroupRec* group; int64_t g0, g1;
+    double theta2; int periodic;
+    uint32_t* lpc; uint32_t* lpp;                 // COUNT pass out: accepted cells / bodies of rejected leaves per group
+    const unsigned long long* pcoff; const unsigned long long* ppoff; // FILL pass in: list offsets per group (exclusive scans)
+    unsigned long long pcbase, ppbase;            // offsets of group g0 (the arena holds one chunk of groups)
+    uint32_t* pclist; uint32_t* pplist;           // FILL pass out: cell indices / body indices
+    uint8_t* pcimg; uint8_t* ppimg;               // periodic: image id (0..124) of every list entry
+    unsigned int* counter;                        // dynamic group scheduler
+    unsigned long long* stat;                     // [0] cells visited, [1] spills (COUNT pass)
+    uint32_t* gstack; int64_t gstack_cap;         // per-warp spill arena (entries per warp)
     int* errflag;
 };
-int force_grid_warps(int order, int periodic, int scap); // resident warps the kernel is launched with
+int walk_grid_warps();
+cudaError_t launch_walk(const WalkArgs& a, bool fill, cudaStream_t st);
+size_t scan_scratch_elems(int64_t n);
+cudaError_t launch_scan_u32_to_u64(const uint32_t* len, int64_t n, unsigned long long* scratch, unsigned long long* off, cudaStream_t st);
+cudaError_t launch_chunk_bounds(const unsigned long long* pcoff, const unsigned long long* ppoff, int64_t ng, unsigned long long cappc,
+                                unsigned long long cappp, int64_t* bounds, int maxchunks, int* nchunks, cudaStream_t st);
+
+// ---- interactions (hot_forces.cu): evaluates the lists of the groups [g0, g1) -------------------------
+struct ForceArgs {
+    const WalkCell* wcell; const CellA* cellA; const CellM2* cellM2; const CellM34* cellM34;
+    const float4* body; const uint32_t* perm; const GroupRec* group; int64_t g0, g1;
+    const unsigned long long* pcoff; const unsigned long long* ppoff; unsigned long long pcbase, ppbase;
+    const uint32_t* pclist; const uint32_t* pplist; const uint8_t* pcimg; const uint8_t* ppimg;
+    float eps2; int order; int periodic;
+    double lo[3], size;
+    float* acc; float* pot;
+    unsigned int* counter;        // dynamic group scheduler
+};
 cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st);
 
 // ---- periodic far field (hot_periodic.cu) -----------------------------------------------------
