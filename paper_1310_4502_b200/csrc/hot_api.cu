@@ -1,4 +1,6 @@
 // hot_api.cu -- the C ABI of include/hot.h: context, allocations, stage orchestration, exports.
+#include <climits>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
@@ -29,9 +31,11 @@ struct Ctx {
     int64_t bytes = 0;
     uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
     // interaction lists (hot_forces)
-    unsigned long long* d_scan = nullptr; int64_t* d_bounds = nullptr;
+    unsigned long long* d_tops = nullptr;
     uint32_t *d_pclist = nullptr, *d_pplist = nullptr; uint8_t *d_pcimg = nullptr, *d_ppimg = nullptr;
+    uint32_t* d_stage = nullptr; uint8_t* d_stage_img = nullptr; int64_t stage_cap = 0; // per-warp list staging (entries per list)
     unsigned long long arena_pc = 0, arena_pp = 0; // entries the list arena holds
+    unsigned long long used_pc = 0, used_pp = 0;   // entries the last hot_forces wrote (sizes the next arena)
     size_t arena_cap_bytes = 0;                     // 0 = as much as fits; else a cap (hot_set_list_arena)
     std::vector<cudaEvent_t> evx;
     bool lists_valid = false;
@@ -104,6 +108,20 @@ int ensure_scratch() {
     }
     return HOT_OK;
 }
+// MAC thresholds (R-7): the criterion is  (double)(s*s) < theta2 * (double)d2  with s = 2^(21-l)
+// and d2 an integer < 2^53.  fl(theta2 * d2) is non-decreasing in d2, so for every level there is one
+// smallest integer T[l] with the criterion true for exactly the d2 >= T[l]; it is found by bisection
+// with that same IEEE double multiply and compare, and the kernel tests d2 >= T[l] in integers.
+void mac_table(double theta2, unsigned long long* T) {
+    for (int l = 0; l < HOT_NLEVELS; ++l) {
+        const double s2 = std::ldexp(1.0, 2 * (HOT_MAXLEVEL - l));
+        auto ok = [&](unsigned long long d2) { volatile double p = theta2 * (double)d2; return s2 < p; };
+        unsigned long long lo = 0, hi = 1ull << 53; // lo fails (0 is never accepted), hi is tested first
+        if (!ok(hi)) { T[l] = ~0ull; continue; }
+        while (hi - lo > 1) { const unsigned long long mid = lo + (hi - lo) / 2; if (ok(mid)) hi = mid; else lo = mid; }
+        T[l] = hi;
+    }
+}
 float ms_between(cudaEvent_t a, cudaEvent_t b) {
     float ms = 0;
     if (cudaEventElapsedTime(&ms, a, b) != cudaSuccess) { cudaGetLastError(); ms = 0; }
@@ -142,7 +160,7 @@ void hot_free(void) {
     if (g.ev_ready) { for (auto& e : g.ev) cudaEventDestroy(e); g.ev_ready = false; }
     for (auto& e : g.evx) cudaEventDestroy(e);
     g.evx.clear();
-    g.arena_pc = g.arena_pp = 0;
+    g.arena_pc = g.arena_pp = 0; g.used_pc = g.used_pp = 0; g.stage_cap = 0;
     cudaFreeHost(g.h_pos); cudaFreeHost(g.h_mass); cudaFreeHost(g.h_acc); cudaFreeHost(g.h_pot);
     cudaFree(g.hd_pos); cudaFree(g.hd_mass); cudaFree(g.hd_acc); cudaFree(g.hd_pot);
     g.h_pos = g.h_mass = g.h_acc = g.h_pot = nullptr; g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
@@ -276,7 +294,10 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         t.mom_order = order;
     }
     CUDA_TRY(cudaEventRecord(g.ev[6], st));
-    // S7 pass 1: list lengths per group, then their exclusive scans = each group's slice of the arena
+    int rc = HOT_OK;
+    // S7: the walk writes every group's lists into the arena; S8/S9/S10 evaluate them.  The arena is
+    // sized from the previous call (first call: a guess); if it is too small the walk reports the
+    // first group that did not fit, the groups before it are evaluated and the walk goes on from there.
     const int nwarps = walk_grid_warps();
     const int64_t gcap = 4096; // spill arena entries per warp
     size_t need = (size_t)nwarps * (size_t)gcap * sizeof(uint32_t) * (t.periodic ? 2 : 1);
@@ -286,114 +307,124 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         g.gstack_bytes = need;
     }
     const int64_t ng = t.ngroups;
-    CUDA_TRY(tree_alloc(&t.pcoff, (size_t)ng + 1));
-    CUDA_TRY(tree_alloc(&t.ppoff, (size_t)ng + 1));
-    CUDA_TRY(tree_alloc(&g.d_scan, scan_scratch_elems(ng)));
-    CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, sizeof(unsigned int), st));
+    CUDA_TRY(tree_alloc(&t.glvis, (size_t)ng));
+    CUDA_TRY(tree_alloc(&t.pcoff, (size_t)ng));
+    CUDA_TRY(tree_alloc(&t.ppoff, (size_t)ng));
+    CUDA_TRY(tree_alloc(&g.d_tops, 2));
+    const size_t esz = t.periodic ? 5 : 4; // bytes per list entry: u32 (+ u8 image id)
+    if (g.stage_cap < 1024) g.stage_cap = 16384;
+    // arena capacity in entries: what the last call needed plus 12%, else a first guess
+    unsigned long long cappc = g.used_pc ? g.used_pc + g.used_pc / 8 + 4096 : (unsigned long long)ng * (t.periodic ? 6000 : 2800) + 65536;
+    unsigned long long cappp = g.used_pp ? g.used_pp + g.used_pp / 8 + 4096 : (unsigned long long)ng * (t.periodic ? 3000 : 1400) + 65536;
+    if (cappc < g.arena_pc) cappc = g.arena_pc; // never shrink what the pool already holds
+    if (cappp < g.arena_pp) cappp = g.arena_pp;
+    auto clamp_arena = [&]() -> int {
+        size_t fre = 0, tot = 0;
+        CUDA_TRY(cudaMemGetInfo(&fre, &tot));
+        double have = 0.7 * (double)fre + (double)(g.arena_pc + g.arena_pp) * (double)esz; // what the pool holds counts as available
+        if (g.arena_cap_bytes > 0 && (double)g.arena_cap_bytes < have) have = (double)g.arena_cap_bytes; // hot_set_list_arena
+        const double want = (double)(cappc + cappp) * (double)esz;
+        if (want > have) { const double f = have / want; cappc = (unsigned long long)(cappc * f) + 1; cappp = (unsigned long long)(cappp * f) + 1; }
+        return HOT_OK;
+    };
+    if (cappc > g.arena_pc || cappp > g.arena_pp || g.arena_cap_bytes > 0) { rc = clamp_arena(); if (rc) return rc; }
+    auto alloc_lists = [&]() -> int {
+        CUDA_TRY(tree_alloc(&g.d_pclist, (size_t)cappc));
+        CUDA_TRY(tree_alloc(&g.d_pplist, (size_t)cappp));
+        if (t.periodic) { CUDA_TRY(tree_alloc(&g.d_pcimg, (size_t)cappc)); CUDA_TRY(tree_alloc(&g.d_ppimg, (size_t)cappp)); }
+        g.arena_pc = cappc; g.arena_pp = cappp;
+        return HOT_OK;
+    };
+    auto alloc_stage = [&]() -> int {
+        CUDA_TRY(tree_alloc(&g.d_stage, (size_t)nwarps * 2 * (size_t)g.stage_cap));
+        if (t.periodic) CUDA_TRY(tree_alloc(&g.d_stage_img, (size_t)nwarps * 2 * (size_t)g.stage_cap));
+        return HOT_OK;
+    };
+    rc = alloc_lists(); if (rc) return rc;
+    rc = alloc_stage(); if (rc) return rc;
     CUDA_TRY(cudaMemsetAsync(g.d_stat, 0, 4 * sizeof(unsigned long long), st));
     CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
     WalkArgs wa{};
-    wa.wcell = t.wcell; wa.group = t.group; wa.g0 = 0; wa.g1 = ng;
-    wa.theta2 = theta * theta; // formed once on the host in double (R-7)
-    wa.periodic = t.periodic; wa.lpc = t.glpc; wa.lpp = t.glpp; wa.pcoff = t.pcoff; wa.ppoff = t.ppoff;
+    wa.wcell = t.wcell; wa.group = t.group; wa.g1 = ng;
+    mac_table(theta * theta, wa.mac_t); // theta^2 formed once on the host in double (R-7)
+    wa.periodic = t.periodic; wa.lpc = t.glpc; wa.lpp = t.glpp; wa.lvis = t.glvis; wa.pcoff = t.pcoff; wa.ppoff = t.ppoff;
+    wa.tops = g.d_tops; wa.first_fail = g.d_flags + 3;
     wa.counter = g.d_counter; wa.stat = g.d_stat; wa.gstack = g.d_gstack; wa.gstack_cap = gcap; wa.errflag = g.d_flags + 2;
-    CUDA_TRY(launch_walk(wa, false, st));
-    CUDA_TRY(launch_scan_u32_to_u64(t.glpc, ng, g.d_scan, t.pcoff, st));
-    CUDA_TRY(launch_scan_u32_to_u64(t.glpp, ng, g.d_scan, t.ppoff, st));
-    unsigned long long totpc = 0, totpp = 0;
-    int flag = 0;
-    CUDA_TRY(cudaMemcpyAsync(&totpc, t.pcoff + ng, sizeof(totpc), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaMemcpyAsync(&totpp, t.ppoff + ng, sizeof(totpp), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaMemcpyAsync(&flag, g.d_flags + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CUDA_TRY(cudaStreamSynchronize(st));
-    if (flag) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted (flag %d)", flag);
-    // the list arena: everything at once if it fits in (most of) the free memory, else chunks of groups
-    const size_t esz = t.periodic ? 5 : 4; // bytes per list entry: u32 index (+ u8 image id)
-    unsigned long long cappc = totpc > 0 ? totpc : 1, cappp = totpp > 0 ? totpp : 1;
-    {
-        size_t fre = 0, tot = 0;
-        CUDA_TRY(cudaMemGetInfo(&fre, &tot));
-        const double have = 0.7 * (double)fre + (double)(g.arena_pc + g.arena_pp) * (double)esz; // what the pool already holds counts
-        const double want = (double)(cappc + cappp) * (double)esz;
-        if (g.arena_cap_bytes > 0 && want > (double)g.arena_cap_bytes) { // test hook: hot_set_list_arena
-            const double f = (double)g.arena_cap_bytes / want;
-            cappc = (unsigned long long)(cappc * f) + 1; cappp = (unsigned long long)(cappp * f) + 1;
-        } else if (want > have) {
-            const double f = have / want;
-            cappc = (unsigned long long)(cappc * f) + 1; cappp = (unsigned long long)(cappp * f) + 1;
-        }
-    }
-    std::vector<int64_t> bounds;
-    if (cappc >= totpc && cappp >= totpp) { bounds = {0, ng}; }
-    else {
-        const int maxchunks = 4096;
-        int64_t* d_bounds = nullptr; int* d_nch = nullptr;
-        CUDA_TRY(tree_alloc(&g.d_bounds, (size_t)maxchunks + 1));
-        d_bounds = g.d_bounds; d_nch = g.d_flags + 3;
-        CUDA_TRY(launch_chunk_bounds(t.pcoff, t.ppoff, ng, cappc, cappp, d_bounds, maxchunks, d_nch, st));
-        int nch = 0;
-        CUDA_TRY(cudaMemcpyAsync(&nch, d_nch, sizeof(int), cudaMemcpyDeviceToHost, st));
-        CUDA_TRY(cudaStreamSynchronize(st));
-        if (nch < 1) return fail(HOT_ENOMEM, "hot_forces: the interaction lists of one sink group (or of %d chunks) do not fit the list arena "
-                                 "(%llu + %llu entries for %llu + %llu in total)", maxchunks, cappc, cappp, totpc, totpp);
-        bounds.resize((size_t)nch + 1);
-        CUDA_TRY(cudaMemcpy(bounds.data(), d_bounds, sizeof(int64_t) * ((size_t)nch + 1), cudaMemcpyDeviceToHost));
-    }
-    CUDA_TRY(tree_alloc(&g.d_pclist, (size_t)cappc));
-    CUDA_TRY(tree_alloc(&g.d_pplist, (size_t)cappp));
-    if (t.periodic) { CUDA_TRY(tree_alloc(&g.d_pcimg, (size_t)cappc)); CUDA_TRY(tree_alloc(&g.d_ppimg, (size_t)cappp)); }
-    g.arena_pc = cappc; g.arena_pp = cappp;
-    std::vector<unsigned long long> h_off; // offsets at the chunk boundaries
-    h_off.resize(2 * bounds.size());
-    if (bounds.size() == 2) { h_off = {0ull, 0ull, totpc, totpp}; }
-    else {
-        for (size_t k = 0; k < bounds.size(); ++k) {
-            CUDA_TRY(cudaMemcpy(&h_off[2 * k], t.pcoff + bounds[k], 8, cudaMemcpyDeviceToHost));
-            CUDA_TRY(cudaMemcpy(&h_off[2 * k + 1], t.ppoff + bounds[k], 8, cudaMemcpyDeviceToHost));
-        }
-    }
-    // S7 pass 2 (lists) and S8/S9/S10 (interactions), chunk by chunk
-    const size_t nchunks = bounds.size() - 1;
-    while (g.evx.size() < 3 * nchunks + 1) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); }
     ForceArgs a{};
     a.wcell = t.wcell; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellM34 = t.cellM34;
     a.body = t.body; a.perm = t.idx[0]; a.group = t.group;
-    a.pcoff = t.pcoff; a.ppoff = t.ppoff; a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
+    a.pcoff = t.pcoff; a.ppoff = t.ppoff; a.lpc = t.glpc; a.lpp = t.glpp;
     a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic;
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
     a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
-    wa.pclist = g.d_pclist; wa.pplist = g.d_pplist; wa.pcimg = g.d_pcimg; wa.ppimg = g.d_ppimg;
-    CUDA_TRY(cudaEventRecord(g.evx[0], st)); // end of the count pass + scans
-    for (size_t k = 0; k < nchunks; ++k) {
-        wa.g0 = a.g0 = bounds[k]; wa.g1 = a.g1 = bounds[k + 1];
-        wa.pcbase = a.pcbase = h_off[2 * k]; wa.ppbase = a.ppbase = h_off[2 * k + 1];
+    int64_t g0 = 0;
+    size_t nrounds = 0;
+    unsigned long long usedpc = 0, usedpp = 0;
+    float ms_walk = 0, ms_eval = 0;
+    if (g.evx.size() < 3) { while (g.evx.size() < 3) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
+    while (g0 < ng) {
+        const int ff0 = INT_MAX;
         CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
-        CUDA_TRY(cudaEventRecord(g.evx[3 * k + 1], st));
-        CUDA_TRY(launch_walk(wa, true, st));
-        CUDA_TRY(cudaEventRecord(g.evx[3 * k + 2], st));
+        CUDA_TRY(cudaMemsetAsync(g.d_tops, 0, 2 * sizeof(unsigned long long), st));
+        CUDA_TRY(cudaMemcpyAsync(g.d_flags + 3, &ff0, sizeof(int), cudaMemcpyHostToDevice, st));
+        wa.g0 = g0;
+        wa.pclist = g.d_pclist; wa.pplist = g.d_pplist; wa.pcimg = g.d_pcimg; wa.ppimg = g.d_ppimg; wa.cappc = cappc; wa.cappp = cappp;
+        wa.stage = g.d_stage; wa.stage_img = g.d_stage_img; wa.stage_cap = g.stage_cap;
+        CUDA_TRY(cudaEventRecord(g.evx[0], st));
+        CUDA_TRY(launch_walk(wa, st));
+        CUDA_TRY(cudaEventRecord(g.evx[1], st));
+        int fl[2] = {0, 0}; // errflag, first_fail
+        unsigned long long tops[2] = {0, 0};
+        CUDA_TRY(cudaMemcpyAsync(fl, g.d_flags + 2, 2 * sizeof(int), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaMemcpyAsync(tops, g.d_tops, sizeof(tops), cudaMemcpyDeviceToHost, st));
+        CUDA_TRY(cudaStreamSynchronize(st));
+        ms_walk += ms_between(g.evx[0], g.evx[1]);
+        if (fl[0] & 4) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted");
+        if (fl[0] & 8) { // a group's lists outgrew the per-warp staging area: enlarge it and walk this range again
+            if (g.stage_cap >= ((int64_t)1 << 26)) return fail(HOT_ENOMEM, "hot_forces: one sink group's interaction list exceeds 2^26 entries");
+            g.stage_cap *= 4;
+            rc = alloc_stage(); if (rc) return rc;
+            CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
+            continue;
+        }
+        const int64_t F = fl[1] < ng ? (int64_t)fl[1] : ng;
+        if (F == g0) { // not even one group fits: enlarge the arena if memory allows
+            const unsigned long long oldpc = cappc, oldpp = cappp;
+            cappc *= 2; cappp *= 2;
+            rc = clamp_arena(); if (rc) return rc;
+            if (cappc <= oldpc + oldpc / 16 && cappp <= oldpp + oldpp / 16)
+                return fail(HOT_ENOMEM, "hot_forces: the interaction lists of one sink group do not fit the list arena (%llu + %llu entries)", oldpc, oldpp);
+            if (cappc < oldpc) cappc = oldpc;
+            if (cappp < oldpp) cappp = oldpp;
+            rc = alloc_lists(); if (rc) return rc;
+            continue;
+        }
+        usedpc += tops[0]; usedpp += tops[1];
+        a.g0 = g0; a.g1 = F;
+        a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
         CUDA_TRY(launch_forces(a, st));
-        CUDA_TRY(cudaEventRecord(g.evx[3 * k + 3], st));
+        CUDA_TRY(cudaEventRecord(g.evx[2], st));
+        if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[1], g.evx[2]); } // the arena is reused
+        g0 = F;
+        ++nrounds;
     }
+    CUDA_TRY(launch_group_stats(t.group, t.glpc, t.glpp, t.glvis, ng, g.d_stat, st));
     CUDA_TRY(cudaEventRecord(g.ev[7], st));
     unsigned long long stat[4];
-    CUDA_TRY(cudaMemcpyAsync(&flag, g.d_flags + 2, sizeof(int), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
-    if (flag) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted (flag %d)", flag);
+    ms_eval += ms_between(g.evx[1], g.evx[2]);
+    g.used_pc = usedpc; g.used_pp = usedpp; // sizes the arena of the next call
     hot_stats_t& s = g.st;
     s.order = order;
     s.cells_visited = stat[0]; s.walk_spills = stat[1]; s.pp_interactions = stat[2]; s.pc_interactions = stat[3];
     s.ms_moments = ms_between(g.ev[5], g.ev[6]);
-    s.ms_walk = ms_between(g.ev[6], g.evx[0]);
-    s.ms_eval = 0;
-    for (size_t k = 0; k < nchunks; ++k) {
-        s.ms_walk += ms_between(g.evx[3 * k + 1], g.evx[3 * k + 2]);
-        s.ms_eval += ms_between(g.evx[3 * k + 2], g.evx[3 * k + 3]);
-    }
+    s.ms_walk = ms_walk;
+    s.ms_eval = ms_eval;
     s.ms_farfield = 0;
     s.ms_forces_total = ms_between(g.ev[5], g.ev[7]);
-    s.list_chunks = (int32_t)nchunks; s.list_entries = totpc + totpp;
+    s.list_chunks = (int32_t)nrounds; s.list_entries = usedpc + usedpp;
     s.bytes_allocated = g.bytes + (int64_t)g.gstack_bytes;
     s.launches_forces = g_hot_launches;
     g.last_order = order;

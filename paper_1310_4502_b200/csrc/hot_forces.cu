@@ -1,6 +1,6 @@
 // hot_forces.cu -- S8 particle-particle and S9 particle-cell interaction kernels, S10 scatter.
 //
-// Input: the interaction lists hot_walk.cu wrote for a chunk of sink groups (cell indices, body
+// Input: the interaction lists hot_walk.cu wrote for a range of sink groups (cell indices, body
 // indices, image ids when periodic).  One warp owns one sink group at a time (persistent grid,
 // dynamic group counter) and evaluates its lists in the m x n blocking of PAPER.md:162-164:
 //
@@ -58,8 +58,8 @@ __device__ __forceinline__ void cp_async_wait_all() {
 // lane evaluates its sinks two at a time; an odd sink count leaves one scalar sink.
 struct f2 { unsigned long long v; };
 __device__ __forceinline__ f2 mk2(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
-__device__ __forceinline__ float lo2(f2 a) { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a.v)); (void)y; return x; }
-__device__ __forceinline__ float hi2(f2 a) { float x, y; asm("mov.b64 {%0, %1}, %2;" : "=f"(x), "=f"(y) : "l"(a.v)); (void)x; return y; }
+__device__ __forceinline__ float lo2(f2 a) { float x; asm("{ .reg .f32 t; mov.b64 {%0, t}, %1; }" : "=f"(x) : "l"(a.v)); return x; }
+__device__ __forceinline__ float hi2(f2 a) { float y; asm("{ .reg .f32 t; mov.b64 {t, %0}, %1; }" : "=f"(y) : "l"(a.v)); return y; }
 __device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
 __device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
 __device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
@@ -323,10 +323,10 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
 
     // ---- S9: the particle-cell list ------------------------------------------------------------------
     {
-        const unsigned long long o0 = P.pcoff[gi], o1 = P.pcoff[gi + 1];
-        const int n = (int)(o1 - o0);
-        const uint32_t* const pl = P.pclist + (o0 - P.pcbase);
-        const uint8_t* const pi = PER ? P.pcimg + (o0 - P.pcbase) : nullptr;
+        const unsigned long long o0 = P.pcoff[gi];
+        const int n = (int)P.lpc[gi];
+        const uint32_t* const pl = P.pclist + o0;
+        const uint8_t* const pi = PER ? P.pcimg + o0 : nullptr;
         const int nb = (n + BATCH - 1) / BATCH;
         CellA cA;
         cA.zx = cA.zy = cA.zz = 0.0; cA.m0 = 0.f; cA.t2 = 0.f;
@@ -407,10 +407,10 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
     }
     // ---- S8: the particle-particle list ------------------------------------------------------------
     {
-        const unsigned long long o0 = P.ppoff[gi], o1 = P.ppoff[gi + 1];
-        const int n = (int)(o1 - o0);
-        const uint32_t* const pl = P.pplist + (o0 - P.ppbase);
-        const uint8_t* const pi = PER ? P.ppimg + (o0 - P.ppbase) : nullptr;
+        const unsigned long long o0 = P.ppoff[gi];
+        const int n = (int)P.lpp[gi];
+        const uint32_t* const pl = P.pplist + o0;
+        const uint8_t* const pi = PER ? P.ppimg + o0 : nullptr;
         const int nb = (n + BATCH - 1) / BATCH;
         float4 pb = make_float4(0.f, 0.f, 0.f, 0.f);
         uint32_t cnext = 0; int inext = 62, pim = 62;

@@ -48,8 +48,8 @@ struct Tree {
     int32_t *cchild = nullptr, *cparent = nullptr;
     WalkCell* wcell = nullptr;
     GroupRec* group = nullptr;
-    uint32_t *glpc = nullptr, *glpp = nullptr;   // list lengths of the last walk (glpp without the group's own bodies)
-    unsigned long long *pcoff = nullptr, *ppoff = nullptr; // [ngroups+1] exclusive scans of them
+    uint32_t *glpc = nullptr, *glpp = nullptr, *glvis = nullptr; // per group, last walk: accepted cells, listed bodies (without the group's own), cells visited
+    unsigned long long *pcoff = nullptr, *ppoff = nullptr; // [ngroups] start of each group's lists in the arena
     // hash
     int64_t hcap = 0;
     uint64_t* hkey = nullptr;
@@ -95,31 +95,38 @@ cudaError_t launch_hash_lookup(const uint64_t* hkey, const int32_t* hval, int64_
 cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st);
 
 // ---- walk (hot_walk.cu): emits the interaction lists of the groups [g0, g1) ---------------------------
+// While a group is walked its particle-particle list is kept as RUNS of bodies, first | (count-1) << 27
+// with count <= 32 (one per rejected leaf; a finest-level leaf with more bodies gives several); the
+// runs are expanded to one body index per entry when the list moves to the arena.
+#define HOT_RUN_SHIFT 27
 struct WalkArgs {
     const WalkCell* wcell; const GroupRec* group; int64_t g0, g1;
-    double theta2; int periodic;
-    uint32_t* lpc; uint32_t* lpp;                 // COUNT pass out: accepted cells / bodies of rejected leaves per group
-    const unsigned long long* pcoff; const unsigned long long* ppoff; // FILL pass in: list offsets per group (exclusive scans)
-    unsigned long long pcbase, ppbase;            // offsets of group g0 (the arena holds one chunk of groups)
-    uint32_t* pclist; uint32_t* pplist;           // FILL pass out: cell indices / body indices
-    uint8_t* pcimg; uint8_t* ppimg;               // periodic: image id (0..124) of every list entry
-    unsigned int* counter;                        // dynamic group scheduler
-    unsigned long long* stat;                     // [0] cells visited, [1] spills (COUNT pass)
-    uint32_t* gstack; int64_t gstack_cap;         // per-warp spill arena (entries per warp)
-    int* errflag;
+    unsigned long long mac_t[HOT_NLEVELS]; // accept a level-l cell iff d2 >= mac_t[l] (R-7, "MAC table")
+    int periodic;
+    uint32_t *lpc, *lpp, *lvis;            // per group: accepted cells, bodies of rejected leaves, cells visited
+    unsigned long long *pcoff, *ppoff;     // per group: where its two lists start in the arena
+    uint32_t* pclist; uint32_t* pplist;    // the arena: cell indices / body indices
+    uint8_t* pcimg; uint8_t* ppimg;        // periodic: image id (0..124) of every list entry
+    unsigned long long cappc, cappp;       // arena capacity in entries
+    unsigned long long* tops;              // [0], [1]: entries handed out so far
+    int* first_fail;                       // smallest group that did not fit the arena (INT_MAX: none)
+    uint32_t* stage; uint8_t* stage_img; int64_t stage_cap; // per-warp staging: [2][stage_cap] entries
+    unsigned int* counter;                 // dynamic group scheduler
+    unsigned long long* stat;              // [1] ring spills
+    uint32_t* gstack; int64_t gstack_cap;  // per-warp spill arena (entries per warp)
+    int* errflag;                          // bit 2: spill arena exhausted, bit 3: staging too small
 };
 int walk_grid_warps();
-cudaError_t launch_walk(const WalkArgs& a, bool fill, cudaStream_t st);
-size_t scan_scratch_elems(int64_t n);
-cudaError_t launch_scan_u32_to_u64(const uint32_t* len, int64_t n, unsigned long long* scratch, unsigned long long* off, cudaStream_t st);
-cudaError_t launch_chunk_bounds(const unsigned long long* pcoff, const unsigned long long* ppoff, int64_t ng, unsigned long long cappc,
-                                unsigned long long cappp, int64_t* bounds, int maxchunks, int* nchunks, cudaStream_t st);
+cudaError_t launch_walk(const WalkArgs& a, cudaStream_t st);
+// stat[0] += cells visited, stat[2] += sum n_G (L_pp + n_G), stat[3] += sum n_G L_pc over the groups [0, ng)
+cudaError_t launch_group_stats(const GroupRec* group, const uint32_t* lpc, const uint32_t* lpp, const uint32_t* lvis, int64_t ng,
+                               unsigned long long* stat, cudaStream_t st);
 
 // ---- interactions (hot_forces.cu): evaluates the lists of the groups [g0, g1) -------------------------
 struct ForceArgs {
     const WalkCell* wcell; const CellA* cellA; const CellM2* cellM2; const CellM34* cellM34;
     const float4* body; const uint32_t* perm; const GroupRec* group; int64_t g0, g1;
-    const unsigned long long* pcoff; const unsigned long long* ppoff; unsigned long long pcbase, ppbase;
+    const unsigned long long* pcoff; const unsigned long long* ppoff; const uint32_t* lpc; const uint32_t* lpp;
     const uint32_t* pclist; const uint32_t* pplist; const uint8_t* pcimg; const uint8_t* ppimg;
     float eps2; int order; int periodic;
     double lo[3], size;
