@@ -115,6 +115,11 @@ int hot_set_stream(void* cuda_stream); /* cudaStream_t; NULL = legacy default st
 void hot_free(void);                   /* releases everything the library owns */
 const char* hot_last_error(void);
 
+/* Host-only, needs no GPU: the 165 Taylor coefficients c_abc (a+b+c <= 8, degree-major, x exponent
+ * descending then y; odd ones are zero) of psi_sm(r) = psi(r) - sum_{|n|_inf<=2} 1/|r-n| about r = 0, in
+ * units of the box: the table of the periodic far field (p = 8, ws = 2).  coef165: host. */
+int hot_far_coefficients(double* coef165);
+
 /* ---- introspection for the parity tests: HOST output arrays, caller-allocated -------------- */
 /* sorted keys and the permutation: key_sorted[i] = key of caller's particle perm[i]; [n] each */
 int hot_export_keys(uint64_t* key_sorted, uint32_t* perm);

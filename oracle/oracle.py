@@ -167,7 +167,10 @@ class Tree:
 
     def __del__(self):
         if getattr(self, "_h", None):
-            lib().orc_destroy(self._h)
+            try:
+                lib().orc_destroy(self._h)
+            except TypeError:  # interpreter shutdown: the module globals are already gone
+                pass
             self._h = None
 
     def keys(self):

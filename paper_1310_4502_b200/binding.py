@@ -59,6 +59,7 @@ def _load():
         lib.hot_set_stream.argtypes = [C.c_void_p]
         lib.hot_set_params.argtypes = [C.c_int, C.c_int]
         lib.hot_set_list_arena.argtypes = [C.c_int64]
+        lib.hot_far_coefficients.argtypes = [C.c_void_p]
         lib.hot_free.restype = None
         lib.hot_export_keys.argtypes = [C.c_void_p, C.c_void_p]
         lib.hot_export_cells.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
@@ -89,6 +90,13 @@ def hot_set_stream(stream=None):
     """Pass a torch.cuda.Stream (or None for the legacy default stream)."""
     ptr = None if stream is None else C.c_void_p(stream.cuda_stream)
     _check(_load().hot_set_stream(ptr))
+
+
+def hot_far_coefficients() -> np.ndarray:
+    """The 165 far-field Taylor coefficients (host computation, no GPU needed)."""
+    out = np.empty(165, dtype=np.float64)
+    _check(_load().hot_far_coefficients(out.ctypes.data_as(C.c_void_p)))
+    return out
 
 
 def hot_set_list_arena(max_bytes: int = 0):

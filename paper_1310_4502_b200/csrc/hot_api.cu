@@ -32,15 +32,17 @@ struct Ctx {
     uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
     // interaction lists (hot_forces)
     unsigned long long* d_tops = nullptr;
+    double* d_farS = nullptr; // periodic: global moments of the box
     uint32_t *d_pclist = nullptr, *d_pplist = nullptr; uint8_t *d_pcimg = nullptr, *d_ppimg = nullptr;
     uint32_t* d_stage = nullptr; uint8_t* d_stage_img = nullptr; int64_t stage_cap = 0; // per-warp list staging (entries per list)
     unsigned long long arena_pc = 0, arena_pp = 0; // entries the list arena holds
     unsigned long long used_pc = 0, used_pp = 0;   // entries the last hot_forces wrote (sizes the next arena)
+    int64_t used_groups = 0;
     size_t arena_cap_bytes = 0;                     // 0 = as much as fits; else a cap (hot_set_list_arena)
     std::vector<cudaEvent_t> evx;
     bool lists_valid = false;
     hot_stats_t st{};
-    cudaEvent_t ev[8] = {};
+    cudaEvent_t ev[9] = {};
     bool ev_ready = false;
     // host staging for hot_step_host
     float *h_pos = nullptr, *h_mass = nullptr, *h_acc = nullptr, *h_pot = nullptr; int64_t h_n = 0;
@@ -139,6 +141,12 @@ int hot_set_stream(void* s) {
     return HOT_OK;
 }
 
+int hot_far_coefficients(double* coef165) {
+    if (!coef165) return fail(HOT_EINVAL, "hot_far_coefficients: NULL output");
+    far_coefficients(coef165);
+    return HOT_OK;
+}
+
 int hot_set_list_arena(int64_t max_bytes) {
     if (max_bytes < 0) return fail(HOT_EINVAL, "hot_set_list_arena: max_bytes must be >= 0");
     g.arena_cap_bytes = (size_t)max_bytes;
@@ -160,7 +168,7 @@ void hot_free(void) {
     if (g.ev_ready) { for (auto& e : g.ev) cudaEventDestroy(e); g.ev_ready = false; }
     for (auto& e : g.evx) cudaEventDestroy(e);
     g.evx.clear();
-    g.arena_pc = g.arena_pp = 0; g.used_pc = g.used_pp = 0; g.stage_cap = 0;
+    g.arena_pc = g.arena_pp = 0; g.used_pc = g.used_pp = 0; g.used_groups = 0; g.stage_cap = 0;
     cudaFreeHost(g.h_pos); cudaFreeHost(g.h_mass); cudaFreeHost(g.h_acc); cudaFreeHost(g.h_pot);
     cudaFree(g.hd_pos); cudaFree(g.hd_mass); cudaFree(g.hd_acc); cudaFree(g.hd_pot);
     g.h_pos = g.h_mass = g.h_acc = g.h_pot = nullptr; g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
@@ -295,6 +303,22 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     }
     CUDA_TRY(cudaEventRecord(g.ev[6], st));
     int rc = HOT_OK;
+    // P2/P3: what the 125 explicit boxes leave of the periodic sum, and the background (hot_periodic.cu);
+    // per body in fp64, added by the interaction kernel before its one rounding to fp32
+    if (t.periodic) {
+        if (!t.far_ready) { // global moments of the box: once per build
+            CUDA_TRY(tree_alloc(&g.d_farS, 165));
+            CUDA_TRY(tree_alloc(&t.far, 4 * (size_t)t.n));
+            CUDA_TRY(launch_far_moments(t, g.d_farS, st));
+            double S[165];
+            CUDA_TRY(cudaMemcpyAsync(S, g.d_farS, sizeof(S), cudaMemcpyDeviceToHost, st));
+            CUDA_TRY(cudaStreamSynchronize(st));
+            far_sink_polynomial(S, t.farD);
+            t.far_ready = true;
+        }
+        CUDA_TRY(launch_far_eval(t, t.farD, t.far, st));
+    }
+    CUDA_TRY(cudaEventRecord(g.ev[8], st));
     // S7: the walk writes every group's lists into the arena; S8/S9/S10 evaluate them.  The arena is
     // sized from the previous call (first call: a guess); if it is too small the walk reports the
     // first group that did not fit, the groups before it are evaluated and the walk goes on from there.
@@ -357,7 +381,17 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic;
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
+    a.far = t.periodic ? t.far : nullptr;
     a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
+    // groups per round: all of them unless the arena is known (or found) to be too small.  The warps
+    // take arena slices in completion order, so in an overfull round the FIRST group may be among
+    // those that fail: then the round is repeated with a quarter of the groups.
+    int64_t budget = ng;
+    if (g.used_pc + g.used_pp > 0 && g.used_groups > 0) {
+        const double per_group = (double)(g.used_pc + g.used_pp) / (double)g.used_groups;
+        const double fit = 0.85 * (double)(cappc + cappp) / (per_group > 1.0 ? per_group : 1.0);
+        if (fit < (double)ng) budget = fit < 1.0 ? 1 : (int64_t)fit;
+    }
     int64_t g0 = 0;
     size_t nrounds = 0;
     unsigned long long usedpc = 0, usedpp = 0;
@@ -368,7 +402,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
         CUDA_TRY(cudaMemsetAsync(g.d_tops, 0, 2 * sizeof(unsigned long long), st));
         CUDA_TRY(cudaMemcpyAsync(g.d_flags + 3, &ff0, sizeof(int), cudaMemcpyHostToDevice, st));
-        wa.g0 = g0;
+        wa.g0 = g0; wa.g1 = g0 + budget < ng ? g0 + budget : ng;
         wa.pclist = g.d_pclist; wa.pplist = g.d_pplist; wa.pcimg = g.d_pcimg; wa.ppimg = g.d_ppimg; wa.cappc = cappc; wa.cappp = cappp;
         wa.stage = g.d_stage; wa.stage_img = g.d_stage_img; wa.stage_cap = g.stage_cap;
         CUDA_TRY(cudaEventRecord(g.evx[0], st));
@@ -388,8 +422,9 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
             CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
             continue;
         }
-        const int64_t F = fl[1] < ng ? (int64_t)fl[1] : ng;
-        if (F == g0) { // not even one group fits: enlarge the arena if memory allows
+        const int64_t F = fl[1] < wa.g1 ? (int64_t)fl[1] : wa.g1;
+        if (F == g0 && wa.g1 - g0 > 1) { budget = (wa.g1 - g0) / 4 > 1 ? (wa.g1 - g0) / 4 : 1; continue; }
+        if (F == g0) { // one group alone does not fit: enlarge the arena if memory allows
             const unsigned long long oldpc = cappc, oldpp = cappp;
             cappc *= 2; cappp *= 2;
             rc = clamp_arena(); if (rc) return rc;
@@ -406,6 +441,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         CUDA_TRY(launch_forces(a, st));
         CUDA_TRY(cudaEventRecord(g.evx[2], st));
         if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[1], g.evx[2]); } // the arena is reused
+        if (F < wa.g1) budget = F - g0; // what fitted this time is a good guess for the next round
         g0 = F;
         ++nrounds;
     }
@@ -415,14 +451,14 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     ms_eval += ms_between(g.evx[1], g.evx[2]);
-    g.used_pc = usedpc; g.used_pp = usedpp; // sizes the arena of the next call
+    g.used_pc = usedpc; g.used_pp = usedpp; g.used_groups = ng; // sizes the arena of the next call
     hot_stats_t& s = g.st;
     s.order = order;
     s.cells_visited = stat[0]; s.walk_spills = stat[1]; s.pp_interactions = stat[2]; s.pc_interactions = stat[3];
     s.ms_moments = ms_between(g.ev[5], g.ev[6]);
     s.ms_walk = ms_walk;
     s.ms_eval = ms_eval;
-    s.ms_farfield = 0;
+    s.ms_farfield = ms_between(g.ev[6], g.ev[8]);
     s.ms_forces_total = ms_between(g.ev[5], g.ev[7]);
     s.list_chunks = (int32_t)nrounds; s.list_entries = usedpc + usedpp;
     s.bytes_allocated = g.bytes + (int64_t)g.gstack_bytes;

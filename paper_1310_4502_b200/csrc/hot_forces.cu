@@ -470,12 +470,16 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
 #pragma unroll
             for (int k = 0; k < 4; ++k) A[i][k] += __shfl_xor_sync(FULL, A[i][k], off);
     }
-    // S10: results to the caller's particle order
+    // S10: results to the caller's particle order (periodic: plus the far field, still in fp64)
     if (strm == 0) {
 #pragma unroll
         for (int i = 0; i < S; ++i) {
             if (sk.me[i] >= 0) {
                 const uint32_t o = P.perm[g.first + sk.me[i]];
+                if (PER) {
+                    const double4 f = reinterpret_cast<const double4*>(P.far)[g.first + sk.me[i]];
+                    A[i][0] += f.x; A[i][1] += f.y; A[i][2] += f.z; A[i][3] += f.w;
+                }
                 P.acc[3 * (int64_t)o] = (float)A[i][0];
                 P.acc[3 * (int64_t)o + 1] = (float)A[i][1];
                 P.acc[3 * (int64_t)o + 2] = (float)A[i][2];

@@ -55,6 +55,10 @@ struct Tree {
     uint64_t* hkey = nullptr;
     int32_t* hval = nullptr;
     int hash_max_probe = 0;
+    // periodic far field: polynomial of the sink position (hot_periodic.cu)
+    bool far_ready = false;
+    double farD[165];
+    double* far = nullptr;                   // [n][4] far field per body, key order
     // moments
     int mom_order = -1;
     CellA* cellA = nullptr;
@@ -128,6 +132,7 @@ struct ForceArgs {
     const float4* body; const uint32_t* perm; const GroupRec* group; int64_t g0, g1;
     const unsigned long long* pcoff; const unsigned long long* ppoff; const uint32_t* lpc; const uint32_t* lpp;
     const uint32_t* pclist; const uint32_t* pplist; const uint8_t* pcimg; const uint8_t* ppimg;
+    const double* far;            // periodic: far field (ax, ay, az, phi) per body in key order, added in fp64; else NULL
     float eps2; int order; int periodic;
     double lo[3], size;
     float* acc; float* pot;
@@ -135,5 +140,8 @@ struct ForceArgs {
 };
 cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st);
 
-// ---- periodic far field (hot_periodic.cu) -----------------------------------------------------
-cudaError_t launch_farfield(const Tree& t, double* scratch, float* acc, float* pot, cudaStream_t st);
+// ---- periodic far field (hot_periodic.cu) ------------------------------------------------------------
+void far_coefficients(double* out165);                    // host: Taylor coefficients of psi_sm, degree-major
+void far_sink_polynomial(const double* S, double* D);     // host: per-sink polynomial from the global moments
+cudaError_t launch_far_moments(const Tree& t, double* S /*device [165]*/, cudaStream_t st);
+cudaError_t launch_far_eval(const Tree& t, const double* D /*host [165]*/, double* far /*device [n][4], key order*/, cudaStream_t st);

@@ -89,3 +89,33 @@ def test_workloads_are_seeded_and_inside_their_boxes():
         t = (a.pos - lo) * np.float32(1.0 / a.size)
         assert (t >= 0).all() and (t < 1).all()
         assert abs(a.mass.astype(np.float64).sum() - 1.0) < 1e-6
+
+
+def test_far_field_table_host_only():
+    """hot_far_coefficients needs no GPU.  The library derives the table from four axis Taylor
+    coefficients and the cubic harmonics; the oracle sums all 35 tensor derivatives (SURVEY C-9).
+    They share no code, so agreement pins both; C0 and the background term are closed forms."""
+    import numpy as np
+
+    from oracle import oracle as O
+    from paper_1310_4502_b200 import binding
+
+    c = binding.hot_far_coefficients()
+    assert c.shape == (165,)
+    assert abs(c[0] - (-60.02450803)) < 1e-7                      # psi_sm(0), SURVEY 8(a) P3
+    assert np.allclose(c[[4, 7, 9]], 2.0 * np.pi / 3.0, rtol=1e-14)  # the uniform background
+    T = O.Tree(np.array([[0.5, 0.5, 0.5]], np.float32), np.array([1.0], np.float32), (0.0, 0.0, 0.0), 1.0, periodic=True)
+    o = T.far_table()
+    assert np.abs(c - o).max() < 1e-11
+    # laplace(psi_sm) = 4 pi: every degree >= 4 part is harmonic
+    k, idx = 0, {}
+    for d in range(9):
+        for a in range(d, -1, -1):
+            for b in range(d - a, -1, -1):
+                idx[(a, b, d - a - b)] = k
+                k += 1
+    for (a, b, cc), k in idx.items():
+        if a + b + cc in (2, 4, 6):  # coefficient of x^a y^b z^c in the Laplacian of the degree+2 part
+            lap = ((a + 2) * (a + 1) * c[idx[(a + 2, b, cc)]] + (b + 2) * (b + 1) * c[idx[(a, b + 2, cc)]]
+                   + (cc + 2) * (cc + 1) * c[idx[(a, b, cc + 2)]])
+            assert abs(lap) < 1e-12, (a, b, cc, lap)

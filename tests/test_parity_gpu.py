@@ -237,3 +237,89 @@ def test_runs_on_a_user_stream(hot):
     finally:
         hot.hot_set_stream(None)
     assert torch.equal(a0, a1) and torch.equal(p0, p1)
+
+
+# ---- periodic boxes: 125 explicit image boxes + far field (R-9) -------------
+PERIODIC_CASES = [  # cfg, lattice side, order, theta
+    (3, 16, 4, 0.5),   # BASELINE configs[3] replica (Zel'dovich lattice, rms 0.3 cells, hexadecapole)
+    (3, 24, 2, 0.5),
+    (4, 16, 2, 0.5),   # BASELINE configs[4] replica (rms 2 cells, quadrupole)
+    (4, 12, 0, 0.7),
+]
+
+
+@pytest.mark.parametrize("cfg,side,order,theta", PERIODIC_CASES)
+def test_periodic_parity(hot, cfg, side, order, theta):
+    w = W.config(cfg, side)
+    assert w.periodic
+    _build(hot, w)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=True)
+    _check_int_artefacts(hot, T)
+    acc, pot = hot.hot_forces(theta, w.eps, order)
+    gg = hot.hot_export_groups()
+    rng = np.random.default_rng(3)
+    sel = np.sort(rng.choice(T.ngroups, min(T.ngroups, 48), replace=False))
+    oa, op, lpc, lpp = T.forces(theta, w.eps, order, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all(), "L_pc summed over the 125 images"
+    assert (gg["lpp"][sel] == lpp.astype(np.uint64)).all(), "L_pp summed over the 125 images"
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]
+    gp = pot.cpu().numpy().astype(np.float64)[m]
+    # a nearly uniform lattice has net forces far below the individual terms: normalise the
+    # acceleration error by the rms acceleration of the set as well
+    arms = np.sqrt((oa[m] ** 2).sum(axis=1).mean())
+    en = np.linalg.norm(ga - oa[m], axis=1) / arms
+    ea = np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    assert np.median(en) <= 1e-5 and np.quantile(en, 0.999) <= 1e-4, (np.median(en), np.quantile(en, 0.999))
+    # the periodic potential is the difference of the explicit image sum, at least
+    # sum_{0<|n|_inf<=2} 1/|n| = 57.187 M/L per body, and the far field -60.02 M/L: fp32 interactions
+    # bound its ABSOLUTE error by that scale, so the relative error is taken against it (R-13)
+    scale = 57.18721055 * float(w.mass.astype(np.float64).sum()) / w.size
+    ep = np.abs(gp - op[m]) / (np.abs(op[m]) + scale)
+    assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
+    assert np.abs(gp - op[m]).max() <= 2e-7 * scale
+    st = hot.hot_stats()
+    assert st["periodic"] == 1 and st["ms_farfield"] > 0
+
+
+def test_periodic_single_body_and_perfect_lattice(hot):
+    """Pins of SURVEY C-9 (O-P1) on the GPU path: one body feels no force and the potential
+    -m xi / L; a perfect K^3 lattice of equal masses has zero force and phi = -xi / K^2 (eps -> 0)."""
+    import torch
+
+    xi = -2.8372974794806
+    hot.hot_set_params(16, 64)
+    pos = torch.tensor([[0.3, 0.6, 0.2]], dtype=torch.float32).cuda()
+    mass = torch.tensor([2.0], dtype=torch.float32).cuda()
+    hot.hot_build(pos, mass, (0.0, 0.0, 0.0), 1.0, True)
+    acc, pot = hot.hot_forces(0.5, 0.0, 4)
+    assert np.abs(acc.cpu().numpy()).max() < 2e-5
+    assert abs(pot.item() - (-2.0 * xi)) < 2e-5 * 2.0 * abs(xi)
+    for K in (2, 3):
+        q = (np.arange(K) + 0.5) / K
+        g = np.stack(np.meshgrid(q, q, q, indexing="ij"), axis=-1).reshape(-1, 3).astype(np.float32)
+        pos = torch.from_numpy(g).cuda()
+        mass = torch.full((K ** 3,), 1.0 / K ** 3, dtype=torch.float32).cuda()
+        hot.hot_build(pos, mass, (0.0, 0.0, 0.0), 1.0, True)
+        acc, pot = hot.hot_forces(0.5, 0.0, 4)
+        assert np.abs(acc.cpu().numpy()).max() < 5e-5
+        assert np.allclose(pot.cpu().numpy(), -xi / K ** 2, rtol=3e-5)
+
+
+def test_small_list_arena_gives_the_same_result_in_rounds(hot):
+    """hot_set_list_arena: when the lists do not fit, groups are walked and evaluated in rounds."""
+    w = W.config(2, 15)
+    _build(hot, w)
+    acc0, pot0 = hot.hot_forces(0.6, w.eps, 2)
+    entries = hot.hot_stats()["list_entries"]
+    try:
+        hot.hot_set_list_arena(max(1 << 16, int(entries * 4 / 5)))  # bytes: a fifth of what all lists need
+        _build(hot, w)
+        acc1, pot1 = hot.hot_forces(0.6, w.eps, 2)
+        st = hot.hot_stats()
+        assert st["list_chunks"] >= 3
+        assert (acc1 == acc0).all() and (pot1 == pot0).all()
+    finally:
+        hot.hot_set_list_arena(0)
+        hot.hot_free()
