@@ -25,9 +25,17 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 # flops per interaction counted from the library's own inner loops:
-# FFMA = 2, FADD/FMUL = 1, rsqrt = 1.
+# FMA = 2, add / multiply = 1, rsqrt = 1; a packed f32x2 instruction counts once per lane-operation.
+#   P-P:          4 add + 3 mul + 6 fma + rsqrt            = 20
+#   P-C order 0:  3 add + 3 mul + 7 fma + rsqrt            = 21
+#   P-C order 2:  6 add + 12 mul + 20 fma + rsqrt          = 59
+#   P-C order 4: 12 add + 73 mul + 95 fma + rsqrt          = 276
 FLOPS_PP = 20
-FLOPS_PC = {0: 20, 2: 62, 4: 275}
+FLOPS_PC = {0: 21, 2: 59, 4: 276}
+# DRAM bytes of one forces_kernel launch from the ncu --set full capture of the default workload
+# (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 13.342 GB + dram__bytes_write.sum 1.197 GB;
+# the lists alone are 4 B x 2.92e9 entries = 11.7 GB of compulsory reads); other workloads: null
+NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2): 14.538e9}
 # FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
@@ -123,14 +131,14 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def cpu_oracle_sample(args, w_full, budget_s=12.0):
+def cpu_oracle_sample(args, w_full, budget_s=15.0):
     """The oracle as it stands, whole path, on a smaller replica of the same workload."""
     import numpy as np
 
     from oracle import oracle as O
     from paper_1310_4502_b200 import workloads as W
 
-    scale = {0: 14, 1: 16, 2: 16, 3: 32, 4: 32}[args.config]
+    scale = {0: 14, 1: 18, 2: 18, 3: 32, 4: 32}[args.config]
     if args.scale is not None:
         scale = min(scale, args.scale)
     w = W.config(args.config, scale)
@@ -242,7 +250,7 @@ def main():
     for _ in range(args.steps):
         step()
         st = hot.hot_stats()
-        for k in ("ms_keygen", "ms_sort", "ms_gather", "ms_tree", "ms_moments", "ms_walk", "ms_eval", "ms_farfield",
+        for k in ("ms_keygen", "ms_sort", "ms_gather", "ms_tree", "ms_moments", "ms_farfield", "ms_walk", "ms_eval",
                   "ms_build_total", "ms_forces_total"):
             stage[k] = stage.get(k, 0.0) + st[k] / args.steps
     e1.record()
@@ -284,6 +292,8 @@ def main():
     flops = st["pp_interactions"] * FLOPS_PP + st["pc_interactions"] * FLOPS_PC[w.order]
     kern_s = stage["ms_eval"] * 1e-3
     achieved = flops / kern_s / 1e12
+    tf_scalar, tf_packed = hot.hot_measure_fp32()  # register-only FMA chains on this device, after the timed region
+    traffic = NCU_TRAFFIC_BYTES.get(("c%d" % args.config, int(round(np.log2(w.n))), w.theta, w.order))
     out = {
         "metric": "interactions_per_second", "value": inter_all / (ms_max * 1e-3) / 1e9, "unit": "Ginteractions/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_max,
@@ -295,18 +305,25 @@ def main():
         "kernel_only_Ginteractions_per_s": inter / kern_s / 1e9,
         "stages_ms": {k: round(v, 4) for k, v in stage.items()},
         "tree": {"n_cells": st["n_cells"], "n_groups": st["n_groups"], "max_level": st["max_level"],
-                 "cells_visited": st["cells_visited"], "walk_spills": st["walk_spills"]},
+                 "cells_visited": st["cells_visited"], "walk_spills": st["walk_spills"],
+                 "list_entries": st["list_entries"], "list_rounds": st["list_chunks"]},
         "hbm_stages": {
             "keygen_GBps": KEYGEN_BYTES_PER_BODY * w.n / (stage["ms_keygen"] * 1e-3) / 1e9,
             "sort_GBps": SORT_BYTES_PER_BODY * w.n / (stage["ms_sort"] * 1e-3) / 1e9,
-            "gather_GBps": GATHER_BYTES_PER_BODY * w.n / (stage["ms_gather"] * 1e-3) / 1e9},
+            "gather_GBps": GATHER_BYTES_PER_BODY * w.n / (stage["ms_gather"] * 1e-3) / 1e9,
+            "walk_list_GBps": 2 * 4 * st["list_entries"] / (stage["ms_walk"] * 1e-3) / 1e9,
+            "walk_Gcells_per_s": st["cells_visited"] / (stage["ms_walk"] * 1e-3) / 1e9},
         "gpu_launches": int((st["launches_build"] + st["launches_forces"]) * args.steps),
         "clocks": clocks,
-        "roofline": {"bound": "alu", "kernel": "forces_kernel (P-P + P-C interaction lists of all sink groups)", "achieved": achieved,
-                     "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS, "traffic": None,
-                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
+        "roofline": {"bound": "alu", "kernel": "forces_kernel (P-P + P-C interaction lists of all sink groups, packed f32x2)",
+                     "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s", "frac": achieved / FP32_PEAK_TFLOPS,
+                     "traffic": traffic,
+                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md Roofline); "
+                                    "MEASURED_PEAKS.json holds no FP32 figure",
+                     "peak_measured_ffma_TFLOPs": {"scalar": tf_scalar, "packed_f32x2": tf_packed},
+                     "frac_of_measured_ffma": achieved / max(tf_scalar, tf_packed),
                      "flops_per_interaction": {"pp": FLOPS_PP, "pc": FLOPS_PC[w.order]},
-                     "kernel_ms": stage["ms_eval"]},
+                     "kernel_ms": stage["ms_eval"], "kernel_share_of_step": stage["ms_eval"] / ms_max},
     }
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))

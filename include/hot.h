@@ -115,6 +115,11 @@ int hot_set_stream(void* cuda_stream); /* cudaStream_t; NULL = legacy default st
 void hot_free(void);                   /* releases everything the library owns */
 const char* hot_last_error(void);
 
+/* Roofline denominator of the interaction kernels measured on the current device: TFLOP/s of a
+ * register-only fused-multiply-add chain, scalar (FFMA) and packed pairs (FFMA2); FMA = 2 flops.
+ * ~10 ms of device time on the library's stream.  Outputs: host. */
+int hot_measure_fp32(double* tflops_scalar, double* tflops_packed);
+
 /* Host-only, needs no GPU: the 165 Taylor coefficients c_abc (a+b+c <= 8, degree-major, x exponent
  * descending then y; odd ones are zero) of psi_sm(r) = psi(r) - sum_{|n|_inf<=2} 1/|r-n| about r = 0, in
  * units of the box: the table of the periodic far field (p = 8, ws = 2).  coef165: host. */

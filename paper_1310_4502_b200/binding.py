@@ -60,6 +60,7 @@ def _load():
         lib.hot_set_params.argtypes = [C.c_int, C.c_int]
         lib.hot_set_list_arena.argtypes = [C.c_int64]
         lib.hot_far_coefficients.argtypes = [C.c_void_p]
+        lib.hot_measure_fp32.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         lib.hot_free.restype = None
         lib.hot_export_keys.argtypes = [C.c_void_p, C.c_void_p]
         lib.hot_export_cells.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
@@ -90,6 +91,13 @@ def hot_set_stream(stream=None):
     """Pass a torch.cuda.Stream (or None for the legacy default stream)."""
     ptr = None if stream is None else C.c_void_p(stream.cuda_stream)
     _check(_load().hot_set_stream(ptr))
+
+
+def hot_measure_fp32():
+    """(scalar FFMA, packed FFMA2) TFLOP/s of a register-only FMA chain on the current device."""
+    a, b = C.c_double(), C.c_double()
+    _check(_load().hot_measure_fp32(C.byref(a), C.byref(b)))
+    return a.value, b.value
 
 
 def hot_far_coefficients() -> np.ndarray:

@@ -141,6 +141,12 @@ int hot_set_stream(void* s) {
     return HOT_OK;
 }
 
+int hot_measure_fp32(double* tflops_scalar, double* tflops_packed) {
+    if (!tflops_scalar || !tflops_packed) return fail(HOT_EINVAL, "hot_measure_fp32: NULL output");
+    CUDA_TRY(measure_fp32(tflops_scalar, tflops_packed, g.stream));
+    return HOT_OK;
+}
+
 int hot_far_coefficients(double* coef165) {
     if (!coef165) return fail(HOT_EINVAL, "hot_far_coefficients: NULL output");
     far_coefficients(coef165);

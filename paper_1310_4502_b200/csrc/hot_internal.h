@@ -145,3 +145,6 @@ void far_coefficients(double* out165);                    // host: Taylor coeffi
 void far_sink_polynomial(const double* S, double* D);     // host: per-sink polynomial from the global moments
 cudaError_t launch_far_moments(const Tree& t, double* S /*device [165]*/, cudaStream_t st);
 cudaError_t launch_far_eval(const Tree& t, const double* D /*host [165]*/, double* far /*device [n][4], key order*/, cudaStream_t st);
+
+// ---- FP32 roofline denominator measured on the device (hot_peak.cu) ------------------------------------
+cudaError_t measure_fp32(double* tf_scalar, double* tf_packed, cudaStream_t st);
