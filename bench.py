@@ -191,6 +191,18 @@ def run_reference(args):
     print(json.dumps(out))
 
 
+def reduce_over_ranks(dist, ms, inter, device):
+    """Whole-job figures of N independent replicas: the slowest rank's time, the interactions of all."""
+    import torch
+
+    tms = torch.tensor([ms], dtype=torch.float64, device=device)
+    tint = torch.tensor([float(inter)], dtype=torch.float64, device=device)
+    if dist is not None:
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        dist.all_reduce(tint, op=dist.ReduceOp.SUM)
+    return float(tms.item()), float(tint.item())
+
+
 def config_dict(args, w):
     return {"workload": f"BASELINE.json configs[{args.config}]: {w.name}, n={w.n}, "
                         f"{'periodic' if w.periodic else 'open'}, eps={w.eps:g}, theta={w.theta:g}, order={w.order}",
@@ -259,12 +271,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     st = hot.hot_stats()
     inter = st["pp_interactions"] + st["pc_interactions"]
-    tms = torch.tensor([ms], dtype=torch.float64, device="cuda")
-    tint = torch.tensor([float(inter)], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
-        dist.all_reduce(tint, op=dist.ReduceOp.SUM)
-    ms_max, inter_all = float(tms.item()), float(tint.item())
+    ms_max, inter_all = reduce_over_ranks(dist, ms, inter, "cuda")
 
     # end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     e2e = None
