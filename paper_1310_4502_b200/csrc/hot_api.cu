@@ -37,7 +37,7 @@ struct Ctx {
     uint32_t* d_stage = nullptr; uint8_t* d_stage_img = nullptr; int64_t stage_cap = 0; // per-warp list staging (entries per list)
     unsigned long long arena_pc = 0, arena_pp = 0; // entries the list arena holds
     unsigned long long used_pc = 0, used_pp = 0;   // entries the last hot_forces wrote (sizes the next arena)
-    int64_t used_groups = 0;
+    int64_t used_groups = 0, last_n = 0; int last_periodic = -1;
     size_t arena_cap_bytes = 0;                     // 0 = as much as fits; else a cap (hot_set_list_arena)
     std::vector<cudaEvent_t> evx;
     bool lists_valid = false;
@@ -191,6 +191,8 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     if (rc) return rc;
     drop_build();
     g_hot_launches = 0;
+    if (g.last_n != n || g.last_periodic != periodic) { g.used_pc = g.used_pp = 0; g.used_groups = 0; } // another problem: forget its list sizes
+    g.last_n = n; g.last_periodic = periodic;
     Tree& t = g.t;
     t.n = n; t.periodic = periodic; t.nleaf = g.nleaf; t.ncrit = g.ncrit; t.box = box;
     for (int k = 0; k < 3; ++k) t.lo[k] = (double)box.lo[k];
@@ -402,7 +404,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     size_t nrounds = 0;
     unsigned long long usedpc = 0, usedpp = 0;
     float ms_walk = 0, ms_eval = 0;
-    if (g.evx.size() < 3) { while (g.evx.size() < 3) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
+    if (g.evx.size() < 4) { while (g.evx.size() < 4) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
     while (g0 < ng) {
         const int ff0 = INT_MAX;
         CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
@@ -444,10 +446,19 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         usedpc += tops[0]; usedpp += tops[1];
         a.g0 = g0; a.g1 = F;
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
+        CUDA_TRY(cudaEventRecord(g.evx[3], st));
         CUDA_TRY(launch_forces(a, st));
         CUDA_TRY(cudaEventRecord(g.evx[2], st));
-        if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[1], g.evx[2]); } // the arena is reused
-        if (F < wa.g1) budget = F - g0; // what fitted this time is a good guess for the next round
+        if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[3], g.evx[2]); } // the arena is reused
+        if (F < wa.g1) { // the arena was too small: enlarge it if memory allows, else keep going in rounds of what fitted
+            const unsigned long long oldpc = cappc, oldpp = cappp;
+            cappc *= 2; cappp *= 2;
+            rc = clamp_arena(); if (rc) return rc;
+            if (cappc < oldpc) cappc = oldpc;
+            if (cappp < oldpp) cappp = oldpp;
+            if (cappc > oldpc || cappp > oldpp) { rc = alloc_lists(); if (rc) return rc; }
+            budget = (F - g0) * (int64_t)((cappc + cappp) / (oldpc + oldpp));
+        }
         g0 = F;
         ++nrounds;
     }
@@ -456,7 +467,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     unsigned long long stat[4];
     CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
-    ms_eval += ms_between(g.evx[1], g.evx[2]);
+    ms_eval += ms_between(g.evx[3], g.evx[2]);
     g.used_pc = usedpc; g.used_pp = usedpp; g.used_groups = ng; // sizes the arena of the next call
     hot_stats_t& s = g.st;
     s.order = order;

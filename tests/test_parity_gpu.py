@@ -323,3 +323,42 @@ def test_small_list_arena_gives_the_same_result_in_rounds(hot):
     finally:
         hot.hot_set_list_arena(0)
         hot.hot_free()
+
+
+# ---- BASELINE.json's full sizes, in the configuration bench.py times, on sampled sink groups -----------
+@pytest.mark.slow
+@pytest.mark.parametrize("cfg,order,theta,nsel", [(2, 2, 0.6, 96), (1, 2, 0.5, 96), (3, 4, 0.5, 24)])
+def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
+    """configs[2] at N = 2^24 (the bench workload), configs[1] at 2^20, configs[3] at 256^3 periodic:
+    integer artefacts in full, forces and list counts on a seeded sample of sink groups (the oracle
+    evaluates a group in milliseconds, the whole set would take hours)."""
+    w = W.config(cfg)
+    _build(hot, w)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic)
+    _check_int_artefacts(hot, T)
+    acc, pot = hot.hot_forces(theta, w.eps, order)
+    gg = hot.hot_export_groups()
+    sel = np.sort(np.random.default_rng(5).choice(T.ngroups, nsel, replace=False))
+    oa, op, lpc, lpp = T.forces(theta, w.eps, order, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]
+    gp = pot.cpu().numpy().astype(np.float64)[m]
+    mtot = float(w.mass.astype(np.float64).sum())
+    scale = 57.18721055 * mtot / w.size if w.periodic else 0.0
+    # periodic: a body's acceleration is what is left of the pull of the 5^3 explicit boxes towards their
+    # centre, (4 pi / 3)(M / L^3) x with |x| up to L/2, after the far field cancels it; fp32 bounds the absolute
+    # error by ~1e-7 of that scale, which on a 256^3 lattice is 2.5e-5 of the net acceleration (DESIGN.md R-14)
+    ascale = (4.0 * np.pi / 3.0) * mtot / w.size ** 2 * 0.5 if w.periodic else 0.0
+    ea = np.linalg.norm(ga - oa[m], axis=1) / (np.linalg.norm(oa[m], axis=1) + ascale)
+    ep = np.abs(gp - op[m]) / (np.abs(op[m]) + scale)
+    print("full-size parity", cfg, "acc median", np.median(ea), "p99.9", np.quantile(ea, 0.999), "plain relative median",
+          np.median(np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)))
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
+    # coverage invariant at full size: every body is in exactly one list entry's range per image
+    cnt = T.cells()["count"]
+    st = hot.hot_stats()
+    assert st["n"] == w.n and st["pp_interactions"] > 0 and st["pc_interactions"] > 0
+    assert np.isfinite(acc.cpu().numpy()).all() and np.isfinite(pot.cpu().numpy()).all()
+    del cnt
