@@ -55,7 +55,7 @@ def parse():
     ap.add_argument("--theta", type=float, default=None)
     ap.add_argument("--order", type=int, default=None)
     ap.add_argument("--nleaf", type=int, default=16)
-    ap.add_argument("--ncrit", type=int, default=64)
+    ap.add_argument("--ncrit", type=int, default=256)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()

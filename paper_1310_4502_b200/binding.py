@@ -112,7 +112,7 @@ def hot_set_list_arena(max_bytes: int = 0):
     _check(_load().hot_set_list_arena(int(max_bytes)))
 
 
-def hot_set_params(nleaf: int = 16, ncrit: int = 64):
+def hot_set_params(nleaf: int = 16, ncrit: int = 256):
     _check(_load().hot_set_params(int(nleaf), int(ncrit)))
 
 

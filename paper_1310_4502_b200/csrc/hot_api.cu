@@ -16,7 +16,7 @@ struct Ctx {
     cudaStream_t stream = nullptr;
     Tree t;
     bool built = false;
-    int nleaf = 16, ncrit = 64;
+    int nleaf = 16, ncrit = 256;
     int last_order = -1;
     char err[512] = "";
     // scratch owned across calls

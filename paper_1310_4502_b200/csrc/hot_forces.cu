@@ -5,7 +5,7 @@
 // dynamic group counter) and evaluates its lists in the m x n blocking of PAPER.md:162-164:
 //
 //   The 32 lanes are split into K = 32/L "source streams" of L lanes.  Every stream holds ALL sinks
-//   of the group in registers (S = ceil(n/L) <= SMAX per lane) and takes every K-th source of a
+//   of the group in registers (S = ceil(n/L) <= SMAX = 6 per lane) and takes every K-th source of a
 //   32-source batch, read from shared memory as broadcast 128-bit loads.  L is the smallest power of
 //   two with ceil(n/L) <= SMAX, so at most L-1 of the L*S sink slots idle whatever the group size;
 //   the K partial sums are combined with shuffles once per group.
@@ -23,11 +23,11 @@
 #define BATCH 32               // sources per staged batch
 #define WARPS_PER_BLOCK 4
 #ifndef HOT_SMAX
-#define HOT_SMAX 4             // sinks per lane (tunable: 4..8)
+#define HOT_SMAX 6             // sinks per lane (tunable 2..8; 6 at 3 blocks/SM measured best with NCRIT >= 128)
 #endif
 #define SMAX HOT_SMAX
 #ifndef HOT_MINBLK
-#define HOT_MINBLK 4           // resident blocks per SM the order 0/2 kernels are compiled for
+#define HOT_MINBLK 3           // resident blocks per SM the order 0/2 kernels are compiled for
 #endif
 #ifndef HOT_UNROLL2
 #define HOT_UNROLL2 0          // evaluate two sources per loop trip (more independent chains, more registers)
@@ -498,7 +498,8 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MIN
         const int64_t gi = P.g0 + (int64_t)__shfl_sync(FULL, q, 0);
         if (gi >= P.g1) break;
         const GroupRec g = P.group[gi];
-        // sinks in chunks of at most 32*SMAX (only groups larger than that need more than one pass)
+        // sinks in chunks of at most 32*SMAX (only groups larger than that need more than one pass; full
+        // chunks first: 6 sinks per lane is the most efficient blocking, measured against an even split)
         for (uint32_t c0 = 0; c0 < g.count; c0 += 32 * SMAX) {
             const uint32_t nc = min((uint32_t)(32 * SMAX), g.count - c0);
             int lgL = 0;

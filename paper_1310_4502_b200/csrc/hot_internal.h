@@ -31,7 +31,7 @@ struct GroupRec { uint32_t first, count, cell, pad; };
 
 struct Tree {
     int64_t n = 0;
-    int periodic = 0, nleaf = 16, ncrit = 64;
+    int periodic = 0, nleaf = 16, ncrit = 256;
     hot_box box{};
     double lo[3], size;
     // bodies

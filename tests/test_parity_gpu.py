@@ -63,6 +63,9 @@ CASES = [  # cfg, scale, nleaf, ncrit, order, theta
     (2, 15, 8, 128, 2, 0.8),
     (1, 14, 4, 32, 4, 0.6),
     (0, 11, 32, 256, 2, 0.5),
+    (2, 16, 16, 256, 2, 0.6),    # the library's default bucket sizes: 5-6 sinks per lane, two-chunk groups
+    (1, 15, 16, 256, 4, 0.5),
+    (2, 15, 16, 192, 0, 0.7),
 ]
 
 
@@ -240,7 +243,7 @@ def test_runs_on_a_user_stream(hot):
 
 
 # ---- periodic boxes: 125 explicit image boxes + far field (R-9) -------------
-PERIODIC_CASES = [  # cfg, lattice side, order, theta
+PERIODIC_CASES = [  # cfg, lattice side, order, theta (+ one case at the default bucket sizes below)
     (3, 16, 4, 0.5),   # BASELINE configs[3] replica (Zel'dovich lattice, rms 0.3 cells, hexadecapole)
     (3, 24, 2, 0.5),
     (4, 16, 2, 0.5),   # BASELINE configs[4] replica (rms 2 cells, quadrupole)
@@ -252,8 +255,9 @@ PERIODIC_CASES = [  # cfg, lattice side, order, theta
 def test_periodic_parity(hot, cfg, side, order, theta):
     w = W.config(cfg, side)
     assert w.periodic
-    _build(hot, w)
-    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=True)
+    ncrit = 256 if (cfg, side) == (4, 16) else 64
+    _build(hot, w, 16, ncrit)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=True, nleaf=16, ncrit=ncrit)
     _check_int_artefacts(hot, T)
     acc, pot = hot.hot_forces(theta, w.eps, order)
     gg = hot.hot_export_groups()
@@ -333,8 +337,8 @@ def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
     integer artefacts in full, forces and list counts on a seeded sample of sink groups (the oracle
     evaluates a group in milliseconds, the whole set would take hours)."""
     w = W.config(cfg)
-    _build(hot, w)
-    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic)
+    _build(hot, w, 16, 256)  # the bucket sizes bench.py times
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic, nleaf=16, ncrit=256)
     _check_int_artefacts(hot, T)
     acc, pot = hot.hot_forces(theta, w.eps, order)
     gg = hot.hot_export_groups()
