@@ -136,25 +136,20 @@ __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ 
     }
     if (threadIdx.x == 0) totals[blockIdx.x] = carry;
 }
+// Stable scatter of one tile: ranks by warp match_any, then the tile is put in digit order in shared
+// memory so that every run of equal digits leaves as one contiguous (coalesced) write.
 __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
                                                                     uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, int64_t n,
                                                                     int shift, const uint32_t* __restrict__ hist,
                                                                     const uint32_t* __restrict__ totals, int64_t nblk) {
     __shared__ uint32_t wcount[SORT_WARPS][256];
-    __shared__ uint32_t gbase[256];
+    __shared__ uint32_t gbase[256];   // global position of the tile's first key of each digit, minus its local start
+    __shared__ uint32_t lstart[256];  // local start of each digit inside the digit-ordered tile
     __shared__ uint32_t wtot[SORT_WARPS];
+    __shared__ uint64_t skey[SORT_TILE]; // the digit-ordered tile: keys first, then (same space) the values
+    __shared__ uint8_t sdig[SORT_TILE];
+    uint32_t* const sval = reinterpret_cast<uint32_t*>(skey);
     int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
-    // digit base = exclusive scan of the 256 row totals + this tile's offset inside the row
-    {
-        uint32_t v = totals[tid], x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
-        if (lane == 31) wtot[w] = x;
-        __syncthreads();
-        uint32_t off = 0;
-        for (int j = 0; j < w; ++j) off += wtot[j];
-        gbase[tid] = off + x - v + hist[(int64_t)tid * nblk + blockIdx.x];
-    }
 #pragma unroll
     for (int j = 0; j < SORT_WARPS; ++j) wcount[j][tid] = 0;
     __syncthreads();
@@ -176,21 +171,60 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64
         rk[k] = d | ((old + r) << 8);
     }
     __syncthreads();
+    uint32_t mine; // this digit's count in the tile
     { // exclusive prefix over the warps of the tile, per digit
         uint32_t run = 0;
 #pragma unroll
         for (int j = 0; j < SORT_WARPS; ++j) { uint32_t t = wcount[j][tid]; wcount[j][tid] = run; run += t; }
+        mine = run;
     }
-    __syncthreads();
+    { // local start of every digit = exclusive scan of the tile's digit counts
+        uint32_t x = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wtot[w] = x;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int j = 0; j < w; ++j) off += wtot[j];
+        lstart[tid] = off + x - mine;
+        __syncthreads();
+    }
+    { // global base of every digit = exclusive scan of the 256 row totals + this tile's offset inside the row
+        uint32_t v = totals[tid], x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wtot[w] = x;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int j = 0; j < w; ++j) off += wtot[j];
+        gbase[tid] = off + x - v + hist[(int64_t)tid * nblk + blockIdx.x] - lstart[tid];
+    }
+    // digit-ordered tile in shared memory: keys
+    uint32_t vv[SORT_ITEMS];
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         int64_t i = base + k * 32 + lane;
-        if (i < n) {
-            uint32_t d = rk[k] & 255u;
-            uint32_t p = gbase[d] + wcount[w][d] + (rk[k] >> 8);
-            kout[p] = kk[k];
-            vout[p] = vin[i];
-        }
+        rk[k] = i < n ? lstart[rk[k] & 255u] + wcount[w][rk[k] & 255u] + (rk[k] >> 8) : 0xffffffffu; // now: position in the tile
+        vv[k] = i < n ? vin[i] : 0u;
+        if (i < n) { skey[rk[k]] = kk[k]; sdig[rk[k]] = (uint8_t)((uint32_t)(kk[k] >> shift) & 255u); }
+    }
+    __syncthreads();
+    const int64_t t0 = (int64_t)blockIdx.x * SORT_TILE;
+    const int cnt = (int)(n - t0 < SORT_TILE ? n - t0 : SORT_TILE);
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        int p = k * SORT_THREADS + tid;
+        if (p < cnt) kout[gbase[sdig[p]] + (uint32_t)p] = skey[p];
+    }
+    __syncthreads();
+    // ... then the values through the same space
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) if (rk[k] != 0xffffffffu) sval[rk[k]] = vv[k];
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        int p = k * SORT_THREADS + tid;
+        if (p < cnt) vout[gbase[sdig[p]] + (uint32_t)p] = sval[p];
     }
 }
 cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st) {
