@@ -40,8 +40,8 @@ NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2): 14.538e9}
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 SORT_BYTES_PER_BODY = 8 * 32          # 8 passes x (8 B histogram read + 12 B read + 12 B write)
-KEYGEN_BYTES_PER_BODY = 24
-GATHER_BYTES_PER_BODY = 36
+KEYGEN_BYTES_PER_BODY = 44          # 12 B pos + 4 B mass read; 8 B key + 4 B index + 16 B float4 body written
+GATHER_BYTES_PER_BODY = 36          # 4 B permutation + 16 B float4 gathered, 16 B written
 
 
 def parse():

@@ -210,6 +210,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(tree_alloc(&t.idx[0], (size_t)n));
     CUDA_TRY(tree_alloc(&t.idx[1], (size_t)n));
     CUDA_TRY(tree_alloc(&t.body, (size_t)n));
+    CUDA_TRY(tree_alloc(&t.bin, (size_t)n));
     CUDA_TRY(tree_alloc(&t.plev, (size_t)n));
     CUDA_TRY(tree_alloc(&d_hist, sort_hist_elems(n)));
     CUDA_TRY(tree_alloc(&d_counts, (size_t)rows * (size_t)nblk));
@@ -217,11 +218,11 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(cudaMemsetAsync(g.d_flags, 0, 4 * sizeof(int), st));
 
     CUDA_TRY(cudaEventRecord(g.ev[0], st));
-    CUDA_TRY(launch_keygen(pos, n, box.lo[0], box.lo[1], box.lo[2], inv, t.key[0], t.idx[0], g.d_flags, st));
+    CUDA_TRY(launch_keygen(pos, mass, n, box.lo[0], box.lo[1], box.lo[2], inv, t.key[0], t.idx[0], t.bin, g.d_flags, st));
     CUDA_TRY(cudaEventRecord(g.ev[1], st));
     CUDA_TRY(launch_radix_sort(t.key, t.idx, n, d_hist, st));
     CUDA_TRY(cudaEventRecord(g.ev[2], st));
-    CUDA_TRY(launch_gather(pos, mass, t.idx[0], n, t.body, st));
+    CUDA_TRY(launch_gather(t.bin, t.idx[0], n, t.body, st));
     CUDA_TRY(cudaEventRecord(g.ev[3], st));
     CUDA_TRY(launch_tree_levels(t.key[0], n, t.nleaf, t.ncrit, t.plev, d_counts, st));
     CUDA_TRY(launch_tree_scan(d_counts, nblk, d_totals, st));

@@ -41,9 +41,11 @@ __device__ __forceinline__ uint64_t body_key(float x, float y, float z, float lo
     return (1ull << 63) | (spread21(ix) << 2) | (spread21(iy) << 1) | spread21(iz);
 }
 // 4 bodies per thread: three 128-bit loads, two 128-bit key stores, one 128-bit index store
-__global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ pos, int64_t n, float lox, float loy,
-                                                     float loz, float inv, uint64_t* __restrict__ key,
-                                                     uint32_t* __restrict__ idx, int* __restrict__ errflag, int vec) {
+// Also writes the bodies as aligned float4 (x,y,z,m) in the caller's order: the gather after the sort
+// then fetches one 32-byte sector per body instead of the 3-4 sectors of the separate pos / mass arrays.
+__global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ pos, const float* __restrict__ mass, int64_t n, float lox,
+                                                     float loy, float loz, float inv, uint64_t* __restrict__ key,
+                                                     uint32_t* __restrict__ idx, float4* __restrict__ bin, int* __restrict__ errflag, int vec) {
     int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; // quad index
     int64_t i0 = q * 4;
     if (i0 >= n) return;
@@ -59,20 +61,26 @@ __global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ p
         ko[0] = make_ulonglong2(k0, k1);
         ko[1] = make_ulonglong2(k2, k3);
         *reinterpret_cast<uint4*>(idx + i0) = make_uint4((uint32_t)i0, (uint32_t)i0 + 1, (uint32_t)i0 + 2, (uint32_t)i0 + 3);
+        const float4 m = __ldg(reinterpret_cast<const float4*>(mass) + q);
+        bin[i0] = make_float4(a.x, a.y, a.z, m.x);
+        bin[i0 + 1] = make_float4(a.w, b.x, b.y, m.y);
+        bin[i0 + 2] = make_float4(b.z, b.w, c.x, m.z);
+        bin[i0 + 3] = make_float4(c.y, c.z, c.w, m.w);
     } else {
         for (int64_t i = i0; i < n && i < i0 + 4; ++i) {
             key[i] = body_key(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], lox, loy, loz, inv, bad);
             idx[i] = (uint32_t)i;
+            bin[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
         }
     }
     if (bad) atomicOr(errflag, 1);
 }
-cudaError_t launch_keygen(const float* pos, int64_t n, float lox, float loy, float loz, float inv,
-                          uint64_t* key, uint32_t* idx, int* errflag, cudaStream_t st) {
+cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float lox, float loy, float loz, float inv,
+                          uint64_t* key, uint32_t* idx, float4* bin, int* errflag, cudaStream_t st) {
     int64_t quads = (n + 3) / 4;
-    int vec = (reinterpret_cast<uintptr_t>(pos) & 15u) == 0; // 128-bit loads need a 16-byte aligned base
+    int vec = ((reinterpret_cast<uintptr_t>(pos) | reinterpret_cast<uintptr_t>(mass)) & 15u) == 0; // 128-bit loads need 16-byte aligned bases
     HOT_LAUNCHED(1);
-    keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, n, lox, loy, loz, inv, key, idx, errflag, vec);
+    keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, mass, n, lox, loy, loz, inv, key, idx, bin, errflag, vec);
     return cudaGetLastError();
 }
 
@@ -83,7 +91,7 @@ cudaError_t launch_keygen(const float* pos, int64_t n, float lox, float loy, flo
 // held warp-striped so the in-tile order is (warp, round, lane).
 // ------------------------------------------------------------------------------------------
 #define SORT_THREADS 256
-#define SORT_ITEMS 16
+#define SORT_ITEMS 8
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_WARPS (SORT_THREADS / 32)
 
@@ -138,7 +146,10 @@ __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ 
 }
 // Stable scatter of one tile: ranks by warp match_any, then the tile is put in digit order in shared
 // memory so that every run of equal digits leaves as one contiguous (coalesced) write.
-__global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+#ifndef SORT_MINBLK
+#define SORT_MINBLK 5
+#endif
+__global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
                                                                     uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, int64_t n,
                                                                     int shift, const uint32_t* __restrict__ hist,
                                                                     const uint32_t* __restrict__ totals, int64_t nblk) {
@@ -157,12 +168,23 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64
     uint64_t kk[SORT_ITEMS];
     uint32_t rk[SORT_ITEMS]; // digit | rank << 8
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
+    for (int k = 0; k < SORT_ITEMS; ++k) { // all loads first: the warp barriers below would serialise them
+        int64_t i = base + k * 32 + lane;
+        kk[k] = i < n ? kin[i] : ~0ull;
+    }
+    uint32_t mm[SORT_ITEMS];
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) { // the 16 matches are independent: issue them back to back
+        int64_t i = base + k * 32 + lane;
+        uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
+        mm[k] = __match_any_sync(FULL, i < n ? d : 256u);
+    }
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) { // ... then the (serial) per-warp digit counters
         int64_t i = base + k * 32 + lane;
         bool valid = i < n;
-        kk[k] = valid ? kin[i] : ~0ull;
         uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
-        uint32_t m = __match_any_sync(FULL, valid ? d : 256u);
+        uint32_t m = mm[k];
         uint32_t r = __popc(m & ((1u << lane) - 1u));
         uint32_t old = valid ? wcount[w][d] : 0;
         __syncwarp();
@@ -204,8 +226,12 @@ __global__ void __launch_bounds__(SORT_THREADS) sort_scatter_kernel(const uint64
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         int64_t i = base + k * 32 + lane;
-        rk[k] = i < n ? lstart[rk[k] & 255u] + wcount[w][rk[k] & 255u] + (rk[k] >> 8) : 0xffffffffu; // now: position in the tile
         vv[k] = i < n ? vin[i] : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        int64_t i = base + k * 32 + lane;
+        rk[k] = i < n ? lstart[rk[k] & 255u] + wcount[w][rk[k] & 255u] + (rk[k] >> 8) : 0xffffffffu; // now: position in the tile
         if (i < n) { skey[rk[k]] = kk[k]; sdig[rk[k]] = (uint8_t)((uint32_t)(kk[k] >> shift) & 255u); }
     }
     __syncthreads();
@@ -246,17 +272,17 @@ cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uin
 
 // ------------------------------------------------------------------------------------------
 // S3 gather into key order as float4 (x,y,z,m): the "structure" the interaction kernels stage.
+// Source: the float4 copy keygen wrote in the caller's order (one aligned 16-byte read per body).
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) gather_kernel(const float* __restrict__ pos, const float* __restrict__ mass,
-                                                     const uint32_t* __restrict__ perm, int64_t n, float4* __restrict__ body) {
+__global__ void __launch_bounds__(256) gather_kernel(const float4* __restrict__ bin, const uint32_t* __restrict__ perm, int64_t n,
+                                                     float4* __restrict__ body) {
     int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    uint32_t j = perm[i];
-    body[i] = make_float4(__ldg(pos + 3 * (int64_t)j), __ldg(pos + 3 * (int64_t)j + 1), __ldg(pos + 3 * (int64_t)j + 2), __ldg(mass + j));
+    body[i] = __ldg(bin + perm[i]);
 }
-cudaError_t launch_gather(const float* pos, const float* mass, const uint32_t* perm, int64_t n, float4* body, cudaStream_t st) {
+cudaError_t launch_gather(const float4* bin, const uint32_t* perm, int64_t n, float4* body, cudaStream_t st) {
     HOT_LAUNCHED(1);
-    gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(pos, mass, perm, n, body);
+    gather_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(bin, perm, n, body);
     return cudaGetLastError();
 }
 

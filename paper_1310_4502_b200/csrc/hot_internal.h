@@ -38,6 +38,7 @@ struct Tree {
     uint64_t* key[2] = {nullptr, nullptr};   // ping-pong, key[0] holds the sorted keys after build
     uint32_t* idx[2] = {nullptr, nullptr};   // idx[0] = perm
     float4* body = nullptr;                  // key-ordered (x,y,z,m)
+    float4* bin = nullptr;                   // the same records in the caller's order (written by keygen, read by the gather)
     uint32_t* plev = nullptr;                // per body: b | Lleaf<<8 | Lgroup<<16
     // cells
     int64_t ncells = 0, nleaves = 0, ngroups = 0;
@@ -68,13 +69,12 @@ struct Tree {
 
 // ---- build stages (hot_build.cu) ------------------------------------------------------------
 // every launcher returns the cudaError_t of its last launch; all work goes to `st`
-cudaError_t launch_keygen(const float* pos, int64_t n, float lox, float loy, float loz, float inv,
-                          uint64_t* key, uint32_t* idx, int* errflag, cudaStream_t st);
+cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float lox, float loy, float loz, float inv,
+                          uint64_t* key, uint32_t* idx, float4* bin, int* errflag, cudaStream_t st);
 // sorts (key,idx) pairs stably, ascending; result ends in key[0]/idx[0]; scratch: hist of sort_hist_elems(n) u32
 size_t sort_hist_elems(int64_t n);
 cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st);
-cudaError_t launch_gather(const float* pos, const float* mass, const uint32_t* perm, int64_t n,
-                          float4* body, cudaStream_t st);
+cudaError_t launch_gather(const float4* bin, const uint32_t* perm, int64_t n, float4* body, cudaStream_t st);
 // tree pass 1: per-body levels + per-block per-level counts.  counts: [HOT_NLEVELS+1][nblk] u32
 int64_t tree_num_blocks(int64_t n);
 cudaError_t launch_tree_levels(const uint64_t* skey, int64_t n, int nleaf, int ncrit, uint32_t* plev,
