@@ -399,7 +399,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (g.used_pc + g.used_pp > 0 && g.used_groups > 0) {
         const double per_group = (double)(g.used_pc + g.used_pp) / (double)g.used_groups;
         const double fit = 0.85 * (double)(cappc + cappp) / (per_group > 1.0 ? per_group : 1.0);
-        if (fit < (double)ng) budget = fit < 1.0 ? 1 : (int64_t)fit;
+        if (fit < 0.8 * (double)ng) budget = fit < 1.0 ? 1 : (int64_t)fit; // clearly too small (a capped arena): plan the rounds
     }
     int64_t g0 = 0;
     size_t nrounds = 0;

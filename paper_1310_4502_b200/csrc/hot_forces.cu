@@ -29,12 +29,6 @@
 #ifndef HOT_MINBLK
 #define HOT_MINBLK 3           // resident blocks per SM the order 0/2 kernels are compiled for
 #endif
-#ifndef HOT_UNROLL2
-#define HOT_UNROLL2 0          // evaluate two sources per loop trip (more independent chains, more registers)
-#endif
-#ifndef HOT_PREFETCH
-#define HOT_PREFETCH 1         // read the next source from shared memory before the arithmetic of the current one
-#endif
 
 template <int ORDER> struct PCQ { static constexpr int v = ORDER >= 4 ? 12 : (ORDER >= 2 ? 3 : 1); }; // float4 per staged cell
 
@@ -368,16 +362,6 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 int j = strm;
                 float4 n0 = st[j < cnt ? j : 0], n1 = n0, n2 = n0;
                 if (ORDER >= 2) { n1 = st[32 + (j < cnt ? j : 0)]; n2 = st[64 + (j < cnt ? j : 0)]; }
-#if HOT_UNROLL2
-#pragma unroll 1
-                for (; j + K < cnt; j += 2 * K) { // two sources per trip: twice the independent chains
-                    const float4 a0 = st[j], a1 = ORDER >= 2 ? st[32 + j] : a0, a2 = ORDER >= 2 ? st[64 + j] : a0;
-                    const float4 b0 = st[j + K], b1 = ORDER >= 2 ? st[32 + j + K] : b0, b2 = ORDER >= 2 ? st[64 + j + K] : b0;
-                    sk.template pc<ORDER>(a0, a1, a2, nullptr, eps2);
-                    sk.template pc<ORDER>(b0, b1, b2, nullptr, eps2);
-                }
-                if (j < cnt) { n0 = st[j]; if (ORDER >= 2) { n1 = st[32 + j]; n2 = st[64 + j]; } }
-#endif
 #pragma unroll 1
                 while (j < cnt) {
                     const float4 q0 = n0, q1 = n1, q2 = n2;
@@ -435,15 +419,6 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
             {
                 int j = strm;
                 float4 nx = st[j < cnt ? j : 0];
-#if HOT_UNROLL2
-#pragma unroll 1
-                for (; j + K < cnt; j += 2 * K) {
-                    const float4 sa = st[j], sb = st[j + K];
-                    sk.pp(sa, eps2);
-                    sk.pp(sb, eps2);
-                }
-                if (j < cnt) nx = st[j];
-#endif
 #pragma unroll 1
                 while (j < cnt) {
                     const float4 sb = nx;

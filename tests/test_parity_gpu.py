@@ -366,3 +366,20 @@ def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
     assert st["n"] == w.n and st["pp_interactions"] > 0 and st["pc_interactions"] > 0
     assert np.isfinite(acc.cpu().numpy()).all() and np.isfinite(pot.cpu().numpy()).all()
     del cnt
+
+
+def test_long_lists_outgrow_the_walk_staging_and_are_retried(hot):
+    """theta = 0.07 with one-body leaves gives more than 16384 accepted cells per group: the walk
+    reports that its per-warp staging area is too small, the library enlarges it and walks again."""
+    w = W.config(0, 15)
+    _build(hot, w, 1, 64)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, nleaf=1, ncrit=64)
+    acc, pot = hot.hot_forces(0.07, w.eps, 2)
+    gg = hot.hot_export_groups()
+    assert gg["lpc"].max() > 16384
+    sel = np.unique(np.append(np.arange(0, T.ngroups, max(1, T.ngroups // 5)), int(np.argmax(gg["lpc"]))))
+    oa, op, lpc, lpp = T.forces(0.07, w.eps, 2, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    ea, ep = _rel_errors(acc, pot, oa, op)
+    assert np.median(ea) <= 1e-5 and np.median(ep) <= 1e-5
+    hot.hot_free()
