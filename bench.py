@@ -33,9 +33,10 @@ if ROOT not in sys.path:
 FLOPS_PP = 20
 FLOPS_PC = {0: 21, 2: 59, 4: 276}
 # DRAM bytes of one forces_kernel launch from the ncu --set full capture of the default workload
-# (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 13.342 GB + dram__bytes_write.sum 1.197 GB;
-# the lists alone are 4 B x 2.92e9 entries = 11.7 GB of compulsory reads); other workloads: null
-NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2): 14.538e9}
+# (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 6.459 GB + dram__bytes_write.sum 1.191 GB;
+# the lists alone are 4 B x 0.88e9 entries = 3.5 GB of compulsory reads, acc + pot 0.27 GB of writes), at the
+# default bucket sizes NLEAF 16 / NCRIT 256; other workloads: null
+NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2, 16, 256): 7.650e9}
 # FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
@@ -300,7 +301,7 @@ def main():
     kern_s = stage["ms_eval"] * 1e-3
     achieved = flops / kern_s / 1e12
     tf_scalar, tf_packed = hot.hot_measure_fp32()  # register-only FMA chains on this device, after the timed region
-    traffic = NCU_TRAFFIC_BYTES.get(("c%d" % args.config, int(round(np.log2(w.n))), w.theta, w.order))
+    traffic = NCU_TRAFFIC_BYTES.get(("c%d" % args.config, int(round(np.log2(w.n))), w.theta, w.order, args.nleaf, args.ncrit))
     out = {
         "metric": "interactions_per_second", "value": inter_all / (ms_max * 1e-3) / 1e9, "unit": "Ginteractions/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_max,
