@@ -191,33 +191,32 @@ void far_sink_polynomial(const double* S, double* D) {
 
 // ---- device: global raw moments about the box centre, box units -------------------------------------
 #define FM_TILE 64
-#define FM_THREADS 192
+#define FM_THREADS 192 // = 3 * FM_TILE: one thread per (coordinate, body) when the power tables are filled
 struct FarIdx { unsigned char a[FAR_N], b[FAR_N], c[FAR_N]; };
 __global__ void __launch_bounds__(FM_THREADS) far_moments_kernel(const float4* __restrict__ body, int64_t n, double cx, double cy, double cz,
                                                                  double inv, const __grid_constant__ FarIdx I, double* __restrict__ S) {
-    __shared__ double pw[3][FAR_P + 1][FM_TILE]; // powers of the three coordinates of a tile of bodies
-    __shared__ double ms[FM_TILE];
+    // powers of the three coordinates of a tile of bodies, exponent fastest: the 165 threads read
+    // <= 9 consecutive doubles per table (no bank conflicts), threads with equal exponents broadcast.
+    // The mass is folded into the x table.
+    __shared__ double pw[3][FM_TILE][FAR_P + 1];
     const int t = threadIdx.x;
     const int ma = t < FAR_N ? I.a[t] : 0, mb = t < FAR_N ? I.b[t] : 0, mc = t < FAR_N ? I.c[t] : 0; // this thread's moment
     double acc = 0.0;
     for (int64_t base = (int64_t)blockIdx.x * FM_TILE; base < n; base += (int64_t)gridDim.x * FM_TILE) {
-        if (t < FM_TILE) {
-            const int64_t j = base + t;
+        { // thread t: coordinate k = t / 64 of body t % 64
+            const int k = t / FM_TILE, jj = t % FM_TILE;
+            const int64_t j = base + jj;
             float4 b = make_float4(0.f, 0.f, 0.f, 0.f);
             if (j < n) b = body[j];
-            const double d[3] = {((double)b.x - cx) * inv, ((double)b.y - cy) * inv, ((double)b.z - cz) * inv};
-            ms[t] = j < n ? (double)b.w : 0.0;
+            const double d = k == 0 ? ((double)b.x - cx) * inv : k == 1 ? ((double)b.y - cy) * inv : ((double)b.z - cz) * inv;
+            double p = k == 0 ? (j < n ? (double)b.w : 0.0) : 1.0;
 #pragma unroll
-            for (int k = 0; k < 3; ++k) {
-                double p = 1.0;
-#pragma unroll
-                for (int e = 0; e <= FAR_P; ++e) { pw[k][e][t] = p; p *= d[k]; }
-            }
+            for (int e = 0; e <= FAR_P; ++e) { pw[k][jj][e] = p; p *= d; }
         }
         __syncthreads();
         if (t < FAR_N) {
 #pragma unroll 8
-            for (int j = 0; j < FM_TILE; ++j) acc += ms[j] * pw[0][ma][j] * pw[1][mb][j] * pw[2][mc][j];
+            for (int j = 0; j < FM_TILE; ++j) acc = fma(pw[0][j][ma] * pw[1][j][mb], pw[2][j][mc], acc);
         }
         __syncthreads();
     }
@@ -235,28 +234,20 @@ __global__ void __launch_bounds__(128) far_eval_kernel(const float4* __restrict_
     if (i >= n) return;
     const float4 b = body[i];
     const double x = ((double)b.x - cx) * inv, y = ((double)b.y - cy) * inv, z = ((double)b.z - cz) * inv;
-    double py[FAR_P + 1], pz[FAR_P + 1];
-    py[0] = pz[0] = 1.0;
-#pragma unroll
-    for (int e = 1; e <= FAR_P; ++e) { py[e] = py[e - 1] * y; pz[e] = pz[e - 1] * z; }
-    // v = sum_a x^a A_a(y,z),  dv/dx = sum_a a x^(a-1) A_a,  dv/dy = sum_a x^a dA_a/dy, ...: Horner in x over a = 8..0
+    // v = sum_a x^a sum_b y^b sum_c z^c D_abc by nested Horner (z innermost), carrying the partial
+    // derivatives along (f' <- f' t + f before f <- f t + c): ~500 fused multiply-adds, no power tables
     double v = 0.0, gx = 0.0, gy = 0.0, gz = 0.0;
 #pragma unroll
     for (int a = FAR_P; a >= 0; --a) {
-        double A = 0.0, Ay = 0.0, Az = 0.0;
+        double B = 0.0, By = 0.0, Bz = 0.0; // sum_b y^b C_ab(z) and its y, z derivatives
 #pragma unroll
-        for (int bb = 0; bb <= FAR_P - a; ++bb)
+        for (int bb = FAR_P - a; bb >= 0; --bb) {
+            double C = 0.0, Cz = 0.0;       // C_ab(z) = sum_c D_abc z^c and dC/dz
 #pragma unroll
-            for (int c = 0; c <= FAR_P - a - bb; ++c) {
-                const double d = D[fidx(a, bb, c)];
-                A += d * py[bb] * pz[c];
-                if (bb > 0) Ay += d * (double)bb * py[bb - 1] * pz[c];
-                if (c > 0) Az += d * (double)c * py[bb] * pz[c - 1];
-            }
-        gx = gx * x + v;      // derivative of the Horner form: v' <- v' x + v before v <- v x + A
-        v = v * x + A;
-        gy = gy * x + Ay;
-        gz = gz * x + Az;
+            for (int c = FAR_P - a - bb; c >= 0; --c) { Cz = fma(Cz, z, C); C = fma(C, z, D[fidx(a, bb, c)]); }
+            By = fma(By, y, B); B = fma(B, y, C); Bz = fma(Bz, y, Cz);
+        }
+        gx = fma(gx, x, v); v = fma(v, x, B); gy = fma(gy, x, By); gz = fma(gz, x, Bz);
     }
     // a_far = grad / L^2, phi_far = -v / L  (inv = 1/L); kept in fp64, key order: the interaction kernel adds
     // it to its fp64 sums before the one rounding to fp32 (the explicit and the far part cancel strongly)
