@@ -315,7 +315,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     // P2/P3: what the 125 explicit boxes leave of the periodic sum, and the background (hot_periodic.cu);
     // per body in fp64, added by the interaction kernel before its one rounding to fp32
     if (t.periodic) {
-        if (!t.far_ready) { // global moments of the box: once per build
+        if (!t.far_ready) { // global moments of the box and the per-body far field: once per build
             CUDA_TRY(tree_alloc(&g.d_farS, 165));
             CUDA_TRY(tree_alloc(&t.far, 4 * (size_t)t.n));
             CUDA_TRY(launch_far_moments(t, g.d_farS, st));
@@ -323,9 +323,9 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
             CUDA_TRY(cudaMemcpyAsync(S, g.d_farS, sizeof(S), cudaMemcpyDeviceToHost, st));
             CUDA_TRY(cudaStreamSynchronize(st));
             far_sink_polynomial(S, t.farD);
+            CUDA_TRY(launch_far_eval(t, t.farD, t.far, st)); // depends on the bodies only: kept for every hot_forces on this build
             t.far_ready = true;
         }
-        CUDA_TRY(launch_far_eval(t, t.farD, t.far, st));
     }
     CUDA_TRY(cudaEventRecord(g.ev[8], st));
     // S7: the walk writes every group's lists into the arena; S8/S9/S10 evaluate them.  The arena is
