@@ -11,7 +11,9 @@ extern long long g_hot_launches; // kernels launched by the library since the la
 
 #define HOT_MAXLEVEL 21
 #define HOT_NLEVELS 22        // levels 0..21
+#ifndef HOT_MAX_NCRIT
 #define HOT_MAX_NCRIT 256
+#endif
 #define HOT_MAX_NLEAF 32
 
 // 16-byte record the walk reads per visited cell (S7).

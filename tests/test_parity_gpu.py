@@ -383,3 +383,49 @@ def test_long_lists_outgrow_the_walk_staging_and_are_retried(hot):
     ea, ep = _rel_errors(acc, pot, oa, op)
     assert np.median(ea) <= 1e-5 and np.median(ep) <= 1e-5
     hot.hot_free()
+
+
+def test_seeded_fuzz_of_sizes_bucket_sizes_orders_and_boundaries(hot):
+    """Seeded random small problems: every sink-blocking variant (1-6 sinks per lane, 1-32 source
+    streams, multi-pass groups), odd sizes, clustered and coincident bodies, open and periodic."""
+    import torch
+
+    rng = np.random.default_rng(20261104)
+    for trial in range(14):
+        n = int(rng.integers(1, 3000))
+        periodic = bool(trial % 3 == 2)
+        nleaf = int(rng.choice([1, 2, 5, 16, 32]))
+        ncrit = int(max(nleaf, rng.choice([1, 7, 33, 64, 200, 256])))
+        order = int(rng.choice([0, 2, 4]))
+        theta = float(rng.choice([0.3, 0.5, 0.75, 0.95]))
+        x = rng.uniform(0.0, 1.0, (n, 3))
+        if trial % 2:  # clumps and a few exactly coincident bodies
+            c = rng.uniform(0.2, 0.8, (8, 3))
+            x = np.clip(c[rng.integers(0, 8, n)] + 0.01 * rng.standard_normal((n, 3)), 0.0, 0.999)
+            x[: n // 10] = x[n // 10: 2 * (n // 10)][: n // 10]
+        pos = np.ascontiguousarray(x.astype(np.float32))
+        pos = np.minimum(pos, np.float32(0.9999))
+        mass = rng.uniform(0.5, 1.5, n).astype(np.float32) / n
+        eps = 1e-3
+        hot.hot_set_params(nleaf, ncrit)
+        hot.hot_build(torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda(), (0.0, 0.0, 0.0), 1.0, periodic)
+        acc, pot = hot.hot_forces(theta, eps, order)
+        T = O.Tree(pos, mass, (0.0, 0.0, 0.0), 1.0, periodic=periodic, nleaf=nleaf, ncrit=ncrit)
+        gk, gp = hot.hot_export_keys()
+        key, skey, perm = T.keys()
+        assert (gk == skey).all() and (gp == perm).all(), trial
+        sel = None if T.ngroups <= 24 else np.sort(rng.choice(T.ngroups, 24, replace=False))
+        oa, op, lpc, lpp = T.forces(theta, eps, order, groups=sel)
+        gg = hot.hot_export_groups()
+        idx = np.arange(T.ngroups) if sel is None else sel
+        assert (gg["lpc"][idx] == lpc.astype(np.uint64)).all() and (gg["lpp"][idx] == lpp.astype(np.uint64)).all(), trial
+        m = ~np.isnan(op)
+        ga = acc.cpu().numpy().astype(np.float64)[m]
+        gpot = pot.cpu().numpy().astype(np.float64)[m]
+        ascale = np.sqrt((oa[m] ** 2).sum(axis=1).mean()) + 1e-300
+        pscale = 57.18721055 * float(mass.astype(np.float64).sum()) if periodic else 0.0
+        ea = np.linalg.norm(ga - oa[m], axis=1) / (np.linalg.norm(oa[m], axis=1) + 1e-3 * ascale)
+        ep = np.abs(gpot - op[m]) / (np.abs(op[m]) + pscale + 1e-300)
+        assert np.median(ea) <= 1e-5 and ea.max() <= 1e-3, (trial, n, nleaf, ncrit, order, theta, periodic, np.median(ea), ea.max())
+        assert np.median(ep) <= 1e-5 and ep.max() <= 1e-3, (trial, n, nleaf, ncrit, order, theta, periodic, np.median(ep), ep.max())
+    hot.hot_set_params(16, 256)
