@@ -263,7 +263,7 @@ def main():
     for _ in range(args.steps):
         step()
         st = hot.hot_stats()
-        for k in ("ms_keygen", "ms_sort", "ms_gather", "ms_tree", "ms_moments", "ms_farfield", "ms_walk", "ms_eval",
+        for k in ("ms_keygen", "ms_sort", "ms_gather", "ms_tree", "ms_moments", "ms_farfield", "ms_walk", "ms_coarse", "ms_eval",
                   "ms_build_total", "ms_forces_total"):
             stage[k] = stage.get(k, 0.0) + st[k] / args.steps
     e1.record()

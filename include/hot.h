@@ -71,7 +71,8 @@ typedef struct {
     float ms_eval;   /* particle-particle / particle-cell interaction kernels (the FP32-bound stage) */
     float ms_farfield;
     float ms_build_total, ms_forces_total;
-    int32_t list_chunks; int32_t pad0; /* group chunks the lists were walked / evaluated in (1 unless the arena is short) */
+    int32_t list_chunks; /* group chunks the lists were walked / evaluated in (1 unless the arena is short) */
+    float ms_coarse;     /* periodic only: fp64 monopoles of the coarsest accepted cells (R-14) */
     uint64_t list_entries;      /* accepted cells + listed bodies over all groups (4 B each, +1 B when periodic) */
     int64_t bytes_allocated;
     int64_t launches_build, launches_forces; /* kernels launched by the last hot_build / hot_forces */

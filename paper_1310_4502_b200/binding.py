@@ -33,7 +33,7 @@ class hot_stats_t(C.Structure):
                 ("ms_keygen", C.c_float), ("ms_sort", C.c_float), ("ms_gather", C.c_float), ("ms_tree", C.c_float),
                 ("ms_moments", C.c_float), ("ms_walk", C.c_float), ("ms_eval", C.c_float), ("ms_farfield", C.c_float),
                 ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float),
-                ("list_chunks", C.c_int32), ("pad0", C.c_int32), ("list_entries", C.c_uint64),
+                ("list_chunks", C.c_int32), ("ms_coarse", C.c_float), ("list_entries", C.c_uint64),
                 ("bytes_allocated", C.c_int64),
                 ("launches_build", C.c_int64), ("launches_forces", C.c_int64)]
 

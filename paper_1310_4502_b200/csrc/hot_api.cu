@@ -318,6 +318,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         if (!t.far_ready) { // global moments of the box and the per-body far field: once per build
             CUDA_TRY(tree_alloc(&g.d_farS, 165));
             CUDA_TRY(tree_alloc(&t.far, 4 * (size_t)t.n));
+            CUDA_TRY(tree_alloc(&t.farc, 4 * (size_t)t.n));
             CUDA_TRY(launch_far_moments(t, g.d_farS, st));
             double S[165];
             CUDA_TRY(cudaMemcpyAsync(S, g.d_farS, sizeof(S), cudaMemcpyDeviceToHost, st));
@@ -404,8 +405,8 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     int64_t g0 = 0;
     size_t nrounds = 0;
     unsigned long long usedpc = 0, usedpp = 0;
-    float ms_walk = 0, ms_eval = 0;
-    if (g.evx.size() < 4) { while (g.evx.size() < 4) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
+    float ms_walk = 0, ms_eval = 0, ms_coarse = 0;
+    if (g.evx.size() < 5) { while (g.evx.size() < 5) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
     while (g0 < ng) {
         const int ff0 = INT_MAX;
         CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
@@ -447,10 +448,15 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         usedpc += tops[0]; usedpp += tops[1];
         a.g0 = g0; a.g1 = F;
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
+        if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
+            CUDA_TRY(cudaEventRecord(g.evx[4], st));
+            CUDA_TRY(launch_coarse_monopoles(a, t.far, t.farc, eps * eps, st));
+            a.far = t.farc;
+        }
         CUDA_TRY(cudaEventRecord(g.evx[3], st));
         CUDA_TRY(launch_forces(a, st));
         CUDA_TRY(cudaEventRecord(g.evx[2], st));
-        if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[3], g.evx[2]); } // the arena is reused
+        if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[3], g.evx[2]); if (t.periodic) ms_coarse += ms_between(g.evx[4], g.evx[3]); } // the arena is reused
         if (F < wa.g1) { // the arena was too small: enlarge it if memory allows, else keep going in rounds of what fitted
             const unsigned long long oldpc = cappc, oldpp = cappp;
             cappc *= 2; cappp *= 2;
@@ -469,6 +475,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     ms_eval += ms_between(g.evx[3], g.evx[2]);
+    if (t.periodic) ms_coarse += ms_between(g.evx[4], g.evx[3]);
     g.used_pc = usedpc; g.used_pp = usedpp; g.used_groups = ng; // sizes the arena of the next call
     hot_stats_t& s = g.st;
     s.order = order;
@@ -476,6 +483,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     s.ms_moments = ms_between(g.ev[5], g.ev[6]);
     s.ms_walk = ms_walk;
     s.ms_eval = ms_eval;
+    s.ms_coarse = ms_coarse;
     s.ms_farfield = ms_between(g.ev[6], g.ev[8]);
     s.ms_forces_total = ms_between(g.ev[5], g.ev[7]);
     s.list_chunks = (int32_t)nrounds; s.list_entries = usedpc + usedpp;

@@ -330,9 +330,10 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
         };
         auto issue = [&](int b) { // gather batch b: centre to registers, moments straight to shared memory
             if (b * BATCH + lane < n) {
-                const uint32_t c = cnext;
+                const uint32_t c = PER ? (cnext & ~HOT_COARSE_FLAG) : cnext;
                 pim = inext;
                 cA = P.cellA[c];
+                if (PER && (cnext & HOT_COARSE_FLAG)) cA.m0 = 0.f; // its monopole is summed in fp64 elsewhere (hot_periodic.cu)
                 float4* const dst = pcst + (b & 1) * NQ * BATCH + lane;
                 if (ORDER >= 2) {
                     const float4* src = reinterpret_cast<const float4*>(P.cellM2 + c);

@@ -62,6 +62,7 @@ struct Tree {
     bool far_ready = false;
     double farD[165];
     double* far = nullptr;                   // [n][4] far field per body, key order
+    double* farc = nullptr;                  // [n][4] far field + fp64 coarse-cell monopoles of the current hot_forces call
     // moments
     int mom_order = -1;
     CellA* cellA = nullptr;
@@ -105,6 +106,13 @@ cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st);
 // with count <= 32 (one per rejected leaf; a finest-level leaf with more bodies gives several); the
 // runs are expanded to one body index per entry when the list moves to the arena.
 #define HOT_RUN_SHIFT 27
+// Periodic boxes: accepted cells of levels <= HOT_COARSE_LEVEL carry HOT_COARSE_FLAG in the cell list.  They are
+// few (~1250 per group at theta = 0.5) but hold the large, nearly cancelling part of the image sum, so their
+// monopole terms are evaluated in fp64 by coarse_monopole_kernel and left out of the fp32 kernel (R-14).
+#ifndef HOT_COARSE_LEVEL
+#define HOT_COARSE_LEVEL 3
+#endif
+#define HOT_COARSE_FLAG 0x80000000u
 struct WalkArgs {
     const WalkCell* wcell; const GroupRec* group; int64_t g0, g1;
     unsigned long long mac_t[HOT_NLEVELS]; // accept a level-l cell iff d2 >= mac_t[l] (R-7, "MAC table")
@@ -147,6 +155,8 @@ void far_coefficients(double* out165);                    // host: Taylor coeffi
 void far_sink_polynomial(const double* S, double* D);     // host: per-sink polynomial from the global moments
 cudaError_t launch_far_moments(const Tree& t, double* S /*device [165]*/, cudaStream_t st);
 cudaError_t launch_far_eval(const Tree& t, const double* D /*host [165]*/, double* far /*device [n][4], key order*/, cudaStream_t st);
+// farc[body] = far[body] + fp64 monopole sum over the flagged cells of the body's group, groups [a.g0, a.g1)
+cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, double* farc, double eps2, cudaStream_t st);
 
 // ---- FP32 roofline denominator measured on the device (hot_peak.cu) ------------------------------------
 cudaError_t measure_fp32(double* tf_scalar, double* tf_packed, cudaStream_t st);

@@ -277,3 +277,82 @@ cudaError_t launch_far_eval(const Tree& t, const double* D, double* far, cudaStr
                                                                   t.lo[2] + 0.5 * t.size, 1.0 / t.size, Q, far);
     return cudaGetLastError();
 }
+
+// ---- fp64 monopoles of the coarse cells (periodic boxes) --------------------------------------------
+// A body of a nearly uniform periodic set feels an O(M/L^2) pull towards the centre of the 5^3 explicit
+// boxes which the far field cancels to the few-percent-of-that net acceleration; fp32 interaction terms
+// carry ~2e-7 of their own size, and the few hundred coarsest cells of the image boxes (levels 0..2, each
+// 1/64 of the box mass or more) carry most of that pull.  Their monopole terms are therefore summed here in
+// fp64 (25 operations each) and added, with the far field, to the fp64 sums of the interaction kernel, which
+// evaluates only their higher moments.  One warp per sink group, two sinks per lane and pass.
+#define CM_WARPS 8
+__global__ void __launch_bounds__(CM_WARPS * 32) coarse_monopole_kernel(const __grid_constant__ ForceArgs P, const double* __restrict__ far,
+                                                                        double* __restrict__ farc, double eps2) {
+    __shared__ double4 s_cell[CM_WARPS][32]; // staged coarse cells of a batch: centre (shifted to its image), mass
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    double4* const sc = s_cell[w];
+    for (int64_t gi = P.g0 + (int64_t)blockIdx.x * CM_WARPS + w; gi < P.g1; gi += (int64_t)gridDim.x * CM_WARPS) {
+        const GroupRec g = P.group[gi];
+        const unsigned long long o0 = P.pcoff[gi];
+        const int n = (int)P.lpc[gi];
+        const uint32_t* const pl = P.pclist + o0;
+        const uint8_t* const pi = P.pcimg + o0;
+        for (uint32_t s0 = 0; s0 < g.count; s0 += 64) {
+            double x[2][3], a[2][4];
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const uint32_t loc = s0 + 32 * i + lane;
+                const float4 b = P.body[g.first + (loc < g.count ? loc : 0u)];
+                x[i][0] = b.x; x[i][1] = b.y; x[i][2] = b.z;
+                a[i][0] = a[i][1] = a[i][2] = a[i][3] = 0.0;
+            }
+            for (int b0 = 0; b0 < n; b0 += 32) {
+                uint32_t e = 0; int im = 62;
+                if (b0 + lane < n) { e = pl[b0 + lane]; im = pi[b0 + lane]; }
+                const bool coarse = (e & HOT_COARSE_FLAG) != 0;
+                const uint32_t m = __ballot_sync(0xffffffffu, coarse);
+                if (m == 0) continue;
+                if (coarse) {
+                    const CellA cA = P.cellA[e & ~HOT_COARSE_FLAG];
+                    double4 r;
+                    r.x = cA.zx + (double)(im / 25 - 2) * P.size; r.y = cA.zy + (double)((im / 5) % 5 - 2) * P.size;
+                    r.z = cA.zz + (double)(im % 5 - 2) * P.size; r.w = (double)cA.m0;
+                    sc[__popc(m & ((1u << lane) - 1u))] = r;
+                }
+                __syncwarp();
+                const int nc = __popc(m);
+                for (int k = 0; k < nc; ++k) {
+                    const double4 c = sc[k];
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        const double Rx = x[i][0] - c.x, Ry = x[i][1] - c.y, Rz = x[i][2] - c.z;
+                        const double ri = rsqrt(fma(Rx, Rx, fma(Ry, Ry, fma(Rz, Rz, eps2))));
+                        const double mr = c.w * ri, mr3 = mr * ri * ri;
+                        a[i][0] = fma(-mr3, Rx, a[i][0]); a[i][1] = fma(-mr3, Ry, a[i][1]); a[i][2] = fma(-mr3, Rz, a[i][2]);
+                        a[i][3] -= mr;
+                    }
+                }
+                __syncwarp();
+            }
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const uint32_t loc = s0 + 32 * i + lane;
+                if (loc < g.count) {
+                    const double4 f = reinterpret_cast<const double4*>(far)[g.first + loc];
+                    double4 r;
+                    r.x = f.x + a[i][0]; r.y = f.y + a[i][1]; r.z = f.z + a[i][2]; r.w = f.w + a[i][3];
+                    reinterpret_cast<double4*>(farc)[g.first + loc] = r;
+                }
+            }
+        }
+    }
+}
+cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, double* farc, double eps2, cudaStream_t st) {
+    const int64_t ng = a.g1 - a.g0;
+    if (ng <= 0) return cudaSuccess;
+    int64_t nb = (ng + CM_WARPS - 1) / CM_WARPS;
+    if (nb > 148 * 16) nb = 148 * 16;
+    HOT_LAUNCHED(1);
+    coarse_monopole_kernel<<<(unsigned)nb, CM_WARPS * 32, 0, st>>>(a, far, farc, eps2);
+    return cudaGetLastError();
+}

@@ -135,7 +135,8 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
             // accepted cells -> P-C list
             if (acc) {
                 const uint32_t p = npc + __popc(macc & lt);
-                if (p < scap) { spc[p] = c; if (PER) ipc[p] = (uint8_t)im; }
+                // periodic: cells of the coarsest levels are marked; their monopoles are summed in fp64 (hot_periodic.cu)
+                if (p < scap) { spc[p] = (PER && lev <= HOT_COARSE_LEVEL) ? (c | HOT_COARSE_FLAG) : c; if (PER) ipc[p] = (uint8_t)im; }
             }
             npc += __popc(macc);
             // rejected leaves -> one body run each (a leaf holds <= 32 bodies except at the finest level)

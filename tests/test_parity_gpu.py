@@ -351,13 +351,12 @@ def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
     mtot = float(w.mass.astype(np.float64).sum())
     scale = 57.18721055 * mtot / w.size if w.periodic else 0.0
     # periodic: a body's acceleration is what is left of the pull of the 5^3 explicit boxes towards their
-    # centre, (4 pi / 3)(M / L^3) x with |x| up to L/2, after the far field cancels it; fp32 bounds the absolute
-    # error by ~1e-7 of that scale, which on a 256^3 lattice is 2.5e-5 of the net acceleration (R-14)
-    ascale = (4.0 * np.pi / 3.0) * mtot / w.size ** 2 * 0.5 if w.periodic else 0.0
-    ea = np.linalg.norm(ga - oa[m], axis=1) / (np.linalg.norm(oa[m], axis=1) + ascale)
+    # centre after the far field cancels it; the monopoles of the coarsest accepted cells, which carry that
+    # pull, are summed in fp64 so that the plain relative criterion holds at 256^3 too (R-14)
+    ea = np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)
     ep = np.abs(gp - op[m]) / (np.abs(op[m]) + scale)
-    print("full-size parity", cfg, "acc median", np.median(ea), "p99.9", np.quantile(ea, 0.999), "plain relative median",
-          np.median(np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)))
+    print("full-size parity", cfg, "acc median", np.median(ea), "p99.9", np.quantile(ea, 0.999),
+          "pot median", np.median(ep), "p99.9", np.quantile(ep, 0.999))
     assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
     assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
     # coverage invariant at full size: every body is in exactly one list entry's range per image
