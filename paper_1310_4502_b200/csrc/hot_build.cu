@@ -87,32 +87,67 @@ cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float 
 // ------------------------------------------------------------------------------------------
 // S2 LSD radix sort of (key, idx), 8-bit digits, 8 passes (PAPER.md:150 names an American-flag
 // radix sort for the on-node sort; a stable LSD sort gives the unique stable permutation).
-// Per pass: tile histogram -> row scan -> stable scatter.  Tile = 256 threads x 16 keys, keys
-// held warp-striped so the in-tile order is (warp, round, lane).
+// One pre-pass counts all eight digits of every key (2048 counters); each pass is then ONE kernel: a tile
+// (256 threads x 8 keys, held warp-striped so the in-tile order is (warp, round, lane)) ranks its keys,
+// publishes its digit counts, finds the counts of all earlier tiles by decoupled look-back and scatters.
+// Scratch (u32): [0,2048) digit counts, [2048,4096) their exclusive scans, [4096,4104) tile tickets,
+// then two look-back state arrays of 256 words per tile (a pass uses one and clears the other).
 // ------------------------------------------------------------------------------------------
 #define SORT_THREADS 256
 #define SORT_ITEMS 8
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_WARPS (SORT_THREADS / 32)
+#define SORT_STATE0 4352
+#define SORT_AGG 0x40000000u     // look-back word: the tile's own count of the digit
+#define SORT_PREFIX 0x80000000u  //                 the count of the digit in this and all earlier tiles
+#define SORT_VALUE 0x3fffffffu
 
 static inline int64_t sort_blocks(int64_t n) { return (n + SORT_TILE - 1) / SORT_TILE; }
-size_t sort_hist_elems(int64_t n) { return (size_t)256 * (size_t)sort_blocks(n) + 256; }
+size_t sort_hist_elems(int64_t n) { return (size_t)SORT_STATE0 + 2 * (size_t)256 * (size_t)sort_blocks(n); }
 
-__global__ void __launch_bounds__(SORT_THREADS) sort_hist_kernel(const uint64_t* __restrict__ key, int64_t n, int shift,
-                                                                 uint32_t* __restrict__ hist, int64_t nblk) {
-    __shared__ uint32_t h[256];
-    h[threadIdx.x] = 0;
-    __syncthreads();
-    int64_t base = (int64_t)blockIdx.x * SORT_TILE;
-    int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+__global__ void __launch_bounds__(256) sort_hist8_kernel(const uint64_t* __restrict__ key, int64_t n, uint32_t* __restrict__ ghist) {
+    __shared__ uint32_t h[8][256];
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
-        int64_t i = base + w * (32 * SORT_ITEMS) + k * 32 + lane;
-        if (i < n) atomicAdd(&h[(uint32_t)(key[i] >> shift) & 255u], 1u);
+    for (int p = 0; p < 8; ++p) h[p][threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t stride = (int64_t)gridDim.x * 256 * 4;
+    for (int64_t i0 = (int64_t)blockIdx.x * 256 * 4 + threadIdx.x; i0 < n; i0 += stride) {
+        uint64_t k[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) k[j] = i0 + j * 256 < n ? key[i0 + j * 256] : 0ull;
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            if (i0 + j * 256 < n) {
+#pragma unroll
+                for (int p = 0; p < 8; ++p) atomicAdd(&h[p][(uint32_t)(k[j] >> (8 * p)) & 255u], 1u);
+            }
     }
     __syncthreads();
-    hist[(int64_t)threadIdx.x * nblk + blockIdx.x] = h[threadIdx.x];
+#pragma unroll
+    for (int p = 0; p < 8; ++p) { uint32_t c = h[p][threadIdx.x]; if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c); }
 }
+// exclusive scan of each of the eight 256-bin histograms; one block of 256 threads
+__global__ void __launch_bounds__(256) sort_scan8_kernel(const uint32_t* __restrict__ ghist, uint32_t* __restrict__ dbase) {
+    __shared__ uint32_t wtot[8];
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    for (int p = 0; p < 8; ++p) {
+        uint32_t v = ghist[p * 256 + tid], x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (lane == 31) wtot[w] = x;
+        __syncthreads();
+        uint32_t off = 0;
+        for (int j = 0; j < w; ++j) off += wtot[j];
+        dbase[p * 256 + tid] = off + x - v;
+        __syncthreads();
+    }
+}
+__device__ __forceinline__ uint32_t ld_relaxed(const uint32_t* p) {
+    uint32_t v;
+    asm volatile("ld.relaxed.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
+__device__ __forceinline__ void st_relaxed(uint32_t* p, uint32_t v) { asm volatile("st.relaxed.gpu.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory"); }
 // in-place exclusive scan of each row (one block per row); totals[row] = row sum
 __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ data, int64_t rowlen, uint32_t* __restrict__ totals) {
     __shared__ uint32_t wsum[32];
@@ -149,46 +184,85 @@ __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ 
 #ifndef SORT_MINBLK
 #define SORT_MINBLK 5
 #endif
+#ifndef SORT_LOOK
+#define SORT_LOOK 8
+#endif
 __global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
                                                                     uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, int64_t n,
-                                                                    int shift, const uint32_t* __restrict__ hist,
-                                                                    const uint32_t* __restrict__ totals, int64_t nblk) {
+                                                                    int shift, const uint32_t* __restrict__ dbase, uint32_t* __restrict__ ticket,
+                                                                    uint32_t* __restrict__ state, uint32_t* __restrict__ state_next) {
     __shared__ uint32_t wcount[SORT_WARPS][256];
     __shared__ uint32_t gbase[256];   // global position of the tile's first key of each digit, minus its local start
     __shared__ uint32_t lstart[256];  // local start of each digit inside the digit-ordered tile
     __shared__ uint32_t wtot[SORT_WARPS];
+    __shared__ uint32_t s_tile;
     __shared__ uint64_t skey[SORT_TILE]; // the digit-ordered tile: keys first, then (same space) the values
-    __shared__ uint8_t sdig[SORT_TILE];
     uint32_t* const sval = reinterpret_cast<uint32_t*>(skey);
-    int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
+    uint32_t(*const wmask)[256] = reinterpret_cast<uint32_t(*)[256]>(skey); // the tile space is free until the ranks are known
 #pragma unroll
-    for (int j = 0; j < SORT_WARPS; ++j) wcount[j][tid] = 0;
+    for (int j = 0; j < SORT_WARPS; ++j) { wcount[j][tid] = 0; wmask[j][tid] = 0; }
+    lstart[tid] = 0;
+    if (tid == 0) s_tile = atomicAdd(ticket, 1u); // tiles are taken in launch order: every earlier tile is running or done
     __syncthreads();
-    int64_t base = (int64_t)blockIdx.x * SORT_TILE + w * (32 * SORT_ITEMS);
+    const int64_t tile = s_tile;
+    const int64_t t0 = tile * SORT_TILE;
+    const int cnt = (int)(n - t0 < SORT_TILE ? n - t0 : SORT_TILE);
+    const int l0 = w * (32 * SORT_ITEMS) + lane; // this thread's keys: tile positions l0 + 32 k
+    const uint64_t* const kt = kin + t0;
     uint64_t kk[SORT_ITEMS];
-    uint32_t rk[SORT_ITEMS]; // digit | rank << 8
+    uint32_t rk[SORT_ITEMS]; // digit | rank << 8, later the position in the digit-ordered tile
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) { // all loads first: the warp barriers below would serialise them
-        int64_t i = base + k * 32 + lane;
-        kk[k] = i < n ? kin[i] : ~0ull;
+    for (int k = 0; k < SORT_ITEMS; ++k) kk[k] = l0 + 32 * k < cnt ? kt[l0 + 32 * k] : ~0ull; // all loads first
+    // The tile's digit counts, by unordered shared-memory atomics, go out before the (long) ranking: the count of
+    // each digit in all earlier tiles is found by decoupled look-back while those tiles are at the same early point.
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k)
+        if (l0 + 32 * k < cnt) atomicAdd(&lstart[(uint32_t)(kk[k] >> shift) & 255u], 1u);
+    __syncthreads();
+    uint32_t excl = 0; // keys with digit tid in earlier tiles
+    {
+        const uint32_t mine = lstart[tid];
+        uint32_t* const mystate = state + tile * 256 + tid;
+        if (tile == 0) st_relaxed(mystate, mine | SORT_PREFIX);
+        else {
+            st_relaxed(mystate, mine | SORT_AGG);
+            // SORT_LOOK earlier tiles per round trip; an unpublished word is read again after a short sleep
+            const uint32_t* q = mystate - 256;
+            int64_t left = tile; // earlier tiles not yet added
+            bool done = false;
+            while (!done) {
+                uint32_t v[SORT_LOOK];
+#pragma unroll
+                for (int j = 0; j < SORT_LOOK; ++j) v[j] = j < left ? ld_relaxed(q - j * 256) : SORT_PREFIX;
+                int used = 0;
+#pragma unroll
+                for (int j = 0; j < SORT_LOOK; ++j) {
+                    const bool ok = !done && used == j && (v[j] & (SORT_AGG | SORT_PREFIX)) != 0u;
+                    if (ok) { excl += v[j] & SORT_VALUE; ++used; done = (v[j] & SORT_PREFIX) != 0u; }
+                }
+                q -= used * 256; left -= used;
+                if (used == 0) __nanosleep(40);
+            }
+            st_relaxed(mystate, (excl + mine) | SORT_PREFIX);
+        }
+        state_next[tile * 256 + tid] = 0u; // the next pass looks back through the other array
     }
-    uint32_t mm[SORT_ITEMS];
+    // Rank inside the warp's 8 x 32 keys.  The lanes holding the same digit find each other through a
+    // shared-memory atomicOr on a per-warp, per-digit lane mask (MATCH.ANY issues once per 64 clocks per SM
+    // on sm_100a -- 115 us of a pass at 2^24 keys; the mask costs five shared-memory operations).
+    const uint32_t below = (1u << lane) - 1u;
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) { // the 16 matches are independent: issue them back to back
-        int64_t i = base + k * 32 + lane;
-        uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
-        mm[k] = __match_any_sync(FULL, i < n ? d : 256u);
-    }
-#pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) { // ... then the (serial) per-warp digit counters
-        int64_t i = base + k * 32 + lane;
-        bool valid = i < n;
-        uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
-        uint32_t m = mm[k];
-        uint32_t r = __popc(m & ((1u << lane) - 1u));
-        uint32_t old = valid ? wcount[w][d] : 0;
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        const bool valid = l0 + 32 * k < cnt;
+        const uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
+        if (valid) atomicOr(&wmask[w][d], 1u << lane);
         __syncwarp();
-        if (valid && r == 0) wcount[w][d] = old + __popc(m);
+        const uint32_t m = valid ? wmask[w][d] : 0u;
+        const uint32_t old = valid ? wcount[w][d] : 0u;
+        const uint32_t r = __popc(m & below);
+        __syncwarp();
+        if (valid && r == 0) { wcount[w][d] = old + __popc(m); wmask[w][d] = 0u; }
         __syncwarp();
         rk[k] = d | ((old + r) << 8);
     }
@@ -209,61 +283,60 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel
         uint32_t off = 0;
         for (int j = 0; j < w; ++j) off += wtot[j];
         lstart[tid] = off + x - mine;
+        gbase[tid] = dbase[tid] + excl - (off + x - mine); // where the tile's run of this digit goes, minus its place in the tile
         __syncthreads();
-    }
-    { // global base of every digit = exclusive scan of the 256 row totals + this tile's offset inside the row
-        uint32_t v = totals[tid], x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
-        if (lane == 31) wtot[w] = x;
-        __syncthreads();
-        uint32_t off = 0;
-        for (int j = 0; j < w; ++j) off += wtot[j];
-        gbase[tid] = off + x - v + hist[(int64_t)tid * nblk + blockIdx.x] - lstart[tid];
     }
     // digit-ordered tile in shared memory: keys
+    const uint32_t* const vt = vin + t0;
     uint32_t vv[SORT_ITEMS];
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
-        int64_t i = base + k * 32 + lane;
-        vv[k] = i < n ? vin[i] : 0u;
-    }
+    for (int k = 0; k < SORT_ITEMS; ++k) vv[k] = l0 + 32 * k < cnt ? vt[l0 + 32 * k] : 0u;
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        int64_t i = base + k * 32 + lane;
-        rk[k] = i < n ? lstart[rk[k] & 255u] + wcount[w][rk[k] & 255u] + (rk[k] >> 8) : 0xffffffffu; // now: position in the tile
-        if (i < n) { skey[rk[k]] = kk[k]; sdig[rk[k]] = (uint8_t)((uint32_t)(kk[k] >> shift) & 255u); }
+        const uint32_t d = rk[k] & 255u;
+        rk[k] = lstart[d] + wcount[w][d] + (rk[k] >> 8); // now: position in the tile
+        if (l0 + 32 * k < cnt) skey[rk[k]] = kk[k];
     }
     __syncthreads();
-    const int64_t t0 = (int64_t)blockIdx.x * SORT_TILE;
-    const int cnt = (int)(n - t0 < SORT_TILE ? n - t0 : SORT_TILE);
+    uint32_t gb[SORT_ITEMS]; // destination of tile position p = k * 256 + tid, for the key and then the value
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        int p = k * SORT_THREADS + tid;
-        if (p < cnt) kout[gbase[sdig[p]] + (uint32_t)p] = skey[p];
+        const int p = k * SORT_THREADS + tid;
+        if (p < cnt) {
+            const uint64_t key = skey[p];
+            gb[k] = gbase[(uint32_t)(key >> shift) & 255u] + (uint32_t)p;
+            kout[gb[k]] = key;
+        }
     }
     __syncthreads();
     // ... then the values through the same space
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) if (rk[k] != 0xffffffffu) sval[rk[k]] = vv[k];
+    for (int k = 0; k < SORT_ITEMS; ++k) if (l0 + 32 * k < cnt) sval[rk[k]] = vv[k];
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
-        int p = k * SORT_THREADS + tid;
-        if (p < cnt) vout[gbase[sdig[p]] + (uint32_t)p] = sval[p];
+        const int p = k * SORT_THREADS + tid;
+        if (p < cnt) vout[gb[k]] = sval[p];
     }
 }
 cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st) {
-    int64_t nblk = sort_blocks(n);
-    uint32_t* totals = hist + (size_t)256 * nblk;
+    const int64_t nblk = sort_blocks(n);
+    uint32_t* const ghist = hist;
+    uint32_t* const dbase = hist + 2048;
+    uint32_t* const ticket = hist + 4096;
+    uint32_t* const state[2] = {hist + SORT_STATE0, hist + SORT_STATE0 + (size_t)256 * nblk};
+    cudaError_t e = cudaMemsetAsync(hist, 0, ((size_t)SORT_STATE0 + (size_t)256 * nblk) * sizeof(uint32_t), st); // counters, tickets, state[0]
+    if (e != cudaSuccess) return e;
+    HOT_LAUNCHED(2);
+    int64_t hb = (n + 1023) / 1024;
+    if (hb > 148 * 8) hb = 148 * 8;
+    sort_hist8_kernel<<<(unsigned)hb, 256, 0, st>>>(key[0], n, ghist);
+    sort_scan8_kernel<<<1, 256, 0, st>>>(ghist, dbase);
     int cur = 0;
     for (int pass = 0; pass < 8; ++pass) {
-        int shift = pass * 8;
-        HOT_LAUNCHED(3);
-        sort_hist_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], n, shift, hist, nblk);
-        scan_rows_kernel<<<256, 1024, 0, st>>>(hist, nblk, totals);
-        sort_scatter_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], idx[cur], key[cur ^ 1], idx[cur ^ 1], n, shift,
-                                                                     hist, totals, nblk);
+        HOT_LAUNCHED(1);
+        sort_scatter_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], idx[cur], key[cur ^ 1], idx[cur ^ 1], n, pass * 8, dbase + pass * 256,
+                                                                     ticket + pass, state[pass & 1], state[(pass & 1) ^ 1]);
         cur ^= 1;
     }
     // 8 passes: the result is back in buffer 0
