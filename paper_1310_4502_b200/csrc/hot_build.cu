@@ -88,13 +88,15 @@ cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float 
 // S2 LSD radix sort of (key, idx), 8-bit digits, 8 passes (PAPER.md:150 names an American-flag
 // radix sort for the on-node sort; a stable LSD sort gives the unique stable permutation).
 // One pre-pass counts all eight digits of every key (2048 counters); each pass is then ONE kernel: a tile
-// (256 threads x 8 keys, held warp-striped so the in-tile order is (warp, round, lane)) ranks its keys,
+// (256 threads x 16 keys, held warp-striped so the in-tile order is (warp, round, lane)) ranks its keys,
 // publishes its digit counts, finds the counts of all earlier tiles by decoupled look-back and scatters.
 // Scratch (u32): [0,2048) digit counts, [2048,4096) their exclusive scans, [4096,4104) tile tickets,
 // then two look-back state arrays of 256 words per tile (a pass uses one and clears the other).
 // ------------------------------------------------------------------------------------------
 #define SORT_THREADS 256
-#define SORT_ITEMS 8
+#ifndef SORT_ITEMS
+#define SORT_ITEMS 16
+#endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_WARPS (SORT_THREADS / 32)
 #define SORT_STATE0 4352
@@ -182,7 +184,7 @@ __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ 
 // Stable scatter of one tile: ranks by warp match_any, then the tile is put in digit order in shared
 // memory so that every run of equal digits leaves as one contiguous (coalesced) write.
 #ifndef SORT_MINBLK
-#define SORT_MINBLK 5
+#define SORT_MINBLK 3
 #endif
 #ifndef SORT_LOOK
 #define SORT_LOOK 8
@@ -248,7 +250,7 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel
         }
         state_next[tile * 256 + tid] = 0u; // the next pass looks back through the other array
     }
-    // Rank inside the warp's 8 x 32 keys.  The lanes holding the same digit find each other through a
+    // Rank inside the warp's 16 x 32 keys.  The lanes holding the same digit find each other through a
     // shared-memory atomicOr on a per-warp, per-digit lane mask (MATCH.ANY issues once per 64 clocks per SM
     // on sm_100a -- 115 us of a pass at 2^24 keys; the mask costs five shared-memory operations).
     const uint32_t below = (1u << lane) - 1u;
