@@ -266,7 +266,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     ea.ckey = t.ckey; ea.cfirst = t.cfirst; ea.ccount = t.ccount; ea.cchild = t.cchild; ea.cparent = t.cparent;
     ea.group = t.group; ea.hkey = t.hkey; ea.hval = t.hval; ea.hmask = t.hcap - 1; ea.maxprobe = g.d_flags + 1;
     CUDA_TRY(launch_tree_emit(ea, st));
-    CUDA_TRY(launch_tree_link(t.ckey, t.cparent, t.cmask, t.ncells, st));
+    CUDA_TRY(launch_tree_link(t.ckey, t.cparent, t.cmask, t.ncells, t.hkey, t.hval, t.hcap - 1, g.d_flags + 1, st));
     CUDA_TRY(launch_tree_finalize(t.ckey, t.cfirst, t.ccount, t.cmask, t.cchild, t.wcell, t.ncells, g.d_flags, st));
     CUDA_TRY(cudaEventRecord(g.ev[4], st));
     CUDA_TRY(cudaMemcpyAsync(flags, g.d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));

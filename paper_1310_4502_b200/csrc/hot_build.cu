@@ -383,10 +383,23 @@ __device__ __forceinline__ int first_diff_level(uint64_t a, uint64_t b) { // 1..
     return 21 - p / 3;
 }
 
+// 32 x 32 bit matrix across the warp: lane r gives row r, lane c receives column c (bit r = bit c of row r)
+__device__ __forceinline__ uint32_t transpose32(uint32_t x, int lane) {
+#pragma unroll
+    for (int s = 16; s >= 1; s >>= 1) {
+        const uint32_t m = s == 16 ? 0x0000ffffu : s == 8 ? 0x00ff00ffu : s == 4 ? 0x0f0f0f0fu : s == 2 ? 0x33333333u : 0x55555555u;
+        const uint32_t y = __shfl_xor_sync(FULL, x, s);
+        x = (lane & s) ? ((x & ~m) | ((y >> s) & m)) : ((x & m) | ((y << s) & ~m));
+    }
+    return x;
+}
+
 __global__ void __launch_bounds__(TREE_TILE) tree_levels_kernel(const uint64_t* __restrict__ skey, int64_t n, int nleaf, int ncrit,
                                                                 uint32_t* __restrict__ plev, uint32_t* __restrict__ counts, int64_t nblk) {
     __shared__ uint64_t sk[TREE_TILE + 2 * HOT_MAX_NCRIT];
-    __shared__ signed char wa[TREE_TILE + HOT_MAX_NCRIT + 32], wb[TREE_TILE + HOT_MAX_NCRIT + 32];
+    // v_q = 1 + cpl(key[q'], key[q'+W]) (0 outside the array), q' = T0 - W + q: plain (W < 32), or its prefix maximum inside
+    // 32-element chunks (sp) with the chunk maxima (sc); the suffix maximum of a thread's own element stays in a register
+    __shared__ uint8_t sp[TREE_TILE + HOT_MAX_NCRIT + 32], sc[(TREE_TILE + HOT_MAX_NCRIT) / 32 + 2];
     __shared__ uint32_t cnt[TREE_ROWS];
     const int tid = threadIdx.x, lane = tid & 31;
     const int64_t T0 = (int64_t)blockIdx.x * TREE_TILE;
@@ -403,42 +416,53 @@ __global__ void __launch_bounds__(TREE_TILE) tree_levels_kernel(const uint64_t* 
 #pragma unroll
     for (int which = 0; which < 2; ++which) {
         const int W = which ? ncrit : nleaf;
-        // w_p = cpl(key[p], key[p+W]) for global p in [T0-W, T0+TILE), -1 outside the array
         const int L = TREE_TILE + W;
-        for (int q = tid; q < L + 32; q += TREE_TILE) {
-            int64_t g = T0 - W + q;
-            signed char v = -1;
-            if (q < L && g >= 0 && g + W < n) v = (signed char)(first_diff_level(sk[q + H - W], sk[q + H]) - 1);
-            wa[q] = v;
+        // the level of body i is the maximum of v over q in [tid, tid + W]
+        int v[2];
+#pragma unroll
+        for (int r = 0; r < 2; ++r) {
+            const int q = tid + r * TREE_TILE;
+            const int64_t g = T0 - W + q;
+            v[r] = (q < L && g >= 0 && g + W < n) ? first_diff_level(sk[q + H - W], sk[q + H]) : 0;
         }
-        __syncthreads();
-        // sliding max over [i-W, i] (length W+1) by doubling: M_k[q] = max w[q .. q+2^k-1]
-        int K = 31 - __clz(W + 1);
-        signed char *src = wa, *dst = wb;
-        for (int k = 0; k < K; ++k) {
-            for (int q = tid; q < L; q += TREE_TILE) {
-                int q2 = q + (1 << k);
-                signed char a = src[q], b = q2 < L ? src[q2] : (signed char)-1;
-                dst[q] = a > b ? a : b;
+        int D;
+        if (W < 32) { // short window: read it
+            sp[tid] = (uint8_t)v[0];
+            if (tid < W) sp[tid + TREE_TILE] = (uint8_t)v[1];
+            __syncthreads();
+            D = v[0];
+            for (int j = 1; j <= W; ++j) D = max(D, (int)sp[tid + j]);
+        } else { // long window: rest of the own chunk, whole chunks, start of the last chunk
+            int suf = v[0];
+#pragma unroll
+            for (int r = 0; r < 2; ++r) {
+                if (r == 1 && (tid & ~31) >= W) break; // warp-uniform: no element of this warp lies below L
+                int s = v[r], p = v[r];
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { // out-of-range lanes return the caller's own value
+                    s = max(s, __shfl_down_sync(FULL, s, o));
+                    p = max(p, __shfl_up_sync(FULL, p, o));
+                }
+                const int q = tid + r * TREE_TILE;
+                sp[q] = (uint8_t)p;
+                if (lane == 0) sc[q >> 5] = (uint8_t)s;
+                if (r == 0) suf = s;
             }
             __syncthreads();
-            signed char* t = src; src = dst; dst = t;
+            const int qe = tid + W;
+            D = max(suf, (int)sp[qe]);
+            for (int c = (tid >> 5) + 1; c < (qe >> 5); ++c) D = max(D, (int)sc[c]);
         }
-        // position i-W is q = tid, position i is q = tid+W
-        signed char a = src[tid], b = src[tid + W - (1 << K) + 1];
-        int D = a > b ? a : b;
-        lev[which] = min(HOT_MAXLEVEL, D + 1);
+        lev[which] = min(HOT_MAXLEVEL, D);
         __syncthreads();
     }
     int b = 0;
     if (valid && i > 0) b = first_diff_level(sk[tid + H - 1], sk[tid + H]);
     const int Lleaf = lev[0], Lgroup = lev[1];
     if (valid) plev[i] = (uint32_t)b | ((uint32_t)Lleaf << 8) | ((uint32_t)Lgroup << 16);
-#pragma unroll 1
-    for (int l = 0; l < HOT_NLEVELS; ++l) {
-        uint32_t m = __ballot_sync(FULL, valid && b <= l && l <= Lleaf);
-        if (lane == 0 && m) atomicAdd(&cnt[l], (uint32_t)__popc(m));
-    }
+    // cells (l, i), b <= l <= Lleaf, counted per level: the lanes' level masks transposed give one level per lane
+    const uint32_t col = transpose32((valid && b <= Lleaf) ? (2u << Lleaf) - (1u << b) : 0u, lane);
+    if (lane < HOT_NLEVELS && col) atomicAdd(&cnt[lane], (uint32_t)__popc(col));
     {
         uint32_t m = __ballot_sync(FULL, valid && b <= Lgroup);
         if (lane == 0 && m) atomicAdd(&cnt[HOT_NLEVELS], (uint32_t)__popc(m));
@@ -473,83 +497,81 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
                                                               int32_t* __restrict__ cparent, GroupRec* __restrict__ group,
                                                               uint64_t* __restrict__ hkey, int32_t* __restrict__ hval, int64_t hmask,
                                                               int* __restrict__ maxprobe) {
-    __shared__ uint32_t wpre[HOT_NLEVELS + 1][32]; // per row, per warp: exclusive prefix inside the tile
-    __shared__ uint32_t boff[HOT_NLEVELS + 1];
+    // per level (row 22: groups) and warp, as lane masks: which bodies start a cell of the level; which bodies
+    // differ from their predecessor at or above the level (= where the cells of the level can end)
+    __shared__ uint32_t sE[HOT_NLEVELS + 1][32], sB[HOT_NLEVELS][32];
+    __shared__ uint32_t wpre[HOT_NLEVELS + 1][32]; // cells of the level in the earlier warps of the tile
+    __shared__ uint32_t boff[HOT_NLEVELS + 1];     // ... and in the earlier tiles
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-    const int64_t i = (int64_t)blockIdx.x * TREE_TILE + tid;
+    const int64_t T0 = (int64_t)blockIdx.x * TREE_TILE;
+    const int64_t i = T0 + tid;
     const bool valid = i < n;
-    uint32_t pl = valid ? plev[i] : 0xffffffu;
-    const int b = valid ? (int)(pl & 255u) : 99, Lleaf = valid ? (int)((pl >> 8) & 255u) : -1, Lgroup = valid ? (int)((pl >> 16) & 255u) : -1;
+    const uint32_t pl = valid ? plev[i] : 0u; // past the end: "differs at level 0", so that every cell ends at n
+    const int b = (int)(pl & 255u), Lleaf = valid ? (int)((pl >> 8) & 255u) : -1, Lgroup = valid ? (int)((pl >> 16) & 255u) : -1;
+    const bool starts = valid && b <= Lleaf;
     const uint32_t lt = (1u << lane) - 1u;
-#pragma unroll 1
-    for (int l = 0; l < HOT_NLEVELS; ++l) {
-        uint32_t m = __ballot_sync(FULL, b <= l && l <= Lleaf);
-        if (lane == 0) wpre[l][w] = __popc(m);
-    }
     {
-        uint32_t m = __ballot_sync(FULL, valid && b <= Lgroup);
-        if (lane == 0) wpre[HOT_NLEVELS][w] = __popc(m);
+        const uint32_t colE = transpose32(starts ? (2u << Lleaf) - (1u << b) : 0u, lane);
+        const uint32_t colB = transpose32(~((1u << b) - 1u), lane);
+        if (lane < HOT_NLEVELS) { sE[lane][w] = colE; sB[lane][w] = colB; }
+        const uint32_t gm = __ballot_sync(FULL, valid && b <= Lgroup);
+        if (lane == 0) sE[HOT_NLEVELS][w] = gm;
     }
     if (tid <= HOT_NLEVELS) boff[tid] = counts[(int64_t)tid * nblk + blockIdx.x];
     __syncthreads();
-    if (tid <= HOT_NLEVELS) {
-        uint32_t run = 0;
-        for (int j = 0; j < 32; ++j) { uint32_t t = wpre[tid][j]; wpre[tid][j] = run; run += t; }
+    if (w <= HOT_NLEVELS) { // warp l: exclusive prefix of row l over the warps
+        const uint32_t c = (uint32_t)__popc(sE[w][lane]);
+        uint32_t x = c;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        wpre[w][lane] = x - c;
     }
     __syncthreads();
-    const uint64_t mykey = valid ? skey[i] : 0;
-    int64_t prev_incl = 0;   // inclusive count at level l-1 (global rank inside the level)
-    int32_t prev_cell = -1;  // index of cell (l-1, i) if it exists
     uint32_t gcount = 0; int32_t gcell = -1;
+    if (starts) {
+        const uint64_t mykey = skey[i];
+        int32_t prev_cell = -1; // cell (l-1, i)
 #pragma unroll 1
-    for (int l = 0; l < HOT_NLEVELS; ++l) {
-        const bool exists = b <= l && l <= Lleaf;
-        uint32_t m = __ballot_sync(FULL, exists);
-        int64_t excl = (int64_t)boff[l] + wpre[l][w] + __popc(m & lt);
-        int64_t incl = excl + (exists ? 1 : 0);
-        if (exists) {
-            int32_t c = (int32_t)(LB.v[l] + excl);
+        for (int l = b; l <= Lleaf; ++l) {
+            const int32_t c = (int32_t)(LB.v[l] + boff[l] + wpre[l][w] + __popc(sE[l][w] & lt));
             const int sh = 63 - 3 * l;
-            uint64_t ck = mykey >> sh;
-            // end of the cell: first j > i whose key leaves the prefix (gallop + bisection)
-            int64_t lo = i, hi;
+            const uint64_t ck = mykey >> sh;
+            // end of the cell: the next body that differs from its predecessor at level <= l; in the tile by the masks,
+            // beyond it by gallop + bisection over the keys
+            int64_t hi;
             if (l == 0) hi = n;
             else {
-                int64_t step = 1, p = i + 1;
-                while (p < n && (skey[p] >> sh) == ck) { lo = p; step <<= 1; p = i + step; }
-                hi = p < n ? p : n;
-                while (hi - lo > 1) {
-                    int64_t mid = (lo + hi) >> 1;
-                    if ((skey[mid] >> sh) == ck) lo = mid; else hi = mid;
+                uint32_t m = sB[l][w] & ~(lt | (1u << lane));
+                int ww = w;
+                while (m == 0u && ++ww < 32) m = sB[l][ww];
+                if (m) hi = T0 + (ww << 5) + __ffs((int)m) - 1;
+                else { // the whole rest of the tile belongs to the cell (and the tile is full)
+                    int64_t lo = T0 + TREE_TILE - 1, step = 1, p = lo + 1;
+                    const int64_t from = lo;
+                    while (p < n && (skey[p] >> sh) == ck) { lo = p; step <<= 1; p = from + step; }
+                    hi = p < n ? p : n;
+                    while (hi - lo > 1) {
+                        int64_t mid = (lo + hi) >> 1;
+                        if ((skey[mid] >> sh) == ck) lo = mid; else hi = mid;
+                    }
                 }
             }
-            uint32_t cnt = (uint32_t)(hi - i);
+            const uint32_t cnt = (uint32_t)(hi - i);
             ckey[c] = ck; cfirst[c] = (uint32_t)i; ccount[c] = cnt;
-            cparent[c] = l == 0 ? -1 : (int32_t)(LB.v[l - 1] + prev_incl - 1);
+            int32_t parent = -1;
+            if (l > b) parent = prev_cell;
+            else if (l > 0) parent = (int32_t)(LB.v[l - 1] + boff[l - 1] + wpre[l - 1][w] + __popc(sE[l - 1][w] & (lt | (1u << lane)))) - 1;
+            cparent[c] = parent;
             if (l == Lleaf) cchild[c] = -1;
             if (prev_cell >= 0) cchild[prev_cell] = c; // cell (l-1, i) is internal: its first child starts at i too
             prev_cell = c;
             if (l == Lgroup) { gcount = cnt; gcell = c; }
-            // hash insert (open addressing, linear probing)
-            uint64_t h = hash64(ck) & (uint64_t)hmask;
-            int probe = 0;
-            while (true) {
-                unsigned long long old = atomicCAS((unsigned long long*)&hkey[h], 0ull, (unsigned long long)ck);
-                if (old == 0ull) { hval[h] = c; break; }
-                h = (h + 1) & (uint64_t)hmask; ++probe;
-            }
-            if (probe > 0 && probe > *((volatile int*)maxprobe)) atomicMax(maxprobe, probe);
-        } else prev_cell = -1;
-        prev_incl = incl;
-    }
-    {
-        bool isg = valid && b <= Lgroup;
-        uint32_t m = __ballot_sync(FULL, isg);
-        if (isg) {
-            int64_t r = (int64_t)boff[HOT_NLEVELS] + wpre[HOT_NLEVELS][w] + __popc(m & lt);
-            GroupRec g; g.first = (uint32_t)i; g.count = gcount; g.cell = (uint32_t)gcell; g.pad = 0;
-            group[r] = g;
         }
+    }
+    if (valid && b <= Lgroup) {
+        const int64_t r = (int64_t)boff[HOT_NLEVELS] + wpre[HOT_NLEVELS][w] + __popc(sE[HOT_NLEVELS][w] & lt);
+        GroupRec g; g.first = (uint32_t)i; g.count = gcount; g.cell = (uint32_t)gcell; g.pad = 0;
+        group[r] = g;
     }
 }
 cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
@@ -560,15 +582,28 @@ cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
                                                              a.cchild, a.cparent, a.group, a.hkey, a.hval, a.hmask, a.maxprobe);
     return cudaGetLastError();
 }
+// per cell: its octant bit into the parent's child mask, and the hash-table entry key -> cell (open addressing,
+// linear probing; one independent insert per thread, so the atomics' latency is covered by the other cells)
 __global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restrict__ ckey, const int32_t* __restrict__ cparent,
-                                                        uint32_t* __restrict__ cmask, int64_t ncells) {
-    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x + 1;
+                                                        uint32_t* __restrict__ cmask, int64_t ncells, uint64_t* __restrict__ hkey,
+                                                        int32_t* __restrict__ hval, int64_t hmask, int* __restrict__ maxprobe) {
+    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= ncells) return;
-    atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ckey[c] & 7ull));
+    const uint64_t ck = ckey[c];
+    if (c > 0) atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ck & 7ull));
+    uint64_t h = hash64(ck) & (uint64_t)hmask;
+    int probe = 0;
+    while (true) {
+        unsigned long long old = atomicCAS((unsigned long long*)&hkey[h], 0ull, (unsigned long long)ck);
+        if (old == 0ull) { hval[h] = (int32_t)c; break; }
+        h = (h + 1) & (uint64_t)hmask; ++probe;
+    }
+    if (probe > 0 && probe > *((volatile int*)maxprobe)) atomicMax(maxprobe, probe);
 }
-cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, cudaStream_t st) {
-    if (ncells > 1) HOT_LAUNCHED(1);
-    if (ncells > 1) tree_link_kernel<<<(unsigned)((ncells - 1 + 255) / 256), 256, 0, st>>>(ckey, cparent, cmask, ncells);
+cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, uint64_t* hkey, int32_t* hval,
+                             int64_t hmask, int* maxprobe, cudaStream_t st) {
+    HOT_LAUNCHED(1);
+    tree_link_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, st>>>(ckey, cparent, cmask, ncells, hkey, hval, hmask, maxprobe);
     return cudaGetLastError();
 }
 __global__ void __launch_bounds__(256) tree_finalize_kernel(const uint64_t* __restrict__ ckey, const uint32_t* __restrict__ cfirst,

@@ -91,7 +91,8 @@ struct TreeEmitArgs {
     GroupRec* group; uint64_t* hkey; int32_t* hval; int64_t hmask; int* maxprobe;
 };
 cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st);
-cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, cudaStream_t st);
+cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, uint64_t* hkey, int32_t* hval,
+                             int64_t hmask, int* maxprobe, cudaStream_t st);
 cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount,
                                  const uint32_t* cmask, const int32_t* cchild, WalkCell* wc,
                                  int64_t ncells, int* errflag, cudaStream_t st);
