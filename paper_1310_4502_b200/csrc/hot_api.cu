@@ -30,6 +30,7 @@ struct Ctx {
     std::vector<Slot> pool;
     int64_t bytes = 0;
     uint32_t *d_hist = nullptr, *d_counts = nullptr, *d_totals = nullptr;
+    int2* d_open = nullptr;
     // interaction lists (hot_forces)
     unsigned long long* d_tops = nullptr;
     double* d_farS = nullptr; // periodic: global moments of the box
@@ -214,6 +215,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(tree_alloc(&t.plev, (size_t)n));
     CUDA_TRY(tree_alloc(&d_hist, sort_hist_elems(n)));
     CUDA_TRY(tree_alloc(&d_counts, (size_t)rows * (size_t)nblk));
+    CUDA_TRY(tree_alloc(&g.d_open, (size_t)HOT_NLEVELS * (size_t)nblk));
     CUDA_TRY(tree_alloc(&d_totals, (size_t)rows));
     CUDA_TRY(cudaMemsetAsync(g.d_flags, 0, 4 * sizeof(int), st));
 
@@ -264,7 +266,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     ea.skey = t.key[0]; ea.plev = t.plev; ea.counts = d_counts; ea.n = n; ea.nblk = nblk;
     for (int l = 0; l <= HOT_NLEVELS; ++l) ea.level_base[l] = t.level_base[l];
     ea.ckey = t.ckey; ea.cfirst = t.cfirst; ea.ccount = t.ccount; ea.cchild = t.cchild; ea.cparent = t.cparent;
-    ea.group = t.group; ea.hkey = t.hkey; ea.hval = t.hval; ea.hmask = t.hcap - 1; ea.maxprobe = g.d_flags + 1;
+    ea.group = t.group; ea.open = g.d_open;
     CUDA_TRY(launch_tree_emit(ea, st));
     CUDA_TRY(launch_tree_link(t.ckey, t.cparent, t.cmask, t.ncells, t.hkey, t.hval, t.hcap - 1, g.d_flags + 1, st));
     CUDA_TRY(launch_tree_finalize(t.ckey, t.cfirst, t.ccount, t.cmask, t.cchild, t.wcell, t.ncells, g.d_flags, st));

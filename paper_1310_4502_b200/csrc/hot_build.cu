@@ -495,8 +495,7 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
                                                               uint64_t* __restrict__ ckey, uint32_t* __restrict__ cfirst,
                                                               uint32_t* __restrict__ ccount, int32_t* __restrict__ cchild,
                                                               int32_t* __restrict__ cparent, GroupRec* __restrict__ group,
-                                                              uint64_t* __restrict__ hkey, int32_t* __restrict__ hval, int64_t hmask,
-                                                              int* __restrict__ maxprobe) {
+                                                              int2* __restrict__ open) {
     // per level (row 22: groups) and warp, as lane masks: which bodies start a cell of the level; which bodies
     // differ from their predecessor at or above the level (= where the cells of the level can end)
     __shared__ uint32_t sE[HOT_NLEVELS + 1][32], sB[HOT_NLEVELS][32];
@@ -518,6 +517,7 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
         if (lane == 0) sE[HOT_NLEVELS][w] = gm;
     }
     if (tid <= HOT_NLEVELS) boff[tid] = counts[(int64_t)tid * nblk + blockIdx.x];
+    if (tid < HOT_NLEVELS) open[(int64_t)blockIdx.x * HOT_NLEVELS + tid] = make_int2(-1, -1);
     __syncthreads();
     if (w <= HOT_NLEVELS) { // warp l: exclusive prefix of row l over the warps
         const uint32_t c = (uint32_t)__popc(sE[w][lane]);
@@ -528,6 +528,7 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
     }
     __syncthreads();
     uint32_t gcount = 0; int32_t gcell = -1;
+    const int64_t grank = (int64_t)boff[HOT_NLEVELS] + wpre[HOT_NLEVELS][w] + __popc(sE[HOT_NLEVELS][w] & lt); // if a group starts here
     if (starts) {
         const uint64_t mykey = skey[i];
         int32_t prev_cell = -1; // cell (l-1, i)
@@ -536,8 +537,8 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
             const int32_t c = (int32_t)(LB.v[l] + boff[l] + wpre[l][w] + __popc(sE[l][w] & lt));
             const int sh = 63 - 3 * l;
             const uint64_t ck = mykey >> sh;
-            // end of the cell: the next body that differs from its predecessor at level <= l; in the tile by the masks,
-            // beyond it by gallop + bisection over the keys
+            // end of the cell: the next body that differs from its predecessor at level <= l, found in the tile's masks;
+            // the one cell per level that runs past the tile is left to tree_open_kernel (count 0 for now)
             int64_t hi;
             if (l == 0) hi = n;
             else {
@@ -545,16 +546,7 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
                 int ww = w;
                 while (m == 0u && ++ww < 32) m = sB[l][ww];
                 if (m) hi = T0 + (ww << 5) + __ffs((int)m) - 1;
-                else { // the whole rest of the tile belongs to the cell (and the tile is full)
-                    int64_t lo = T0 + TREE_TILE - 1, step = 1, p = lo + 1;
-                    const int64_t from = lo;
-                    while (p < n && (skey[p] >> sh) == ck) { lo = p; step <<= 1; p = from + step; }
-                    hi = p < n ? p : n;
-                    while (hi - lo > 1) {
-                        int64_t mid = (lo + hi) >> 1;
-                        if ((skey[mid] >> sh) == ck) lo = mid; else hi = mid;
-                    }
-                }
+                else { hi = i; open[(int64_t)blockIdx.x * HOT_NLEVELS + l] = make_int2(c, l == Lgroup ? (int)grank : -1); }
             }
             const uint32_t cnt = (uint32_t)(hi - i);
             ckey[c] = ck; cfirst[c] = (uint32_t)i; ccount[c] = cnt;
@@ -569,17 +561,42 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
         }
     }
     if (valid && b <= Lgroup) {
-        const int64_t r = (int64_t)boff[HOT_NLEVELS] + wpre[HOT_NLEVELS][w] + __popc(sE[HOT_NLEVELS][w] & lt);
         GroupRec g; g.first = (uint32_t)i; g.count = gcount; g.cell = (uint32_t)gcell; g.pad = 0;
-        group[r] = g;
+        group[grank] = g;
     }
+}
+// the cells that run past the tile of their first body (at most one per level and tile): end by gallop + bisection
+// over the sorted keys, one cell per thread
+__global__ void __launch_bounds__(256) tree_open_kernel(const int2* __restrict__ open, int64_t nslots, const uint64_t* __restrict__ skey, int64_t n,
+                                                        const uint32_t* __restrict__ cfirst, uint32_t* __restrict__ ccount,
+                                                        GroupRec* __restrict__ group) {
+    const int64_t s = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= nslots) return;
+    const int2 e = open[s];
+    if (e.x < 0) return;
+    const int l = (int)(s % HOT_NLEVELS);
+    const int sh = 63 - 3 * l;
+    const int64_t i = cfirst[e.x];
+    const uint64_t ck = skey[i] >> sh;
+    const int64_t from = (s / HOT_NLEVELS) * TREE_TILE + TREE_TILE - 1; // the tile's last body is inside the cell
+    int64_t lo = from, step = 1, p = from + 1;
+    while (p < n && (skey[p] >> sh) == ck) { lo = p; step <<= 1; p = from + step; }
+    int64_t hi = p < n ? p : n;
+    while (hi - lo > 1) {
+        int64_t mid = (lo + hi) >> 1;
+        if ((skey[mid] >> sh) == ck) lo = mid; else hi = mid;
+    }
+    ccount[e.x] = (uint32_t)(hi - i);
+    if (e.y >= 0) group[e.y].count = (uint32_t)(hi - i);
 }
 cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
     LevelBase LB;
     for (int l = 0; l <= HOT_NLEVELS; ++l) LB.v[l] = a.level_base[l];
-    HOT_LAUNCHED(1);
+    HOT_LAUNCHED(2);
     tree_emit_kernel<<<(unsigned)a.nblk, TREE_TILE, 0, st>>>(a.skey, a.plev, a.counts, a.n, a.nblk, LB, a.ckey, a.cfirst, a.ccount,
-                                                             a.cchild, a.cparent, a.group, a.hkey, a.hval, a.hmask, a.maxprobe);
+                                                             a.cchild, a.cparent, a.group, a.open);
+    const int64_t nslots = a.nblk * HOT_NLEVELS;
+    tree_open_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, st>>>(a.open, nslots, a.skey, a.n, a.cfirst, a.ccount, a.group);
     return cudaGetLastError();
 }
 // per cell: its octant bit into the parent's child mask, and the hash-table entry key -> cell (open addressing,

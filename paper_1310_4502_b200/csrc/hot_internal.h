@@ -88,7 +88,8 @@ struct TreeEmitArgs {
     const uint64_t* skey; const uint32_t* plev; const uint32_t* counts; int64_t n, nblk;
     int64_t level_base[HOT_NLEVELS + 1];
     uint64_t* ckey; uint32_t* cfirst; uint32_t* ccount; int32_t* cchild; int32_t* cparent;
-    GroupRec* group; uint64_t* hkey; int32_t* hval; int64_t hmask; int* maxprobe;
+    GroupRec* group;
+    int2* open; // [nblk][HOT_NLEVELS] scratch: the cells whose end lies beyond the tile of their first body
 };
 cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st);
 cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, uint64_t* hkey, int32_t* hval,
