@@ -258,7 +258,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(tree_alloc(&t.glpp, (size_t)t.ngroups));
     CUDA_TRY(tree_alloc(&t.hkey, (size_t)t.hcap));
     CUDA_TRY(tree_alloc(&t.hval, (size_t)t.hcap));
-    CUDA_TRY(cudaMemsetAsync(t.hkey, 0, sizeof(uint64_t) * (size_t)t.hcap, st));
+    CUDA_TRY(cudaMemsetAsync(t.hval, 0xff, sizeof(int32_t) * (size_t)t.hcap, st)); // -1: free slot
     CUDA_TRY(cudaMemsetAsync(t.cmask, 0, sizeof(uint32_t) * (size_t)t.ncells, st));
     CUDA_TRY(cudaMemsetAsync(t.glpc, 0, sizeof(uint32_t) * (size_t)t.ngroups, st));
     CUDA_TRY(cudaMemsetAsync(t.glpp, 0, sizeof(uint32_t) * (size_t)t.ngroups, st));

@@ -488,6 +488,7 @@ __device__ __forceinline__ uint64_t hash64(uint64_t k) {
     k ^= k >> 33; k *= 0xff51afd7ed558ccdull; k ^= k >> 33; k *= 0xc4ceb9fe1a85ec53ull; k ^= k >> 33;
     return k;
 }
+__device__ __forceinline__ uint64_t hash_slot(uint64_t key, uint64_t hmask) { return hash64(key) & hmask; } // home slot of a cell key
 struct LevelBase { int64_t v[HOT_NLEVELS + 1]; };
 
 __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __restrict__ skey, const uint32_t* __restrict__ plev,
@@ -604,18 +605,23 @@ cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
 __global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restrict__ ckey, const int32_t* __restrict__ cparent,
                                                         uint32_t* __restrict__ cmask, int64_t ncells, uint64_t* __restrict__ hkey,
                                                         int32_t* __restrict__ hval, int64_t hmask, int* __restrict__ maxprobe) {
-    int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncells) return;
-    const uint64_t ck = ckey[c];
-    if (c > 0) atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ck & 7ull));
-    uint64_t h = hash64(ck) & (uint64_t)hmask;
+    __shared__ int s_probe;
+    if (threadIdx.x == 0) s_probe = 0;
+    __syncthreads();
+    const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int probe = 0;
-    while (true) {
-        unsigned long long old = atomicCAS((unsigned long long*)&hkey[h], 0ull, (unsigned long long)ck);
-        if (old == 0ull) { hval[h] = (int32_t)c; break; }
-        h = (h + 1) & (uint64_t)hmask; ++probe;
+    if (c < ncells) {
+        const uint64_t ck = ckey[c];
+        if (c > 0) atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ck & 7ull));
+        uint64_t h = hash_slot(ck, (uint64_t)hmask);
+        while (atomicCAS(&hval[h], -1, (int32_t)c) != -1) { h = (h + 1) & (uint64_t)hmask; ++probe; } // a slot is free iff its value is -1
+        hkey[h] = ck;
     }
-    if (probe > 0 && probe > *((volatile int*)maxprobe)) atomicMax(maxprobe, probe);
+    // longest probe sequence: one global atomic per block at most (every thread reading the one counter queues in its L2 slice)
+    probe = __reduce_max_sync(FULL, probe);
+    if ((threadIdx.x & 31) == 0 && probe > 0) atomicMax(&s_probe, probe);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_probe > 0 && s_probe > *((volatile int*)maxprobe)) atomicMax(maxprobe, s_probe);
 }
 cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, uint64_t* hkey, int32_t* hval,
                              int64_t hmask, int* maxprobe, cudaStream_t st) {
@@ -657,11 +663,11 @@ __global__ void hash_lookup_kernel(const uint64_t* __restrict__ hkey, const int3
     uint64_t k = keys[q];
     int32_t r = -1;
     if (k != 0) {
-        uint64_t h = hash64(k) & (uint64_t)hmask;
+        uint64_t h = hash_slot(k, (uint64_t)hmask);
         while (true) {
-            uint64_t s = hkey[h];
-            if (s == k) { r = hval[h]; break; }
-            if (s == 0) break;
+            const int32_t v = hval[h];
+            if (v < 0) break;
+            if (hkey[h] == k) { r = v; break; }
             h = (h + 1) & (uint64_t)hmask;
         }
     }
