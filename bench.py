@@ -40,7 +40,7 @@ NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2, 16, 256): 7.650e9}
 # FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-SORT_BYTES_PER_BODY = 8 * 32          # 8 passes x (8 B histogram read + 12 B read + 12 B write)
+SORT_BYTES_PER_BODY = 8 + 8 * 24      # one 8 B read for the digit histograms + 8 passes x (12 B read + 12 B write)
 KEYGEN_BYTES_PER_BODY = 44          # 12 B pos + 4 B mass read; 8 B key + 4 B index + 16 B float4 body written
 GATHER_BYTES_PER_BODY = 36          # 4 B permutation + 16 B float4 gathered, 16 B written
 

@@ -362,7 +362,7 @@ cudaError_t launch_gather(const float4* bin, const uint32_t* perm, int64_t n, fl
 }
 
 // ------------------------------------------------------------------------------------------
-// S4/S5 tree from the sorted keys in one sweep (DESIGN.md "Tree build").
+// S4/S5 tree from the sorted keys in one sweep (DESIGN.md "The tree build").
 // For sorted position i:
 //   b_i      = level at which key[i-1] and key[i] first differ (0 for i = 0, 22 if equal)
 //   Lleaf_i  = level of the leaf holding i   = min(21, 1 + max_{j in [i-NLEAF,i]} cpl(key[j], key[j+NLEAF]))
