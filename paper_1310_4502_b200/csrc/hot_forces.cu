@@ -465,6 +465,51 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
     }
 }
 
+// one pass over the group's lists for sinks [c0, c0 + nc) with L = 1 << lgL lanes per source stream
+template <int ORDER, bool PER>
+__device__ __forceinline__ void run_chunk(const ForceArgs& P, const int w, const GroupRec g, const int64_t gi, const uint32_t c0,
+                                          const uint32_t nc, const int lgL, const int lane) {
+    const int S = (int)((nc + (1u << lgL) - 1) >> lgL);
+    if (S <= 1) eval_chunk<ORDER, PER, 1>(P, w, g, gi, c0, nc, lgL, lane);
+#if SMAX <= 2
+    else eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
+#elif SMAX <= 3
+    else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
+    else eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
+#else
+    else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 3) eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
+#endif
+#if SMAX <= 3
+#elif SMAX <= 4
+    else eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
+#else
+    else if (S == 4) eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 5) eval_chunk<ORDER, PER, 5>(P, w, g, gi, c0, nc, lgL, lane);
+#if SMAX <= 6
+    else eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
+#else
+    else if (S == 6) eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 7) eval_chunk<ORDER, PER, 7>(P, w, g, gi, c0, nc, lgL, lane);
+    else eval_chunk<ORDER, PER, 8>(P, w, g, gi, c0, nc, lgL, lane);
+#endif
+#endif
+}
+// smallest stream width that holds n sinks with at most SMAX per lane
+__device__ __forceinline__ int fit_lgL(uint32_t n) {
+    int lgL = 0;
+    while (((n + (1u << lgL) - 1) >> lgL) > SMAX) ++lgL;
+    return lgL;
+}
+// Relative time of a pass: L lanes per stream each spend (PLAN_A + PLAN_B * S) per source, 32 / L sources at a time;
+// PLAN_C is what a pass costs whatever its sinks (list reads, staging of the sources).
+#ifndef HOT_PLAN_A
+#define HOT_PLAN_A 1
+#define HOT_PLAN_B 3
+#define HOT_PLAN_C 12
+#endif
+__device__ __forceinline__ int pass_cost(int lgL, uint32_t n) { return (HOT_PLAN_A + HOT_PLAN_B * (int)((n + (1u << lgL) - 1) >> lgL)) << lgL; }
+
 template <int ORDER, bool PER>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -474,37 +519,26 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MIN
         const int64_t gi = P.g0 + (int64_t)__shfl_sync(FULL, q, 0);
         if (gi >= P.g1) break;
         const GroupRec g = P.group[gi];
-        // sinks in chunks of at most 32*SMAX (only groups larger than that need more than one pass; full
-        // chunks first: 6 sinks per lane is the most efficient blocking, measured against an even split)
+        // sinks in passes of at most 32*SMAX (full passes first: 6 sinks per lane is the most efficient blocking,
+        // measured against an even split).  The last nc sinks: one pass with ceil(nc / L) sinks per lane leaves up to
+        // L - 1 of its slots idle; when cheaper, a pass with floor(nc / L) full slots per lane is followed by a
+        // narrow pass for the < L sinks left over (e.g. 100 sinks: 32 x 3 + 4 x 1 instead of 32 x 4).
         for (uint32_t c0 = 0; c0 < g.count; c0 += 32 * SMAX) {
             const uint32_t nc = min((uint32_t)(32 * SMAX), g.count - c0);
-            int lgL = 0;
-            while (((nc + (1u << lgL) - 1) >> lgL) > SMAX) ++lgL;
-            const int S = (int)((nc + (1u << lgL) - 1) >> lgL);
-            if (S <= 1) eval_chunk<ORDER, PER, 1>(P, w, g, gi, c0, nc, lgL, lane);
-#if SMAX <= 2
-            else eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
-#elif SMAX <= 3
-            else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
-            else eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
-#else
-            else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
-            else if (S == 3) eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
-#endif
-#if SMAX <= 3
-#elif SMAX <= 4
-            else eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
-#else
-            else if (S == 4) eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
-            else if (S == 5) eval_chunk<ORDER, PER, 5>(P, w, g, gi, c0, nc, lgL, lane);
-#if SMAX <= 6
-            else eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
-#else
-            else if (S == 6) eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
-            else if (S == 7) eval_chunk<ORDER, PER, 7>(P, w, g, gi, c0, nc, lgL, lane);
-            else eval_chunk<ORDER, PER, 8>(P, w, g, gi, c0, nc, lgL, lane);
-#endif
-#endif
+            int lgL = fit_lgL(nc);
+            uint32_t nmain = nc;
+            int best = pass_cost(lgL, nc);
+#pragma unroll 1
+            for (int lg = 0; lg <= 5; ++lg) {
+                const uint32_t sf = nc >> lg;
+                if (sf < 1 || sf > SMAX) continue;
+                const uint32_t r = nc - (sf << lg);
+                if (r == 0) continue; // an exact fit is the single pass already
+                const int c = pass_cost(lg, sf << lg) + pass_cost(fit_lgL(r), r) + HOT_PLAN_C;
+                if (c < best) { best = c; lgL = lg; nmain = sf << lg; }
+            }
+            run_chunk<ORDER, PER>(P, w, g, gi, c0, nmain, lgL, lane);
+            if (nmain < nc) run_chunk<ORDER, PER>(P, w, g, gi, c0 + nmain, nc - nmain, fit_lgL(nc - nmain), lane);
         }
     }
 }
