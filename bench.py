@@ -28,10 +28,10 @@ if ROOT not in sys.path:
 # FMA = 2, add / multiply = 1, rsqrt = 1; a packed f32x2 instruction counts once per lane-operation.
 #   P-P:          4 add + 3 mul + 6 fma + rsqrt            = 20
 #   P-C order 0:  3 add + 3 mul + 7 fma + rsqrt            = 21
-#   P-C order 2:  6 add + 12 mul + 20 fma + rsqrt          = 59
-#   P-C order 4: 12 add + 70 mul + 95 fma + rsqrt          = 273   (as compiled: FADD2 / FMUL2 / FFMA2 per sink pair in SASS)
+#   P-C order 2:  4 add + 11 mul + 21 fma + rsqrt          = 58    (constant factors folded into the staged moments)
+#   P-C order 4: 10 add + 68 mul + 96 fma + rsqrt          = 271   (as compiled: FADD2 / FMUL2 / FFMA2 per sink pair in SASS)
 FLOPS_PP = 20
-FLOPS_PC = {0: 21, 2: 59, 4: 273}
+FLOPS_PC = {0: 21, 2: 58, 4: 271}
 # DRAM bytes of one forces_kernel launch from the ncu --set full capture of the default workload
 # (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 6.459 GB + dram__bytes_write.sum 1.191 GB;
 # the lists alone are 4 B x 0.88e9 entries = 3.5 GB of compulsory reads, acc + pot 0.27 GB of writes), at the

@@ -307,7 +307,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     // S6: moments, cached per build at the highest order asked so far
     if (t.mom_order < order) {
         if (!t.cellA) CUDA_TRY(tree_alloc(&t.cellA, (size_t)t.ncells));
-        if (order >= 2 && !t.cellM2) CUDA_TRY(tree_alloc(&t.cellM2, (size_t)t.ncells));
+        if (order >= 2 && !t.cellM2) { CUDA_TRY(tree_alloc(&t.cellM2, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellE2, (size_t)t.ncells)); }
         if (order >= 4 && !t.cellM34) CUDA_TRY(tree_alloc(&t.cellM34, (size_t)t.ncells));
         CUDA_TRY(launch_moments(t, order, st));
         t.mom_order = order;
@@ -387,7 +387,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     wa.tops = g.d_tops; wa.first_fail = g.d_flags + 3;
     wa.counter = g.d_counter; wa.stat = g.d_stat; wa.gstack = g.d_gstack; wa.gstack_cap = gcap; wa.errflag = g.d_flags + 2;
     ForceArgs a{};
-    a.wcell = t.wcell; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellM34 = t.cellM34;
+    a.wcell = t.wcell; a.cellA = t.cellA; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34;
     a.body = t.body; a.perm = t.idx[0]; a.group = t.group;
     a.pcoff = t.pcoff; a.ppoff = t.ppoff; a.lpc = t.glpc; a.lpp = t.glpp;
     a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic;

@@ -95,7 +95,7 @@ __device__ __forceinline__ void pp_one_self(const float4 ns, const bool same, co
 // Staged cell j of a batch: float4 slot q of the record sits at st[q*32 + j] (slot-major, so the
 // K streams of a warp read K consecutive float4 -- no bank conflicts for any K):
 //   slot 0: (-zx, -zy, -zz, -M0)  NEGATED centre of mass relative to the group origin, negated mass
-//   slot 1: (xx, xy, xz, yy)  slot 2: (yz, zz, t2, -)                        ORDER >= 2
+//   slot 1: 3 (xx, xy, xz, yy)  slot 2: (3 yz, 3 zz, 1.5 t2, 0.5 t2)          ORDER >= 2  (the cellE2 record)
 //   slots 3..11: M3 (10) M4 (15) t3 (3) T4 (6: xx xy xz yy yz zz) t4 (1) pad   ORDER >= 4
 template <int ORDER, class T>
 __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const float4 q2, const float* __restrict__ m,
@@ -111,18 +111,17 @@ __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const f
         a[3] = vfma(nm0, ri, a[3]);
         return;
     }
-    // quadrupole, with p5 = 1.5 u^-5/2 and w = -5 u^-1:
-    //   phi = -M0 ri + 0.5 t2 ri3 - p5 Q2;   a = R (-M0 ri3 + t2 p5 + w p5 Q2) + 2 p5 (M2 R)
-    const T p5 = ri3 * (splat<T>(1.5f) * ri2), w5 = splat<T>(-5.0f) * ri2;
+    // quadrupole with the staged N = 3 M2, 1.5 t2 and 0.5 t2; ri5 = u^-5/2, w7 = -2.5 u^-1:
+    //   phi = -M0 ri + 0.5 t2 ri3 - 0.5 ri5 (R N R);   a = R (-M0 ri3 + 1.5 t2 ri5 + w7 ri5 (R N R)) + ri5 (N R)
+    const T ri5 = ri3 * ri2, w7 = splat<T>(-2.5f) * ri2;
     const T Mx = vfma(splat<T>(q1.x), Rx, vfma(splat<T>(q1.y), Ry, splat<T>(q1.z) * Rz));
     const T My = vfma(splat<T>(q1.y), Rx, vfma(splat<T>(q1.w), Ry, splat<T>(q2.x) * Rz));
     const T Mz = vfma(splat<T>(q1.z), Rx, vfma(splat<T>(q2.x), Ry, splat<T>(q2.y) * Rz));
     const T Q2 = vfma(Mx, Rx, vfma(My, Ry, Mz * Rz));
-    const T t2 = splat<T>(q2.z), ht2 = splat<T>(0.5f * q2.z);
-    const T hQ = p5 * Q2;                                   // 1.5 u^-5/2 Q2
-    T cR = vfma(hQ, w5, vfma(t2, p5, nm0 * ri3));           // -7.5 u^-7/2 Q2 + 1.5 t2 u^-5/2 - M0 u^-3/2
-    T ph = vfma(ht2, ri3, nm0 * ri) - hQ;
-    const T D2 = p5 + p5;
+    const T hQ = ri5 * Q2;                                          // 3 u^-5/2 (R M2 R)
+    T cR = vfma(hQ, w7, vfma(splat<T>(q2.z), ri5, nm0 * ri3));      // -7.5 u^-7/2 Q2 + 1.5 t2 u^-5/2 - M0 u^-3/2
+    T ph = vfma(splat<T>(-0.5f), hQ, vfma(splat<T>(q2.w), ri3, nm0 * ri));
+    const T D2 = ri5;                                               // multiplies N R = 3 M2 R
     if (ORDER < 4) { // accumulate straight into the partial sums
         a[0] = vfma(cR, Rx, vfma(D2, Mx, a[0]));
         a[1] = vfma(cR, Ry, vfma(D2, My, a[1]));
@@ -336,7 +335,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 if (PER && (cnext & HOT_COARSE_FLAG)) cA.m0 = 0.f; // its monopole is summed in fp64 elsewhere (hot_periodic.cu)
                 float4* const dst = pcst + (b & 1) * NQ * BATCH + lane;
                 if (ORDER >= 2) {
-                    const float4* src = reinterpret_cast<const float4*>(P.cellM2 + c);
+                    const float4* src = reinterpret_cast<const float4*>(P.cellE2 + c);
                     cp_async16(dst + 1 * BATCH, src);
                     cp_async16(dst + 2 * BATCH, src + 1);
                 }

@@ -26,6 +26,8 @@ struct __align__(16) WalkCell { uint32_t x, y, z, w; };
 // per-cell expansion data (S6), gathered when a cell is accepted
 struct __align__(16) CellA { double zx, zy, zz; float m0; float t2; };   // centre of mass, mass, trace M2
 struct __align__(16) CellM2 { float xx, xy, xz, yy, yz, zz, t2, pad1; };     // t2 = trace
+// the same record as the P-C kernel stages it (cellE2): 3 xx, 3 xy, 3 xz, 3 yy, 3 yz, 3 zz, 1.5 t2, 0.5 t2 -- the
+// constant factors of the order-2 terms folded in once per cell instead of once per interaction
 // order 4: M3 (10) + M4 (15) + traces t3 (3), T4 (6), t4 (1) = 35 floats -> 36
 struct __align__(16) CellM34 { float v[36]; };
 
@@ -67,6 +69,7 @@ struct Tree {
     int mom_order = -1;
     CellA* cellA = nullptr;
     CellM2* cellM2 = nullptr;
+    CellM2* cellE2 = nullptr; // evaluation form of cellM2 (see CellM2)
     CellM34* cellM34 = nullptr;
 };
 
@@ -140,7 +143,7 @@ cudaError_t launch_group_stats(const GroupRec* group, const uint32_t* lpc, const
 
 // ---- interactions (hot_forces.cu): evaluates the lists of the groups [g0, g1) -------------------------
 struct ForceArgs {
-    const WalkCell* wcell; const CellA* cellA; const CellM2* cellM2; const CellM34* cellM34;
+    const WalkCell* wcell; const CellA* cellA; const CellM2* cellE2; const CellM34* cellM34;
     const float4* body; const uint32_t* perm; const GroupRec* group; int64_t g0, g1;
     const unsigned long long* pcoff; const unsigned long long* ppoff; const uint32_t* lpc; const uint32_t* lpp;
     const uint32_t* pclist; const uint32_t* pplist; const uint8_t* pcimg; const uint8_t* ppimg;

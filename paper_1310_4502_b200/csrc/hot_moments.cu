@@ -67,7 +67,7 @@ __device__ __forceinline__ void add_shifted(double* M, const double* C, double m
 
 template <int ORDER>
 __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, double zy, double zz, const double* M,
-                                           CellA* cellA, CellM2* cellM2, CellM34* cellM34) {
+                                           CellA* cellA, CellM2* cellM2, CellM2* cellE2, CellM34* cellM34) {
     CellA A; A.zx = zx; A.zy = zy; A.zz = zz; A.m0 = (float)m0; A.t2 = 0.f;
     if (ORDER >= 2) {
         CellM2 Q;
@@ -76,6 +76,10 @@ __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, doub
         A.t2 = Q.xx + Q.yy + Q.zz;
         Q.t2 = A.t2; Q.pad1 = 0.f; // the trace rides in the record the P-C kernel stages with cp.async
         cellM2[c] = Q;
+        CellM2 E; // what the P-C kernel stages: phi2 = 0.5 t2 ri^3 - 0.5 ri^5 R.(3 M2).R, a2 = R (1.5 t2 ri^5 - 2.5 ri^7 R.(3 M2).R) + ri^5 (3 M2) R
+        E.xx = 3.f * Q.xx; E.xy = 3.f * Q.xy; E.xz = 3.f * Q.xz; E.yy = 3.f * Q.yy; E.yz = 3.f * Q.yz; E.zz = 3.f * Q.zz;
+        E.t2 = 1.5f * A.t2; E.pad1 = 0.5f * A.t2;
+        cellE2[c] = E;
     }
     cellA[c] = A;
     if (ORDER >= 4) {
@@ -117,7 +121,7 @@ template <int ORDER>
 __global__ void __launch_bounds__(128) moments_level_kernel(int64_t cbeg, int64_t cend, const uint32_t* __restrict__ cfirst,
                                                             const uint32_t* __restrict__ ccount, const uint32_t* __restrict__ cmask,
                                                             const int32_t* __restrict__ cchild, const float4* __restrict__ body,
-                                                            CellA* __restrict__ cellA, CellM2* __restrict__ cellM2,
+                                                            CellA* __restrict__ cellA, CellM2* __restrict__ cellM2, CellM2* __restrict__ cellE2,
                                                             CellM34* __restrict__ cellM34) {
     int64_t c = cbeg + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= cend) return;
@@ -154,7 +158,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(int64_t cbeg, int64_
                 add_shifted<ORDER>(M, C, (double)A.m0, A.zx - zx, A.zy - zy, A.zz - zz);
             }
     }
-    store_cell<ORDER>(c, m0, zx, zy, zz, M, cellA, cellM2, cellM34);
+    store_cell<ORDER>(c, m0, zx, zy, zz, M, cellA, cellM2, cellE2, cellM34);
 }
 
 cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
@@ -164,11 +168,11 @@ cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
         unsigned nb = (unsigned)((ce - cb + 127) / 128);
         HOT_LAUNCHED(1);
         if (order >= 4)
-            moments_level_kernel<4><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellM34);
+            moments_level_kernel<4><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellE2, t.cellM34);
         else if (order >= 2)
-            moments_level_kernel<2><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellM34);
+            moments_level_kernel<2><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellE2, t.cellM34);
         else
-            moments_level_kernel<0><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellM34);
+            moments_level_kernel<0><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellE2, t.cellM34);
     }
     return cudaGetLastError();
 }
