@@ -26,6 +26,9 @@
 #define HOT_SMAX 6             // sinks per lane (tunable 2..8; 6 at 3 blocks/SM measured best with NCRIT >= 128)
 #endif
 #define SMAX HOT_SMAX
+#ifndef HOT_UNROLL2_S
+#define HOT_UNROLL2_S 6
+#endif
 #ifndef HOT_MINBLK
 #define HOT_MINBLK 3           // resident blocks per SM the order 0/2 kernels are compiled for
 #endif
@@ -362,6 +365,17 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 int j = strm;
                 float4 n0 = st[j < cnt ? j : 0], n1 = n0, n2 = n0;
                 if (ORDER >= 2) { n1 = st[32 + (j < cnt ? j : 0)]; n2 = st[64 + (j < cnt ? j : 0)]; }
+                if (S >= HOT_UNROLL2_S) { // two sources per trip: the sums stay in their registers (no copies at the loop end)
+#pragma unroll 2
+                while (j < cnt) {
+                    const float4 q0 = n0, q1 = n1, q2 = n2;
+                    j += K;
+                    const int jn = j < cnt ? j : strm;
+                    n0 = st[jn];
+                    if (ORDER >= 2) { n1 = st[32 + jn]; n2 = st[64 + jn]; }
+                    sk.template pc<ORDER>(q0, q1, q2, nullptr, eps2);
+                }
+                } else {
 #pragma unroll 1
                 while (j < cnt) {
                     const float4 q0 = n0, q1 = n1, q2 = n2;
@@ -370,6 +384,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                     n0 = st[jn];
                     if (ORDER >= 2) { n1 = st[32 + jn]; n2 = st[64 + jn]; }
                     sk.template pc<ORDER>(q0, q1, q2, nullptr, eps2);
+                }
                 }
             } else {
 #pragma unroll 1
