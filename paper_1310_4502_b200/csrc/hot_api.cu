@@ -22,6 +22,7 @@ struct Ctx {
     // scratch owned across calls
     int* d_flags = nullptr;               // [0] build error bits, [1] hash max probe, [2] forces error bits
     unsigned int* d_counter = nullptr;
+    uint4* d_items = nullptr; // work items of the interaction kernel
     unsigned long long* d_stat = nullptr; // 4 counters
     uint32_t* d_gstack = nullptr; size_t gstack_bytes = 0; int64_t gstack_cap = 0;
     // device buffers of the build, pooled across hot_build calls: a slot is keyed by the address of
@@ -102,7 +103,7 @@ void drop_build() { // forgets the build; its buffers stay pooled for the next o
 int ensure_scratch() {
     if (!g.d_flags) {
         CUDA_TRY(cudaMalloc(&g.d_flags, 4 * sizeof(int)));
-        CUDA_TRY(cudaMalloc(&g.d_counter, 2 * sizeof(unsigned int)));
+        CUDA_TRY(cudaMalloc(&g.d_counter, 18 * sizeof(unsigned int))); // walk and interaction schedulers, 16 work-item class counters
         CUDA_TRY(cudaMalloc(&g.d_stat, 4 * sizeof(unsigned long long)));
     }
     if (!g.ev_ready) {
@@ -394,7 +395,9 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
     a.far = t.periodic ? t.far : nullptr;
-    a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
+    a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1; a.cls = g.d_counter + 2;
+    CUDA_TRY(tree_alloc(&g.d_items, (size_t)(HOT_MAX_NCRIT / 64 + 2) * (size_t)ng)); // passes per group: full ones of >= 64 sinks, one split in two
+    a.items = g.d_items;
     // groups per round: all of them unless the arena is known (or found) to be too small.  The warps
     // take arena slices in completion order, so in an overfull round the FIRST group may be among
     // those that fail: then the round is repeated with a quarter of the groups.
@@ -411,7 +414,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (g.evx.size() < 5) { while (g.evx.size() < 5) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
     while (g0 < ng) {
         const int ff0 = INT_MAX;
-        CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
+        CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 18 * sizeof(unsigned int), st));
         CUDA_TRY(cudaMemsetAsync(g.d_tops, 0, 2 * sizeof(unsigned long long), st));
         CUDA_TRY(cudaMemcpyAsync(g.d_flags + 3, &ff0, sizeof(int), cudaMemcpyHostToDevice, st));
         wa.g0 = g0; wa.g1 = g0 + budget < ng ? g0 + budget : ng;
@@ -450,6 +453,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         usedpc += tops[0]; usedpp += tops[1];
         a.g0 = g0; a.g1 = F;
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
+        CUDA_TRY(launch_plan(a, st));
         if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
             CUDA_TRY(cudaEventRecord(g.evx[4], st));
             CUDA_TRY(launch_coarse_monopoles(a, t.far, t.farc, eps * eps, st));

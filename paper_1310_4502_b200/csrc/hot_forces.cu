@@ -524,36 +524,84 @@ __device__ __forceinline__ int fit_lgL(uint32_t n) {
 #endif
 __device__ __forceinline__ int pass_cost(int lgL, uint32_t n) { return (HOT_PLAN_A + HOT_PLAN_B * (int)((n + (1u << lgL) - 1) >> lgL)) << lgL; }
 
+// The passes of one group.  Sinks in passes of at most 32*SMAX (full passes first: 6 sinks per lane is the most
+// efficient blocking, measured against an even split).  The last nc sinks: one pass with ceil(nc / L) sinks per lane
+// leaves up to L - 1 of its slots idle; when cheaper, a pass with floor(nc / L) full slots per lane is followed by a
+// narrow pass for the < L sinks left over (e.g. 100 sinks: 32 x 3 + 4 x 1 instead of 32 x 4).
+template <class F>
+__device__ __forceinline__ void plan_group(const uint32_t count, F&& emit) {
+    for (uint32_t c0 = 0; c0 < count; c0 += 32 * SMAX) {
+        const uint32_t nc = min((uint32_t)(32 * SMAX), count - c0);
+        int lgL = fit_lgL(nc);
+        uint32_t nmain = nc;
+        int best = pass_cost(lgL, nc);
+#pragma unroll 1
+        for (int lg = 0; lg <= 5; ++lg) {
+            const uint32_t sf = nc >> lg;
+            if (sf < 1 || sf > SMAX) continue;
+            const uint32_t r = nc - (sf << lg);
+            if (r == 0) continue; // an exact fit is the single pass already
+            const int c = pass_cost(lg, sf << lg) + pass_cost(fit_lgL(r), r) + HOT_PLAN_C;
+            if (c < best) { best = c; lgL = lg; nmain = sf << lg; }
+        }
+        emit(c0, nmain, lgL);
+        if (nmain < nc) emit(c0 + nmain, nc - nmain, fit_lgL(nc - nmain));
+    }
+}
+#ifndef HOT_FORCES_PERIODIC_TU
+// Work items of the interaction kernel, one per pass: (group - g0, first sink, sinks, lg2 lanes per stream), ordered by
+// sinks per lane, 6 first.  The SMAX variants of the loops together do not fit the instruction cache (unrolling all of
+// them: 76 -> 105 ms); with the items in this order the warps of an SM run the same variant most of the time, and the
+// long items start first.  FILL = false counts the items per class, FILL = true places them.
+template <bool FILL>
+__global__ void __launch_bounds__(256) plan_kernel(const __grid_constant__ ForceArgs P) {
+    __shared__ unsigned int s_cnt[8], s_base[8];
+    if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
+    __syncthreads();
+    const int64_t gi = P.g0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const uint32_t count = gi < P.g1 ? P.group[gi].count : 0u;
+    plan_group(count, [&](uint32_t, uint32_t nc, int lgL) { atomicAdd(&s_cnt[SMAX - (int)((nc + (1u << lgL) - 1) >> lgL)], 1u); });
+    __syncthreads();
+    if (!FILL) {
+        if (threadIdx.x < 8 && s_cnt[threadIdx.x]) atomicAdd(&P.cls[threadIdx.x], s_cnt[threadIdx.x]);
+        return;
+    }
+    if (threadIdx.x < 8) { // the block's range in every class: start of the class + a cursor
+        unsigned int base = 0;
+        for (int c = 0; c < (int)threadIdx.x; ++c) base += P.cls[c];
+        s_base[threadIdx.x] = base + (s_cnt[threadIdx.x] ? atomicAdd(&P.cls[8 + threadIdx.x], s_cnt[threadIdx.x]) : 0u);
+        s_cnt[threadIdx.x] = 0;
+    }
+    __syncthreads();
+    plan_group(count, [&](uint32_t c0, uint32_t nc, int lgL) {
+        const int c = SMAX - (int)((nc + (1u << lgL) - 1) >> lgL);
+        P.items[s_base[c] + atomicAdd(&s_cnt[c], 1u)] = make_uint4((uint32_t)(gi - P.g0), c0, nc, (uint32_t)lgL);
+    });
+}
+cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st) {
+    const int64_t ng = a.g1 - a.g0;
+    if (ng <= 0) return cudaSuccess;
+    HOT_LAUNCHED(2);
+    plan_kernel<false><<<(unsigned)((ng + 255) / 256), 256, 0, st>>>(a);
+    plan_kernel<true><<<(unsigned)((ng + 255) / 256), 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+#endif
+
 template <int ORDER, bool PER>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    unsigned int total = lane < SMAX ? P.cls[lane] : 0u;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(FULL, total, o);
     while (true) {
         unsigned int q = 0;
         if (lane == 0) q = atomicAdd(P.counter, 1u);
-        const int64_t gi = P.g0 + (int64_t)__shfl_sync(FULL, q, 0);
-        if (gi >= P.g1) break;
-        const GroupRec g = P.group[gi];
-        // sinks in passes of at most 32*SMAX (full passes first: 6 sinks per lane is the most efficient blocking,
-        // measured against an even split).  The last nc sinks: one pass with ceil(nc / L) sinks per lane leaves up to
-        // L - 1 of its slots idle; when cheaper, a pass with floor(nc / L) full slots per lane is followed by a
-        // narrow pass for the < L sinks left over (e.g. 100 sinks: 32 x 3 + 4 x 1 instead of 32 x 4).
-        for (uint32_t c0 = 0; c0 < g.count; c0 += 32 * SMAX) {
-            const uint32_t nc = min((uint32_t)(32 * SMAX), g.count - c0);
-            int lgL = fit_lgL(nc);
-            uint32_t nmain = nc;
-            int best = pass_cost(lgL, nc);
-#pragma unroll 1
-            for (int lg = 0; lg <= 5; ++lg) {
-                const uint32_t sf = nc >> lg;
-                if (sf < 1 || sf > SMAX) continue;
-                const uint32_t r = nc - (sf << lg);
-                if (r == 0) continue; // an exact fit is the single pass already
-                const int c = pass_cost(lg, sf << lg) + pass_cost(fit_lgL(r), r) + HOT_PLAN_C;
-                if (c < best) { best = c; lgL = lg; nmain = sf << lg; }
-            }
-            run_chunk<ORDER, PER>(P, w, g, gi, c0, nmain, lgL, lane);
-            if (nmain < nc) run_chunk<ORDER, PER>(P, w, g, gi, c0 + nmain, nc - nmain, fit_lgL(nc - nmain), lane);
-        }
+        q = __shfl_sync(FULL, q, 0);
+        if (q >= total) break;
+        const uint4 it = P.items[q];
+        const int64_t gi = P.g0 + (int64_t)it.x;
+        run_chunk<ORDER, PER>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
     }
 }
 

@@ -151,9 +151,12 @@ struct ForceArgs {
     float eps2; int order; int periodic;
     double lo[3], size;
     float* acc; float* pot;
-    unsigned int* counter;        // dynamic group scheduler
+    unsigned int* counter;        // dynamic scheduler over the work items
+    uint4* items;                 // one per pass of a group, ordered by sinks per lane (launch_plan)
+    unsigned int* cls;            // [0..7] items per class (SMAX - sinks per lane), [8..15] fill cursors
 };
-cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st);
+cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st);   // fills items / cls for groups [g0, g1); cls must be zero
+cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st); // after launch_plan
 
 // ---- periodic far field (hot_periodic.cu) ------------------------------------------------------------
 void far_coefficients(double* out165);                    // host: Taylor coefficients of psi_sm, degree-major
