@@ -26,6 +26,11 @@
 #define HOT_SMAX 6             // sinks per lane (tunable 2..8; 6 at 3 blocks/SM measured best with NCRIT >= 128)
 #endif
 #define SMAX HOT_SMAX
+#ifndef HOT_PP_UNROLL
+#define HOT_PP_UNROLL 2
+#endif
+#define HOT_STR(x) #x
+#define HOT_UNROLL(n) _Pragma(HOT_STR(unroll n))
 #ifndef HOT_UNROLL2_S
 #define HOT_UNROLL2_S 6
 #endif
@@ -434,7 +439,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
             {
                 int j = strm;
                 float4 nx = st[j < cnt ? j : 0];
-#pragma unroll 1
+HOT_UNROLL(HOT_PP_UNROLL)
                 while (j < cnt) {
                     const float4 sb = nx;
                     j += K;
