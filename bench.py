@@ -33,10 +33,10 @@ if ROOT not in sys.path:
 FLOPS_PP = 20
 FLOPS_PC = {0: 21, 2: 58, 4: 271}
 # DRAM bytes of one forces_kernel launch from the ncu --set full capture of the default workload
-# (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 6.834 GB + dram__bytes_write.sum 1.193 GB;
+# (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 14.563 GB + dram__bytes_write.sum 1.201 GB;
 # the lists alone are 4 B x 0.88e9 entries = 3.5 GB of compulsory reads, acc + pot 0.27 GB of writes), at the
 # default bucket sizes NLEAF 16 / NCRIT 256; other workloads: null
-NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2, 16, 256): 8.027e9}
+NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2, 16, 256): 15.764e9}
 # FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
