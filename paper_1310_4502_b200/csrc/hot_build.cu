@@ -40,12 +40,12 @@ __device__ __forceinline__ uint64_t body_key(float x, float y, float z, float lo
     uint32_t ix = grid_coord(x, lox, inv, bad), iy = grid_coord(y, loy, inv, bad), iz = grid_coord(z, loz, inv, bad);
     return (1ull << 63) | (spread21(ix) << 2) | (spread21(iy) << 1) | spread21(iz);
 }
-// 4 bodies per thread: three 128-bit loads, two 128-bit key stores, one 128-bit index store
+// 4 bodies per thread: three 128-bit loads, two 128-bit key stores (the sort's first pass takes the index from the position)
 // Also writes the bodies as aligned float4 (x,y,z,m) in the caller's order: the gather after the sort
 // then fetches one 32-byte sector per body instead of the 3-4 sectors of the separate pos / mass arrays.
 __global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ pos, const float* __restrict__ mass, int64_t n, float lox,
                                                      float loy, float loz, float inv, uint64_t* __restrict__ key,
-                                                     uint32_t* __restrict__ idx, float4* __restrict__ bin, int* __restrict__ errflag, int vec) {
+                                                     float4* __restrict__ bin, int* __restrict__ errflag, int vec) {
     int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; // quad index
     int64_t i0 = q * 4;
     if (i0 >= n) return;
@@ -60,7 +60,6 @@ __global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ p
         ulonglong2* ko = reinterpret_cast<ulonglong2*>(key + i0);
         ko[0] = make_ulonglong2(k0, k1);
         ko[1] = make_ulonglong2(k2, k3);
-        *reinterpret_cast<uint4*>(idx + i0) = make_uint4((uint32_t)i0, (uint32_t)i0 + 1, (uint32_t)i0 + 2, (uint32_t)i0 + 3);
         const float4 m = __ldg(reinterpret_cast<const float4*>(mass) + q);
         bin[i0] = make_float4(a.x, a.y, a.z, m.x);
         bin[i0 + 1] = make_float4(a.w, b.x, b.y, m.y);
@@ -69,18 +68,17 @@ __global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ p
     } else {
         for (int64_t i = i0; i < n && i < i0 + 4; ++i) {
             key[i] = body_key(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], lox, loy, loz, inv, bad);
-            idx[i] = (uint32_t)i;
             bin[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
         }
     }
     if (bad) atomicOr(errflag, 1);
 }
 cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float lox, float loy, float loz, float inv,
-                          uint64_t* key, uint32_t* idx, float4* bin, int* errflag, cudaStream_t st) {
+                          uint64_t* key, float4* bin, int* errflag, cudaStream_t st) {
     int64_t quads = (n + 3) / 4;
     int vec = ((reinterpret_cast<uintptr_t>(pos) | reinterpret_cast<uintptr_t>(mass)) & 15u) == 0; // 128-bit loads need 16-byte aligned bases
     HOT_LAUNCHED(1);
-    keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, mass, n, lox, loy, loz, inv, key, idx, bin, errflag, vec);
+    keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, mass, n, lox, loy, loz, inv, key, bin, errflag, vec);
     return cudaGetLastError();
 }
 
@@ -181,54 +179,108 @@ __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ 
     }
     if (threadIdx.x == 0) totals[blockIdx.x] = carry;
 }
-// Stable scatter of one tile: ranks by warp match_any, then the tile is put in digit order in shared
-// memory so that every run of equal digits leaves as one contiguous (coalesced) write.
+// Stable scatter of one tile.  PASS is a template parameter so that a digit is one byte of one key half (PRMT);
+// FULLT marks a full tile (every tile but the last): no per-key bounds predicates.
+// Shared memory: the digit-ordered tile (keys 32 KB + values 16 KB, dynamic) and 10.5 KB of counters.
 #ifndef SORT_MINBLK
 #define SORT_MINBLK 3
 #endif
 #ifndef SORT_LOOK
-#define SORT_LOOK 8
+#define SORT_LOOK 4
 #endif
-__global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
-                                                                    uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, int64_t n,
-                                                                    int shift, const uint32_t* __restrict__ dbase, uint32_t* __restrict__ ticket,
-                                                                    uint32_t* __restrict__ state, uint32_t* __restrict__ state_next) {
-    __shared__ uint32_t wcount[SORT_WARPS][256];
-    __shared__ uint32_t gbase[256];   // global position of the tile's first key of each digit, minus its local start
-    __shared__ uint32_t lstart[256];  // local start of each digit inside the digit-ordered tile
-    __shared__ uint32_t wtot[SORT_WARPS];
-    __shared__ uint32_t s_tile;
-    __shared__ uint64_t skey[SORT_TILE]; // the digit-ordered tile: keys first, then (same space) the values
-    uint32_t* const sval = reinterpret_cast<uint32_t*>(skey);
+#define SORT_SMEM_BYTES (SORT_TILE * 12)
+template <int PASS> __device__ __forceinline__ uint32_t sort_digit(uint64_t k) {
+    const uint32_t h = PASS < 4 ? (uint32_t)k : (uint32_t)(k >> 32);
+    return __byte_perm(h, 0u, 0x4440u + (PASS & 3));
+}
+struct SortShared {
+    uint32_t wcount[SORT_WARPS][256]; // per warp and digit: keys ranked so far; later the warp's start inside the tile
+    uint32_t gbase[256];              // global position of the tile's first key of each digit, minus its local start
+    uint32_t wtot[SORT_WARPS];
+    uint32_t tile;
+};
+template <int PASS, bool FULLT>
+__device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __restrict__ skey, const int64_t tile, const int cnt,
+                                                  const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+                                                  uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
+                                                  const uint32_t* __restrict__ dbase, uint32_t* __restrict__ state,
+                                                  uint32_t* __restrict__ state_next) {
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
-    uint32_t(*const wmask)[256] = reinterpret_cast<uint32_t(*)[256]>(skey); // the tile space is free until the ranks are known
-#pragma unroll
-    for (int j = 0; j < SORT_WARPS; ++j) { wcount[j][tid] = 0; wmask[j][tid] = 0; }
-    lstart[tid] = 0;
-    if (tid == 0) s_tile = atomicAdd(ticket, 1u); // tiles are taken in launch order: every earlier tile is running or done
-    __syncthreads();
-    const int64_t tile = s_tile;
+    uint32_t* const sval = reinterpret_cast<uint32_t*>(skey + SORT_TILE);
+    // two per-warp lane-mask arrays, used by alternate ranking rounds; the tile space is free until the ranks are known
+    uint32_t* const wm0 = reinterpret_cast<uint32_t*>(skey) + w * 256;
+    uint32_t* const wm1 = wm0 + SORT_WARPS * 256;
+    uint32_t* const wc = sh.wcount[w];
     const int64_t t0 = tile * SORT_TILE;
-    const int cnt = (int)(n - t0 < SORT_TILE ? n - t0 : SORT_TILE);
     const int l0 = w * (32 * SORT_ITEMS) + lane; // this thread's keys: tile positions l0 + 32 k
-    const uint64_t* const kt = kin + t0;
+    const uint64_t* const kt = kin + t0 + l0;
     uint64_t kk[SORT_ITEMS];
-    uint32_t rk[SORT_ITEMS]; // digit | rank << 8, later the position in the digit-ordered tile
+    uint32_t rk[SORT_ITEMS]; // rank among the warp's keys of the same digit, later the position in the digit-ordered tile
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) kk[k] = l0 + 32 * k < cnt ? kt[l0 + 32 * k] : ~0ull; // all loads first
-    // The tile's digit counts, by unordered shared-memory atomics, go out before the (long) ranking: the count of
-    // each digit in all earlier tiles is found by decoupled look-back while those tiles are at the same early point.
+    for (int k = 0; k < SORT_ITEMS; ++k) kk[k] = (FULLT || l0 + 32 * k < cnt) ? __ldg(kt + 32 * k) : ~0ull; // all loads first
+    // Rank inside the warp's 16 x 32 keys.  The lanes holding the same digit find each other through a
+    // shared-memory atomicOr on a per-warp, per-digit lane mask (MATCH.ANY issues once per 64 clocks per SM
+    // on sm_100a -- 115 us of a pass at 2^24 keys; eight ballots per key are no faster than the mask).  Round k
+    // uses mask array k & 1: its leader clears the word after the round's reads, and the next atomicOr on that
+    // array is two warp barriers later.
+    const uint32_t lanebit = 1u << lane, below = lanebit - 1u;
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k)
-        if (l0 + 32 * k < cnt) atomicAdd(&lstart[(uint32_t)(kk[k] >> shift) & 255u], 1u);
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        const bool valid = FULLT || l0 + 32 * k < cnt;
+        const uint32_t d = sort_digit<PASS>(kk[k]);
+        uint32_t* const mp = ((k & 1) ? wm1 : wm0) + d;
+        if (valid) atomicOr(mp, lanebit);
+        __syncwarp();
+        const uint32_t m = valid ? *mp : 0u;
+        const uint32_t old = wc[d];
+        const uint32_t r = __popc(m & below);
+        __syncwarp();
+        if (valid && r == 0) { wc[d] = old + __popc(m); *mp = 0u; }
+        rk[k] = old + r;
+    }
     __syncthreads();
-    uint32_t excl = 0; // keys with digit tid in earlier tiles
+    // The tile's count of digit tid (the column sum of the warps' counts) is published now; the counts of the earlier
+    // tiles are looked up after the tile has been laid out in digit order, when most of them have been published.
+    uint32_t mine = 0;
+#pragma unroll
+    for (int j = 0; j < SORT_WARPS; ++j) mine += sh.wcount[j][tid];
+    uint32_t* const mystate = state + tile * 256 + tid;
+    st_relaxed(mystate, mine | (tile == 0 ? SORT_PREFIX : SORT_AGG));
+    state_next[tile * 256 + tid] = 0u; // the next pass looks back through the other array
+    uint32_t off; // start of digit tid in the tile (exclusive scan of the counts)
     {
-        const uint32_t mine = lstart[tid];
-        uint32_t* const mystate = state + tile * 256 + tid;
-        if (tile == 0) st_relaxed(mystate, mine | SORT_PREFIX);
-        else {
-            st_relaxed(mystate, mine | SORT_AGG);
+        uint32_t x = mine;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (lane == 31) sh.wtot[w] = x;
+        __syncthreads();
+        off = x - mine;
+#pragma unroll
+        for (int j = 0; j < SORT_WARPS; ++j) off += j < w ? sh.wtot[j] : 0u;
+        uint32_t run = off; // ... and of every warp's keys inside the digit
+#pragma unroll
+        for (int j = 0; j < SORT_WARPS; ++j) { const uint32_t t = sh.wcount[j][tid]; sh.wcount[j][tid] = run; run += t; }
+        __syncthreads();
+    }
+    // digit-ordered tile in shared memory: keys ...
+#pragma unroll
+    for (int k = 0; k < SORT_ITEMS; ++k) {
+        rk[k] += wc[sort_digit<PASS>(kk[k])]; // now: position in the tile
+        if (FULLT || l0 + 32 * k < cnt) skey[rk[k]] = kk[k];
+    }
+    // The values are fetched now and arrive while the keys leave (pass 0: the index is the key's position).
+    uint32_t vv[SORT_ITEMS];
+    if (PASS == 0) {
+#pragma unroll
+        for (int k = 0; k < SORT_ITEMS; ++k) vv[k] = (uint32_t)(t0 + l0) + 32u * k;
+    } else {
+        const uint32_t* const vt = vin + t0 + l0;
+#pragma unroll
+        for (int k = 0; k < SORT_ITEMS; ++k) vv[k] = (FULLT || l0 + 32 * k < cnt) ? __ldg(vt + 32 * k) : 0u;
+    }
+    {
+        uint32_t excl = 0; // keys with digit tid in earlier tiles
+        if (tile != 0) {
             // SORT_LOOK earlier tiles per round trip; an unpublished word is read again after a short sleep
             const uint32_t* q = mystate - 256;
             int64_t left = tile; // earlier tiles not yet added
@@ -248,78 +300,61 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel
             }
             st_relaxed(mystate, (excl + mine) | SORT_PREFIX);
         }
-        state_next[tile * 256 + tid] = 0u; // the next pass looks back through the other array
-    }
-    // Rank inside the warp's 16 x 32 keys.  The lanes holding the same digit find each other through a
-    // shared-memory atomicOr on a per-warp, per-digit lane mask (MATCH.ANY issues once per 64 clocks per SM
-    // on sm_100a -- 115 us of a pass at 2^24 keys; the mask costs five shared-memory operations).
-    const uint32_t below = (1u << lane) - 1u;
-#pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
-        const bool valid = l0 + 32 * k < cnt;
-        const uint32_t d = (uint32_t)(kk[k] >> shift) & 255u;
-        if (valid) atomicOr(&wmask[w][d], 1u << lane);
-        __syncwarp();
-        const uint32_t m = valid ? wmask[w][d] : 0u;
-        const uint32_t old = valid ? wcount[w][d] : 0u;
-        const uint32_t r = __popc(m & below);
-        __syncwarp();
-        if (valid && r == 0) { wcount[w][d] = old + __popc(m); wmask[w][d] = 0u; }
-        __syncwarp();
-        rk[k] = d | ((old + r) << 8);
-    }
-    __syncthreads();
-    uint32_t mine; // this digit's count in the tile
-    { // exclusive prefix over the warps of the tile, per digit
-        uint32_t run = 0;
-#pragma unroll
-        for (int j = 0; j < SORT_WARPS; ++j) { uint32_t t = wcount[j][tid]; wcount[j][tid] = run; run += t; }
-        mine = run;
-    }
-    { // local start of every digit = exclusive scan of the tile's digit counts
-        uint32_t x = mine;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
-        if (lane == 31) wtot[w] = x;
-        __syncthreads();
-        uint32_t off = 0;
-        for (int j = 0; j < w; ++j) off += wtot[j];
-        lstart[tid] = off + x - mine;
-        gbase[tid] = dbase[tid] + excl - (off + x - mine); // where the tile's run of this digit goes, minus its place in the tile
-        __syncthreads();
-    }
-    // digit-ordered tile in shared memory: keys
-    const uint32_t* const vt = vin + t0;
-    uint32_t vv[SORT_ITEMS];
-#pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) vv[k] = l0 + 32 * k < cnt ? vt[l0 + 32 * k] : 0u;
-#pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) {
-        const uint32_t d = rk[k] & 255u;
-        rk[k] = lstart[d] + wcount[w][d] + (rk[k] >> 8); // now: position in the tile
-        if (l0 + 32 * k < cnt) skey[rk[k]] = kk[k];
+        sh.gbase[tid] = dbase[tid] + excl - off; // where the tile's run of this digit goes, minus its place in the tile
     }
     __syncthreads();
     uint32_t gb[SORT_ITEMS]; // destination of tile position p = k * 256 + tid, for the key and then the value
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         const int p = k * SORT_THREADS + tid;
-        if (p < cnt) {
+        if (FULLT || p < cnt) {
             const uint64_t key = skey[p];
-            gb[k] = gbase[(uint32_t)(key >> shift) & 255u] + (uint32_t)p;
+            gb[k] = sh.gbase[sort_digit<PASS>(key)] + (uint32_t)p;
             kout[gb[k]] = key;
         }
     }
-    __syncthreads();
-    // ... then the values through the same space
+    // ... then the values (their own space: no barrier between)
 #pragma unroll
-    for (int k = 0; k < SORT_ITEMS; ++k) if (l0 + 32 * k < cnt) sval[rk[k]] = vv[k];
+    for (int k = 0; k < SORT_ITEMS; ++k)
+        if (FULLT || l0 + 32 * k < cnt) sval[rk[k]] = vv[k];
     __syncthreads();
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
         const int p = k * SORT_THREADS + tid;
-        if (p < cnt) vout[gb[k]] = sval[p];
+        if (FULLT || p < cnt) vout[gb[k]] = sval[p];
     }
+}
+template <int PASS>
+__global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel(const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
+                                                                    uint64_t* __restrict__ kout, uint32_t* __restrict__ vout, int64_t n,
+                                                                    const uint32_t* __restrict__ dbase, uint32_t* __restrict__ ticket,
+                                                                    uint32_t* __restrict__ state, uint32_t* __restrict__ state_next) {
+    __shared__ SortShared sh;
+    extern __shared__ __align__(16) uint64_t sort_tile_space[];
+    const int tid = threadIdx.x;
+    uint32_t* const z = reinterpret_cast<uint32_t*>(sort_tile_space); // both mask arrays
+#pragma unroll
+    for (int j = 0; j < SORT_WARPS; ++j) { sh.wcount[j][tid] = 0; z[j * 256 + tid] = 0; z[(SORT_WARPS + j) * 256 + tid] = 0; }
+    if (tid == 0) sh.tile = atomicAdd(ticket, 1u); // tiles are taken in launch order: every earlier tile is running or done
+    __syncthreads();
+    const int64_t tile = sh.tile;
+    const int64_t left = n - tile * SORT_TILE;
+    if (left >= SORT_TILE) sort_scatter_tile<PASS, true>(sh, sort_tile_space, tile, SORT_TILE, kin, vin, kout, vout, dbase, state, state_next);
+    else sort_scatter_tile<PASS, false>(sh, sort_tile_space, tile, (int)left, kin, vin, kout, vout, dbase, state, state_next);
+}
+template <int PASS>
+static cudaError_t launch_sort_pass(uint64_t* key[2], uint32_t* idx[2], int cur, int64_t n, int64_t nblk, uint32_t* dbase, uint32_t* ticket,
+                                    uint32_t* const state[2], cudaStream_t st) {
+    static bool attr_set = false; // the 48 KB tile is dynamic shared memory above the default limit
+    if (!attr_set) {
+        cudaError_t e = cudaFuncSetAttribute(sort_scatter_kernel<PASS>, cudaFuncAttributeMaxDynamicSharedMemorySize, SORT_SMEM_BYTES);
+        if (e != cudaSuccess) return e;
+        attr_set = true;
+    }
+    HOT_LAUNCHED(1);
+    sort_scatter_kernel<PASS><<<(unsigned)nblk, SORT_THREADS, SORT_SMEM_BYTES, st>>>(key[cur], idx[cur], key[cur ^ 1], idx[cur ^ 1], n, dbase + PASS * 256,
+                                                                                     ticket + PASS, state[PASS & 1], state[(PASS & 1) ^ 1]);
+    return cudaGetLastError();
 }
 cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st) {
     const int64_t nblk = sort_blocks(n);
@@ -334,15 +369,15 @@ cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uin
     if (hb > 148 * 8) hb = 148 * 8;
     sort_hist8_kernel<<<(unsigned)hb, 256, 0, st>>>(key[0], n, ghist);
     sort_scan8_kernel<<<1, 256, 0, st>>>(ghist, dbase);
-    int cur = 0;
-    for (int pass = 0; pass < 8; ++pass) {
-        HOT_LAUNCHED(1);
-        sort_scatter_kernel<<<(unsigned)nblk, SORT_THREADS, 0, st>>>(key[cur], idx[cur], key[cur ^ 1], idx[cur ^ 1], n, pass * 8, dbase + pass * 256,
-                                                                     ticket + pass, state[pass & 1], state[(pass & 1) ^ 1]);
-        cur ^= 1;
-    }
-    // 8 passes: the result is back in buffer 0
-    return cudaGetLastError();
+    // 8 passes: the result is back in buffer 0.  Pass 0 takes the index from the key's position (idx[0] is not read).
+    if ((e = launch_sort_pass<0>(key, idx, 0, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    if ((e = launch_sort_pass<1>(key, idx, 1, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    if ((e = launch_sort_pass<2>(key, idx, 0, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    if ((e = launch_sort_pass<3>(key, idx, 1, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    if ((e = launch_sort_pass<4>(key, idx, 0, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    if ((e = launch_sort_pass<5>(key, idx, 1, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    if ((e = launch_sort_pass<6>(key, idx, 0, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;
+    return launch_sort_pass<7>(key, idx, 1, n, nblk, dbase, ticket, state, st);
 }
 
 // ------------------------------------------------------------------------------------------

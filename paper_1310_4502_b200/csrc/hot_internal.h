@@ -76,8 +76,9 @@ struct Tree {
 // ---- build stages (hot_build.cu) ------------------------------------------------------------
 // every launcher returns the cudaError_t of its last launch; all work goes to `st`
 cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float lox, float loy, float loz, float inv,
-                          uint64_t* key, uint32_t* idx, float4* bin, int* errflag, cudaStream_t st);
-// sorts (key,idx) pairs stably, ascending; result ends in key[0]/idx[0]; scratch: hist of sort_hist_elems(n) u32
+                          uint64_t* key, float4* bin, int* errflag, cudaStream_t st);
+// sorts (key, position) pairs stably, ascending: idx[0] need not be initialised (the first pass takes a key's index from
+// its position); result ends in key[0]/idx[0]; scratch: hist of sort_hist_elems(n) u32
 size_t sort_hist_elems(int64_t n);
 cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st);
 cudaError_t launch_gather(const float4* bin, const uint32_t* perm, int64_t n, float4* body, cudaStream_t st);
