@@ -221,7 +221,7 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(cudaMemsetAsync(g.d_flags, 0, 4 * sizeof(int), st));
 
     CUDA_TRY(cudaEventRecord(g.ev[0], st));
-    CUDA_TRY(launch_keygen(pos, mass, n, box.lo[0], box.lo[1], box.lo[2], inv, t.key[0], t.bin, g.d_flags, st));
+    CUDA_TRY(launch_keygen(pos, mass, n, box.lo[0], box.lo[1], box.lo[2], inv, t.key[0], t.bin, d_hist, g.d_flags, st));
     CUDA_TRY(cudaEventRecord(g.ev[1], st));
     CUDA_TRY(launch_radix_sort(t.key, t.idx, n, d_hist, st));
     CUDA_TRY(cudaEventRecord(g.ev[2], st));

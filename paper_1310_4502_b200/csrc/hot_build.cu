@@ -40,45 +40,72 @@ __device__ __forceinline__ uint64_t body_key(float x, float y, float z, float lo
     uint32_t ix = grid_coord(x, lox, inv, bad), iy = grid_coord(y, loy, inv, bad), iz = grid_coord(z, loz, inv, bad);
     return (1ull << 63) | (spread21(ix) << 2) | (spread21(iy) << 1) | spread21(iz);
 }
-// 4 bodies per thread: three 128-bit loads, two 128-bit key stores (the sort's first pass takes the index from the position)
-// Also writes the bodies as aligned float4 (x,y,z,m) in the caller's order: the gather after the sort
+// 4 bodies per thread and trip: three 128-bit loads, two 128-bit key stores (the sort's first pass takes the index from
+// the position).  Also writes the bodies as aligned float4 (x,y,z,m) in the caller's order: the gather after the sort
 // then fetches one 32-byte sector per body instead of the 3-4 sectors of the separate pos / mass arrays.
+// The sort's eight digit histograms are counted here as well (shared-memory atomics, added to `ghist` at the end of
+// the block's grid-stride loop): the kernel is HBM-bound, the shared-memory pipe is free.
+static cudaError_t sort_clear_scratch(uint32_t* hist, int64_t n, cudaStream_t st);
+__device__ __forceinline__ void key_digits(uint32_t (*h)[256], uint64_t k) {
+    const uint32_t lo = (uint32_t)k, hi = (uint32_t)(k >> 32);
+#pragma unroll
+    for (int p = 0; p < 4; ++p) {
+        atomicAdd(&h[p][__byte_perm(lo, 0u, 0x4440u + p)], 1u);
+        atomicAdd(&h[4 + p][__byte_perm(hi, 0u, 0x4440u + p)], 1u);
+    }
+}
 __global__ void __launch_bounds__(256) keygen_kernel(const float* __restrict__ pos, const float* __restrict__ mass, int64_t n, float lox,
                                                      float loy, float loz, float inv, uint64_t* __restrict__ key,
-                                                     float4* __restrict__ bin, int* __restrict__ errflag, int vec) {
-    int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; // quad index
-    int64_t i0 = q * 4;
-    if (i0 >= n) return;
+                                                     float4* __restrict__ bin, uint32_t* __restrict__ ghist, int* __restrict__ errflag, int vec) {
+    __shared__ uint32_t h[8][256];
+#pragma unroll
+    for (int p = 0; p < 8; ++p) h[p][threadIdx.x] = 0;
+    __syncthreads();
     bool bad = false;
-    if (vec && i0 + 4 <= n) {
-        const float4* p4 = reinterpret_cast<const float4*>(pos) + q * 3;
-        float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
-        uint64_t k0 = body_key(a.x, a.y, a.z, lox, loy, loz, inv, bad);
-        uint64_t k1 = body_key(a.w, b.x, b.y, lox, loy, loz, inv, bad);
-        uint64_t k2 = body_key(b.z, b.w, c.x, lox, loy, loz, inv, bad);
-        uint64_t k3 = body_key(c.y, c.z, c.w, lox, loy, loz, inv, bad);
-        ulonglong2* ko = reinterpret_cast<ulonglong2*>(key + i0);
-        ko[0] = make_ulonglong2(k0, k1);
-        ko[1] = make_ulonglong2(k2, k3);
-        const float4 m = __ldg(reinterpret_cast<const float4*>(mass) + q);
-        bin[i0] = make_float4(a.x, a.y, a.z, m.x);
-        bin[i0 + 1] = make_float4(a.w, b.x, b.y, m.y);
-        bin[i0 + 2] = make_float4(b.z, b.w, c.x, m.z);
-        bin[i0 + 3] = make_float4(c.y, c.z, c.w, m.w);
-    } else {
-        for (int64_t i = i0; i < n && i < i0 + 4; ++i) {
-            key[i] = body_key(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], lox, loy, loz, inv, bad);
-            bin[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+    const int64_t quads = (n + 3) / 4;
+    for (int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; q < quads; q += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t i0 = q * 4;
+        if (vec && i0 + 4 <= n) {
+            const float4* p4 = reinterpret_cast<const float4*>(pos) + q * 3;
+            float4 a = __ldg(p4), b = __ldg(p4 + 1), c = __ldg(p4 + 2);
+            const float4 m = __ldg(reinterpret_cast<const float4*>(mass) + q);
+            uint64_t k0 = body_key(a.x, a.y, a.z, lox, loy, loz, inv, bad);
+            uint64_t k1 = body_key(a.w, b.x, b.y, lox, loy, loz, inv, bad);
+            uint64_t k2 = body_key(b.z, b.w, c.x, lox, loy, loz, inv, bad);
+            uint64_t k3 = body_key(c.y, c.z, c.w, lox, loy, loz, inv, bad);
+            ulonglong2* ko = reinterpret_cast<ulonglong2*>(key + i0);
+            ko[0] = make_ulonglong2(k0, k1);
+            ko[1] = make_ulonglong2(k2, k3);
+            bin[i0] = make_float4(a.x, a.y, a.z, m.x);
+            bin[i0 + 1] = make_float4(a.w, b.x, b.y, m.y);
+            bin[i0 + 2] = make_float4(b.z, b.w, c.x, m.z);
+            bin[i0 + 3] = make_float4(c.y, c.z, c.w, m.w);
+            key_digits(h, k0); key_digits(h, k1); key_digits(h, k2); key_digits(h, k3);
+        } else {
+            for (int64_t i = i0; i < n && i < i0 + 4; ++i) {
+                const uint64_t k = body_key(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], lox, loy, loz, inv, bad);
+                key[i] = k;
+                bin[i] = make_float4(pos[3 * i], pos[3 * i + 1], pos[3 * i + 2], mass[i]);
+                key_digits(h, k);
+            }
         }
     }
     if (bad) atomicOr(errflag, 1);
+    __syncthreads();
+#pragma unroll
+    for (int p = 0; p < 8; ++p) { const uint32_t c = h[p][threadIdx.x]; if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c); }
 }
+// `hist` is the sort's scratch (sort_hist_elems(n) words): cleared here, its first 2048 words receive the digit counts
 cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float lox, float loy, float loz, float inv,
-                          uint64_t* key, float4* bin, int* errflag, cudaStream_t st) {
+                          uint64_t* key, float4* bin, uint32_t* hist, int* errflag, cudaStream_t st) {
+    cudaError_t e = sort_clear_scratch(hist, n, st);
+    if (e != cudaSuccess) return e;
     int64_t quads = (n + 3) / 4;
+    int64_t blocks = (quads + 255) / 256;
+    if (blocks > 148 * 8) blocks = 148 * 8;
     int vec = ((reinterpret_cast<uintptr_t>(pos) | reinterpret_cast<uintptr_t>(mass)) & 15u) == 0; // 128-bit loads need 16-byte aligned bases
     HOT_LAUNCHED(1);
-    keygen_kernel<<<(unsigned)((quads + 255) / 256), 256, 0, st>>>(pos, mass, n, lox, loy, loz, inv, key, bin, errflag, vec);
+    keygen_kernel<<<(unsigned)blocks, 256, 0, st>>>(pos, mass, n, lox, loy, loz, inv, key, bin, hist, errflag, vec);
     return cudaGetLastError();
 }
 
@@ -105,27 +132,6 @@ cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float 
 static inline int64_t sort_blocks(int64_t n) { return (n + SORT_TILE - 1) / SORT_TILE; }
 size_t sort_hist_elems(int64_t n) { return (size_t)SORT_STATE0 + 2 * (size_t)256 * (size_t)sort_blocks(n); }
 
-__global__ void __launch_bounds__(256) sort_hist8_kernel(const uint64_t* __restrict__ key, int64_t n, uint32_t* __restrict__ ghist) {
-    __shared__ uint32_t h[8][256];
-#pragma unroll
-    for (int p = 0; p < 8; ++p) h[p][threadIdx.x] = 0;
-    __syncthreads();
-    const int64_t stride = (int64_t)gridDim.x * 256 * 4;
-    for (int64_t i0 = (int64_t)blockIdx.x * 256 * 4 + threadIdx.x; i0 < n; i0 += stride) {
-        uint64_t k[4];
-#pragma unroll
-        for (int j = 0; j < 4; ++j) k[j] = i0 + j * 256 < n ? key[i0 + j * 256] : 0ull;
-#pragma unroll
-        for (int j = 0; j < 4; ++j)
-            if (i0 + j * 256 < n) {
-#pragma unroll
-                for (int p = 0; p < 8; ++p) atomicAdd(&h[p][(uint32_t)(k[j] >> (8 * p)) & 255u], 1u);
-            }
-    }
-    __syncthreads();
-#pragma unroll
-    for (int p = 0; p < 8; ++p) { uint32_t c = h[p][threadIdx.x]; if (c) atomicAdd(&ghist[p * 256 + threadIdx.x], c); }
-}
 // exclusive scan of each of the eight 256-bin histograms; one block of 256 threads
 __global__ void __launch_bounds__(256) sort_scan8_kernel(const uint32_t* __restrict__ ghist, uint32_t* __restrict__ dbase) {
     __shared__ uint32_t wtot[8];
@@ -222,7 +228,7 @@ __device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __re
     // shared-memory atomicOr on a per-warp, per-digit lane mask (MATCH.ANY issues once per 64 clocks per SM
     // on sm_100a -- 115 us of a pass at 2^24 keys; eight ballots per key are no faster than the mask).  Round k
     // uses mask array k & 1: its leader clears the word after the round's reads, and the next atomicOr on that
-    // array is two warp barriers later.
+    // array is two rounds (two warp barriers) later.
     const uint32_t lanebit = 1u << lane, below = lanebit - 1u;
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
@@ -232,10 +238,11 @@ __device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __re
         if (valid) atomicOr(mp, lanebit);
         __syncwarp();
         const uint32_t m = valid ? *mp : 0u;
-        const uint32_t old = wc[d];
         const uint32_t r = __popc(m & below);
-        __syncwarp();
-        if (valid && r == 0) { wc[d] = old + __popc(m); *mp = 0u; }
+        uint32_t old = 0;
+        if (valid && r == 0) old = atomicAdd(&wc[d], (uint32_t)__popc(m)); // the lowest lane of the digit counts for all
+        old = __shfl_sync(FULL, old, (__ffs((int)m) - 1) & 31); // source lane depends on m: every lane has read the mask by now
+        if (valid && r == 0) *mp = 0u;
         rk[k] = old + r;
     }
     __syncthreads();
@@ -356,18 +363,18 @@ static cudaError_t launch_sort_pass(uint64_t* key[2], uint32_t* idx[2], int cur,
                                                                                      ticket + PASS, state[PASS & 1], state[(PASS & 1) ^ 1]);
     return cudaGetLastError();
 }
+// digit counters, tile tickets and the first look-back array start at zero
+static cudaError_t sort_clear_scratch(uint32_t* hist, int64_t n, cudaStream_t st) {
+    return cudaMemsetAsync(hist, 0, ((size_t)SORT_STATE0 + (size_t)256 * sort_blocks(n)) * sizeof(uint32_t), st);
+}
 cudaError_t launch_radix_sort(uint64_t* key[2], uint32_t* idx[2], int64_t n, uint32_t* hist, cudaStream_t st) {
     const int64_t nblk = sort_blocks(n);
     uint32_t* const ghist = hist;
     uint32_t* const dbase = hist + 2048;
     uint32_t* const ticket = hist + 4096;
     uint32_t* const state[2] = {hist + SORT_STATE0, hist + SORT_STATE0 + (size_t)256 * nblk};
-    cudaError_t e = cudaMemsetAsync(hist, 0, ((size_t)SORT_STATE0 + (size_t)256 * nblk) * sizeof(uint32_t), st); // counters, tickets, state[0]
-    if (e != cudaSuccess) return e;
-    HOT_LAUNCHED(2);
-    int64_t hb = (n + 1023) / 1024;
-    if (hb > 148 * 8) hb = 148 * 8;
-    sort_hist8_kernel<<<(unsigned)hb, 256, 0, st>>>(key[0], n, ghist);
+    cudaError_t e;
+    HOT_LAUNCHED(1);
     sort_scan8_kernel<<<1, 256, 0, st>>>(ghist, dbase);
     // 8 passes: the result is back in buffer 0.  Pass 0 takes the index from the key's position (idx[0] is not read).
     if ((e = launch_sort_pass<0>(key, idx, 0, n, nblk, dbase, ticket, state, st)) != cudaSuccess) return e;

@@ -76,7 +76,8 @@ struct Tree {
 // ---- build stages (hot_build.cu) ------------------------------------------------------------
 // every launcher returns the cudaError_t of its last launch; all work goes to `st`
 cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float lox, float loy, float loz, float inv,
-                          uint64_t* key, float4* bin, int* errflag, cudaStream_t st);
+                          uint64_t* key, float4* bin, uint32_t* hist, int* errflag, cudaStream_t st);
+// launch_keygen also clears the sort's scratch `hist` and counts the eight digit histograms of the keys into it.
 // sorts (key, position) pairs stably, ascending: idx[0] need not be initialised (the first pass takes a key's index from
 // its position); result ends in key[0]/idx[0]; scratch: hist of sort_hist_elems(n) u32
 size_t sort_hist_elems(int64_t n);
