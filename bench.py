@@ -40,8 +40,9 @@ NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2, 16, 256): 15.764e9}
 # FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
-SORT_BYTES_PER_BODY = 8 + 8 * 24      # one 8 B read for the digit histograms + 8 passes x (12 B read + 12 B write)
-KEYGEN_BYTES_PER_BODY = 44          # 12 B pos + 4 B mass read; 8 B key + 4 B index + 16 B float4 body written
+SORT_BYTES_PER_BODY = 8 * 24 - 4      # 8 passes x (12 B read + 12 B write); pass 0 reads no index (it is the position)
+SORT_BYTES_SURVEY = 8 + 8 * 24        # SURVEY 8(d) count for d = 8 (with a histogram pre-pass over the keys; here keygen counts)
+KEYGEN_BYTES_PER_BODY = 40          # 12 B pos + 4 B mass read; 8 B key + 16 B float4 body written (+ digit histograms)
 GATHER_BYTES_PER_BODY = 36          # 4 B permutation + 16 B float4 gathered, 16 B written
 
 
@@ -318,6 +319,7 @@ def main():
         "hbm_stages": {
             "keygen_GBps": KEYGEN_BYTES_PER_BODY * w.n / (stage["ms_keygen"] * 1e-3) / 1e9,
             "sort_GBps": SORT_BYTES_PER_BODY * w.n / (stage["ms_sort"] * 1e-3) / 1e9,
+            "sort_GBps_survey_count": SORT_BYTES_SURVEY * w.n / (stage["ms_sort"] * 1e-3) / 1e9,
             "gather_GBps": GATHER_BYTES_PER_BODY * w.n / (stage["ms_gather"] * 1e-3) / 1e9,
             "walk_list_GBps": 2 * 4 * st["list_entries"] / (stage["ms_walk"] * 1e-3) / 1e9,
             "walk_Gcells_per_s": st["cells_visited"] / (stage["ms_walk"] * 1e-3) / 1e9},

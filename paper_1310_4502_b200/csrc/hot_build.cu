@@ -112,9 +112,12 @@ cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float 
 // ------------------------------------------------------------------------------------------
 // S2 LSD radix sort of (key, idx), 8-bit digits, 8 passes (PAPER.md:150 names an American-flag
 // radix sort for the on-node sort; a stable LSD sort gives the unique stable permutation).
-// One pre-pass counts all eight digits of every key (2048 counters); each pass is then ONE kernel: a tile
+// keygen_kernel counts all eight digits of every key (2048 counters); each pass is then ONE kernel: a tile
 // (256 threads x 16 keys, held warp-striped so the in-tile order is (warp, round, lane)) ranks its keys,
-// publishes its digit counts, finds the counts of all earlier tiles by decoupled look-back and scatters.
+// publishes its digit counts, lays the tile out in digit order in shared memory, finds the counts of all earlier
+// tiles by decoupled look-back and scatters.  The kernel is bound by the shared-memory / LSU data pipe (ncu:
+// l1tex__data_pipe_lsu_wavefronts 75% of peak, 51 wavefronts per 32 keys), so its design minimises
+// shared-memory operations per key, not instructions.
 // Scratch (u32): [0,2048) digit counts, [2048,4096) their exclusive scans, [4096,4104) tile tickets,
 // then two look-back state arrays of 256 words per tile (a pass uses one and clears the other).
 // ------------------------------------------------------------------------------------------
@@ -206,7 +209,8 @@ struct SortShared {
     uint32_t tile;
 };
 template <int PASS, bool FULLT>
-__device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __restrict__ skey, const int64_t tile, const int cnt,
+__device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __restrict__ skey, uint32_t* __restrict__ wmbase,
+                                                  const int64_t tile, const int cnt,
                                                   const uint64_t* __restrict__ kin, const uint32_t* __restrict__ vin,
                                                   uint64_t* __restrict__ kout, uint32_t* __restrict__ vout,
                                                   const uint32_t* __restrict__ dbase, uint32_t* __restrict__ state,
@@ -214,7 +218,7 @@ __device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __re
     const int tid = threadIdx.x, w = tid >> 5, lane = tid & 31;
     uint32_t* const sval = reinterpret_cast<uint32_t*>(skey + SORT_TILE);
     // two per-warp lane-mask arrays, used by alternate ranking rounds; the tile space is free until the ranks are known
-    uint32_t* const wm0 = reinterpret_cast<uint32_t*>(skey) + w * 256;
+    uint32_t* const wm0 = wmbase + w * 256;
     uint32_t* const wm1 = wm0 + SORT_WARPS * 256;
     uint32_t* const wc = sh.wcount[w];
     const int64_t t0 = tile * SORT_TILE;
@@ -346,8 +350,8 @@ __global__ void __launch_bounds__(SORT_THREADS, SORT_MINBLK) sort_scatter_kernel
     __syncthreads();
     const int64_t tile = sh.tile;
     const int64_t left = n - tile * SORT_TILE;
-    if (left >= SORT_TILE) sort_scatter_tile<PASS, true>(sh, sort_tile_space, tile, SORT_TILE, kin, vin, kout, vout, dbase, state, state_next);
-    else sort_scatter_tile<PASS, false>(sh, sort_tile_space, tile, (int)left, kin, vin, kout, vout, dbase, state, state_next);
+    if (left >= SORT_TILE) sort_scatter_tile<PASS, true>(sh, sort_tile_space, z, tile, SORT_TILE, kin, vin, kout, vout, dbase, state, state_next);
+    else sort_scatter_tile<PASS, false>(sh, sort_tile_space, z, tile, (int)left, kin, vin, kout, vout, dbase, state, state_next);
 }
 template <int PASS>
 static cudaError_t launch_sort_pass(uint64_t* key[2], uint32_t* idx[2], int cur, int64_t n, int64_t nblk, uint32_t* dbase, uint32_t* ticket,
