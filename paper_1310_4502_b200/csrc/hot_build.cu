@@ -231,8 +231,9 @@ __device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __re
     // Rank inside the warp's 16 x 32 keys.  The lanes holding the same digit find each other through a
     // shared-memory atomicOr on a per-warp, per-digit lane mask (MATCH.ANY issues once per 64 clocks per SM
     // on sm_100a -- 115 us of a pass at 2^24 keys; eight ballots per key are no faster than the mask).  Round k
-    // uses mask array k & 1: its leader clears the word after the round's reads, and the next atomicOr on that
-    // array is two rounds (two warp barriers) later.
+    // uses mask array k & 1: its leader clears the word after the round's reads (second warp barrier), and the next
+    // atomicOr on that array is two rounds later; the lowest lane of a digit adds the lanes' number to the warp's
+    // count of the digit with one atomicAdd and hands the old count to the others by a shuffle.
     const uint32_t lanebit = 1u << lane, below = lanebit - 1u;
 #pragma unroll
     for (int k = 0; k < SORT_ITEMS; ++k) {
@@ -245,7 +246,8 @@ __device__ __forceinline__ void sort_scatter_tile(SortShared& sh, uint64_t* __re
         const uint32_t r = __popc(m & below);
         uint32_t old = 0;
         if (valid && r == 0) old = atomicAdd(&wc[d], (uint32_t)__popc(m)); // the lowest lane of the digit counts for all
-        old = __shfl_sync(FULL, old, (__ffs((int)m) - 1) & 31); // source lane depends on m: every lane has read the mask by now
+        old = __shfl_sync(FULL, old, (__ffs((int)m) - 1) & 31);
+        __syncwarp(); // every lane has read the mask
         if (valid && r == 0) *mp = 0u;
         rk[k] = old + r;
     }
