@@ -169,6 +169,35 @@ def test_ragged_and_tiny_sizes(hot, n):
         assert ea.max() <= 1e-4 and ep.max() <= 1e-5
 
 
+@pytest.mark.parametrize("n,kind", [(4095, "uniform"), (4096, "uniform"), (4097, "dup"), (8191, "corner"), (8193, "dup"),
+                                    (3 * 4096, "corner"), (37 * 4096 + 5, "dup"), (37 * 4096 + 5, "uniform"), (65536, "planes")])
+def test_sort_tile_edges_duplicates_and_skewed_digits(hot, n, kind):
+    """Keys, stable permutation, cells and groups bit-exact where the radix sort's tiles (4096 keys) end exactly, one
+    short or one over, with equal keys running across tiles ("dup": ties keep the caller's order), with all bodies in
+    one finest-level corner region ("corner": the leading digits are all equal, the look-back sees one digit only) and
+    with two coordinates quantised to 8 values ("planes": few distinct digits per pass, long runs)."""
+    rng = np.random.default_rng(n + len(kind))
+    pos = rng.uniform(0, 1, (n, 3)).astype(np.float32) * np.float32(0.999)
+    if kind == "dup":
+        src = rng.integers(0, 7, n)  # seven points, each hit n/7 times in random caller order
+        pts = rng.uniform(0, 1, (7, 3)).astype(np.float32) * np.float32(0.999)
+        half = rng.random(n) < 0.8
+        pos[half] = pts[src[half]]
+    elif kind == "corner":
+        pos = (pos * np.float32(2.0 ** -12)).astype(np.float32)
+    elif kind == "planes":
+        pos[:, :2] = (np.floor(pos[:, :2] * 8) / 8 + 1 / 16).astype(np.float32)
+    mass = np.full(n, 1.0 / n, np.float32)
+    w = W.Workload("t", pos, mass, (0, 0, 0), 1.0, False, 1e-2, 0.5, 2)
+    _build(hot, w, 8, 32)
+    T = O.Tree(pos, mass, w.lo, w.size, nleaf=8, ncrit=32, moments=False)
+    _check_int_artefacts(hot, T)
+    key, skey, perm = T.keys()
+    assert (skey[1:] >= skey[:-1]).all() and (np.sort(perm) == np.arange(n)).all()
+    same = skey[1:] == skey[:-1]
+    assert (perm[1:][same] > perm[:-1][same]).all(), "ties keep ascending caller index"
+
+
 def test_coincident_particles_and_finest_level_group(hot):
     """Duplicated keys: a level-21 leaf above NLEAF and a sink group above NCRIT (kernels chunk)."""
     rng = np.random.default_rng(5)
