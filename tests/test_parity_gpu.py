@@ -396,6 +396,33 @@ def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
     del cnt
 
 
+@pytest.mark.slow
+def test_maximum_size_keys_and_stable_sort(hot):
+    """n = 2^27 (the library's maximum, configs[4]'s size): 32768 sort tiles.  Seeded uniform bodies made on the GPU; the
+    oracle computes the 2^27 keys (seconds), the sorted keys and the permutation are checked by the properties that fix them
+    uniquely: key_sorted == key[perm], non-decreasing, perm a permutation, equal keys in ascending caller index."""
+    import torch
+    n = 1 << 27
+    g = torch.Generator(device="cuda"); g.manual_seed(1310450227)
+    pos = torch.rand(n, 3, device="cuda", generator=g) * 0.999 + 0.0003
+    pos[: n // 64] = pos[n // 64: n // 32]  # 2^21 duplicated bodies: equal keys far apart in caller order
+    mass = torch.full((n,), 1.0 / n, device="cuda")
+    hot.hot_set_params(16, 256)
+    try:
+        hot.hot_build(pos, mass, (0.0, 0.0, 0.0), 1.0, False)
+        skey, perm = hot.hot_export_keys()
+    finally:
+        hot.hot_free()
+    key = O.keys(pos.cpu().numpy(), (0.0, 0.0, 0.0), 1.0)
+    del pos, mass
+    assert (skey == key[perm]).all(), "sorted keys are the caller's keys through the permutation"
+    assert (skey[1:] >= skey[:-1]).all(), "ascending"
+    seen = np.zeros(n, np.bool_); seen[perm] = True
+    assert seen.all(), "permutation"
+    same = skey[1:] == skey[:-1]
+    assert same.sum() >= n // 64 and (perm[1:][same] > perm[:-1][same]).all(), "ties keep ascending caller index"
+
+
 def test_long_lists_outgrow_the_walk_staging_and_are_retried(hot):
     """theta = 0.07 with one-body leaves gives more than 16384 accepted cells per group: the walk
     reports that its per-warp staging area is too small, the library enlarges it and walks again."""
