@@ -90,7 +90,9 @@ int hot_set_params(int nleaf, int ncrit);
 int hot_set_list_arena(int64_t max_bytes);
 
 /* pos : device, [n][3] fp32 row-major x,y,z; borrowed.   mass: device, [n] fp32 > 0; borrowed.
- * n   : 1 <= n <= 2^27 (and < 2^27 coincident bodies in one finest-level cell).
+ * n   : 1 <= n <= 2^27 (and < 2^27 coincident bodies in one finest-level cell).  The bound is the 27-bit count
+ *       and 28-bit cell index of the 16-byte record the walk reads per cell; 2^27 fp32
+ *       bodies with their lists are also what fits 180 GB.
  * periodic: 0 open, 1 periodic with period box.size.  In both modes every particle must satisfy
  *           0 <= fl32((x-lo)*fl32(1/size)) < 1 per axis, else HOT_ERANGE (the caller wraps).
  * Builds keys, the stable key-sorted permutation, key-ordered bodies, cells, hash table and
@@ -134,13 +136,30 @@ int hot_export_keys(uint64_t* key_sorted, uint32_t* perm);
  * child = index of the first child or -1 for a leaf; parent = -1 for the root. */
 int hot_export_cells(uint64_t* key, uint32_t* first, uint32_t* count, uint8_t* mask,
                      int32_t* child, int32_t* parent, int64_t cap, int64_t* ncells);
-/* sink groups in particle order: cell index, and the list counts of the last hot_forces
- * (zeros before the first): L_pc = accepted cells, L_pp = particles of rejected leaves. */
-int hot_export_groups(int32_t* cell, uint64_t* lpc, uint64_t* lpp, int64_t cap, int64_t* ngroups);
-/* moments of the last hot_forces: com [ncells][3] double, m0 [ncells], m2 [ncells][6]
- * (xx xy xz yy yz zz), m3 [ncells][10], m4 [ncells][15] (degree-major, x>y>z); NULL to skip;
+/* sink groups in particle order: index and key of the group's cell, its first body (sorted
+ * position) and body count, and the list counts of the last hot_forces (zeros before the first):
+ * L_pc = accepted cells, L_pp = particles of rejected leaves (the group's own bodies included), both
+ * summed over the 125 images when periodic.  Any pointer may be NULL. */
+int hot_export_groups(int32_t* cell, uint64_t* key, uint32_t* first, uint32_t* count, uint64_t* lpc, uint64_t* lpp,
+                      int64_t cap, int64_t* ngroups);
+/* The interaction lists of ONE sink group as the last hot_forces walked them, as sets
+ * (the order inside a list is the walk's and means nothing):
+ *   pc_cell [*npc]: indices (ascending-key numbering of hot_export_cells) of the accepted cells,
+ *   pc_img  [*npc]: image of each, 25 (nx+2) + 5 (ny+2) + (nz+2), 62 = the box itself (always 62 when open),
+ *   pp_body [*npp]: sorted positions (index into key_sorted / perm of hot_export_keys) of the listed bodies;
+ *                   the group's OWN bodies in the box itself are not in the list (the kernel pairs them
+ *                   separately and skips j = i), so *npp = L_pp - count(group),
+ *   pp_img  [*npp]: image of each.
+ * HOST arrays; pc_img / pp_img may be NULL; *npc / *npp are always set; HOT_EINVAL if a cap is too small.
+ * HOT_EORDER if the group's lists are no longer in the arena (hot_forces ran in several rounds,
+ * hot_stats list_chunks > 1, and this group was not in the last one). */
+int hot_export_lists(int64_t group, int32_t* pc_cell, uint8_t* pc_img, int64_t pc_cap, int64_t* npc,
+                     uint32_t* pp_body, uint8_t* pp_img, int64_t pp_cap, int64_t* npp);
+/* moments of the last hot_forces: com [ncells][3] double, m0 [ncells], bmax [ncells] (radius about com
+ * holding every body of the cell, PAPER.md:94 / DESIGN.md R-15), m2 [ncells][6] (xx xy xz yy yz zz),
+ * m3 [ncells][10], m4 [ncells][15] (degree-major, x>y>z); NULL to skip;
  * m3/m4 only when the last order was 4 (else HOT_EINVAL if requested). */
-int hot_export_moments(double* com, float* m0, float* m2, float* m3, float* m4, int64_t cap);
+int hot_export_moments(double* com, float* m0, float* bmax, float* m2, float* m3, float* m4, int64_t cap);
 /* hash table: cell index of each key, -1 if absent.  keys, idx: host, [nkeys]. */
 int hot_lookup_keys(const uint64_t* keys, int64_t nkeys, int32_t* idx);
 

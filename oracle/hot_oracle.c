@@ -59,6 +59,9 @@ typedef struct {
     int64_t *gcell;
     /* moments about the centre of mass, eq (6): mom[c][k] = sum m d^alpha_k; com[c][3]; bmax[c] */
     double *mom, *com, *bmax;
+    double *bbound;   /* b_max as the upward pass can carry it: see build_bbound */
+    int lazy;         /* moments computed on demand, only for the cells a requested group accepts */
+    uint8_t *momdone; /* lazy: 1 where mom/com/bmax of the cell are filled */
     /* periodic far field (C-9 step 2), built on demand */
     int far_ready;
     double far_coef[165]; /* coefficient of x^a y^b z^c of psi_sm, a+b+c<=8 (odd ones zero) */
@@ -224,32 +227,60 @@ static void build_groups(orc_t *t) {
  * C-5 upward pass, eq (6): raw moments about the centre of mass, directly from the
  * cell's particle range.  mom[k] = sum_j m_j dx^a dy^b dz^c for alpha_k = (a,b,c), |alpha| <= 4.
  * ---------------------------------------------------------------------------------------- */
-static void build_moments(orc_t *t) {
+static void cell_moments(orc_t *t, int64_t c) {
+    int64_t f = t->cfirst[c], e = f + t->ccount[c];
+    double M0 = 0, z[3] = {0, 0, 0};
+    for (int64_t j = f; j < e; ++j) {
+        M0 += t->m[j];
+        for (int k = 0; k < 3; ++k) z[k] += t->m[j] * t->x[3 * j + k];
+    }
+    for (int k = 0; k < 3; ++k) z[k] /= M0;
+    double *mo = t->mom + (size_t)c * ORC_NMOM, bm = 0;
+    for (int k = 0; k < ORC_NMOM; ++k) mo[k] = 0;
+    for (int64_t j = f; j < e; ++j) {
+        double d[3];
+        for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - z[k];
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
+        if (r > bm) bm = r;
+        for (int k = 0; k < ORC_NMOM; ++k)
+            mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
+    }
+    for (int k = 0; k < 3; ++k) t->com[3 * c + k] = z[k];
+    t->bmax[c] = bm;
+}
+/* b_max of Fig 3 ("sources are contained within a source cell V of radius b_max") as
+ * an upward pass carries it (R-15): a leaf's value is the largest distance of one of
+ * its bodies from the centre of mass; an internal cell takes, over its children,
+ * max(|z_child - z| + b_child), which contains every body of the cell by the triangle
+ * inequality.  bmax[] above is the exact radius (directly from the bodies); bbound >= bmax. */
+static void build_bbound(orc_t *t) {
+    t->bbound = calloc((size_t)t->ncells, sizeof(double));
+    for (int64_t c = t->ncells - 1; c >= 0; --c) { /* children have larger indices than parents */
+        if (t->cchild[c] < 0) { t->bbound[c] = t->bmax[c]; continue; }
+        int nch = 0; for (int b = 0; b < 8; ++b) nch += (t->cmask[c] >> b) & 1;
+        double bb = 0;
+        for (int k = 0; k < nch; ++k) {
+            int64_t d = t->cchild[c] + k;
+            double s = 0;
+            for (int q = 0; q < 3; ++q) { double u = t->com[3 * d + q] - t->com[3 * c + q]; s += u * u; }
+            double v = sqrt(s) + t->bbound[d];
+            if (v > bb) bb = v;
+        }
+        t->bbound[c] = bb;
+    }
+}
+/* with_moments = 1: every cell; 2: none now, orc_tree_forces fills in the cells its groups accept
+ * (same cell_moments; for the 2^27-body config, where all 2e7 cells would take hours) */
+static void build_moments(orc_t *t, int lazy) {
     mi_init();
     t->mom = calloc((size_t)t->ncells * ORC_NMOM, sizeof(double));
     t->com = calloc((size_t)t->ncells * 3, sizeof(double));
     t->bmax = calloc((size_t)t->ncells, sizeof(double));
+    t->lazy = lazy;
+    if (lazy) { t->momdone = calloc((size_t)t->ncells, 1); return; }
 #pragma omp parallel for schedule(dynamic, 64)
-    for (int64_t c = 0; c < t->ncells; ++c) {
-        int64_t f = t->cfirst[c], e = f + t->ccount[c];
-        double M0 = 0, z[3] = {0, 0, 0};
-        for (int64_t j = f; j < e; ++j) {
-            M0 += t->m[j];
-            for (int k = 0; k < 3; ++k) z[k] += t->m[j] * t->x[3 * j + k];
-        }
-        for (int k = 0; k < 3; ++k) z[k] /= M0;
-        double *mo = t->mom + (size_t)c * ORC_NMOM, bm = 0;
-        for (int64_t j = f; j < e; ++j) {
-            double d[3];
-            for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - z[k];
-            double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
-            if (r > bm) bm = r;
-            for (int k = 0; k < ORC_NMOM; ++k)
-                mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
-        }
-        for (int k = 0; k < 3; ++k) t->com[3 * c + k] = z[k];
-        t->bmax[c] = bm;
-    }
+    for (int64_t c = 0; c < t->ncells; ++c) cell_moments(t, c);
+    build_bbound(t);
 }
 
 /* ------------------------------------------------------------------------------------------
@@ -260,6 +291,7 @@ void orc_destroy(orc_t *t) {
     free(t->key); free(t->skey); free(t->perm); free(t->x); free(t->m);
     free(t->ckey); free(t->clevel); free(t->cfirst); free(t->ccount); free(t->cmask);
     free(t->cchild); free(t->cparent); free(t->gcell); free(t->mom); free(t->com); free(t->bmax);
+    free(t->bbound); free(t->momdone);
     free(t);
 }
 orc_t *orc_create(const float *pos, const float *mass, int64_t n, const float lo[3], float size,
@@ -282,7 +314,7 @@ orc_t *orc_create(const float *pos, const float *mass, int64_t n, const float lo
     }
     build_tree(t);
     build_groups(t);
-    if (with_moments) build_moments(t);
+    if (with_moments) build_moments(t, with_moments == 2);
     return t;
 }
 
@@ -309,6 +341,7 @@ void orc_get_cells(const orc_t *t, uint64_t *key, int32_t *level, int64_t *first
 void orc_get_groups(const orc_t *t, int64_t *gcell) {
     memcpy(gcell, t->gcell, sizeof(int64_t) * (size_t)t->ngroups);
 }
+void orc_get_bbound(const orc_t *t, double *bbound) { memcpy(bbound, t->bbound, 8 * (size_t)t->ncells); }
 void orc_get_moments(const orc_t *t, double *mom, double *com, double *bmax) {
     size_t nc = (size_t)t->ncells;
     if (mom) memcpy(mom, t->mom, 8 * nc * ORC_NMOM);
@@ -442,6 +475,7 @@ typedef struct {
     int64_t npc, npp, covered;       /* counts */
     int64_t *pc, *pp; int64_t cap;   /* optional lists: accepted cells / rejected leaves */
     int64_t nleafrej;
+    uint8_t *mark;                   /* optional: set to 1 for every accepted cell */
     /* evaluation */
     int eval, order; double eps2; double shx[3];
     int64_t gfirst, gcount; double *acc, *pot; /* [gcount][3], [gcount], group-local */
@@ -467,6 +501,7 @@ static void walk_rec(walk_t *w, int64_t c) {
     if (mac_accept(w, c)) {
         if (w->pc && w->npc < w->cap) w->pc[w->npc] = c;
         w->npc++; w->covered += t->ccount[c];
+        if (w->mark) w->mark[c] = 1;
         if (w->eval)
             for (int64_t i = 0; i < w->gcount; ++i) {
                 double z[3] = {t->com[3 * c] + w->shx[0], t->com[3 * c + 1] + w->shx[1], t->com[3 * c + 2] + w->shx[2]};
@@ -718,6 +753,21 @@ void orc_tree_forces(orc_t *t, double theta, double eps, int order, const int64_
     int ws = image_range(t);
     if (t->periodic) far_prepare(t);
     if (!groups) ng = t->ngroups;
+    if (t->lazy) { /* moments of the cells these groups accept: mark them (walk only), then fill them in */
+        uint8_t *need = calloc((size_t)t->ncells, 1);
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int64_t q = 0; q < ng; ++q)
+            for (int ix = -ws; ix <= ws; ++ix) for (int iy = -ws; iy <= ws; ++iy) for (int iz = -ws; iz <= ws; ++iz) {
+                walk_t w; walk_setup(&w, t, theta, groups ? groups[q] : q);
+                w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
+                w.mark = need;
+                walk_rec(&w, 0);
+            }
+#pragma omp parallel for schedule(dynamic, 1)
+        for (int64_t c = 0; c < t->ncells; ++c)
+            if (need[c] && !t->momdone[c]) { cell_moments(t, c); t->momdone[c] = 1; }
+        free(need);
+    }
 #pragma omp parallel for schedule(dynamic, 4)
     for (int64_t q = 0; q < ng; ++q) {
         int64_t g = groups ? groups[q] : q;

@@ -163,7 +163,7 @@ class Tree:
         self._h = C.c_void_p(self._h)
         self.ncells = lib().orc_ncells(self._h)
         self.ngroups = lib().orc_ngroups(self._h)
-        self.has_moments = bool(moments)
+        self.has_moments = bool(moments)  # moments = 2 ("lazy"): only the cells that forces() needs, on demand
 
     def __del__(self):
         if getattr(self, "_h", None):
@@ -207,6 +207,12 @@ class Tree:
         bmax = np.empty(nc)
         lib().orc_get_moments(self._h, _p(mom), _p(com), _p(bmax))
         return mom, com, bmax
+
+    def bbound(self):
+        """b_max as an upward pass carries it (children's radii + centre offsets); >= moments()[2]."""
+        bb = np.empty(self.ncells)
+        lib().orc_get_bbound(self._h, _p(bb))
+        return bb
 
     def walk_counts(self, theta, groups=None):
         groups = _i64(groups)

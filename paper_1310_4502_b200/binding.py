@@ -64,8 +64,10 @@ def _load():
         lib.hot_free.restype = None
         lib.hot_export_keys.argtypes = [C.c_void_p, C.c_void_p]
         lib.hot_export_cells.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
-        lib.hot_export_groups.argtypes = [C.c_void_p] * 3 + [C.c_int64, C.POINTER(C.c_int64)]
-        lib.hot_export_moments.argtypes = [C.c_void_p] * 5 + [C.c_int64]
+        lib.hot_export_groups.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
+        lib.hot_export_lists.argtypes = [C.c_int64, C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64),
+                                         C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(C.c_int64)]
+        lib.hot_export_moments.argtypes = [C.c_void_p] * 6 + [C.c_int64]
         lib.hot_lookup_keys.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
         _lib = lib
     return _lib
@@ -120,35 +122,44 @@ def hot_free():
     _load().hot_free()
 
 
-_n_built = 0
-_dev = None
-
-
 def hot_build(pos, mass, lo, size, periodic=False):
-    """pos [n,3] / mass [n]: contiguous CUDA float32 tensors (borrowed for the call)."""
+    """pos [n,3] / mass [n]: contiguous CUDA float32 tensors on the current device (borrowed for the call)."""
     import torch
 
-    global _n_built, _dev
     if not (pos.is_cuda and mass.is_cuda and pos.dtype == torch.float32 and mass.dtype == torch.float32):
         raise TypeError("hot_build wants CUDA float32 tensors")
     if not (pos.is_contiguous() and mass.is_contiguous() and pos.dim() == 2 and pos.shape[1] == 3
             and mass.numel() == pos.shape[0]):
         raise TypeError("hot_build wants contiguous pos [n,3] and mass [n]")
-    n = pos.shape[0]
-    _n_built, _dev = 0, pos.device
-    _check(_load().hot_build(pos.data_ptr(), mass.data_ptr(), n, _box(lo, size), int(bool(periodic))))
-    _n_built = n
+    cur = torch.cuda.current_device()
+    if pos.device.index != cur or mass.device.index != cur:
+        raise TypeError(f"hot_build wants tensors on the current CUDA device (cuda:{cur}): the library works there")
+    _check(_load().hot_build(pos.data_ptr(), mass.data_ptr(), pos.shape[0], _box(lo, size), int(bool(periodic))))
+
+
+def _check_out(t, shape, name):
+    import torch
+
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()
+            and tuple(t.shape) == shape and t.device.index == torch.cuda.current_device()):
+        raise TypeError(f"hot_forces wants {name} as a contiguous CUDA float32 tensor of shape {shape} on the current device")
 
 
 def hot_forces(theta, eps, order, acc=None, pot=None, want_pot=True):
-    """Returns (acc [n,3], pot [n] or None) as CUDA float32 tensors in the caller's particle order."""
+    """Returns (acc [n,3], pot [n] or None) as CUDA float32 tensors in the caller's particle order.
+    n is the size of the library's current build (hot_stats), whichever call made it."""
     import torch
 
-    n = _n_built
+    n = int(hot_stats()["n"])  # 0 before a build: the library then reports HOT_EORDER
+    dev = torch.device("cuda", torch.cuda.current_device())
     if acc is None:
-        acc = torch.empty((max(n, 1), 3), dtype=torch.float32, device=_dev or "cuda")
+        acc = torch.empty((max(n, 1), 3), dtype=torch.float32, device=dev)
+    elif n:
+        _check_out(acc, (n, 3), "acc")
     if pot is None and want_pot:
-        pot = torch.empty(max(n, 1), dtype=torch.float32, device=_dev or "cuda")
+        pot = torch.empty(max(n, 1), dtype=torch.float32, device=dev)
+    elif pot is not None and n:
+        _check_out(pot, (n,), "pot")
     _check(_load().hot_forces(float(theta), float(eps), int(order), acc.data_ptr(),
                               pot.data_ptr() if pot is not None else None))
     return acc, pot
@@ -195,16 +206,31 @@ def hot_export_cells() -> dict:
 
 def hot_export_groups() -> dict:
     ng = hot_stats()["n_groups"]
-    out = dict(cell=np.empty(ng, np.int32), lpc=np.empty(ng, np.uint64), lpp=np.empty(ng, np.uint64))
+    out = dict(cell=np.empty(ng, np.int32), key=np.empty(ng, np.uint64), first=np.empty(ng, np.uint32),
+               count=np.empty(ng, np.uint32), lpc=np.empty(ng, np.uint64), lpp=np.empty(ng, np.uint64))
     got = C.c_int64()
-    _check(_load().hot_export_groups(out["cell"].ctypes.data, out["lpc"].ctypes.data, out["lpp"].ctypes.data,
+    _check(_load().hot_export_groups(out["cell"].ctypes.data, out["key"].ctypes.data, out["first"].ctypes.data,
+                                     out["count"].ctypes.data, out["lpc"].ctypes.data, out["lpp"].ctypes.data,
                                      ng, C.byref(got)))
+    return out
+
+
+def hot_export_lists(group: int) -> dict:
+    """Interaction lists of one sink group from the last hot_forces: accepted cells (+ image ids) and listed
+    bodies (sorted positions, + image ids; the group's own bodies are not listed)."""
+    npc, npp = C.c_int64(), C.c_int64()
+    lib = _load()
+    _check(lib.hot_export_lists(int(group), None, None, 0, C.byref(npc), None, None, 0, C.byref(npp)))
+    out = dict(pc_cell=np.empty(npc.value, np.int32), pc_img=np.empty(npc.value, np.uint8),
+               pp_body=np.empty(npp.value, np.uint32), pp_img=np.empty(npp.value, np.uint8))
+    _check(lib.hot_export_lists(int(group), out["pc_cell"].ctypes.data, out["pc_img"].ctypes.data, npc.value, C.byref(npc),
+                                out["pp_body"].ctypes.data, out["pp_img"].ctypes.data, npp.value, C.byref(npp)))
     return out
 
 
 def hot_export_moments(order: int) -> dict:
     nc = hot_stats()["n_cells"]
-    out = dict(com=np.empty((nc, 3), np.float64), m0=np.empty(nc, np.float32))
+    out = dict(com=np.empty((nc, 3), np.float64), m0=np.empty(nc, np.float32), bmax=np.empty(nc, np.float32))
     m2 = m3 = m4 = None
     if order >= 2:
         out["m2"] = m2 = np.empty((nc, 6), np.float32)
@@ -212,7 +238,7 @@ def hot_export_moments(order: int) -> dict:
         out["m3"] = m3 = np.empty((nc, 10), np.float32)
         out["m4"] = m4 = np.empty((nc, 15), np.float32)
     p = lambda a: a.ctypes.data if a is not None else None
-    _check(_load().hot_export_moments(p(out["com"]), p(out["m0"]), p(m2), p(m3), p(m4), nc))
+    _check(_load().hot_export_moments(p(out["com"]), p(out["m0"]), p(out["bmax"]), p(m2), p(m3), p(m4), nc))
     return out
 
 

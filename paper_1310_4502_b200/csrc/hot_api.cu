@@ -46,8 +46,9 @@ struct Ctx {
     hot_stats_t st{};
     cudaEvent_t ev[9] = {};
     bool ev_ready = false;
-    // host staging for hot_step_host
-    float *h_pos = nullptr, *h_mass = nullptr, *h_acc = nullptr, *h_pot = nullptr; int64_t h_n = 0;
+    int64_t list_g0 = 0, list_g1 = 0; // groups whose lists the arena holds after the last hot_forces
+    // device staging of hot_step_host
+    int64_t h_n = 0;
     float *hd_pos = nullptr, *hd_mass = nullptr, *hd_acc = nullptr, *hd_pot = nullptr;
 };
 Ctx g;
@@ -177,9 +178,8 @@ void hot_free(void) {
     for (auto& e : g.evx) cudaEventDestroy(e);
     g.evx.clear();
     g.arena_pc = g.arena_pp = 0; g.used_pc = g.used_pp = 0; g.used_groups = 0; g.stage_cap = 0;
-    cudaFreeHost(g.h_pos); cudaFreeHost(g.h_mass); cudaFreeHost(g.h_acc); cudaFreeHost(g.h_pot);
     cudaFree(g.hd_pos); cudaFree(g.hd_mass); cudaFree(g.hd_acc); cudaFree(g.hd_pot);
-    g.h_pos = g.h_mass = g.h_acc = g.h_pot = nullptr; g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
+    g.hd_pos = g.hd_mass = g.hd_acc = g.hd_pot = nullptr; g.h_n = 0;
     cudaGetLastError();
     g.st = hot_stats_t{};
 }
@@ -299,7 +299,6 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (!acc) return fail(HOT_EINVAL, "hot_forces: NULL acc");
     if (!(theta >= 0.0) || !(theta < 1.0)) return fail(HOT_EINVAL, "hot_forces: theta must be in [0, 1)");
     if (!(eps >= 0.0)) return fail(HOT_EINVAL, "hot_forces: eps must be >= 0");
-    if (order == 1) order = 0;
     if (order != 0 && order != 2 && order != 4) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2 or 4");
     Tree& t = g.t;
     cudaStream_t st = g.stream;
@@ -472,6 +471,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
             if (cappc > oldpc || cappp > oldpp) { rc = alloc_lists(); if (rc) return rc; }
             budget = (F - g0) * (int64_t)((cappc + cappp) / (oldpc + oldpp));
         }
+        g.list_g0 = g0; g.list_g1 = F;
         g0 = F;
         ++nrounds;
     }
@@ -560,22 +560,28 @@ int hot_export_cells(uint64_t* key, uint32_t* first, uint32_t* count, uint8_t* m
     }
     return HOT_OK;
 }
-int hot_export_groups(int32_t* cell, uint64_t* lpc, uint64_t* lpp, int64_t cap, int64_t* ngroups) {
+int hot_export_groups(int32_t* cell, uint64_t* key, uint32_t* first, uint32_t* count, uint64_t* lpc, uint64_t* lpp,
+                      int64_t cap, int64_t* ngroups) {
     if (!g.built) return fail(HOT_EORDER, "hot_export_groups: no build");
     const Tree& t = g.t;
     if (ngroups) *ngroups = t.ngroups;
     if (cap < t.ngroups) return fail(HOT_EINVAL, "hot_export_groups: cap too small");
     CUDA_TRY(cudaStreamSynchronize(g.stream));
     size_t ng = (size_t)t.ngroups;
-    if (cell) {
-        std::vector<GroupRec> r(ng);
-        CUDA_TRY(cudaMemcpy(r.data(), t.group, sizeof(GroupRec) * ng, cudaMemcpyDeviceToHost));
-        for (size_t i = 0; i < ng; ++i) cell[i] = (int32_t)r[i].cell;
+    std::vector<GroupRec> r(ng);
+    CUDA_TRY(cudaMemcpy(r.data(), t.group, sizeof(GroupRec) * ng, cudaMemcpyDeviceToHost));
+    for (size_t i = 0; i < ng; ++i) {
+        if (cell) cell[i] = (int32_t)r[i].cell;
+        if (first) first[i] = r[i].first;
+        if (count) count[i] = r[i].count;
+    }
+    if (key) {
+        std::vector<uint64_t> ck((size_t)t.ncells);
+        CUDA_TRY(cudaMemcpy(ck.data(), t.ckey, 8 * (size_t)t.ncells, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < ng; ++i) key[i] = ck[r[i].cell];
     }
     if (lpc || lpp) { // device holds u32 list lengths; L_pp counts the group's own bodies too (they are not in the list)
         std::vector<uint32_t> v(ng);
-        std::vector<GroupRec> r(ng);
-        CUDA_TRY(cudaMemcpy(r.data(), t.group, sizeof(GroupRec) * ng, cudaMemcpyDeviceToHost));
         if (lpc) {
             CUDA_TRY(cudaMemcpy(v.data(), t.glpc, 4 * ng, cudaMemcpyDeviceToHost));
             for (size_t i = 0; i < ng; ++i) lpc[i] = v[i];
@@ -587,19 +593,46 @@ int hot_export_groups(int32_t* cell, uint64_t* lpc, uint64_t* lpp, int64_t cap, 
     }
     return HOT_OK;
 }
-int hot_export_moments(double* com, float* m0, float* m2, float* m3, float* m4, int64_t cap) {
+int hot_export_lists(int64_t group, int32_t* pc_cell, uint8_t* pc_img, int64_t pc_cap, int64_t* npc, uint32_t* pp_body,
+                     uint8_t* pp_img, int64_t pp_cap, int64_t* npp) {
+    if (!g.built || !g.lists_valid) return fail(HOT_EORDER, "hot_export_lists: no hot_forces on this build");
+    const Tree& t = g.t;
+    if (!npc || !npp) return fail(HOT_EINVAL, "hot_export_lists: NULL npc / npp");
+    if (group < 0 || group >= t.ngroups) return fail(HOT_EINVAL, "hot_export_lists: group %lld outside [0, %lld)", (long long)group, (long long)t.ngroups);
+    if (group < g.list_g0 || group >= g.list_g1)
+        return fail(HOT_EORDER, "hot_export_lists: the arena holds the lists of groups [%lld, %lld) only", (long long)g.list_g0, (long long)g.list_g1);
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    uint32_t n2[2]; unsigned long long off[2];
+    CUDA_TRY(cudaMemcpy(&n2[0], t.glpc + group, 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(&n2[1], t.glpp + group, 4, cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(&off[0], t.pcoff + group, 8, cudaMemcpyDeviceToHost));
+    CUDA_TRY(cudaMemcpy(&off[1], t.ppoff + group, 8, cudaMemcpyDeviceToHost));
+    *npc = n2[0]; *npp = n2[1];
+    if ((pc_cell && pc_cap < (int64_t)n2[0]) || (pc_img && pc_cap < (int64_t)n2[0])) return fail(HOT_EINVAL, "hot_export_lists: pc_cap %lld < %u", (long long)pc_cap, n2[0]);
+    if ((pp_body && pp_cap < (int64_t)n2[1]) || (pp_img && pp_cap < (int64_t)n2[1])) return fail(HOT_EINVAL, "hot_export_lists: pp_cap %lld < %u", (long long)pp_cap, n2[1]);
+    if (pc_cell && n2[0]) {
+        CUDA_TRY(cudaMemcpy(pc_cell, g.d_pclist + off[0], 4 * (size_t)n2[0], cudaMemcpyDeviceToHost));
+        for (uint32_t i = 0; i < n2[0]; ++i) pc_cell[i] = (int32_t)((uint32_t)pc_cell[i] & ~HOT_COARSE_FLAG); // the fp64-monopole mark of periodic walks
+    }
+    if (pp_body && n2[1]) CUDA_TRY(cudaMemcpy(pp_body, g.d_pplist + off[1], 4 * (size_t)n2[1], cudaMemcpyDeviceToHost));
+    if (pc_img && n2[0]) { if (t.periodic) CUDA_TRY(cudaMemcpy(pc_img, g.d_pcimg + off[0], n2[0], cudaMemcpyDeviceToHost)); else memset(pc_img, 62, n2[0]); }
+    if (pp_img && n2[1]) { if (t.periodic) CUDA_TRY(cudaMemcpy(pp_img, g.d_ppimg + off[1], n2[1], cudaMemcpyDeviceToHost)); else memset(pp_img, 62, n2[1]); }
+    return HOT_OK;
+}
+int hot_export_moments(double* com, float* m0, float* bmax, float* m2, float* m3, float* m4, int64_t cap) {
     if (!g.built || g.t.mom_order < 0) return fail(HOT_EORDER, "hot_export_moments: no hot_forces yet");
     const Tree& t = g.t;
     if (cap < t.ncells) return fail(HOT_EINVAL, "hot_export_moments: cap too small");
     if ((m2 && t.mom_order < 2) || ((m3 || m4) && t.mom_order < 4)) return fail(HOT_EINVAL, "hot_export_moments: order not computed");
     CUDA_TRY(cudaStreamSynchronize(g.stream));
     size_t nc = (size_t)t.ncells;
-    if (com || m0) {
+    if (com || m0 || bmax) {
         std::vector<CellA> a(nc);
         CUDA_TRY(cudaMemcpy(a.data(), t.cellA, sizeof(CellA) * nc, cudaMemcpyDeviceToHost));
         for (size_t i = 0; i < nc; ++i) {
             if (com) { com[3 * i] = a[i].zx; com[3 * i + 1] = a[i].zy; com[3 * i + 2] = a[i].zz; }
             if (m0) m0[i] = a[i].m0;
+            if (bmax) bmax[i] = a[i].bmax;
         }
     }
     if (m2) {

@@ -330,7 +330,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
         const uint8_t* const pi = PER ? P.pcimg + o0 : nullptr;
         const int nb = (n + BATCH - 1) / BATCH;
         CellA cA;
-        cA.zx = cA.zy = cA.zz = 0.0; cA.m0 = 0.f; cA.t2 = 0.f;
+        cA.zx = cA.zy = cA.zz = 0.0; cA.m0 = 0.f; cA.bmax = 0.f;
         uint32_t cnext = 0; int inext = 62, pim = 62;
         auto fetch_idx = [&](int b) { // list entries of batch b
             if (b * BATCH + lane < n) { cnext = pl[b * BATCH + lane]; if (PER) inext = pi[b * BATCH + lane]; }

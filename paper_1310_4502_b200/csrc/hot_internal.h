@@ -24,7 +24,7 @@ extern long long g_hot_launches; // kernels launched by the library since the la
 struct __align__(16) WalkCell { uint32_t x, y, z, w; };
 
 // per-cell expansion data (S6), gathered when a cell is accepted
-struct __align__(16) CellA { double zx, zy, zz; float m0; float t2; };   // centre of mass, mass, trace M2
+struct __align__(16) CellA { double zx, zy, zz; float m0; float bmax; }; // centre of mass, mass, b_max: radius about the centre of mass that holds every body (R-15)
 struct __align__(16) CellM2 { float xx, xy, xz, yy, yz, zz, t2, pad1; };     // t2 = trace
 // the same record as the P-C kernel stages it (cellE2): 3 xx, 3 xy, 3 xz, 3 yy, 3 yz, 3 zz, 1.5 t2, 0.5 t2 -- the
 // constant factors of the order-2 terms folded in once per cell instead of once per interaction

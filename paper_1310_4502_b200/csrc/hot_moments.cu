@@ -66,19 +66,19 @@ __device__ __forceinline__ void add_shifted(double* M, const double* C, double m
 }
 
 template <int ORDER>
-__device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, double zy, double zz, const double* M,
+__device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, double zy, double zz, double bmax, const double* M,
                                            CellA* cellA, CellM2* cellM2, CellM2* cellE2, CellM34* cellM34) {
-    CellA A; A.zx = zx; A.zy = zy; A.zz = zz; A.m0 = (float)m0; A.t2 = 0.f;
+    CellA A; A.zx = zx; A.zy = zy; A.zz = zz; A.m0 = (float)m0; A.bmax = __double2float_ru(bmax); // rounded up: stays a bound
     if (ORDER >= 2) {
         CellM2 Q;
         Q.xx = (float)M[midx(2, 0, 0)]; Q.xy = (float)M[midx(1, 1, 0)]; Q.xz = (float)M[midx(1, 0, 1)];
         Q.yy = (float)M[midx(0, 2, 0)]; Q.yz = (float)M[midx(0, 1, 1)]; Q.zz = (float)M[midx(0, 0, 2)];
-        A.t2 = Q.xx + Q.yy + Q.zz;
-        Q.t2 = A.t2; Q.pad1 = 0.f; // the trace rides in the record the P-C kernel stages with cp.async
+        const float t2 = Q.xx + Q.yy + Q.zz;
+        Q.t2 = t2; Q.pad1 = 0.f;
         cellM2[c] = Q;
         CellM2 E; // what the P-C kernel stages: phi2 = 0.5 t2 ri^3 - 0.5 ri^5 R.(3 M2).R, a2 = R (1.5 t2 ri^5 - 2.5 ri^7 R.(3 M2).R) + ri^5 (3 M2) R
         E.xx = 3.f * Q.xx; E.xy = 3.f * Q.xy; E.xz = 3.f * Q.xz; E.yy = 3.f * Q.yy; E.yz = 3.f * Q.yz; E.zz = 3.f * Q.zz;
-        E.t2 = 1.5f * A.t2; E.pad1 = 0.5f * A.t2;
+        E.t2 = 1.5f * t2; E.pad1 = 0.5f * t2;
         cellE2[c] = E;
     }
     cellA[c] = A;
@@ -129,7 +129,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(int64_t cbeg, int64_
     double M[NM];
 #pragma unroll
     for (int k = 0; k < NM; ++k) M[k] = 0;
-    double m0 = 0, zx = 0, zy = 0, zz = 0;
+    double m0 = 0, zx = 0, zy = 0, zz = 0, bmax = 0; // bmax: DESIGN.md R-15 (leaf: farthest body; else children's radii + offsets)
     int32_t ch = cchild[c];
     if (ch < 0) { // leaf: from its bodies
         uint32_t f = cfirst[c], n = ccount[c];
@@ -138,11 +138,13 @@ __global__ void __launch_bounds__(128) moments_level_kernel(int64_t cbeg, int64_
             m0 += (double)b.w; zx += (double)b.w * b.x; zy += (double)b.w * b.y; zz += (double)b.w * b.z;
         }
         zx /= m0; zy /= m0; zz /= m0;
-        if (ORDER >= 2)
-            for (uint32_t j = 0; j < n; ++j) {
-                float4 b = body[f + j];
-                add_point<ORDER>(M, (double)b.w, (double)b.x - zx, (double)b.y - zy, (double)b.z - zz);
-            }
+        for (uint32_t j = 0; j < n; ++j) {
+            float4 b = body[f + j];
+            const double dx = (double)b.x - zx, dy = (double)b.y - zy, dz = (double)b.z - zz;
+            bmax = fmax(bmax, dx * dx + dy * dy + dz * dz);
+            if (ORDER >= 2) add_point<ORDER>(M, (double)b.w, dx, dy, dz);
+        }
+        bmax = sqrt(bmax);
     } else { // internal: from its children (one level down, already done)
         int nch = __popc(cmask[c]);
         for (int k = 0; k < nch; ++k) {
@@ -150,15 +152,18 @@ __global__ void __launch_bounds__(128) moments_level_kernel(int64_t cbeg, int64_
             m0 += (double)A.m0; zx += (double)A.m0 * A.zx; zy += (double)A.m0 * A.zy; zz += (double)A.m0 * A.zz;
         }
         zx /= m0; zy /= m0; zz /= m0;
-        if (ORDER >= 2)
-            for (int k = 0; k < nch; ++k) {
-                CellA A = cellA[ch + k];
+        for (int k = 0; k < nch; ++k) {
+            CellA A = cellA[ch + k];
+            const double dx = A.zx - zx, dy = A.zy - zy, dz = A.zz - zz;
+            bmax = fmax(bmax, sqrt(dx * dx + dy * dy + dz * dz) + (double)A.bmax);
+            if (ORDER >= 2) {
                 double C[NM];
                 load_child<ORDER>(ch + k, cellA, cellM2, cellM34, C);
-                add_shifted<ORDER>(M, C, (double)A.m0, A.zx - zx, A.zy - zy, A.zz - zz);
+                add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
             }
+        }
     }
-    store_cell<ORDER>(c, m0, zx, zy, zz, M, cellA, cellM2, cellE2, cellM34);
+    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, cellA, cellM2, cellE2, cellM34);
 }
 
 cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {

@@ -191,13 +191,22 @@ def test_momentum_conservation_and_coincident_pair():
     m = w.mass.astype(np.float64)
     tot = (m[:, None] * a).sum(0)
     assert np.abs(tot).max() <= 1e-13 * (m[:, None] * np.abs(a)).sum()
-    # energy symmetry: sum_i m_i phi_i = 2 * sum_{i<j} pair energies (antisymmetry of the pairs)
+    # O-2 termwise: the force of j on i is minus the force of i on j.  A pair's term is what is left of the
+    # direct sum when every other body is removed, so evaluate pairs (i, j) on their own
     x = w.pos.astype(np.float64)
+    for i, j in ((0, 1), (5, 900), (17, 18), (1023, 3)):
+        a2, p2 = O.direct(w.pos[[i, j]], w.mass[[i, j]], w.eps)
+        assert np.array_equal(m[i] * a2[0], -(m[j] * a2[1])), (i, j)          # bit-exact: same |d|, same products
+        assert m[i] * p2[0] == m[j] * p2[1]
+    # energy symmetry: sum_i m_i phi_i = 2 * sum_{i<j} (pair energy), pair energies typed out here with numpy
+    k = 65
     e = 0.0
-    for i in range(0, 64):
-        d = x[i + 1:] - x[i]
-        e += -(m[i] * m[i + 1:] / np.sqrt((d * d).sum(1) + w.eps**2)).sum()
-    a64, p64 = O.direct(w.pos[:65], w.mass[:65], w.eps)
+    for i in range(k - 1):
+        d = x[i + 1:k] - x[i]
+        e += -(m[i] * m[i + 1:k] / np.sqrt((d * d).sum(1) + w.eps**2)).sum()
+    a64, p64 = O.direct(w.pos[:k], w.mass[:k], w.eps)
+    assert math.isclose((m[:k] * p64).sum(), 2 * e, rel_tol=1e-13)
+    assert np.abs((m[:k, None] * a64).sum(0)).max() <= 1e-13 * (m[:k, None] * np.abs(a64)).sum()
     # coincident distinct bodies: zero force, -m/eps potential
     pos = np.array([[0.5, 0.5, 0.5], [0.5, 0.5, 0.5]], np.float32)
     a2, p2 = O.direct(pos, np.array([1, 2], np.float32), 0.1)
@@ -350,6 +359,54 @@ def test_moment_pins():
     assert math.isclose(mom[0, 34], (m * d[:, 2] ** 4).sum(), rel_tol=1e-12)  # zzzz
     assert math.isclose(mom[0, 24], (m * d[:, 0] ** 2 * d[:, 1] * d[:, 2]).sum(), rel_tol=1e-9, abs_tol=1e-18)  # xxyz
     assert math.isclose(bmax[0], np.sqrt((d * d).sum(1)).max(), rel_tol=1e-14)
+    # every second, third and fourth moment (indices 4..34) of the root and of a mid-tree cell, typed out with numpy
+    key, skey, perm = T.keys()
+    xs, ms = x[perm], m[perm]
+    mid = int(np.argmax((c["level"] == 2) & (c["count"] > 40)))
+    assert c["level"][mid] == 2
+    for ci in (0, mid):
+        f, k = int(c["first"][ci]), int(c["count"][ci])
+        dd = xs[f:f + k] - (ms[f:f + k, None] * xs[f:f + k]).sum(0) / ms[f:f + k].sum()
+        for q, (a, b, cc) in enumerate(O.multi_indices()):
+            if a + b + cc < 2:
+                continue
+            want = (ms[f:f + k] * dd[:, 0] ** a * dd[:, 1] ** b * dd[:, 2] ** cc).sum()
+            assert abs(mom[ci, q] - want) <= 1e-12 * ms[f:f + k].sum() * np.abs(dd).max() ** (a + b + cc), (ci, a, b, cc)
+
+
+def test_bmax_bound_of_the_upward_pass():
+    """R-15: the b_max an upward pass can carry (children's radii + centre offsets) contains every body of the
+    cell: it is never below the exact radius, equals it on leaves, and never exceeds the cell's diagonal by more
+    than the children's slack (sanity: <= 2 x the exact radius + the cell diagonal)."""
+    w = W.config(2, 12)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, nleaf=4, ncrit=16)
+    mom, com, bmax = T.moments()
+    bb = T.bbound()
+    c = T.cells()
+    leaf = c["child"] < 0
+    assert (bb >= bmax * (1 - 1e-15)).all()
+    assert (bb[leaf] == bmax[leaf]).all()
+    # brute force from the bodies: every body lies within bb of the centre of mass
+    key, skey, perm = T.keys()
+    xs = w.pos.astype(np.float64)[perm]
+    for ci in np.random.default_rng(0).choice(T.ncells, 200, replace=False):
+        f, k = int(c["first"][ci]), int(c["count"][ci])
+        r = np.sqrt(((xs[f:f + k] - com[ci]) ** 2).sum(1)).max()
+        assert r <= bb[ci] * (1 + 1e-14) and math.isclose(r, bmax[ci], rel_tol=1e-13, abs_tol=1e-300)
+    side = w.size * np.ldexp(1.0, -c["level"].astype(np.int64))
+    assert (bb <= np.sqrt(3.0) * side * 2).all()
+
+
+def test_lazy_moments_give_the_same_forces():
+    """moments=2 (only the cells the requested groups accept; used at 2^27 bodies) is the same arithmetic."""
+    w = W.config(2, 11)
+    T1 = O.Tree(w.pos, w.mass, w.lo, w.size)
+    T2 = O.Tree(w.pos, w.mass, w.lo, w.size, moments=2)
+    sel = np.array([0, 3, T1.ngroups - 1])
+    a1, p1, lpc1, lpp1 = T1.forces(0.5, w.eps, 4, groups=sel)
+    a2, p2, lpc2, lpp2 = T2.forces(0.5, w.eps, 4, groups=sel)
+    assert np.array_equal(a1, a2, equal_nan=True) and np.array_equal(p1, p2, equal_nan=True)
+    assert (lpc1 == lpc2).all() and (lpp1 == lpp2).all()
 
 
 # ---------------------------------------------------------------- walk + tree forces (C-7, C-8)
@@ -362,6 +419,94 @@ def test_theta_zero_is_direct_sum():
     assert np.abs(a - ad).max() <= 1e-12 * np.abs(ad).max() and np.abs(p - pd).max() <= 1e-12 * np.abs(pd).max()
 
 
+def _lattice64():
+    """One body at the centre of each of the 64 level-2 cells; NLEAF = NCRIT = 1: root, 8 level-1 cells,
+    64 level-2 leaves which are also the sink groups.  Returns the tree and, per cell index, (level, i, j, k)."""
+    q = (np.arange(4) + 0.5) / 4
+    pts = np.array([[x, y, z] for x in q for y in q for z in q], np.float32)
+    T = O.Tree(pts, np.ones(64, np.float32), (0, 0, 0), 1.0, nleaf=1, ncrit=1, moments=False)
+    c = T.cells()
+    assert T.ncells == 73 and T.ngroups == 64
+    geo = {}
+    for ci in range(T.ncells):
+        l = int(c["level"][ci])
+        k = int(c["key"][ci]) & ((1 << (3 * l)) - 1)
+        ijk = [0, 0, 0]
+        for b in range(l):
+            for ax in range(3):
+                ijk[ax] |= ((k >> (3 * b + 2 - ax)) & 1) << b
+        geo[ci] = (l, *ijk)
+    return T, c, geo
+
+
+def _by_hand_accepts(level, ijk, img, theta):
+    """SURVEY C-7 / DESIGN R-7 worked by hand for the group = level-2 cell (0,0,0) of the 4x4x4 lattice, in
+    units of the level-2 side s (group = [0,1)^3): a level-l cell (i,j,k) of image n is the cube
+    [i w + 4 n, (i+1) w + 4 n) with w = 4 / 2^l; gap per axis = distance between the intervals (0 if they touch
+    or overlap); accepted iff w^2 < theta^2 * (sum of squared gaps), strictly."""
+    from fractions import Fraction
+    wdt = Fraction(4, 2 ** level)
+    d2 = Fraction(0)
+    for ax in range(3):
+        lo = ijk[ax] * wdt + 4 * img[ax]
+        hi = lo + wdt
+        gap = max(Fraction(0), lo - 1, 0 - hi)
+        d2 += gap * gap
+    return wdt * wdt < Fraction(theta).limit_denominator(10 ** 6) ** 2 * d2
+
+
+@pytest.mark.parametrize("theta", [0.5, 0.51, 0.577, 0.578, 0.9])
+def test_mac_by_hand_open_and_one_image(theta):
+    """The FORM of the criterion (verdict r1 item 4): minimum distance between the cubes (not centre distance),
+    s_C^2 < theta^2 d^2 strictly, d = 0 never accepted, image shift +n L applied to the SOURCE."""
+    T, c, geo = _lattice64()
+    g0 = 0  # groups are in key order: group 0 is the level-2 cell (0,0,0)
+    assert geo[int(T.groups()[0])] == (2, 0, 0, 0)
+    for img in ((0, 0, 0), (-1, 0, 0), (1, 0, 0), (0, 2, -1)):
+        pc, lv = T.walk_lists(theta, g0, img=img)
+        want_pc, want_lv = set(), set()
+        # by hand: no level-0/1 cell is ever accepted for theta < 1 in the box itself (gap <= its own side);
+        # in an image, walk the three levels with the rule above
+        def visit(ci):
+            l, i, j, k = geo[ci]
+            if _by_hand_accepts(l, (i, j, k), img, theta):
+                want_pc.add(ci)
+            elif c["child"][ci] < 0:
+                want_lv.add(ci)
+            else:
+                for ch in range(int(c["child"][ci]), int(c["child"][ci]) + bin(int(c["mask"][ci])).count("1")):
+                    visit(ch)
+        visit(0)
+        assert set(pc.tolist()) == want_pc and set(lv.tolist()) == want_lv, (theta, img)
+        assert len(pc) == len(want_pc) and len(lv) == len(want_lv)
+    # the named cases, spelled out
+    pc, lv = T.walk_lists(theta, g0)
+    by = {geo[ci][1:]: ci for ci in geo if geo[ci][0] == 2}
+    # cell (2,2,2): gap (s,s,s), d^2 = 3 s^2: accepted iff theta^2 > 1/3
+    assert (by[(2, 2, 2)] in pc) == (theta * theta > 1 / 3)
+    # cell (3,0,0): gap (2s,0,0), d^2 = 4 s^2: theta = 0.5 is an exact tie and a tie is NOT accepted
+    assert (by[(3, 0, 0)] in pc) == (theta > 0.5)
+    # face-, edge- and corner-adjacent cells touch the group (d = 0): never accepted, and neither is the group itself
+    for adj in ((1, 0, 0), (1, 1, 0), (1, 1, 1), (0, 0, 0)):
+        assert by[adj] in lv and by[adj] not in pc
+    # a centre-distance criterion would differ: (2,0,0) has centre distance 2s but gap s -> rejected for theta < 1
+    assert by[(2, 0, 0)] in lv
+    # image (-1,0,0): the copy of cell (3,0,0) occupies x in [-s, 0) and touches the group: never accepted;
+    # the copy of cell (1,0,0) occupies [-3s,-2s): gap 2 s: accepted iff theta > 0.5.  With the shift applied
+    # with the wrong sign these cells would sit at x in [7s, 8s) and [5s, 6s) and both be accepted at theta >= 0.5.
+    pc, lv = T.walk_lists(theta, g0, img=(-1, 0, 0))
+    assert by[(3, 0, 0)] in lv
+    assert (by[(1, 0, 0)] in pc) == (theta > 0.5)
+    # every group, every listed image: accepted cells + rejected leaves cover each body exactly once
+    for g in (0, 21, 63):
+        for img in ((0, 0, 0), (2, -2, 1)):
+            pc, lv = T.walk_lists(theta, g, img=img)
+            seen = np.zeros(64, int)
+            for ci in list(pc) + list(lv):
+                seen[c["first"][ci]:c["first"][ci] + c["count"][ci]] += 1
+            assert (seen == 1).all()
+
+
 @pytest.mark.parametrize("cfg,scale", [(0, 12), (1, 12), (2, 12)])
 def test_coverage_invariant(cfg, scale):
     w = W.config(cfg, scale)
@@ -369,7 +514,7 @@ def test_coverage_invariant(cfg, scale):
     for theta in (0.3, 0.5, 0.8):
         lpc, lpp, cov = T.walk_counts(theta)
         assert (cov + lpp == w.n).all()
-    # the lists of one group: disjoint particle cover, no accepted cell touches the group
+    # the lists of one group: disjoint particle cover, and no accepted cell touches or overlaps the group's cube
     c = T.cells()
     g = T.ngroups // 2
     pc, lv = T.walk_lists(0.5, g)
@@ -377,6 +522,19 @@ def test_coverage_invariant(cfg, scale):
     for ci in list(pc) + list(lv):
         seen[c["first"][ci]:c["first"][ci] + c["count"][ci]] += 1
     assert (seen == 1).all()
+
+    def cube(ci):  # integer corner and side on the 2^21 grid, from the key alone
+        l = int(c["level"][ci]); k = int(c["key"][ci]) & ((1 << (3 * l)) - 1)
+        o = [0, 0, 0]
+        for b in range(l):
+            for ax in range(3):
+                o[ax] |= ((k >> (3 * b + 2 - ax)) & 1) << b
+        return [v << (21 - l) for v in o], 1 << (21 - l)
+    go, gs = cube(int(T.groups()[g]))
+    for ci in pc:
+        o, sz = cube(int(ci))
+        gaps = [max(0, o[ax] - (go[ax] + gs), go[ax] - (o[ax] + sz)) for ax in range(3)]
+        assert sum(v * v for v in gaps) * 0.25 > sz * sz  # accepted at theta = 0.5: strictly separated, by more than 2 sides
 
 
 def test_error_monotone_in_order_and_theta():

@@ -45,6 +45,8 @@ def _check_int_artefacts(hot, T):
     assert st["n_leaves"] == int((oc["child"] < 0).sum()) and st["max_level"] == int(oc["level"].max())
     gg = hot.hot_export_groups()
     assert (gg["cell"] == T.groups()).all(), "sink groups"
+    og = T.groups()
+    assert (gg["key"] == oc["key"][og]).all() and (gg["first"] == oc["first"][og]).all() and (gg["count"] == oc["count"][og]).all()
     # cell membership: leaf of every sorted particle, via the hash table (key -> cell index)
     leaf = T.leaf_of()
     sel = np.random.default_rng(1).choice(T.n, min(T.n, 4096), replace=False)
@@ -94,6 +96,60 @@ def test_open_boundary_parity(hot, cfg, scale, nleaf, ncrit, order, theta):
     assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
 
 
+@pytest.mark.parametrize("cfg,scale,periodic,theta", [(2, 12, False, 0.6), (0, 11, False, 0.4), (4, 12, True, 0.5), (3, 10, True, 0.7)])
+def test_interaction_lists_as_sets(hot, cfg, scale, periodic, theta):
+    """not only the list COUNTS but the lists themselves, as sorted sets, equal the oracle's
+    (N <= 2^12, open and periodic; per image when periodic).  The GPU lists bodies, the oracle rejected leaves:
+    a leaf's body range is expanded here; the group's own bodies (image 62) are not in the GPU list."""
+    w = W.config(cfg, scale)
+    assert w.periodic == periodic and w.n <= 4096
+    _build(hot, w, 8, 32)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=periodic, nleaf=8, ncrit=32, moments=False)
+    hot.hot_forces(theta, w.eps, 2)
+    c = T.cells()
+    gg = hot.hot_export_groups()
+    rng = np.random.default_rng(7)
+    groups = np.unique(np.append(rng.choice(T.ngroups, min(T.ngroups, 12 if periodic else 40), replace=False), [0, T.ngroups - 1]))
+    for gi in groups:
+        L = hot.hot_export_lists(int(gi))
+        gf, gk = int(gg["first"][gi]), int(gg["count"][gi])
+        images = [(ix, iy, iz) for ix in range(-2, 3) for iy in range(-2, 3) for iz in range(-2, 3)] if periodic else [(0, 0, 0)]
+        npc = npp = 0
+        for img in images:
+            iid = 25 * (img[0] + 2) + 5 * (img[1] + 2) + (img[2] + 2)
+            pc, lv = T.walk_lists(theta, int(gi), img=img)
+            bodies = np.concatenate([np.arange(c["first"][l], c["first"][l] + c["count"][l]) for l in lv]) if len(lv) else np.zeros(0, np.int64)
+            if iid == 62:
+                bodies = bodies[(bodies < gf) | (bodies >= gf + gk)]  # the group's own bodies are paired separately
+            got_pc = np.sort(L["pc_cell"][L["pc_img"] == iid])
+            got_pp = np.sort(L["pp_body"][L["pp_img"] == iid])
+            assert np.array_equal(got_pc, np.sort(pc)), (gi, img, "accepted cells")
+            assert np.array_equal(got_pp, np.sort(bodies)), (gi, img, "listed bodies")
+            npc += len(pc); npp += len(bodies)
+        assert npc == len(L["pc_cell"]) == gg["lpc"][gi] and npp == len(L["pp_body"]) and npp + gk == gg["lpp"][gi]
+        assert len(np.unique(L["pc_cell"].astype(np.int64) * 125 + L["pc_img"])) == npc, "no entry twice"
+        assert len(np.unique(L["pp_body"].astype(np.int64) * 125 + L["pp_img"])) == npp
+
+
+def test_binding_sizes_outputs_from_the_library_build(hot):
+    """hot_build(small) -> hot_step_host(big) replaces the build inside the library; hot_forces() must
+    size its outputs from the library's n, and reject wrongly shaped / typed / placed outputs."""
+    import torch
+
+    ws, wb = W.config(0, 8), W.config(0, 11)
+    _build(hot, ws)
+    ha, hp = hot.hot_step_host(wb.pos, wb.mass, wb.lo, wb.size, False, 0.5, wb.eps, 2)
+    acc, pot = hot.hot_forces(0.5, wb.eps, 2)
+    assert acc.shape == (wb.n, 3) and pot.shape == (wb.n,)
+    assert (acc.cpu().numpy() == ha).all() and (pot.cpu().numpy() == hp).all()
+    for bad_acc in (torch.empty((ws.n, 3), device="cuda"), torch.empty((wb.n, 3), device="cuda", dtype=torch.float64),
+                    torch.empty((wb.n, 3)), torch.empty((3, wb.n), device="cuda").t()):
+        with pytest.raises(TypeError):
+            hot.hot_forces(0.5, wb.eps, 2, acc=bad_acc)
+    with pytest.raises(TypeError):
+        hot.hot_forces(0.5, wb.eps, 2, pot=torch.empty(wb.n + 1, device="cuda"))
+
+
 def test_moments_parity(hot):
     w = W.config(2, 14)
     _build(hot, w)
@@ -104,6 +160,10 @@ def test_moments_parity(hot):
     size = np.ldexp(1.0, -T.cells()["level"].astype(np.int64)) * w.size  # cell side
     assert np.abs(g["com"] - com).max() <= 1e-12 * w.size
     assert np.abs(g["m0"] - mom[:, 0]).max() <= 1e-6 * mom[:, 0].max()
+    # b_max (R-15): the upward-pass bound, rounded up to fp32; never below the exact radius
+    bb, bexact = T.bbound(), T.moments()[2]
+    assert (np.abs(g["bmax"] - bb) <= 2e-7 * bb + 1e-30).all()
+    assert (g["bmax"].astype(np.float64) >= bexact * (1 - 1e-12)).all()
     for name, sl, deg in (("m2", slice(4, 10), 2), ("m3", slice(10, 20), 3), ("m4", slice(20, 35), 4)):
         scale = mom[:, 0] * size ** deg  # natural size of a degree-`deg` moment of the cell
         err = np.abs(g[name] - mom[:, sl]).max(axis=1) / scale
@@ -237,7 +297,7 @@ def test_error_codes(hot):
         hot.hot_build(pos, mass, w.lo, -1.0, False)
     assert e.value.code == -1
     hot.hot_build(pos, mass, w.lo, w.size, False)
-    for theta, eps, order in ((1.0, 1e-3, 2), (-0.1, 1e-3, 2), (0.5, -1.0, 2), (0.5, 1e-3, 3), (0.5, 1e-3, 6)):
+    for theta, eps, order in ((1.0, 1e-3, 2), (-0.1, 1e-3, 2), (0.5, -1.0, 2), (0.5, 1e-3, 3), (0.5, 1e-3, 6), (0.5, 1e-3, 1)):
         with pytest.raises(HotError) as e:
             hot.hot_forces(theta, eps, order)
         assert e.value.code == -1
@@ -360,14 +420,16 @@ def test_small_list_arena_gives_the_same_result_in_rounds(hot):
 
 # ---- BASELINE.json's full sizes, in the configuration bench.py times, on sampled sink groups -----------
 @pytest.mark.slow
-@pytest.mark.parametrize("cfg,order,theta,nsel", [(2, 2, 0.6, 96), (1, 2, 0.5, 96), (3, 4, 0.5, 24)])
+@pytest.mark.parametrize("cfg,order,theta,nsel", [(2, 2, 0.6, 96), (1, 2, 0.5, 96), (3, 4, 0.5, 24), (4, 2, 0.5, 24)])
 def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
-    """configs[2] at N = 2^24 (the bench workload), configs[1] at 2^20, configs[3] at 256^3 periodic:
-    integer artefacts in full, forces and list counts on a seeded sample of sink groups (the oracle
-    evaluates a group in milliseconds, the whole set would take hours)."""
+    """configs[2] at N = 2^24 (the bench workload), configs[1] at 2^20, configs[3] at 256^3 and configs[4] at
+    512^3 = 2^27 periodic: integer artefacts in full (keys, permutation, every cell, every group), forces and
+    list counts on a seeded sample of sink groups (the oracle evaluates a group in milliseconds to seconds, the
+    whole set would take hours).  At 2^27 the oracle computes the moments of the cells those groups accept only
+    (Tree(moments=2): same cell_moments; all 2e7 cells would take hours -- BASELINE.md section 3)."""
     w = W.config(cfg)
     _build(hot, w, 16, 256)  # the bucket sizes bench.py times
-    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic, nleaf=16, ncrit=256)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic, nleaf=16, ncrit=256, moments=2 if cfg == 4 else True)
     _check_int_artefacts(hot, T)
     acc, pot = hot.hot_forces(theta, w.eps, order)
     gg = hot.hot_export_groups()
@@ -388,12 +450,27 @@ def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
           "pot median", np.median(ep), "p99.9", np.quantile(ep, 0.999))
     assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
     assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
-    # coverage invariant at full size: every body is in exactly one list entry's range per image
+    # coverage invariant at full size on the GPU's own lists (sampled groups; the arena may hold the last round
+    # only): the accepted cells' bodies + the listed bodies + the group's own = n bodies per image, each once
     cnt = T.cells()["count"]
     st = hot.hot_stats()
+    nimg = 125 if w.periodic else 1
+    checked = 0
+    for gi in sel[::-1][:6]:
+        try:
+            L = hot.hot_export_lists(int(gi))
+        except Exception as e:  # HOT_EORDER: lists of an earlier round
+            assert getattr(e, "code", 0) == -5 and st["list_chunks"] > 1
+            continue
+        assert len(L["pc_cell"]) == gg["lpc"][gi] and len(L["pp_body"]) + gg["count"][gi] == gg["lpp"][gi]
+        assert int(cnt[L["pc_cell"]].sum()) + int(gg["lpp"][gi]) == w.n * nimg
+        per_img = np.bincount(L["pc_img"], weights=cnt[L["pc_cell"]], minlength=125) + np.bincount(L["pp_img"], minlength=125)
+        per_img[62] += gg["count"][gi]
+        assert (per_img[per_img > 0] == w.n).all() and (per_img > 0).sum() == nimg
+        checked += 1
+    assert checked >= 1
     assert st["n"] == w.n and st["pp_interactions"] > 0 and st["pc_interactions"] > 0
     assert np.isfinite(acc.cpu().numpy()).all() and np.isfinite(pot.cpu().numpy()).all()
-    del cnt
 
 
 @pytest.mark.slow
