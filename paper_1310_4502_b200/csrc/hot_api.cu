@@ -9,6 +9,8 @@
 #include "hot_internal.h"
 
 long long g_hot_launches = 0;
+unsigned long long g_hot_dbg_mask = ~0ull;
+int g_hot_sb_shift = 16; // groups per superblock of the interaction kernel's work-item order (hot_forces.cu), log2
 
 namespace {
 
@@ -23,6 +25,7 @@ struct Ctx {
     int* d_flags = nullptr;               // [0] build error bits, [1] hash max probe, [2] forces error bits
     unsigned int* d_counter = nullptr;
     uint4* d_items = nullptr; // work items of the interaction kernel
+    unsigned int* d_cls = nullptr; // ... and their per-superblock class counters (launch_plan)
     unsigned long long* d_stat = nullptr; // 4 counters
     uint32_t* d_gstack = nullptr; size_t gstack_bytes = 0; int64_t gstack_cap = 0;
     // device buffers of the build, pooled across hot_build calls: a slot is keyed by the address of
@@ -104,7 +107,7 @@ void drop_build() { // forgets the build; its buffers stay pooled for the next o
 int ensure_scratch() {
     if (!g.d_flags) {
         CUDA_TRY(cudaMalloc(&g.d_flags, 4 * sizeof(int)));
-        CUDA_TRY(cudaMalloc(&g.d_counter, 18 * sizeof(unsigned int))); // walk and interaction schedulers, 16 work-item class counters
+        CUDA_TRY(cudaMalloc(&g.d_counter, 2 * sizeof(unsigned int))); // walk and interaction schedulers
         CUDA_TRY(cudaMalloc(&g.d_stat, 4 * sizeof(unsigned long long)));
     }
     if (!g.ev_ready) {
@@ -136,6 +139,9 @@ float ms_between(cudaEvent_t a, cudaEvent_t b) {
 } // namespace
 
 extern "C" {
+
+int hot_debug_set_mask(unsigned long long m) { g_hot_dbg_mask = m; return HOT_OK; }
+int hot_debug_set_sb_shift(int s) { if (s < 8 || s > 30) return HOT_EINVAL; g_hot_sb_shift = s; return HOT_OK; } // TEMP sweep hook
 
 const char* hot_last_error(void) { return g.err; }
 
@@ -255,21 +261,20 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     CUDA_TRY(tree_alloc(&t.cparent, (size_t)t.ncells));
     CUDA_TRY(tree_alloc(&t.wcell, (size_t)t.ncells));
     CUDA_TRY(tree_alloc(&t.group, (size_t)t.ngroups));
+    CUDA_TRY(tree_alloc(&t.leafcell, (size_t)t.nleaves));
     CUDA_TRY(tree_alloc(&t.glpc, (size_t)t.ngroups));
     CUDA_TRY(tree_alloc(&t.glpp, (size_t)t.ngroups));
-    CUDA_TRY(tree_alloc(&t.hkey, (size_t)t.hcap));
     CUDA_TRY(tree_alloc(&t.hval, (size_t)t.hcap));
     CUDA_TRY(cudaMemsetAsync(t.hval, 0xff, sizeof(int32_t) * (size_t)t.hcap, st)); // -1: free slot
-    CUDA_TRY(cudaMemsetAsync(t.cmask, 0, sizeof(uint32_t) * (size_t)t.ncells, st));
     CUDA_TRY(cudaMemsetAsync(t.glpc, 0, sizeof(uint32_t) * (size_t)t.ngroups, st));
     CUDA_TRY(cudaMemsetAsync(t.glpp, 0, sizeof(uint32_t) * (size_t)t.ngroups, st));
     TreeEmitArgs ea;
     ea.skey = t.key[0]; ea.plev = t.plev; ea.counts = d_counts; ea.n = n; ea.nblk = nblk;
     for (int l = 0; l <= HOT_NLEVELS; ++l) ea.level_base[l] = t.level_base[l];
     ea.ckey = t.ckey; ea.cfirst = t.cfirst; ea.ccount = t.ccount; ea.cchild = t.cchild; ea.cparent = t.cparent;
-    ea.group = t.group; ea.open = g.d_open;
+    ea.group = t.group; ea.leafcell = t.leafcell; ea.open = g.d_open;
     CUDA_TRY(launch_tree_emit(ea, st));
-    CUDA_TRY(launch_tree_link(t.ckey, t.cparent, t.cmask, t.ncells, t.hkey, t.hval, t.hcap - 1, g.d_flags + 1, st));
+    CUDA_TRY(launch_tree_link(t.ckey, t.ncells, t.hval, t.hcap - 1, g.d_flags + 1, st));
     CUDA_TRY(launch_tree_finalize(t.ckey, t.cfirst, t.ccount, t.cmask, t.cchild, t.wcell, t.ncells, g.d_flags, st));
     CUDA_TRY(cudaEventRecord(g.ev[4], st));
     CUDA_TRY(cudaMemcpyAsync(flags, g.d_flags, sizeof(flags), cudaMemcpyDeviceToHost, st));
@@ -394,7 +399,10 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
     a.far = t.periodic ? t.far : nullptr;
-    a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1; a.cls = g.d_counter + 2;
+    a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
+    a.sb_shift = g_hot_sb_shift; a.dbg_mask = g_hot_dbg_mask;
+    CUDA_TRY(tree_alloc(&g.d_cls, plan_cls_elems(ng, a.sb_shift)));
+    a.cls = g.d_cls;
     CUDA_TRY(tree_alloc(&g.d_items, (size_t)(HOT_MAX_NCRIT / 64 + 2) * (size_t)ng)); // passes per group: full ones of >= 64 sinks, one split in two
     a.items = g.d_items;
     // groups per round: all of them unless the arena is known (or found) to be too small.  The warps
@@ -413,7 +421,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (g.evx.size() < 5) { while (g.evx.size() < 5) { cudaEvent_t e; CUDA_TRY(cudaEventCreate(&e)); g.evx.push_back(e); } }
     while (g0 < ng) {
         const int ff0 = INT_MAX;
-        CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 18 * sizeof(unsigned int), st));
+        CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
         CUDA_TRY(cudaMemsetAsync(g.d_tops, 0, 2 * sizeof(unsigned long long), st));
         CUDA_TRY(cudaMemcpyAsync(g.d_flags + 3, &ff0, sizeof(int), cudaMemcpyHostToDevice, st));
         wa.g0 = g0; wa.g1 = g0 + budget < ng ? g0 + budget : ng;
@@ -451,6 +459,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         }
         usedpc += tops[0]; usedpp += tops[1];
         a.g0 = g0; a.g1 = F;
+        a.nsb = (unsigned int)((F - g0 + ((int64_t)1 << a.sb_shift) - 1) >> a.sb_shift);
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
         CUDA_TRY(launch_plan(a, st));
         if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
@@ -661,7 +670,7 @@ int hot_lookup_keys(const uint64_t* keys, int64_t nkeys, int32_t* idx) {
     CUDA_TRY(cudaMalloc(&dk, 8 * (size_t)nkeys));
     cudaError_t e = cudaMalloc(&di, 4 * (size_t)nkeys);
     if (e == cudaSuccess) e = cudaMemcpyAsync(dk, keys, 8 * (size_t)nkeys, cudaMemcpyHostToDevice, g.stream);
-    if (e == cudaSuccess) e = launch_hash_lookup(g.t.hkey, g.t.hval, g.t.hcap - 1, dk, nkeys, di, g.stream);
+    if (e == cudaSuccess) e = launch_hash_lookup(g.t.ckey, g.t.hval, g.t.hcap - 1, dk, nkeys, di, g.stream);
     if (e == cudaSuccess) e = cudaMemcpyAsync(idx, di, 4 * (size_t)nkeys, cudaMemcpyDeviceToHost, g.stream);
     if (e == cudaSuccess) e = cudaStreamSynchronize(g.stream);
     cudaFree(dk); cudaFree(di);

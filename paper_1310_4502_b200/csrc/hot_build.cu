@@ -543,13 +543,14 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
                                                               const uint32_t* __restrict__ counts, int64_t n, int64_t nblk, LevelBase LB,
                                                               uint64_t* __restrict__ ckey, uint32_t* __restrict__ cfirst,
                                                               uint32_t* __restrict__ ccount, int32_t* __restrict__ cchild,
-                                                              int32_t* __restrict__ cparent, GroupRec* __restrict__ group,
+                                                              int32_t* __restrict__ cparent,
+                                                              GroupRec* __restrict__ group, int32_t* __restrict__ leafcell,
                                                               int2* __restrict__ open) {
-    // per level (row 22: groups) and warp, as lane masks: which bodies start a cell of the level; which bodies
-    // differ from their predecessor at or above the level (= where the cells of the level can end)
-    __shared__ uint32_t sE[HOT_NLEVELS + 1][32], sB[HOT_NLEVELS][32];
-    __shared__ uint32_t wpre[HOT_NLEVELS + 1][32]; // cells of the level in the earlier warps of the tile
-    __shared__ uint32_t boff[HOT_NLEVELS + 1];     // ... and in the earlier tiles
+    // per level (row 22: groups, row 23: leaves) and warp, as lane masks: which bodies start a cell of the level; which
+    // bodies differ from their predecessor at or above the level (= where the cells of the level can end)
+    __shared__ uint32_t sE[HOT_NLEVELS + 2][32], sB[HOT_NLEVELS][32];
+    __shared__ uint32_t wpre[HOT_NLEVELS + 2][32]; // cells of the level in the earlier warps of the tile
+    __shared__ uint32_t boff[HOT_NLEVELS + 2];     // ... and in the earlier tiles
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
     const int64_t T0 = (int64_t)blockIdx.x * TREE_TILE;
     const int64_t i = T0 + tid;
@@ -563,12 +564,13 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
         const uint32_t colB = transpose32(~((1u << b) - 1u), lane);
         if (lane < HOT_NLEVELS) { sE[lane][w] = colE; sB[lane][w] = colB; }
         const uint32_t gm = __ballot_sync(FULL, valid && b <= Lgroup);
-        if (lane == 0) sE[HOT_NLEVELS][w] = gm;
+        const uint32_t lm = __ballot_sync(FULL, starts); // a leaf starts wherever a cell starts: the cell (Lleaf, i)
+        if (lane == 0) { sE[HOT_NLEVELS][w] = gm; sE[HOT_NLEVELS + 1][w] = lm; }
     }
-    if (tid <= HOT_NLEVELS) boff[tid] = counts[(int64_t)tid * nblk + blockIdx.x];
+    if (tid <= HOT_NLEVELS + 1) boff[tid] = counts[(int64_t)tid * nblk + blockIdx.x];
     if (tid < HOT_NLEVELS) open[(int64_t)blockIdx.x * HOT_NLEVELS + tid] = make_int2(-1, -1);
     __syncthreads();
-    if (w <= HOT_NLEVELS) { // warp l: exclusive prefix of row l over the warps
+    if (w <= HOT_NLEVELS + 1) { // warp l: exclusive prefix of row l over the warps
         const uint32_t c = (uint32_t)__popc(sE[w][lane]);
         uint32_t x = c;
 #pragma unroll
@@ -603,7 +605,7 @@ __global__ void __launch_bounds__(TREE_TILE) tree_emit_kernel(const uint64_t* __
             if (l > b) parent = prev_cell;
             else if (l > 0) parent = (int32_t)(LB.v[l - 1] + boff[l - 1] + wpre[l - 1][w] + __popc(sE[l - 1][w] & (lt | (1u << lane)))) - 1;
             cparent[c] = parent;
-            if (l == Lleaf) cchild[c] = -1;
+            if (l == Lleaf) { cchild[c] = -1; leafcell[(int64_t)boff[HOT_NLEVELS + 1] + wpre[HOT_NLEVELS + 1][w] + __popc(sE[HOT_NLEVELS + 1][w] & lt)] = c; }
             if (prev_cell >= 0) cchild[prev_cell] = c; // cell (l-1, i) is internal: its first child starts at i too
             prev_cell = c;
             if (l == Lgroup) { gcount = cnt; gcell = c; }
@@ -643,27 +645,25 @@ cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st) {
     for (int l = 0; l <= HOT_NLEVELS; ++l) LB.v[l] = a.level_base[l];
     HOT_LAUNCHED(2);
     tree_emit_kernel<<<(unsigned)a.nblk, TREE_TILE, 0, st>>>(a.skey, a.plev, a.counts, a.n, a.nblk, LB, a.ckey, a.cfirst, a.ccount,
-                                                             a.cchild, a.cparent, a.group, a.open);
+                                                             a.cchild, a.cparent, a.group, a.leafcell, a.open);
     const int64_t nslots = a.nblk * HOT_NLEVELS;
     tree_open_kernel<<<(unsigned)((nslots + 255) / 256), 256, 0, st>>>(a.open, nslots, a.skey, a.n, a.cfirst, a.ccount, a.group);
     return cudaGetLastError();
 }
-// per cell: its octant bit into the parent's child mask, and the hash-table entry key -> cell (open addressing,
-// linear probing; one independent insert per thread, so the atomics' latency is covered by the other cells)
-__global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restrict__ ckey, const int32_t* __restrict__ cparent,
-                                                        uint32_t* __restrict__ cmask, int64_t ncells, uint64_t* __restrict__ hkey,
-                                                        int32_t* __restrict__ hval, int64_t hmask, int* __restrict__ maxprobe) {
+// The hash table key -> cell, open addressing with linear probing.  A slot holds the cell INDEX only
+// (-1 = free): the key it stands for is ckey[index], which a lookup compares against -- so an insert is one 32-bit CAS
+// and the table is 4 bytes per slot (33-67 MB at 2^24 bodies: L2-resident; with keys stored beside the indices it was
+// 201 MB and every insert two DRAM sector read-modify-writes).  One independent insert per thread.
+__global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restrict__ ckey, int64_t ncells, int32_t* __restrict__ hval,
+                                                        int64_t hmask, int* __restrict__ maxprobe) {
     __shared__ int s_probe;
     if (threadIdx.x == 0) s_probe = 0;
     __syncthreads();
     const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     int probe = 0;
     if (c < ncells) {
-        const uint64_t ck = ckey[c];
-        if (c > 0) atomicOr(&cmask[cparent[c]], 1u << (uint32_t)(ck & 7ull));
-        uint64_t h = hash_slot(ck, (uint64_t)hmask);
-        while (atomicCAS(&hval[h], -1, (int32_t)c) != -1) { h = (h + 1) & (uint64_t)hmask; ++probe; } // a slot is free iff its value is -1
-        hkey[h] = ck;
+        uint64_t h = hash_slot(ckey[c], (uint64_t)hmask);
+        while (atomicCAS(&hval[h], -1, (int32_t)c) != -1) { h = (h + 1) & (uint64_t)hmask; ++probe; }
     }
     // longest probe sequence: one global atomic per block at most (every thread reading the one counter queues in its L2 slice)
     probe = __reduce_max_sync(FULL, probe);
@@ -671,14 +671,15 @@ __global__ void __launch_bounds__(256) tree_link_kernel(const uint64_t* __restri
     __syncthreads();
     if (threadIdx.x == 0 && s_probe > 0 && s_probe > *((volatile int*)maxprobe)) atomicMax(maxprobe, s_probe);
 }
-cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, uint64_t* hkey, int32_t* hval,
-                             int64_t hmask, int* maxprobe, cudaStream_t st) {
+cudaError_t launch_tree_link(const uint64_t* ckey, int64_t ncells, int32_t* hval, int64_t hmask, int* maxprobe, cudaStream_t st) {
     HOT_LAUNCHED(1);
-    tree_link_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, st>>>(ckey, cparent, cmask, ncells, hkey, hval, hmask, maxprobe);
+    tree_link_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, st>>>(ckey, ncells, hval, hmask, maxprobe);
     return cudaGetLastError();
 }
+// per cell: the child mask (the children are the cells from cchild on whose key is this key extended by one octant:
+// at most eight consecutive, sorted keys -- no atomics) and the 16-byte record the walk reads
 __global__ void __launch_bounds__(256) tree_finalize_kernel(const uint64_t* __restrict__ ckey, const uint32_t* __restrict__ cfirst,
-                                                            const uint32_t* __restrict__ ccount, const uint32_t* __restrict__ cmask,
+                                                            const uint32_t* __restrict__ ccount, uint32_t* __restrict__ cmask,
                                                             const int32_t* __restrict__ cchild, WalkCell* __restrict__ wc,
                                                             int64_t ncells, int* __restrict__ errflag) {
     int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -688,23 +689,34 @@ __global__ void __launch_bounds__(256) tree_finalize_kernel(const uint64_t* __re
     uint64_t mort = k & ((1ull << (3 * level)) - 1ull);
     int up = HOT_MAXLEVEL - level;
     uint64_t ox = (uint64_t)compact21(mort >> 2) << up, oy = (uint64_t)compact21(mort >> 1) << up, oz = (uint64_t)compact21(mort) << up;
-    bool leaf = cchild[c] < 0;
-    uint32_t cnt = leaf ? ccount[c] : (uint32_t)__popc(cmask[c]);
+    const int32_t ch = cchild[c];
+    bool leaf = ch < 0;
+    uint32_t mask = 0;
+    if (!leaf) {
+#pragma unroll 1
+        for (int j = 0; j < 8 && ch + j < ncells; ++j) {
+            const uint64_t kk = ckey[ch + j];
+            if ((kk >> 3) != k) break;
+            mask |= 1u << (uint32_t)(kk & 7ull);
+        }
+    }
+    cmask[c] = mask;
+    uint32_t cnt = leaf ? ccount[c] : (uint32_t)__popc(mask);
     if (cnt >= (1u << 27)) { atomicOr(errflag, 2); cnt = (1u << 27) - 1; }
     uint64_t packed = ox | (oy << 21) | (oz << 42) | (leaf ? (1ull << 63) : 0ull);
     WalkCell r;
     r.x = (uint32_t)packed; r.y = (uint32_t)(packed >> 32);
-    r.z = leaf ? cfirst[c] : (uint32_t)cchild[c];
+    r.z = leaf ? cfirst[c] : (uint32_t)ch;
     r.w = ((uint32_t)level << 27) | cnt;
     wc[c] = r;
 }
-cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount, const uint32_t* cmask,
+cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount, uint32_t* cmask,
                                  const int32_t* cchild, WalkCell* wc, int64_t ncells, int* errflag, cudaStream_t st) {
     HOT_LAUNCHED(1);
     tree_finalize_kernel<<<(unsigned)((ncells + 255) / 256), 256, 0, st>>>(ckey, cfirst, ccount, cmask, cchild, wc, ncells, errflag);
     return cudaGetLastError();
 }
-__global__ void hash_lookup_kernel(const uint64_t* __restrict__ hkey, const int32_t* __restrict__ hval, int64_t hmask,
+__global__ void hash_lookup_kernel(const uint64_t* __restrict__ ckey, const int32_t* __restrict__ hval, int64_t hmask,
                                    const uint64_t* __restrict__ keys, int64_t nkeys, int32_t* __restrict__ out) {
     int64_t q = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (q >= nkeys) return;
@@ -715,14 +727,14 @@ __global__ void hash_lookup_kernel(const uint64_t* __restrict__ hkey, const int3
         while (true) {
             const int32_t v = hval[h];
             if (v < 0) break;
-            if (hkey[h] == k) { r = v; break; }
+            if (ckey[v] == k) { r = v; break; }
             h = (h + 1) & (uint64_t)hmask;
         }
     }
     out[q] = r;
 }
-cudaError_t launch_hash_lookup(const uint64_t* hkey, const int32_t* hval, int64_t hmask, const uint64_t* keys, int64_t nkeys,
+cudaError_t launch_hash_lookup(const uint64_t* ckey, const int32_t* hval, int64_t hmask, const uint64_t* keys, int64_t nkeys,
                                int32_t* out, cudaStream_t st) {
-    if (nkeys > 0) hash_lookup_kernel<<<(unsigned)((nkeys + 255) / 256), 256, 0, st>>>(hkey, hval, hmask, keys, nkeys, out);
+    if (nkeys > 0) hash_lookup_kernel<<<(unsigned)((nkeys + 255) / 256), 256, 0, st>>>(ckey, hval, hmask, keys, nkeys, out);
     return cudaGetLastError();
 }

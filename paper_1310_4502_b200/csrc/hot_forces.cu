@@ -21,7 +21,12 @@
 
 #define FULL 0xffffffffu
 #define BATCH 32               // sources per staged batch
+#ifndef WARPS_PER_BLOCK
 #define WARPS_PER_BLOCK 4
+#endif
+#ifndef HOT_FLUSH_N
+#define HOT_FLUSH_N 64     // sources a lane sums in fp32 before the partial sums go to the fp64 running sums
+#endif
 #ifndef HOT_SMAX
 #define HOT_SMAX 6             // sinks per lane (tunable 2..8; 6 at 3 blocks/SM measured best with NCRIT >= 128)
 #endif
@@ -62,10 +67,15 @@ struct f2 { unsigned long long v; };
 __device__ __forceinline__ f2 mk2(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ float lo2(f2 a) { float x; asm("{ .reg .f32 t; mov.b64 {%0, t}, %1; }" : "=f"(x) : "l"(a.v)); return x; }
 __device__ __forceinline__ float hi2(f2 a) { float y; asm("{ .reg .f32 t; mov.b64 {t, %0}, %1; }" : "=f"(y) : "l"(a.v)); return y; }
-__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 vfma(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
+#ifdef HOT_ASM_VOLATILE
+#define HOT_ASM asm volatile
+#else
+#define HOT_ASM asm
+#endif
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; HOT_ASM("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; HOT_ASM("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; HOT_ASM("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ f2 vfma(f2 a, f2 b, f2 c) { f2 r; HOT_ASM("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
 __device__ __forceinline__ float vfma(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ f2 vrsqrt(f2 a) { return mk2(rsqrt_approx(lo2(a)), rsqrt_approx(hi2(a))); }
 __device__ __forceinline__ float vrsqrt(float a) { return rsqrt_approx(a); }
@@ -190,6 +200,134 @@ __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const f
     a[3] = a[3] + ph;
 }
 
+// ---- all NP sink pairs of a lane against one source, instruction order chosen for the operand-reuse cache ----------
+// A packed instruction that reads three different registers occupies the FP32 pipe for three cycles instead of two
+// (measured).  An operand that the previous instruction used in the same position comes
+// from the reuse cache instead.  The same arithmetic as pp_one / pc_one per pair, written so that consecutive
+// instructions share either the source's scalar (across the pairs) or a per-pair quantity (across the components).
+#ifdef HOT_BLOCK_ORDER
+template <int NP>
+__device__ __forceinline__ void pp_block(const float4 ns, const f2 (&x)[NP][3], const float eps2, f2 (&a)[NP][4]) {
+    f2 d[NP][3], r2[NP], ri[NP], nmr[NP], nmr3[NP];
+    const f2 sx = splat<f2>(ns.x), sy = splat<f2>(ns.y), sz = splat<f2>(ns.z), sw = splat<f2>(ns.w), e2 = splat<f2>(eps2);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) d[p][2] = x[p][2] + sz;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) d[p][1] = x[p][1] + sy;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) d[p][0] = x[p][0] + sx;
+#pragma unroll
+    for (int p = 0; p < NP; ++p) r2[p] = vfma(d[p][2], d[p][2], e2);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) r2[p] = vfma(d[p][1], d[p][1], r2[p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) r2[p] = vfma(d[p][0], d[p][0], r2[p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) ri[p] = vrsqrt(r2[p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) nmr[p] = sw * ri[p];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { const f2 ri2 = ri[p] * ri[p]; nmr3[p] = nmr[p] * ri2; }
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        a[p][0] = vfma(nmr3[p], d[p][0], a[p][0]);
+        a[p][1] = vfma(nmr3[p], d[p][1], a[p][1]);
+        a[p][2] = vfma(nmr3[p], d[p][2], a[p][2]);
+        a[p][3] = a[p][3] + nmr[p];
+    }
+}
+template <int ORDER, int NP>
+__device__ __forceinline__ void pc_block(const float4 q0, const float4 q1, const float4 q2, const f2 (&x)[NP][3], const float eps2, f2 (&a)[NP][4]) {
+    static_assert(ORDER <= 2, "orders 0 and 2");
+    f2 R[NP][3], u[NP], ri[NP], ri2[NP], ri3[NP];
+    const f2 e2 = splat<f2>(eps2), nm0 = splat<f2>(q0.w);
+    { const f2 s = splat<f2>(q0.z);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) R[p][2] = x[p][2] + s; }
+    { const f2 s = splat<f2>(q0.y);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) R[p][1] = x[p][1] + s; }
+    { const f2 s = splat<f2>(q0.x);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) R[p][0] = x[p][0] + s; }
+#pragma unroll
+    for (int p = 0; p < NP; ++p) u[p] = vfma(R[p][2], R[p][2], e2);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) u[p] = vfma(R[p][1], R[p][1], u[p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) u[p] = vfma(R[p][0], R[p][0], u[p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) ri[p] = vrsqrt(u[p]);
+#pragma unroll
+    for (int p = 0; p < NP; ++p) { ri2[p] = ri[p] * ri[p]; ri3[p] = ri[p] * ri2[p]; }
+    if (ORDER < 2) {
+#pragma unroll
+        for (int p = 0; p < NP; ++p) {
+            const f2 c = nm0 * ri3[p];
+            a[p][0] = vfma(c, R[p][0], a[p][0]); a[p][1] = vfma(c, R[p][1], a[p][1]); a[p][2] = vfma(c, R[p][2], a[p][2]);
+        }
+#pragma unroll
+        for (int p = 0; p < NP; ++p) a[p][3] = vfma(nm0, ri[p], a[p][3]);
+        return;
+    }
+    // M = N R with N = 3 M2 (symmetric): column l of N times R_l, the scalar shared by the pairs, snake over (k, p)
+    f2 M[NP][3];
+    { const f2 nxx = splat<f2>(q1.x), nxy = splat<f2>(q1.y), nxz = splat<f2>(q1.z), nyy = splat<f2>(q1.w), nyz = splat<f2>(q2.x), nzz = splat<f2>(q2.y);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) M[p][0] = nxz * R[p][2];
+#pragma unroll
+      for (int p = NP - 1; p >= 0; --p) M[p][1] = nyz * R[p][2];
+#pragma unroll
+      for (int p = 0; p < NP; ++p) M[p][2] = nzz * R[p][2];
+#pragma unroll
+      for (int p = NP - 1; p >= 0; --p) M[p][2] = vfma(nyz, R[p][1], M[p][2]);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) M[p][1] = vfma(nyy, R[p][1], M[p][1]);
+#pragma unroll
+      for (int p = NP - 1; p >= 0; --p) M[p][0] = vfma(nxy, R[p][1], M[p][0]);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) M[p][0] = vfma(nxx, R[p][0], M[p][0]);
+#pragma unroll
+      for (int p = NP - 1; p >= 0; --p) M[p][1] = vfma(nxy, R[p][0], M[p][1]);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) M[p][2] = vfma(nxz, R[p][0], M[p][2]);
+    }
+    f2 ri5[NP], cR[NP], ph[NP];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) ri5[p] = ri3[p] * ri2[p];
+    { const f2 t15 = splat<f2>(q2.z), t05 = splat<f2>(q2.w);
+#pragma unroll
+      for (int p = 0; p < NP; ++p) cR[p] = nm0 * ri3[p];
+#pragma unroll
+      for (int p = NP - 1; p >= 0; --p) ph[p] = nm0 * ri[p];
+#pragma unroll
+      for (int p = 0; p < NP; ++p) ph[p] = vfma(t05, ri3[p], ph[p]);
+#pragma unroll
+      for (int p = NP - 1; p >= 0; --p) cR[p] = vfma(t15, ri5[p], cR[p]);
+    }
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        f2 Q2 = M[p][0] * R[p][0];
+        Q2 = vfma(M[p][1], R[p][1], Q2);
+        Q2 = vfma(M[p][2], R[p][2], Q2);
+        const f2 hQ = ri5[p] * Q2;                       // 3 u^-5/2 (R M2 R)
+        const f2 w7 = splat<f2>(-2.5f) * ri2[p];
+        cR[p] = vfma(hQ, w7, cR[p]);
+        ph[p] = vfma(splat<f2>(-0.5f), hQ, ph[p]);
+    }
+#pragma unroll
+    for (int p = 0; p < NP; ++p) {
+        a[p][0] = vfma(ri5[p], M[p][0], a[p][0]);
+        a[p][1] = vfma(ri5[p], M[p][1], a[p][1]);
+        a[p][2] = vfma(ri5[p], M[p][2], a[p][2]);
+        a[p][0] = vfma(cR[p], R[p][0], a[p][0]);
+        a[p][1] = vfma(cR[p], R[p][1], a[p][1]);
+        a[p][2] = vfma(cR[p], R[p][2], a[p][2]);
+        a[p][3] = a[p][3] + ph[p];
+    }
+}
+#endif
+
 // ---- the sinks of one lane: NP pairs + (S odd) one scalar ------------------------------------------
 template <int S> struct Sinks {
     static constexpr int NP = S / 2, TAIL = S & 1;
@@ -215,29 +353,35 @@ template <int S> struct Sinks {
         return (i & 1) ? hi2(a2[i >> 1][k]) : lo2(a2[i >> 1][k]);
     }
     __device__ __forceinline__ void pp(const float4 ns, float eps2) {
+#ifdef HOT_BLOCK_ORDER
+        if (NP) pp_block<NP ? NP : 1>(ns, x2, eps2, a2);
+#else
 #pragma unroll
         for (int p = 0; p < NP; ++p) pp_one<f2>(ns, x2[p], eps2, a2[p]);
+#endif
         if (TAIL) pp_one<float>(ns, x1, eps2, a1);
     }
-    __device__ __forceinline__ void pp_self(const float4 ns, int j, float eps2) { // scalar: a few bodies per group only
+    // the group's own bodies: the same packed arithmetic, the j = i slot masked by index through ri = 0 (works for eps = 0)
+    __device__ __forceinline__ void pp_self(const float4 ns, int j, float eps2) {
 #pragma unroll
-        for (int i = 0; i < S; ++i) {
-            float xs[3], as[4] = {0.f, 0.f, 0.f, 0.f};
-            if (TAIL && i == S - 1) { xs[0] = x1[0]; xs[1] = x1[1]; xs[2] = x1[2]; }
-            else if (i & 1) { xs[0] = hi2(x2[i >> 1][0]); xs[1] = hi2(x2[i >> 1][1]); xs[2] = hi2(x2[i >> 1][2]); }
-            else { xs[0] = lo2(x2[i >> 1][0]); xs[1] = lo2(x2[i >> 1][1]); xs[2] = lo2(x2[i >> 1][2]); }
-            pp_one_self(ns, j == me[i], xs, eps2, as);
-            if (TAIL && i == S - 1) {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) a1[k] += as[k];
-            } else {
-#pragma unroll
-                for (int k = 0; k < 4; ++k) a2[i >> 1][k] = a2[i >> 1][k] + ((i & 1) ? mk2(0.f, as[k]) : mk2(as[k], 0.f));
-            }
+        for (int p = 0; p < NP; ++p) {
+            const f2 dx = x2[p][0] + splat<f2>(ns.x), dy = x2[p][1] + splat<f2>(ns.y), dz = x2[p][2] + splat<f2>(ns.z);
+            const f2 r2 = vfma(dx, dx, vfma(dy, dy, vfma(dz, dz, splat<f2>(eps2))));
+            const float r0 = rsqrt_approx(lo2(r2)), r1 = rsqrt_approx(hi2(r2));
+            const f2 ri = mk2(j == me[2 * p] ? 0.0f : r0, j == me[2 * p + 1] ? 0.0f : r1);
+            const f2 ri2 = ri * ri, nmr = splat<f2>(ns.w) * ri, nmr3 = nmr * ri2;
+            a2[p][0] = vfma(nmr3, dx, a2[p][0]); a2[p][1] = vfma(nmr3, dy, a2[p][1]); a2[p][2] = vfma(nmr3, dz, a2[p][2]);
+            a2[p][3] = a2[p][3] + nmr;
         }
+        if (TAIL) pp_one_self(ns, j == me[S - 1], x1, eps2, a1);
     }
     template <int ORDER>
     __device__ __forceinline__ void pc(const float4 q0, const float4 q1, const float4 q2, const float* m, float eps2) {
+#ifdef HOT_BLOCK_ORDER
+        if (ORDER <= 2) {
+            if (NP) pc_block<(ORDER <= 2 ? ORDER : 2), NP ? NP : 1>(q0, q1, q2, x2, eps2, a2);
+        } else
+#endif
 #pragma unroll
         for (int p = 0; p < NP; ++p) pc_one<ORDER, f2>(q0, q1, q2, m, x2[p], eps2, a2[p]);
         if (TAIL) pc_one<ORDER, float>(q0, q1, q2, m, x1, eps2, a1);
@@ -405,7 +549,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 }
             }
             nacc += (cnt + K - 1) >> lgK;
-            if (nacc >= 32) flush();
+            if (nacc >= HOT_FLUSH_N) flush();
         }
         __syncwarp();
     }
@@ -448,7 +592,7 @@ HOT_UNROLL(HOT_PP_UNROLL)
                 }
             }
             nacc += (cnt + K - 1) >> lgK;
-            if (nacc >= 32) flush();
+            if (nacc >= HOT_FLUSH_N) flush();
         }
         __syncwarp();
     }
@@ -554,27 +698,28 @@ __device__ __forceinline__ void plan_group(const uint32_t count, F&& emit) {
     }
 }
 #ifndef HOT_FORCES_PERIODIC_TU
-// Work items of the interaction kernel, one per pass: (group - g0, first sink, sinks, lg2 lanes per stream), ordered by
-// sinks per lane, 6 first.  The SMAX variants of the loops together do not fit the instruction cache (unrolling all of
-// them: 76 -> 105 ms); with the items in this order the warps of an SM run the same variant most of the time, and the
-// long items start first.  FILL = false counts the items per class, FILL = true places them.
+// Work items of the interaction kernel, one per pass: (group - g0, first sink, sinks, lg2 lanes per stream).  The SMAX
+// variants of the loops together do not fit the instruction cache (unrolling all of them: 76 -> 105 ms), so the items are
+// ordered by sinks per lane, 6 first -- but only INSIDE superblocks of 2^sb_shift consecutive groups (key order), so that
+// the groups in flight at any time are neighbours in space and share the cells and bodies of their lists in L2.
+// cls: [nsb][8] items per (superblock, class = SMAX - sinks per lane), [nsb][8] where each starts, [nsb][8] fill cursors,
+// [1] total.  FILL = false counts, plan_scan_kernel places the classes, FILL = true fills.
 template <bool FILL>
 __global__ void __launch_bounds__(256) plan_kernel(const __grid_constant__ ForceArgs P) {
     __shared__ unsigned int s_cnt[8], s_base[8];
     if (threadIdx.x < 8) s_cnt[threadIdx.x] = 0;
     __syncthreads();
     const int64_t gi = P.g0 + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const unsigned int sb = (unsigned int)(((int64_t)blockIdx.x * blockDim.x) >> P.sb_shift); // sb_shift >= 8: one superblock per block
     const uint32_t count = gi < P.g1 ? P.group[gi].count : 0u;
     plan_group(count, [&](uint32_t, uint32_t nc, int lgL) { atomicAdd(&s_cnt[SMAX - (int)((nc + (1u << lgL) - 1) >> lgL)], 1u); });
     __syncthreads();
     if (!FILL) {
-        if (threadIdx.x < 8 && s_cnt[threadIdx.x]) atomicAdd(&P.cls[threadIdx.x], s_cnt[threadIdx.x]);
+        if (threadIdx.x < 8 && s_cnt[threadIdx.x]) atomicAdd(&P.cls[8 * sb + threadIdx.x], s_cnt[threadIdx.x]);
         return;
     }
     if (threadIdx.x < 8) { // the block's range in every class: start of the class + a cursor
-        unsigned int base = 0;
-        for (int c = 0; c < (int)threadIdx.x; ++c) base += P.cls[c];
-        s_base[threadIdx.x] = base + (s_cnt[threadIdx.x] ? atomicAdd(&P.cls[8 + threadIdx.x], s_cnt[threadIdx.x]) : 0u);
+        s_base[threadIdx.x] = P.cls[8 * (P.nsb + sb) + threadIdx.x] + (s_cnt[threadIdx.x] ? atomicAdd(&P.cls[8 * (2 * P.nsb + sb) + threadIdx.x], s_cnt[threadIdx.x]) : 0u);
         s_cnt[threadIdx.x] = 0;
     }
     __syncthreads();
@@ -583,11 +728,29 @@ __global__ void __launch_bounds__(256) plan_kernel(const __grid_constant__ Force
         P.items[s_base[c] + atomicAdd(&s_cnt[c], 1u)] = make_uint4((uint32_t)(gi - P.g0), c0, nc, (uint32_t)lgL);
     });
 }
+// exclusive scan of the 8 nsb (superblock, class) counts in that order; one warp
+__global__ void __launch_bounds__(32) plan_scan_kernel(unsigned int* __restrict__ cls, unsigned int nsb) {
+    const int lane = threadIdx.x;
+    unsigned int carry = 0;
+    for (unsigned int b = 0; b < 8 * nsb; b += 32) {
+        const unsigned int v = b + lane < 8 * nsb ? cls[b + lane] : 0u;
+        unsigned int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { const unsigned int y = __shfl_up_sync(FULL, x, o); if (lane >= o) x += y; }
+        if (b + lane < 8 * nsb) cls[8 * nsb + b + lane] = carry + x - v;
+        carry += __shfl_sync(FULL, x, 31);
+    }
+    if (lane == 0) cls[24 * nsb] = carry;
+}
+size_t plan_cls_elems(int64_t ng, int sb_shift) { return 24 * (size_t)((ng + ((int64_t)1 << sb_shift) - 1) >> sb_shift) + 1; }
 cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st) {
     const int64_t ng = a.g1 - a.g0;
     if (ng <= 0) return cudaSuccess;
-    HOT_LAUNCHED(2);
+    cudaError_t e = cudaMemsetAsync(a.cls, 0, plan_cls_elems(ng, a.sb_shift) * sizeof(unsigned int), st);
+    if (e != cudaSuccess) return e;
+    HOT_LAUNCHED(3);
     plan_kernel<false><<<(unsigned)((ng + 255) / 256), 256, 0, st>>>(a);
+    plan_scan_kernel<<<1, 32, 0, st>>>(a.cls, a.nsb);
     plan_kernel<true><<<(unsigned)((ng + 255) / 256), 256, 0, st>>>(a);
     return cudaGetLastError();
 }
@@ -596,15 +759,16 @@ cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st) {
 template <int ORDER, bool PER>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
-    unsigned int total = lane < SMAX ? P.cls[lane] : 0u;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) total += __shfl_xor_sync(FULL, total, o);
+    const unsigned int total = P.cls[24 * P.nsb];
     while (true) {
         unsigned int q = 0;
         if (lane == 0) q = atomicAdd(P.counter, 1u);
         q = __shfl_sync(FULL, q, 0);
         if (q >= total) break;
         const uint4 it = P.items[q];
+#ifdef HOT_DEBUG_HOOKS
+        { const int S_ = (int)((it.z + (1u << it.w) - 1) >> it.w); if (!((P.dbg_mask >> (S_ + 8 * (int)it.w)) & 1ull)) continue; }
+#endif
         const int64_t gi = P.g0 + (int64_t)it.x;
         run_chunk<ORDER, PER>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
     }

@@ -51,14 +51,14 @@ struct Tree {
     uint64_t* ckey = nullptr;
     uint32_t *cfirst = nullptr, *ccount = nullptr, *cmask = nullptr;
     int32_t *cchild = nullptr, *cparent = nullptr;
+    int32_t* leafcell = nullptr;             // [nleaves] cell index of every leaf, in body order (the upward pass starts here)
     WalkCell* wcell = nullptr;
     GroupRec* group = nullptr;
     uint32_t *glpc = nullptr, *glpp = nullptr, *glvis = nullptr; // per group, last walk: accepted cells, listed bodies (without the group's own), cells visited
     unsigned long long *pcoff = nullptr, *ppoff = nullptr; // [ngroups] start of each group's lists in the arena
     // hash
     int64_t hcap = 0;
-    uint64_t* hkey = nullptr;
-    int32_t* hval = nullptr;
+    int32_t* hval = nullptr;                 // slot -> cell index or -1; the slot's key is ckey[index]
     int hash_max_probe = 0;
     // periodic far field: polynomial of the sink position (hot_periodic.cu)
     bool far_ready = false;
@@ -93,16 +93,15 @@ struct TreeEmitArgs {
     const uint64_t* skey; const uint32_t* plev; const uint32_t* counts; int64_t n, nblk;
     int64_t level_base[HOT_NLEVELS + 1];
     uint64_t* ckey; uint32_t* cfirst; uint32_t* ccount; int32_t* cchild; int32_t* cparent;
-    GroupRec* group;
+    GroupRec* group; int32_t* leafcell;
     int2* open; // [nblk][HOT_NLEVELS] scratch: the cells whose end lies beyond the tile of their first body
 };
 cudaError_t launch_tree_emit(const TreeEmitArgs& a, cudaStream_t st);
-cudaError_t launch_tree_link(const uint64_t* ckey, const int32_t* cparent, uint32_t* cmask, int64_t ncells, uint64_t* hkey, int32_t* hval,
-                             int64_t hmask, int* maxprobe, cudaStream_t st);
+cudaError_t launch_tree_link(const uint64_t* ckey, int64_t ncells, int32_t* hval, int64_t hmask, int* maxprobe, cudaStream_t st);
 cudaError_t launch_tree_finalize(const uint64_t* ckey, const uint32_t* cfirst, const uint32_t* ccount,
-                                 const uint32_t* cmask, const int32_t* cchild, WalkCell* wc,
+                                 uint32_t* cmask /* out */, const int32_t* cchild, WalkCell* wc,
                                  int64_t ncells, int* errflag, cudaStream_t st);
-cudaError_t launch_hash_lookup(const uint64_t* hkey, const int32_t* hval, int64_t hmask,
+cudaError_t launch_hash_lookup(const uint64_t* ckey, const int32_t* hval, int64_t hmask,
                                const uint64_t* keys, int64_t nkeys, int32_t* out, cudaStream_t st);
 
 // ---- upward pass (hot_moments.cu) -------------------------------------------------------------
@@ -155,9 +154,12 @@ struct ForceArgs {
     float* acc; float* pot;
     unsigned int* counter;        // dynamic scheduler over the work items
     uint4* items;                 // one per pass of a group, ordered by sinks per lane (launch_plan)
-    unsigned int* cls;            // [0..7] items per class (SMAX - sinks per lane), [8..15] fill cursors
+    unsigned int* cls;            // plan_cls_elems(g1 - g0, sb_shift) words: per-(superblock, class) counts, starts, cursors, total
+    unsigned long long dbg_mask; // HOT_DEBUG_HOOKS builds only: bit (S + 8 lgL) enables the class
+    int sb_shift; unsigned int nsb; // 2^sb_shift groups per superblock (>= 8), number of superblocks of [g0, g1)
 };
-cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st);   // fills items / cls for groups [g0, g1); cls must be zero
+size_t plan_cls_elems(int64_t ngroups, int sb_shift);
+cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st);   // fills items / cls for groups [g0, g1)
 cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st); // after launch_plan
 
 // ---- periodic far field (hot_periodic.cu) ------------------------------------------------------------

@@ -1,5 +1,5 @@
-// hot_moments.cu -- S6 upward pass: mass, centre of mass and raw Cartesian moments of eq (6)
-// about the centre of mass, per cell, level by level from the leaves up.
+// hot_moments.cu -- S6 upward pass: mass, centre of mass, raw Cartesian moments of eq (6)
+// about the centre of mass and b_max, per cell, from the leaves up.
 // Leaves sum their bodies; internal cells combine their children with the parallel-axis shift
 //   M'_alpha = sum_{beta<=alpha} C(alpha,beta) M_beta d^(alpha-beta),  d = z_child - z_parent.
 // Arithmetic is fp64 (the stage is HBM/latency bound); results are stored as the fp32 records the
@@ -104,80 +104,176 @@ __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, doub
     }
 }
 template <int ORDER>
-__device__ __forceinline__ void load_child(int64_t c, const CellA* cellA, const CellM2* cellM2, const CellM34* cellM34, double* C) {
+__device__ __forceinline__ void load_child(int64_t c, const CellM2* cellM2, const CellM34* cellM34, double* C) {
     if (ORDER >= 2) {
-        CellM2 Q = cellM2[c];
-        C[midx(2, 0, 0)] = Q.xx; C[midx(1, 1, 0)] = Q.xy; C[midx(1, 0, 1)] = Q.xz;
-        C[midx(0, 2, 0)] = Q.yy; C[midx(0, 1, 1)] = Q.yz; C[midx(0, 0, 2)] = Q.zz;
+        const float4 q0 = reinterpret_cast<const float4*>(cellM2 + c)[0], q1 = reinterpret_cast<const float4*>(cellM2 + c)[1];
+        C[midx(2, 0, 0)] = q0.x; C[midx(1, 1, 0)] = q0.y; C[midx(1, 0, 1)] = q0.z;
+        C[midx(0, 2, 0)] = q0.w; C[midx(0, 1, 1)] = q1.x; C[midx(0, 0, 2)] = q1.y;
     }
     if (ORDER >= 4) {
-        const CellM34& R = cellM34[c];
+        const float4* r = reinterpret_cast<const float4*>(cellM34 + c);
 #pragma unroll
-        for (int k = 0; k < 25; ++k) C[10 + k] = R.v[k];
+        for (int k = 0; k < 6; ++k) {
+            const float4 v = r[k];
+            C[10 + 4 * k] = v.x; C[11 + 4 * k] = v.y; C[12 + 4 * k] = v.z; C[13 + 4 * k] = v.w;
+        }
+        C[34] = reinterpret_cast<const float*>(cellM34 + c)[24];
     }
 }
 
+// Leaves, one thread each, in BODY order (leafcell, written by tree_emit): neighbouring threads read neighbouring
+// bodies (a leaf holds 4 bodies on average at NLEAF = 16, so the lines a warp touches are shared through L1).
+struct MomArgs {
+    const int32_t* leafcell; int64_t nleaves;
+    const uint32_t *cfirst, *ccount, *cmask; const int32_t* cchild; const float4* body;
+    CellA* cellA; CellM2* cellM2; CellM2* cellE2; CellM34* cellM34;
+};
 template <int ORDER>
-__global__ void __launch_bounds__(128) moments_level_kernel(int64_t cbeg, int64_t cend, const uint32_t* __restrict__ cfirst,
-                                                            const uint32_t* __restrict__ ccount, const uint32_t* __restrict__ cmask,
-                                                            const int32_t* __restrict__ cchild, const float4* __restrict__ body,
-                                                            CellA* __restrict__ cellA, CellM2* __restrict__ cellM2, CellM2* __restrict__ cellE2,
-                                                            CellM34* __restrict__ cellM34) {
-    int64_t c = cbeg + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= cend) return;
+__global__ void __launch_bounds__(128) moments_leaves_kernel(const __grid_constant__ MomArgs P) {
     constexpr int NM = NMom<ORDER>::v;
+    const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= P.nleaves) return;
+    const int32_t c0 = P.leafcell[k];
+    const uint32_t f = P.cfirst[c0], n = P.ccount[c0];
     double M[NM];
 #pragma unroll
-    for (int k = 0; k < NM; ++k) M[k] = 0;
-    double m0 = 0, zx = 0, zy = 0, zz = 0, bmax = 0; // bmax: DESIGN.md R-15 (leaf: farthest body; else children's radii + offsets)
-    int32_t ch = cchild[c];
-    if (ch < 0) { // leaf: from its bodies
-        uint32_t f = cfirst[c], n = ccount[c];
-        for (uint32_t j = 0; j < n; ++j) {
-            float4 b = body[f + j];
-            m0 += (double)b.w; zx += (double)b.w * b.x; zy += (double)b.w * b.y; zz += (double)b.w * b.z;
+    for (int q = 0; q < NM; ++q) M[q] = 0;
+    double m0 = 0, zx = 0, zy = 0, zz = 0, bmax = 0; // bmax: DESIGN.md R-15 (leaf: its farthest body)
+    const float4* const src = P.body + f;
+    for (uint32_t j = 0; j < n; ++j) {
+        const float4 b = __ldg(src + j);
+        m0 += (double)b.w; zx += (double)b.w * b.x; zy += (double)b.w * b.y; zz += (double)b.w * b.z;
+    }
+    zx /= m0; zy /= m0; zz /= m0;
+    for (uint32_t j = 0; j < n; ++j) {
+        const float4 b = __ldg(src + j);
+        const double dx = (double)b.x - zx, dy = (double)b.y - zy, dz = (double)b.z - zz;
+        bmax = fmax(bmax, dx * dx + dy * dy + dz * dz);
+        if (ORDER >= 2) add_point<ORDER>(M, (double)b.w, dx, dy, dz);
+    }
+    store_cell<ORDER>(c0, m0, zx, zy, zz, sqrt(bmax), M, P.cellA, P.cellM2, P.cellE2, P.cellM34);
+}
+// an internal cell from its children (one level down, already done): parallel-axis shift, fixed child order
+template <int ORDER>
+__device__ __forceinline__ void combine_children(const MomArgs& P, int64_t c) {
+    constexpr int NM = NMom<ORDER>::v;
+    const int32_t ch = P.cchild[c];
+    if (ch < 0) return; // a leaf: done by moments_leaves_kernel
+    const int nch = __popc(P.cmask[c]);
+    double M[NM];
+#pragma unroll
+    for (int q = 0; q < NM; ++q) M[q] = 0;
+    double m0 = 0, zx = 0, zy = 0, zz = 0, bmax = 0; // bmax: DESIGN.md R-15 (children's radii + centre offsets)
+    for (int q = 0; q < nch; ++q) {
+        const CellA A = P.cellA[ch + q];
+        m0 += (double)A.m0; zx += (double)A.m0 * A.zx; zy += (double)A.m0 * A.zy; zz += (double)A.m0 * A.zz;
+    }
+    zx /= m0; zy /= m0; zz /= m0;
+    for (int q = 0; q < nch; ++q) {
+        const CellA A = P.cellA[ch + q];
+        const double dx = A.zx - zx, dy = A.zy - zy, dz = A.zz - zz;
+        bmax = fmax(bmax, sqrt(dx * dx + dy * dy + dz * dz) + (double)A.bmax);
+        if (ORDER >= 2) {
+            double C[NM];
+            load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C);
+            add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
+        }
+    }
+    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34);
+}
+// One level of internal cells.  A warp looks at 32 consecutive cells of the level, keeps the internal ones (one in eight
+// on average) and hands each to an OCTET of lanes: lane q of the octet loads child q (all children of the warp's cells in
+// parallel instead of one dependent load chain per cell), the octet sums mass and centre of mass by shuffles, every lane
+// shifts its child's moments to the parent's centre, and the octet sums them.  Four cells per trip.
+template <int ORDER>
+__global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constant__ MomArgs P, int64_t cbeg, int64_t cend) {
+    constexpr int NM = NMom<ORDER>::v;
+    const int lane = threadIdx.x & 31, oct = lane >> 3, q = lane & 7;
+    const int64_t c = cbeg + (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int32_t ch0 = c < cend ? P.cchild[c] : -1;
+    uint32_t todo = __ballot_sync(0xffffffffu, ch0 >= 0);
+    const uint32_t mymask = ch0 >= 0 ? P.cmask[c] : 0u;
+    while (todo) { // warp-uniform
+        // the octet's cell: the oct-th set bit of todo
+        uint32_t t = todo;
+        for (int i = 0; i < oct; ++i) t &= t - 1;
+        const int src = t ? __ffs((int)t) - 1 : 0;
+        const bool have = t != 0;
+        const int32_t ch = __shfl_sync(0xffffffffu, ch0, src);
+        const int nch = __popc(__shfl_sync(0xffffffffu, mymask, src));
+        const int64_t cell = (c - lane) + src;
+        const bool mine = have && q < nch;
+        CellA A; A.zx = A.zy = A.zz = 0.0; A.m0 = 0.f; A.bmax = 0.f;
+        if (mine) A = P.cellA[ch + q];
+        double m0 = (double)A.m0, zx = m0 * A.zx, zy = m0 * A.zy, zz = m0 * A.zz;
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) {
+            m0 += __shfl_xor_sync(0xffffffffu, m0, o); zx += __shfl_xor_sync(0xffffffffu, zx, o);
+            zy += __shfl_xor_sync(0xffffffffu, zy, o); zz += __shfl_xor_sync(0xffffffffu, zz, o);
         }
         zx /= m0; zy /= m0; zz /= m0;
-        for (uint32_t j = 0; j < n; ++j) {
-            float4 b = body[f + j];
-            const double dx = (double)b.x - zx, dy = (double)b.y - zy, dz = (double)b.z - zz;
-            bmax = fmax(bmax, dx * dx + dy * dy + dz * dz);
-            if (ORDER >= 2) add_point<ORDER>(M, (double)b.w, dx, dy, dz);
-        }
-        bmax = sqrt(bmax);
-    } else { // internal: from its children (one level down, already done)
-        int nch = __popc(cmask[c]);
-        for (int k = 0; k < nch; ++k) {
-            CellA A = cellA[ch + k];
-            m0 += (double)A.m0; zx += (double)A.m0 * A.zx; zy += (double)A.m0 * A.zy; zz += (double)A.m0 * A.zz;
-        }
-        zx /= m0; zy /= m0; zz /= m0;
-        for (int k = 0; k < nch; ++k) {
-            CellA A = cellA[ch + k];
+        double M[NM];
+#pragma unroll
+        for (int k = 0; k < NM; ++k) M[k] = 0;
+        double bmax = 0; // DESIGN.md R-15: children's radii + centre offsets
+        if (mine) {
             const double dx = A.zx - zx, dy = A.zy - zy, dz = A.zz - zz;
-            bmax = fmax(bmax, sqrt(dx * dx + dy * dy + dz * dz) + (double)A.bmax);
+            bmax = sqrt(dx * dx + dy * dy + dz * dz) + (double)A.bmax;
             if (ORDER >= 2) {
                 double C[NM];
-                load_child<ORDER>(ch + k, cellA, cellM2, cellM34, C);
+                load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C);
                 add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
             }
         }
+#pragma unroll
+        for (int o = 1; o < 8; o <<= 1) {
+            bmax = fmax(bmax, __shfl_xor_sync(0xffffffffu, bmax, o));
+            if (ORDER >= 2) {
+#pragma unroll
+                for (int k = 4; k < NM; ++k) M[k] += __shfl_xor_sync(0xffffffffu, M[k], o);
+            }
+        }
+        if (have && q == 0) store_cell<ORDER>(cell, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34);
+        // drop the four cells just done
+        for (int i = 0; i < 4 && todo; ++i) todo &= todo - 1;
     }
-    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, cellA, cellM2, cellE2, cellM34);
+}
+// the shallow levels ltop .. 0 (a few thousand cells in all) in one block: no launch per level
+struct LevelBases { int64_t v[HOT_NLEVELS + 1]; };
+template <int ORDER>
+__global__ void __launch_bounds__(256) moments_top_kernel(const __grid_constant__ MomArgs P, const __grid_constant__ LevelBases LB, int ltop) {
+    for (int l = ltop; l >= 0; --l) {
+        for (int64_t c = LB.v[l] + threadIdx.x; c < LB.v[l + 1]; c += blockDim.x) combine_children<ORDER>(P, c);
+        __syncthreads(); // this block wrote the level: visible to its own threads after the barrier
+    }
 }
 
-cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
-    for (int l = t.max_level; l >= 0; --l) {
-        int64_t cb = t.level_base[l], ce = t.level_base[l + 1];
+template <int ORDER> static cudaError_t moments_run(const Tree& t, const MomArgs& a, cudaStream_t st) {
+    HOT_LAUNCHED(1);
+    moments_leaves_kernel<ORDER><<<(unsigned)((t.nleaves + 127) / 128), 128, 0, st>>>(a);
+    // deepest level such that levels 0 .. ltop are cheap enough for ONE block (the order-4 shift is ~2000 fp64 operations per child)
+    const int64_t top_cells = ORDER >= 4 ? 128 : 640;
+    int ltop = -1;
+    while (ltop + 1 <= t.max_level && t.level_base[ltop + 2] <= top_cells) ++ltop;
+    for (int l = t.max_level - 1; l > ltop; --l) { // the deepest level holds leaves only
+        const int64_t cb = t.level_base[l], ce = t.level_base[l + 1];
         if (ce <= cb) continue;
-        unsigned nb = (unsigned)((ce - cb + 127) / 128);
         HOT_LAUNCHED(1);
-        if (order >= 4)
-            moments_level_kernel<4><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellE2, t.cellM34);
-        else if (order >= 2)
-            moments_level_kernel<2><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellE2, t.cellM34);
-        else
-            moments_level_kernel<0><<<nb, 128, 0, st>>>(cb, ce, t.cfirst, t.ccount, t.cmask, t.cchild, t.body, t.cellA, t.cellM2, t.cellE2, t.cellM34);
+        moments_level_kernel<ORDER><<<(unsigned)((ce - cb + 127) / 128), 128, 0, st>>>(a, cb, ce);
+    }
+    if (ltop >= 0) {
+        LevelBases LB;
+        for (int l = 0; l <= HOT_NLEVELS; ++l) LB.v[l] = t.level_base[l];
+        HOT_LAUNCHED(1);
+        moments_top_kernel<ORDER><<<1, 256, 0, st>>>(a, LB, ltop < t.max_level ? ltop : t.max_level);
     }
     return cudaGetLastError();
+}
+cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
+    MomArgs a;
+    a.leafcell = t.leafcell; a.nleaves = t.nleaves; a.cfirst = t.cfirst; a.ccount = t.ccount; a.cmask = t.cmask; a.cchild = t.cchild;
+    a.body = t.body; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34;
+    if (order >= 4) return moments_run<4>(t, a, st);
+    if (order >= 2) return moments_run<2>(t, a, st);
+    return moments_run<0>(t, a, st);
 }
