@@ -56,6 +56,7 @@ def parse():
     ap.add_argument("--scale", type=int, default=None)
     ap.add_argument("--theta", type=float, default=None)
     ap.add_argument("--order", type=int, default=None)
+    ap.add_argument("--tol", type=float, default=None, help="error-bound criterion (hot_forces_tol): absolute acceleration tolerance per interaction; not the BASELINE workload")
     ap.add_argument("--nleaf", type=int, default=16)
     ap.add_argument("--ncrit", type=int, default=256)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -244,7 +245,10 @@ def main():
 
     def step():
         hot.hot_build(pos, mass, w.lo, w.size, w.periodic)
-        hot.hot_forces(w.theta, w.eps, w.order, acc=acc, pot=pot)
+        if args.tol is not None:
+            hot.hot_forces_tol(args.tol, w.eps, acc=acc, pot=pot)
+        else:
+            hot.hot_forces(w.theta, w.eps, w.order, acc=acc, pot=pot)
 
     def barrier():
         torch.cuda.synchronize()

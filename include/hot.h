@@ -76,6 +76,9 @@ typedef struct {
     uint64_t list_entries;      /* accepted cells + listed bodies over all groups (4 B each, +1 B when periodic) */
     int64_t bytes_allocated;
     int64_t launches_build, launches_forces; /* kernels launched by the last hot_build / hot_forces */
+    /* pc_interactions by expansion order (sum over groups of n_G x accepted cells of that order): all in one entry after
+     * hot_forces, a mix after hot_forces_tol ("hexadecapole ... quadrupole ... monopole interactions") */
+    uint64_t pc_monopole, pc_quadrupole, pc_hexadecapole;
 } hot_stats_t;
 
 /* Bucket sizes of the tree: a cell with more than nleaf bodies is split (down
@@ -106,6 +109,18 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
  * pot  : device, [n] fp32 or NULL; overwritten.
  * May be called repeatedly on one build with different theta / eps / order. */
 int hot_forces(double theta, double eps, int order, float* acc, float* pot);
+
+/* The same evaluation with the paper's kind of acceptance criterion: an ABSOLUTE bound on the acceleration error of each
+ * accepted interaction, with the expansion order chosen per interaction ("MAC based on an absolute error",
+ * 90-94 and Fig 3, 238: a mix of monopole, quadrupole and hexadecapole interactions).  The paper prints no formula; the
+ * reading is DESIGN.md R-16: a cell of radius b_max about its centre of mass z with B_n = sum m |y - z|^n, at distance
+ * R > b_max from the nearest point of the sink group's cube, truncated after order p, is off by at most
+ * (p+2) B_(p+1) / (R^(p+1) (R - b_max)^2); the cheapest of monopole (p = 1 about the centre of mass), quadrupole and
+ * hexadecapole whose bound is <= tol is taken, else the cell is opened (a leaf: its bodies interact directly).
+ * tol: absolute acceleration error per interaction, in the caller's units (G = 1), >= 0 (0: only exact interactions).
+ * The criterion compares floating-point numbers: list counts are reproducible run to run, but a borderline cell may
+ * fall differently from another implementation of the same formulas.  Other arguments as hot_forces. */
+int hot_forces_tol(double tol, double eps, float* acc, float* pot);
 
 int hot_stats(hot_stats_t* out);
 
@@ -142,6 +157,8 @@ int hot_export_cells(uint64_t* key, uint32_t* first, uint32_t* count, uint8_t* m
  * summed over the 125 images when periodic.  Any pointer may be NULL. */
 int hot_export_groups(int32_t* cell, uint64_t* key, uint32_t* first, uint32_t* count, uint64_t* lpc, uint64_t* lpp,
                       int64_t cap, int64_t* ngroups);
+/* accepted cells per sink group by expansion order, last hot_forces / hot_forces_tol; HOST arrays [ngroups], NULL to skip */
+int hot_export_group_orders(uint64_t* lmono, uint64_t* lquad, uint64_t* lhexa, int64_t cap, int64_t* ngroups);
 /* The interaction lists of ONE sink group as the last hot_forces walked them, as sets
  * (the order inside a list is the walk's and means nothing):
  *   pc_cell [*npc]: indices (ascending-key numbering of hot_export_cells) of the accepted cells,

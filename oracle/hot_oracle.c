@@ -476,6 +476,8 @@ typedef struct {
     int64_t *pc, *pp; int64_t cap;   /* optional lists: accepted cells / rejected leaves */
     int64_t nleafrej;
     uint8_t *mark;                   /* optional: set to 1 for every accepted cell */
+    int tolmode; double tol; double gc[3], gh; /* error-bound MAC: tolerance, group cube centre and half side */
+    int64_t npc_o[3];                /* accepted cells by order: monopole, quadrupole, hexadecapole */
     /* evaluation */
     int eval, order; double eps2; double shx[3];
     int64_t gfirst, gcount; double *acc, *pot; /* [gcount][3], [gcount], group-local */
@@ -496,16 +498,57 @@ static int mac_accept(const walk_t *w, int64_t c) {
     }
     return (double)((uint64_t)(s * s)) < w->theta2 * (double)d2;
 }
+/* ------------------------------------------------------------------------------------------
+ * f-2: error-bound MAC with per-interaction order (Fig 3).  The paper
+ * prints no formula (it cites refs [45, 68]); the reading taken is DESIGN.md R-16.  A cell with
+ * expansion centre z (its centre of mass), radius b = bbound and absolute moments
+ * B_n = sum_j m_j |y_j - z|^n, truncated after order p, evaluated at distance R > b from z, is off by
+ *     |delta a| <= (p+2) B_(p+1) / (R^(p+1) (R - b)^2)
+ * (the Legendre series of 1/|R - d| summed beyond order p, each term's gradient bounded by
+ * (n+1) |d|^n / R^(n+2); the softened kernel is bounded by the same expression).  About the centre
+ * of mass the dipole vanishes, so "monopole" is p = 1.  B_2 = trace M2 and B_4 = M4_iijj are exact
+ * from the moments; B_3 <= sqrt(B_2 B_4) (Cauchy-Schwarz) and B_5 <= b B_4.
+ * R is the distance from z to the nearest point of the sink group's cube.  The cheapest order in
+ * {monopole, quadrupole, hexadecapole} whose bound is <= tol is taken; if none, the cell is opened.
+ * Returns 0, 2 or 4, or -1 (open).
+ * ---------------------------------------------------------------------------------------- */
+double orc_mac_bound(const double *mom35, double b, double R, int p) {
+    double B2 = mom35[4] + mom35[7] + mom35[9];
+    double B4 = mom35[20] + mom35[30] + mom35[34] + 2.0 * (mom35[23] + mom35[25] + mom35[32]);
+    if (!(R > b)) return INFINITY;
+    double den = (R - b) * (R - b);
+    if (p <= 1) return 3.0 * B2 / (R * R * den);
+    if (p == 2) return 4.0 * sqrt(B2 * B4) / (R * R * R * den);
+    return 6.0 * b * B4 / (R * R * R * R * R * den);
+}
+static int mac_tol(const walk_t *w, int64_t c) {
+    const orc_t *t = w->t;
+    double d2 = 0;
+    for (int k = 0; k < 3; ++k) {
+        double g = fabs(t->com[3 * c + k] + w->shx[k] - w->gc[k]) - w->gh;
+        if (g > 0) d2 += g * g;
+    }
+    double R = sqrt(d2), b = t->bbound[c];
+    const double *mo = t->mom + (size_t)c * ORC_NMOM;
+    if (orc_mac_bound(mo, b, R, 1) <= w->tol) return 0;
+    if (orc_mac_bound(mo, b, R, 2) <= w->tol) return 2;
+    if (orc_mac_bound(mo, b, R, 4) <= w->tol) return 4;
+    return -1;
+}
 static void walk_rec(walk_t *w, int64_t c) {
     const orc_t *t = w->t;
-    if (mac_accept(w, c)) {
+    int ord = w->order, acc_ = 0;
+    if (w->tolmode) { ord = mac_tol(w, c); acc_ = ord >= 0; }
+    else acc_ = mac_accept(w, c);
+    if (acc_) {
+        if (w->tolmode) w->npc_o[ord / 2]++;
         if (w->pc && w->npc < w->cap) w->pc[w->npc] = c;
         w->npc++; w->covered += t->ccount[c];
         if (w->mark) w->mark[c] = 1;
         if (w->eval)
             for (int64_t i = 0; i < w->gcount; ++i) {
                 double z[3] = {t->com[3 * c] + w->shx[0], t->com[3 * c + 1] + w->shx[1], t->com[3 * c + 2] + w->shx[2]};
-                cell_on_sink(t->mom + (size_t)c * ORC_NMOM, z, w->order, t->x + 3 * (w->gfirst + i),
+                cell_on_sink(t->mom + (size_t)c * ORC_NMOM, z, ord, t->x + 3 * (w->gfirst + i),
                              w->eps2, w->acc + 3 * i, w->pot + i);
             }
     } else if (t->cchild[c] < 0) {
@@ -794,6 +837,49 @@ void orc_tree_forces(orc_t *t, double theta, double eps, int order, const int64_
             for (int k = 0; k < 3; ++k) acc[3 * o + k] = a[3 * i + k];
             pot[o] = p[i];
         }
+        free(a); free(p);
+    }
+}
+/* f-2: the same evaluation with the error-bound MAC; list counts per order (summed over images) */
+void orc_tree_forces_tol(orc_t *t, double tol, double eps, const int64_t *groups, int64_t ng,
+                         double *acc, double *pot, int64_t *Lpc0, int64_t *Lpc2, int64_t *Lpc4, int64_t *Lpp) {
+    mi_init();
+    int ws = image_range(t);
+    if (t->periodic) far_prepare(t);
+    if (!groups) ng = t->ngroups;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t q = 0; q < ng; ++q) {
+        int64_t g = groups ? groups[q] : q;
+        walk_t w; walk_setup(&w, t, 0.0, g);
+        int64_t nG = w.gcount, n0 = 0, n2 = 0, n4 = 0, npp = 0;
+        double *a = calloc((size_t)nG * 3, sizeof(double)), *p = calloc((size_t)nG, sizeof(double));
+        for (int ix = -ws; ix <= ws; ++ix) for (int iy = -ws; iy <= ws; ++iy) for (int iz = -ws; iz <= ws; ++iz) {
+            walk_setup(&w, t, 0.0, g);
+            w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
+            w.shx[0] = ix * t->size; w.shx[1] = iy * t->size; w.shx[2] = iz * t->size;
+            w.eval = acc != NULL; w.eps2 = eps * eps; w.acc = a; w.pot = p;
+            w.tolmode = 1; w.tol = tol;
+            double h = t->size / 2097152.0; /* grid spacing: the group's cube from its integer corner and side */
+            w.gh = 0.5 * (double)w.gs * h;
+            for (int k = 0; k < 3; ++k) w.gc[k] = t->lo[k] + ((double)w.go[k] + 0.5 * (double)w.gs) * h;
+            walk_rec(&w, 0);
+            n0 += w.npc_o[0]; n2 += w.npc_o[1]; n4 += w.npc_o[2]; npp += w.npp;
+        }
+        if (Lpc0) Lpc0[q] = n0;
+        if (Lpc2) Lpc2[q] = n2;
+        if (Lpc4) Lpc4[q] = n4;
+        if (Lpp) Lpp[q] = npp;
+        if (acc)
+            for (int64_t i = 0; i < nG; ++i) {
+                int64_t s = w.gfirst + i, o = (int64_t)t->perm[s];
+                if (t->periodic) {
+                    double v, gr[3]; far_on_sink(t, t->x + 3 * s, &v, gr);
+                    p[i] -= v / t->size;
+                    for (int k = 0; k < 3; ++k) a[3 * i + k] += gr[k] / (t->size * t->size);
+                }
+                for (int k = 0; k < 3; ++k) acc[3 * o + k] = a[3 * i + k];
+                pot[o] = p[i];
+            }
         free(a); free(p);
     }
 }

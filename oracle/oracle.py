@@ -40,6 +40,7 @@ def lib():
         _lib.orc_dg.restype = C.c_double
         _lib.orc_psi_smooth.restype = C.c_double
         _lib.orc_ewald_xi.restype = C.c_double
+        _lib.orc_mac_bound.restype = C.c_double
     return _lib
 
 
@@ -139,6 +140,12 @@ def cell_on_sink(mom, z, order, x, eps):
     pot = C.c_double()
     lib().orc_cell_on_sink(_p(mom), _p(z), order, _p(x), C.c_double(eps), _p(acc), C.byref(pot))
     return acc, pot.value
+
+
+def mac_bound(mom35, b, R, p):
+    """Error bound of DESIGN.md R-16 for a cell with moments mom35 (about its centre of mass), radius b, at distance R."""
+    mom35 = np.ascontiguousarray(mom35, dtype=np.float64)
+    return lib().orc_mac_bound(_p(mom35), C.c_double(b), C.c_double(R), int(p))
 
 
 def num_threads():
@@ -246,6 +253,18 @@ class Tree:
         lib().orc_tree_forces(self._h, C.c_double(theta), C.c_double(eps), int(order), _p(groups),
                               C.c_int64(ng), _p(acc), _p(pot), _p(lpc), _p(lpp))
         return acc, pot, lpc, lpp
+
+    def forces_tol(self, tol, eps, groups=None, evaluate=True):
+        """Error-bound MAC with per-interaction order (R-16): acc, pot, and per listed group the accepted cells by
+        order (monopole, quadrupole, hexadecapole) and L_pp."""
+        groups = _i64(groups)
+        ng = self.ngroups if groups is None else groups.shape[0]
+        acc = np.full((self.n, 3), np.nan) if evaluate else None
+        pot = np.full(self.n, np.nan) if evaluate else None
+        l0, l2, l4, lpp = (np.empty(ng, np.int64) for _ in range(4))
+        lib().orc_tree_forces_tol(self._h, C.c_double(tol), C.c_double(eps), _p(groups), C.c_int64(ng),
+                                  _p(acc), _p(pot), _p(l0), _p(l2), _p(l4), _p(lpp))
+        return acc, pot, l0, l2, l4, lpp
 
     def far_table(self):
         co = np.empty(165)

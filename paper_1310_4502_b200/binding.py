@@ -35,7 +35,8 @@ class hot_stats_t(C.Structure):
                 ("ms_build_total", C.c_float), ("ms_forces_total", C.c_float),
                 ("list_chunks", C.c_int32), ("ms_coarse", C.c_float), ("list_entries", C.c_uint64),
                 ("bytes_allocated", C.c_int64),
-                ("launches_build", C.c_int64), ("launches_forces", C.c_int64)]
+                ("launches_build", C.c_int64), ("launches_forces", C.c_int64),
+                ("pc_monopole", C.c_uint64), ("pc_quadrupole", C.c_uint64), ("pc_hexadecapole", C.c_uint64)]
 
 
 def library_path() -> str:
@@ -54,6 +55,8 @@ def _load():
         lib.hot_build.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, hot_box, C.c_int]
         lib.hot_forces.argtypes = [C.c_double, C.c_double, C.c_int, C.c_void_p, C.c_void_p]
         lib.hot_stats.argtypes = [C.POINTER(hot_stats_t)]
+        lib.hot_forces_tol.argtypes = [C.c_double, C.c_double, C.c_void_p, C.c_void_p]
+        lib.hot_export_group_orders.argtypes = [C.c_void_p] * 3 + [C.c_int64, C.POINTER(C.c_int64)]
         lib.hot_step_host.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, hot_box, C.c_int, C.c_double,
                                       C.c_double, C.c_int, C.c_void_p, C.c_void_p]
         lib.hot_set_stream.argtypes = [C.c_void_p]
@@ -135,6 +138,33 @@ def hot_build(pos, mass, lo, size, periodic=False):
     if pos.device.index != cur or mass.device.index != cur:
         raise TypeError(f"hot_build wants tensors on the current CUDA device (cuda:{cur}): the library works there")
     _check(_load().hot_build(pos.data_ptr(), mass.data_ptr(), pos.shape[0], _box(lo, size), int(bool(periodic))))
+
+
+def hot_forces_tol(tol, eps, acc=None, pot=None, want_pot=True):
+    """hot_forces with the error-bound criterion (absolute acceleration tolerance per interaction, order chosen per
+    interaction).  Returns (acc [n,3], pot [n] or None)."""
+    import torch
+
+    n = int(hot_stats()["n"])
+    dev = torch.device("cuda", torch.cuda.current_device())
+    if acc is None:
+        acc = torch.empty((max(n, 1), 3), dtype=torch.float32, device=dev)
+    elif n:
+        _check_out(acc, (n, 3), "acc")
+    if pot is None and want_pot:
+        pot = torch.empty(max(n, 1), dtype=torch.float32, device=dev)
+    elif pot is not None and n:
+        _check_out(pot, (n,), "pot")
+    _check(_load().hot_forces_tol(float(tol), float(eps), acc.data_ptr(), pot.data_ptr() if pot is not None else None))
+    return acc, pot
+
+
+def hot_export_group_orders() -> dict:
+    ng = hot_stats()["n_groups"]
+    out = dict(mono=np.empty(ng, np.uint64), quad=np.empty(ng, np.uint64), hexa=np.empty(ng, np.uint64))
+    got = C.c_int64()
+    _check(_load().hot_export_group_orders(out["mono"].ctypes.data, out["quad"].ctypes.data, out["hexa"].ctypes.data, ng, C.byref(got)))
+    return out
 
 
 def _check_out(t, shape, name):

@@ -19,7 +19,7 @@ struct Ctx {
     Tree t;
     bool built = false;
     int nleaf = 16, ncrit = 256;
-    int last_order = -1;
+    int last_order = -1, last_tolmode = 0;
     char err[512] = "";
     // scratch owned across calls
     int* d_flags = nullptr;               // [0] build error bits, [1] hash max probe, [2] forces error bits
@@ -108,7 +108,7 @@ int ensure_scratch() {
     if (!g.d_flags) {
         CUDA_TRY(cudaMalloc(&g.d_flags, 4 * sizeof(int)));
         CUDA_TRY(cudaMalloc(&g.d_counter, 2 * sizeof(unsigned int))); // walk and interaction schedulers
-        CUDA_TRY(cudaMalloc(&g.d_stat, 4 * sizeof(unsigned long long)));
+        CUDA_TRY(cudaMalloc(&g.d_stat, 6 * sizeof(unsigned long long)));
     }
     if (!g.ev_ready) {
         for (auto& e : g.ev) CUDA_TRY(cudaEventCreate(&e));
@@ -299,12 +299,11 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
     return HOT_OK;
 }
 
-int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
-    if (!g.built) return fail(HOT_EORDER, "hot_forces: no successful hot_build");
-    if (!acc) return fail(HOT_EINVAL, "hot_forces: NULL acc");
-    if (!(theta >= 0.0) || !(theta < 1.0)) return fail(HOT_EINVAL, "hot_forces: theta must be in [0, 1)");
-    if (!(eps >= 0.0)) return fail(HOT_EINVAL, "hot_forces: eps must be >= 0");
-    if (order != 0 && order != 2 && order != 4) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2 or 4");
+} // extern "C"
+namespace {
+// hot_forces (tolmode 0: opening angle theta, one expansion order) and hot_forces_tol (tolmode 1: error-bound criterion
+// with the order chosen per interaction, R-16) share everything but the criterion and the evaluation launches
+int forces_impl(const int tolmode, const double theta, const double tol, const double eps, int order, float* acc, float* pot) {
     Tree& t = g.t;
     cudaStream_t st = g.stream;
     g_hot_launches = 0;
@@ -313,7 +312,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (t.mom_order < order) {
         if (!t.cellA) CUDA_TRY(tree_alloc(&t.cellA, (size_t)t.ncells));
         if (order >= 2 && !t.cellM2) { CUDA_TRY(tree_alloc(&t.cellM2, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellE2, (size_t)t.ncells)); }
-        if (order >= 4 && !t.cellM34) CUDA_TRY(tree_alloc(&t.cellM34, (size_t)t.ncells));
+        if (order >= 4 && !t.cellM34) { CUDA_TRY(tree_alloc(&t.cellM34, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellMac, (size_t)t.ncells)); }
         CUDA_TRY(launch_moments(t, order, st));
         t.mom_order = order;
     }
@@ -383,11 +382,15 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     };
     rc = alloc_lists(); if (rc) return rc;
     rc = alloc_stage(); if (rc) return rc;
-    CUDA_TRY(cudaMemsetAsync(g.d_stat, 0, 4 * sizeof(unsigned long long), st));
+    CUDA_TRY(cudaMemsetAsync(g.d_stat, 0, 6 * sizeof(unsigned long long), st));
     CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
     WalkArgs wa{};
     wa.wcell = t.wcell; wa.group = t.group; wa.g1 = ng;
     mac_table(theta * theta, wa.mac_t); // theta^2 formed once on the host in double (R-7)
+    wa.tolmode = tolmode; wa.tol = tol; wa.size = t.size; wa.cellA = t.cellA; wa.cellMac = t.cellMac;
+    for (int k = 0; k < 3; ++k) wa.lo[k] = t.lo[k];
+    if (tolmode) { CUDA_TRY(tree_alloc(&t.glpc0, (size_t)ng)); CUDA_TRY(tree_alloc(&t.glpc2, (size_t)ng)); }
+    wa.lpc0 = t.glpc0; wa.lpc2 = t.glpc2;
     wa.periodic = t.periodic; wa.lpc = t.glpc; wa.lpp = t.glpp; wa.lvis = t.glvis; wa.pcoff = t.pcoff; wa.ppoff = t.ppoff;
     wa.tops = g.d_tops; wa.first_fail = g.d_flags + 3;
     wa.counter = g.d_counter; wa.stat = g.d_stat; wa.gstack = g.d_gstack; wa.gstack_cap = gcap; wa.errflag = g.d_flags + 2;
@@ -399,6 +402,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
     a.far = t.periodic ? t.far : nullptr;
+    a.seg = -1; a.lpc0 = t.glpc0; a.lpc2 = t.glpc2; a.do_pp = 1; a.accumulate = 0;
     a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
     a.sb_shift = g_hot_sb_shift; a.dbg_mask = g_hot_dbg_mask;
     CUDA_TRY(tree_alloc(&g.d_cls, plan_cls_elems(ng, a.sb_shift)));
@@ -468,7 +472,16 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
             a.far = t.farc;
         }
         CUDA_TRY(cudaEventRecord(g.evx[3], st));
-        CUDA_TRY(launch_forces(a, st));
+        if (!tolmode) CUDA_TRY(launch_forces(a, st));
+        else { // one launch per order over its part of the cell lists; the first also takes the bodies and the far field
+            ForceArgs b = a;
+            b.seg = 0; b.order = 0; CUDA_TRY(launch_forces(b, st));
+            b.do_pp = 0; b.accumulate = 1; b.far = nullptr;
+            for (int sgm = 1; sgm < 3; ++sgm) {
+                CUDA_TRY(cudaMemsetAsync(g.d_counter + 1, 0, sizeof(unsigned int), st)); // the work-item scheduler starts over
+                b.seg = sgm; b.order = 2 * sgm; CUDA_TRY(launch_forces(b, st));
+            }
+        }
         CUDA_TRY(cudaEventRecord(g.evx[2], st));
         if (F < ng) { CUDA_TRY(cudaStreamSynchronize(st)); ms_eval += ms_between(g.evx[3], g.evx[2]); if (t.periodic) ms_coarse += ms_between(g.evx[4], g.evx[3]); } // the arena is reused
         if (F < wa.g1) { // the arena was too small: enlarge it if memory allows, else keep going in rounds of what fitted
@@ -484,9 +497,9 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
         g0 = F;
         ++nrounds;
     }
-    CUDA_TRY(launch_group_stats(t.group, t.glpc, t.glpp, t.glvis, ng, g.d_stat, st));
+    CUDA_TRY(launch_group_stats(t.group, t.glpc, t.glpp, t.glvis, tolmode ? t.glpc0 : nullptr, tolmode ? t.glpc2 : nullptr, ng, g.d_stat, st));
     CUDA_TRY(cudaEventRecord(g.ev[7], st));
-    unsigned long long stat[4];
+    unsigned long long stat[6];
     CUDA_TRY(cudaMemcpyAsync(stat, g.d_stat, sizeof(stat), cudaMemcpyDeviceToHost, st));
     CUDA_TRY(cudaStreamSynchronize(st));
     ms_eval += ms_between(g.evx[3], g.evx[2]);
@@ -495,6 +508,10 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     hot_stats_t& s = g.st;
     s.order = order;
     s.cells_visited = stat[0]; s.walk_spills = stat[1]; s.pp_interactions = stat[2]; s.pc_interactions = stat[3];
+    s.pc_monopole = s.pc_quadrupole = s.pc_hexadecapole = 0;
+    if (tolmode) { s.pc_monopole = stat[4]; s.pc_quadrupole = stat[5]; s.pc_hexadecapole = stat[3] - stat[4] - stat[5]; }
+    else (order == 0 ? s.pc_monopole : order == 2 ? s.pc_quadrupole : s.pc_hexadecapole) = stat[3];
+    g.last_tolmode = tolmode;
     s.ms_moments = ms_between(g.ev[5], g.ev[6]);
     s.ms_walk = ms_walk;
     s.ms_eval = ms_eval;
@@ -506,6 +523,44 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     s.launches_forces = g_hot_launches;
     g.last_order = order;
     g.lists_valid = true;
+    return HOT_OK;
+}
+} // namespace
+extern "C" {
+int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
+    if (!g.built) return fail(HOT_EORDER, "hot_forces: no successful hot_build");
+    if (!acc) return fail(HOT_EINVAL, "hot_forces: NULL acc");
+    if (!(theta >= 0.0) || !(theta < 1.0)) return fail(HOT_EINVAL, "hot_forces: theta must be in [0, 1)");
+    if (!(eps >= 0.0)) return fail(HOT_EINVAL, "hot_forces: eps must be >= 0");
+    if (order != 0 && order != 2 && order != 4) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2 or 4");
+    return forces_impl(0, theta, 0.0, eps, order, acc, pot);
+}
+int hot_forces_tol(double tol, double eps, float* acc, float* pot) {
+    if (!g.built) return fail(HOT_EORDER, "hot_forces_tol: no successful hot_build");
+    if (!acc) return fail(HOT_EINVAL, "hot_forces_tol: NULL acc");
+    if (!(tol >= 0.0) || !(tol < 3.0e38)) return fail(HOT_EINVAL, "hot_forces_tol: tol must be finite and >= 0");
+    if (!(eps >= 0.0)) return fail(HOT_EINVAL, "hot_forces_tol: eps must be >= 0");
+    return forces_impl(1, 0.0, tol, eps, 4, acc, pot);
+}
+int hot_export_group_orders(uint64_t* lmono, uint64_t* lquad, uint64_t* lhexa, int64_t cap, int64_t* ngroups) {
+    if (!g.built || !g.lists_valid) return fail(HOT_EORDER, "hot_export_group_orders: no hot_forces on this build");
+    const Tree& t = g.t;
+    if (ngroups) *ngroups = t.ngroups;
+    if (cap < t.ngroups) return fail(HOT_EINVAL, "hot_export_group_orders: cap too small");
+    CUDA_TRY(cudaStreamSynchronize(g.stream));
+    const size_t ng = (size_t)t.ngroups;
+    std::vector<uint32_t> tot(ng), a0(ng, 0), a2(ng, 0);
+    CUDA_TRY(cudaMemcpy(tot.data(), t.glpc, 4 * ng, cudaMemcpyDeviceToHost));
+    if (g.last_tolmode) {
+        CUDA_TRY(cudaMemcpy(a0.data(), t.glpc0, 4 * ng, cudaMemcpyDeviceToHost));
+        CUDA_TRY(cudaMemcpy(a2.data(), t.glpc2, 4 * ng, cudaMemcpyDeviceToHost));
+    } else if (g.last_order == 0) a0 = tot;
+    else if (g.last_order == 2) a2 = tot;
+    for (size_t i = 0; i < ng; ++i) {
+        if (lmono) lmono[i] = a0[i];
+        if (lquad) lquad[i] = a2[i];
+        if (lhexa) lhexa[i] = (uint64_t)tot[i] - a0[i] - a2[i];
+    }
     return HOT_OK;
 }
 

@@ -453,7 +453,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
     // sources are staged NEGATED (origin - position, -mass): the kernels then need no negations
 
     // ---- the group's own bodies (the "self block"): the walk leaves the group cell out ----------
-    for (uint32_t j0 = 0; j0 < g.count; j0 += BATCH) {
+    for (uint32_t j0 = 0; j0 < (P.do_pp ? g.count : 0u); j0 += BATCH) {
         const int cnt = (int)min((uint32_t)BATCH, g.count - j0);
         if (lane < cnt) {
             const float4 b = P.body[g.first + j0 + lane];
@@ -468,8 +468,14 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
 
     // ---- S9: the particle-cell list ------------------------------------------------------------------
     {
-        const unsigned long long o0 = P.pcoff[gi];
-        const int n = (int)P.lpc[gi];
+        unsigned long long o0 = P.pcoff[gi];
+        int n = (int)P.lpc[gi];
+        if (P.seg >= 0) { // tolerance mode: the list is monopoles | quadrupoles | hexadecapoles, this launch takes one part
+            const int n0 = (int)P.lpc0[gi], n2 = (int)P.lpc2[gi];
+            if (P.seg == 0) n = n0;
+            else if (P.seg == 1) { o0 += n0; n = n2; }
+            else { o0 += n0 + n2; n -= n0 + n2; }
+        }
         const uint32_t* const pl = P.pclist + o0;
         const uint8_t* const pi = PER ? P.pcimg + o0 : nullptr;
         const int nb = (n + BATCH - 1) / BATCH;
@@ -556,7 +562,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
     // ---- S8: the particle-particle list ------------------------------------------------------------
     {
         const unsigned long long o0 = P.ppoff[gi];
-        const int n = (int)P.lpp[gi];
+        const int n = P.do_pp ? (int)P.lpp[gi] : 0;
         const uint32_t* const pl = P.pplist + o0;
         const uint8_t* const pi = PER ? P.ppimg + o0 : nullptr;
         const int nb = (n + BATCH - 1) / BATCH;
@@ -615,9 +621,13 @@ HOT_UNROLL(HOT_PP_UNROLL)
         for (int i = 0; i < S; ++i) {
             if (sk.me[i] >= 0) {
                 const uint32_t o = P.perm[g.first + sk.me[i]];
-                if (PER) {
+                if (PER && P.far) {
                     const double4 f = reinterpret_cast<const double4*>(P.far)[g.first + sk.me[i]];
                     A[i][0] += f.x; A[i][1] += f.y; A[i][2] += f.z; A[i][3] += f.w;
+                }
+                if (P.accumulate) { // a later launch of the same hot_forces call (tolerance mode: one launch per order)
+                    A[i][0] += (double)P.acc[3 * (int64_t)o]; A[i][1] += (double)P.acc[3 * (int64_t)o + 1]; A[i][2] += (double)P.acc[3 * (int64_t)o + 2];
+                    if (P.pot) A[i][3] += (double)P.pot[o];
                 }
                 P.acc[3 * (int64_t)o] = (float)A[i][0];
                 P.acc[3 * (int64_t)o + 1] = (float)A[i][1];

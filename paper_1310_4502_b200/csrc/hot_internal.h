@@ -71,6 +71,8 @@ struct Tree {
     CellM2* cellM2 = nullptr;
     CellM2* cellE2 = nullptr; // evaluation form of cellM2 (see CellM2)
     CellM34* cellM34 = nullptr;
+    float4* cellMac = nullptr;               // order 4 only: b, 3 B2, 4 sqrt(B2 B4), 6 b B4 (the error bounds of R-16, numerators)
+    uint32_t *glpc0 = nullptr, *glpc2 = nullptr; // per group, tolerance mode: accepted monopoles, quadrupoles
 };
 
 // ---- build stages (hot_build.cu) ------------------------------------------------------------
@@ -135,12 +137,17 @@ struct WalkArgs {
     unsigned long long* stat;              // [1] ring spills
     uint32_t* gstack; int64_t gstack_cap;  // per-warp spill arena (entries per warp)
     int* errflag;                          // bit 2: spill arena exhausted, bit 3: staging too small
+    // error-bound criterion (tolmode != 0; R-16): accept at the cheapest order whose bound is <= tol
+    int tolmode; double tol; double lo[3], size;
+    const CellA* cellA; const float4* cellMac;   // per cell: centre of mass / (b, 3 B2, 4 sqrt(B2 B4), 6 b B4)
+    uint32_t *lpc0, *lpc2;                 // per group: accepted monopoles, quadrupoles (the list is ordered mono | quad | hexa)
 };
 int walk_grid_warps();
 cudaError_t launch_walk(const WalkArgs& a, cudaStream_t st);
-// stat[0] += cells visited, stat[2] += sum n_G (L_pp + n_G), stat[3] += sum n_G L_pc over the groups [0, ng)
-cudaError_t launch_group_stats(const GroupRec* group, const uint32_t* lpc, const uint32_t* lpp, const uint32_t* lvis, int64_t ng,
-                               unsigned long long* stat, cudaStream_t st);
+// stat[0] += cells visited, stat[2] += sum n_G (L_pp + n_G), stat[3] += sum n_G L_pc over the groups [0, ng);
+// with lpc0 / lpc2 (tolerance mode): stat[4], stat[5] += sum n_G x accepted monopoles / quadrupoles
+cudaError_t launch_group_stats(const GroupRec* group, const uint32_t* lpc, const uint32_t* lpp, const uint32_t* lvis,
+                               const uint32_t* lpc0, const uint32_t* lpc2, int64_t ng, unsigned long long* stat, cudaStream_t st);
 
 // ---- interactions (hot_forces.cu): evaluates the lists of the groups [g0, g1) -------------------------
 struct ForceArgs {
@@ -155,6 +162,8 @@ struct ForceArgs {
     unsigned int* counter;        // dynamic scheduler over the work items
     uint4* items;                 // one per pass of a group, ordered by sinks per lane (launch_plan)
     unsigned int* cls;            // plan_cls_elems(g1 - g0, sb_shift) words: per-(superblock, class) counts, starts, cursors, total
+    // tolerance mode: one launch per order over its segment of the cell lists (seg = 0, 1, 2; -1: the whole list)
+    int seg; const uint32_t *lpc0, *lpc2; int do_pp, accumulate;
     unsigned long long dbg_mask; // HOT_DEBUG_HOOKS builds only: bit (S + 8 lgL) enables the class
     int sb_shift; unsigned int nsb; // 2^sb_shift groups per superblock (>= 8), number of superblocks of [g0, g1)
 };

@@ -67,7 +67,7 @@ __device__ __forceinline__ void add_shifted(double* M, const double* C, double m
 
 template <int ORDER>
 __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, double zy, double zz, double bmax, const double* M,
-                                           CellA* cellA, CellM2* cellM2, CellM2* cellE2, CellM34* cellM34) {
+                                           CellA* cellA, CellM2* cellM2, CellM2* cellE2, CellM34* cellM34, float4* cellMac = nullptr) {
     CellA A; A.zx = zx; A.zy = zy; A.zz = zz; A.m0 = (float)m0; A.bmax = __double2float_ru(bmax); // rounded up: stays a bound
     if (ORDER >= 2) {
         CellM2 Q;
@@ -101,6 +101,11 @@ __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, doub
         v[34] = v[28] + v[31] + v[33];                 // t4
         v[35] = 0.f;
         cellM34[c] = R;
+        if (cellMac) { // numerators of the error bounds of DESIGN.md R-16, rounded up: b, 3 B2, 4 sqrt(B2 B4), 6 b B4
+            const double B2 = M[midx(2, 0, 0)] + M[midx(0, 2, 0)] + M[midx(0, 0, 2)];
+            const double B4 = M[midx(4, 0, 0)] + M[midx(0, 4, 0)] + M[midx(0, 0, 4)] + 2.0 * (M[midx(2, 2, 0)] + M[midx(2, 0, 2)] + M[midx(0, 2, 2)]);
+            cellMac[c] = make_float4(A.bmax, __double2float_ru(3.0 * B2), __double2float_ru(4.0 * sqrt(B2 * B4)), __double2float_ru(6.0 * (double)A.bmax * B4));
+        }
     }
 }
 template <int ORDER>
@@ -126,7 +131,7 @@ __device__ __forceinline__ void load_child(int64_t c, const CellM2* cellM2, cons
 struct MomArgs {
     const int32_t* leafcell; int64_t nleaves;
     const uint32_t *cfirst, *ccount, *cmask; const int32_t* cchild; const float4* body;
-    CellA* cellA; CellM2* cellM2; CellM2* cellE2; CellM34* cellM34;
+    CellA* cellA; CellM2* cellM2; CellM2* cellE2; CellM34* cellM34; float4* cellMac;
 };
 template <int ORDER>
 __global__ void __launch_bounds__(128) moments_leaves_kernel(const __grid_constant__ MomArgs P) {
@@ -151,7 +156,7 @@ __global__ void __launch_bounds__(128) moments_leaves_kernel(const __grid_consta
         bmax = fmax(bmax, dx * dx + dy * dy + dz * dz);
         if (ORDER >= 2) add_point<ORDER>(M, (double)b.w, dx, dy, dz);
     }
-    store_cell<ORDER>(c0, m0, zx, zy, zz, sqrt(bmax), M, P.cellA, P.cellM2, P.cellE2, P.cellM34);
+    store_cell<ORDER>(c0, m0, zx, zy, zz, sqrt(bmax), M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac);
 }
 // an internal cell from its children (one level down, already done): parallel-axis shift, fixed child order
 template <int ORDER>
@@ -179,7 +184,7 @@ __device__ __forceinline__ void combine_children(const MomArgs& P, int64_t c) {
             add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
         }
     }
-    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34);
+    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac);
 }
 // One level of internal cells.  A warp looks at 32 consecutive cells of the level, keeps the internal ones (one in eight
 // on average) and hands each to an OCTET of lanes: lane q of the octet loads child q (all children of the warp's cells in
@@ -233,7 +238,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constan
                 for (int k = 4; k < NM; ++k) M[k] += __shfl_xor_sync(0xffffffffu, M[k], o);
             }
         }
-        if (have && q == 0) store_cell<ORDER>(cell, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34);
+        if (have && q == 0) store_cell<ORDER>(cell, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac);
         // drop the four cells just done
         for (int i = 0; i < 4 && todo; ++i) todo &= todo - 1;
     }
@@ -272,7 +277,7 @@ template <int ORDER> static cudaError_t moments_run(const Tree& t, const MomArgs
 cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
     MomArgs a;
     a.leafcell = t.leafcell; a.nleaves = t.nleaves; a.cfirst = t.cfirst; a.ccount = t.ccount; a.cmask = t.cmask; a.cchild = t.cchild;
-    a.body = t.body; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34;
+    a.body = t.body; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34; a.cellMac = order >= 4 ? t.cellMac : nullptr;
     if (order >= 4) return moments_run<4>(t, a, st);
     if (order >= 2) return moments_run<2>(t, a, st);
     return moments_run<0>(t, a, st);

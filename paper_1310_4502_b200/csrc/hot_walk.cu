@@ -29,7 +29,12 @@
 // the warp pops the OLDEST entries (breadth-first: keeps the frontier wide and the 32 lanes busy);
 // once it holds RING/4 entries it pops the NEWEST (depth-first: bounded growth).  If it still fills
 // up, the oldest entries spill to a per-warp arena in global memory.
-template <bool PER>
+// TOL: the error-bound criterion with per-interaction order (R-16) instead of the
+// opening angle: a lane also reads the cell's centre of mass, radius and moment bounds and takes the cheapest of
+// monopole / quadrupole / hexadecapole whose bound at the distance to the group's cube is below the tolerance; the
+// order rides in bits 29-30 of the staged entry and the list is laid out monopoles | quadrupoles | hexadecapoles.
+#define HOT_ORDER_SHIFT 29
+template <bool PER, bool TOL>
 __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_constant__ WalkArgs P) {
     __shared__ uint32_t s_ring[WALK_WARPS][RING];
     __shared__ uint8_t s_img[PER ? WALK_WARPS : 1][PER ? RING : 1];
@@ -59,6 +64,13 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
         const int gs = 1 << (HOT_MAXLEVEL - (int)(gw.w >> 27));
         const int gox = (int)(gw.x & 0x1fffffu), goy = (int)((gw.x >> 21) | ((gw.y & 0x3ffu) << 11)), goz = (int)((gw.y >> 10) & 0x1fffffu);
         const int ghx = gox + gs, ghy = goy + gs, ghz = goz + gs;
+        double gcx = 0, gcy = 0, gcz = 0, gh = 0; // TOL: the group's cube as centre and half side, in the caller's units
+        if (TOL) {
+            const double h = P.size * (1.0 / 2097152.0);
+            gcx = P.lo[0] + ((double)gox + 0.5 * gs) * h; gcy = P.lo[1] + ((double)goy + 0.5 * gs) * h; gcz = P.lo[2] + ((double)goz + 0.5 * gs) * h;
+            gh = 0.5 * (double)gs * h;
+        }
+        uint32_t n0 = 0, n2 = 0; // TOL: accepted monopoles, quadrupoles
         uint32_t npc = 0, nrun = 0, nbody = 0, nvis = 0; // list lengths, bodies in the runs, cells visited
         int head = 0, top = 0, gtop = 0, next_img = 0;
         while (true) {
@@ -127,7 +139,25 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
             const uint32_t gy = (uint32_t)max(0, max(cy - ghy, goy - (cy + s)));
             const uint32_t gz = (uint32_t)max(0, max(cz - ghz, goz - (cz + s)));
             const unsigned long long d2 = (unsigned long long)gx * gx + (unsigned long long)gy * gy + (unsigned long long)gz * gz;
-            const bool acc = v && d2 >= P.mac_t[lev]; // == (double)(s*s) < theta^2 * (double)d2, see mac_table()
+            bool acc; int ocode = 0;
+            if (!TOL) acc = v && d2 >= P.mac_t[lev]; // == (double)(s*s) < theta^2 * (double)d2, see mac_table()
+            else {
+                acc = false;
+                if (v) {
+                    const CellA A = P.cellA[c];
+                    const float4 mb = P.cellMac[c]; // b, 3 B2, 4 sqrt(B2 B4), 6 b B4
+                    double zx = A.zx, zy = A.zy, zz = A.zz;
+                    if (PER) { zx += (double)(im / 25 - 2) * P.size; zy += (double)((im / 5) % 5 - 2) * P.size; zz += (double)(im % 5 - 2) * P.size; }
+                    const double ax = fmax(fabs(zx - gcx) - gh, 0.0), ay = fmax(fabs(zy - gcy) - gh, 0.0), az = fmax(fabs(zz - gcz) - gh, 0.0);
+                    const double R2 = ax * ax + ay * ay + az * az, R = sqrt(R2), b = (double)mb.x;
+                    if (R > b) {
+                        const double t = P.tol * (R - b) * (R - b); // bound_p <= tol  <=>  c_p <= tol (R-b)^2 R^(p+1)
+                        if ((double)mb.y <= t * R2) { acc = true; ocode = 0; }
+                        else if ((double)mb.z <= t * R2 * R) { acc = true; ocode = 1; }
+                        else if ((double)mb.w <= t * R2 * R2 * R) { acc = true; ocode = 2; }
+                    }
+                }
+            }
             const bool self = v && c == gcell && (!PER || im == 62);
             const bool rej_leaf = v && !acc && leaf && !self;
             const bool open = v && !acc && !leaf && !self;
@@ -136,9 +166,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
             if (acc) {
                 const uint32_t p = npc + __popc(macc & lt);
                 // periodic: cells of the coarsest levels are marked; their monopoles are summed in fp64 (hot_periodic.cu)
-                if (p < scap) { spc[p] = (PER && lev <= HOT_COARSE_LEVEL) ? (c | HOT_COARSE_FLAG) : c; if (PER) ipc[p] = (uint8_t)im; }
+                if (p < scap) { spc[p] = ((PER && lev <= HOT_COARSE_LEVEL) ? (c | HOT_COARSE_FLAG) : c) | (TOL ? (uint32_t)ocode << HOT_ORDER_SHIFT : 0u); if (PER) ipc[p] = (uint8_t)im; }
             }
             npc += __popc(macc);
+            if (TOL) { n0 += __popc(__ballot_sync(FULL, acc && ocode == 0)); n2 += __popc(__ballot_sync(FULL, acc && ocode == 1)); }
             // rejected leaves -> one body run each (a leaf holds <= 32 bodies except at the finest level)
             if (mrej) {
                 uint32_t nb = rej_leaf ? cnt : 0u;
@@ -190,7 +221,24 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
         if (!ok) continue;
         pcb = __shfl_sync(FULL, pcb, 0); ppb = __shfl_sync(FULL, ppb, 0);
         __syncwarp();
-        for (uint32_t j = lane; j < npc; j += 32) { P.pclist[pcb + j] = spc[j]; if (PER) P.pcimg[pcb + j] = ipc[j]; }
+        if (!TOL) {
+            for (uint32_t j = lane; j < npc; j += 32) { P.pclist[pcb + j] = spc[j]; if (PER) P.pcimg[pcb + j] = ipc[j]; }
+        } else { // three stable passes: monopoles, quadrupoles, hexadecapoles; the order bits are dropped
+            uint32_t base = 0;
+            for (uint32_t o = 0; o < 3; ++o)
+                for (uint32_t j0 = 0; j0 < npc; j0 += 32) {
+                    const uint32_t j = j0 + lane;
+                    const uint32_t e = j < npc ? spc[j] : 0u;
+                    const bool hit = j < npc && ((e >> HOT_ORDER_SHIFT) & 3u) == o;
+                    const uint32_t m = __ballot_sync(FULL, hit);
+                    if (hit) {
+                        const uint32_t q = base + __popc(m & lt);
+                        P.pclist[pcb + q] = e & ~(3u << HOT_ORDER_SHIFT);
+                        if (PER) P.pcimg[pcb + q] = ipc[j];
+                    }
+                    base += __popc(m);
+                }
+        }
         {
             uint32_t r = 0, roff = 0, out = 0; // next run, bodies of it already written, entries written
             while (out < nbody) {
@@ -217,6 +265,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
         }
         if (lane == 0) {
             P.lpc[gi] = npc; P.lpp[gi] = nbody; P.lvis[gi] = nvis;
+            if (TOL) { P.lpc0[gi] = n0; P.lpc2[gi] = n2; }
             P.pcoff[gi] = pcb; P.ppoff[gi] = ppb;
         }
         __syncwarp();
@@ -230,8 +279,10 @@ int walk_grid_warps() { // resident warps of the walk grid: blocks/SM of the var
         int dev = 0, nsm = 0, occ = 1 << 20, o = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false, true>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, true>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
         if (occ == 1 << 20) occ = 1;
         cudaGetLastError();
         nw = nsm * occ * WALK_WARPS;
@@ -241,30 +292,36 @@ int walk_grid_warps() { // resident warps of the walk grid: blocks/SM of the var
 cudaError_t launch_walk(const WalkArgs& a, cudaStream_t st) {
     const int nb = walk_grid_warps() / WALK_WARPS;
     HOT_LAUNCHED(1);
-    if (a.periodic) walk_kernel<true><<<nb, WALK_WARPS * 32, 0, st>>>(a);
-    else walk_kernel<false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+    if (a.tolmode) {
+        if (a.periodic) walk_kernel<true, true><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+        else walk_kernel<false, true><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+    } else if (a.periodic) walk_kernel<true, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+    else walk_kernel<false, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
     return cudaGetLastError();
 }
 
 // interaction and visit counts of the last walk, summed over the groups
 __global__ void __launch_bounds__(256) group_stats_kernel(const GroupRec* __restrict__ group, const uint32_t* __restrict__ lpc,
-                                                          const uint32_t* __restrict__ lpp, const uint32_t* __restrict__ lvis, int64_t ng,
+                                                          const uint32_t* __restrict__ lpp, const uint32_t* __restrict__ lvis,
+                                                          const uint32_t* __restrict__ lpc0, const uint32_t* __restrict__ lpc2, int64_t ng,
                                                           unsigned long long* __restrict__ stat) {
-    unsigned long long vis = 0, spp = 0, spc = 0;
+    unsigned long long vis = 0, spp = 0, spc = 0, s0 = 0, s2 = 0;
     for (int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; i < ng; i += (int64_t)gridDim.x * blockDim.x) {
         const unsigned long long n = group[i].count;
         vis += lvis[i]; spc += n * lpc[i]; spp += n * ((unsigned long long)lpp[i] + n); // L_pp counts the group's own bodies too
+        if (lpc0) { s0 += n * lpc0[i]; s2 += n * lpc2[i]; }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         vis += __shfl_xor_sync(FULL, vis, o); spp += __shfl_xor_sync(FULL, spp, o); spc += __shfl_xor_sync(FULL, spc, o);
+        s0 += __shfl_xor_sync(FULL, s0, o); s2 += __shfl_xor_sync(FULL, s2, o);
     }
-    if ((threadIdx.x & 31) == 0) { atomicAdd(&stat[0], vis); atomicAdd(&stat[2], spp); atomicAdd(&stat[3], spc); }
+    if ((threadIdx.x & 31) == 0) { atomicAdd(&stat[0], vis); atomicAdd(&stat[2], spp); atomicAdd(&stat[3], spc); if (lpc0) { atomicAdd(&stat[4], s0); atomicAdd(&stat[5], s2); } }
 }
-cudaError_t launch_group_stats(const GroupRec* group, const uint32_t* lpc, const uint32_t* lpp, const uint32_t* lvis, int64_t ng,
-                               unsigned long long* stat, cudaStream_t st) {
+cudaError_t launch_group_stats(const GroupRec* group, const uint32_t* lpc, const uint32_t* lpp, const uint32_t* lvis,
+                               const uint32_t* lpc0, const uint32_t* lpc2, int64_t ng, unsigned long long* stat, cudaStream_t st) {
     HOT_LAUNCHED(1);
     const unsigned nb = (unsigned)((ng + 255) / 256 < 1184 ? (ng + 255) / 256 : 1184);
-    group_stats_kernel<<<nb, 256, 0, st>>>(group, lpc, lpp, lvis, ng, stat);
+    group_stats_kernel<<<nb, 256, 0, st>>>(group, lpc, lpp, lvis, lpc0, lpc2, ng, stat);
     return cudaGetLastError();
 }

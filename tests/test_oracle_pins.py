@@ -550,3 +550,69 @@ def test_error_monotone_in_order_and_theta():
     for o in (0, 2, 4):
         assert e[(0.4, o)] < e[(0.6, o)] < e[(0.8, o)]
     assert e[(0.4, 4)] < 1e-5
+
+
+# ---------------------------------------------------------------- f-2: error-bound MAC (R-16)
+def test_error_bound_holds_for_random_cells():
+    """Fig 6's set-up: 512 random particles in a unit cube, a sink at distance r.  The bound of R-16
+    must never be below the actual truncation error of the expansion about the centre of mass -- for every order it
+    is used with, every direction, softened or not -- and must not be uselessly loose either."""
+    rng = np.random.default_rng(68)
+    worst = {0: 0.0, 2: 0.0, 4: 0.0}
+    loose = {0: [], 2: [], 4: []}
+    for trial in range(6):
+        n = 512 if trial < 3 else 9
+        y = rng.uniform(-0.5, 0.5, (n, 3)) * (1.0 if trial % 2 == 0 else np.array([1.0, 0.2, 0.05]))
+        m = rng.uniform(0.5, 1.5, n) / n
+        mom, z = O.moments_of(y, m)
+        b = np.sqrt(((y - z) ** 2).sum(1)).max()
+        for eps in (0.0, 0.05):
+            for r in (1.05 * b, 1.5 * b, 1.0, 2.0, 4.0, 16.0):
+                if r <= b:
+                    continue
+                for _ in range(8):
+                    u = rng.standard_normal(3); u /= np.linalg.norm(u)
+                    x = z + r * u
+                    ad, pd = _direct_on(x, y, m, eps)
+                    for order, p in ((0, 1), (2, 2), (4, 4)):
+                        a, ph = O.cell_on_sink(mom, z, order, x, eps)
+                        err = np.linalg.norm(a - ad)
+                        bound = O.mac_bound(mom, b, r, p)
+                        assert err <= bound * (1 + 1e-9) + 1e-15 * np.linalg.norm(ad), (trial, eps, r, order, err, bound)
+                        worst[order] = max(worst[order], err / bound)
+                        if r >= 2 * b and eps == 0.0 and n == 512:
+                            loose[order].append(bound / max(err, 1e-300))
+    assert all(v > 0.02 for v in worst.values()), worst           # the bound is approached within a factor of 50
+    assert all(np.median(v) < 2000 for v in loose.values()), {k: np.median(v) for k, v in loose.items()}
+    assert O.mac_bound(mom, b, 0.9 * b, 2) == np.inf                # inside the cell's radius: never accepted
+
+
+def test_error_bound_tree_properties():
+    """Tolerance -> 0: everything particle-particle = the direct sum.  Larger tolerance: fewer, lower-order
+    interactions and a larger error, always below tolerance x accepted cells; coverage invariant."""
+    w = W.config(2, 11)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, nleaf=8, ncrit=32)
+    ad, pd = O.direct(w.pos, w.mass, w.eps)
+    a, p, l0, l2, l4, lpp = T.forces_tol(0.0, w.eps)
+    # tolerance 0 accepts only cells whose bound is 0: single bodies, whose monopole is exact
+    assert (l2 + l4 == 0).all() and (l0 + lpp == w.n).all()
+    assert np.abs(a - ad).max() <= 1e-12 * np.abs(ad).max()
+    arms = np.sqrt((ad ** 2).sum(1).mean())
+    prev_cost, prev_err = None, None
+    for tol in (1e-5 * arms, 1e-3 * arms, 1e-1 * arms):
+        a, p, l0, l2, l4, lpp = T.forces_tol(tol, w.eps)
+        err = np.linalg.norm(a - ad, axis=1)
+        # every particle's error is below tol x (number of cells its group accepted)
+        gcount = T.cells()["count"][T.groups()]
+        per_body = np.repeat(l0 + l2 + l4, gcount)          # in key order
+        perm = T.keys()[2]
+        bound = np.empty(w.n); bound[perm] = per_body * tol
+        assert (err <= bound + 1e-12 * arms).all()
+        cost = (gcount * (l0 + 3 * l2 + 13 * l4 + lpp)).sum()
+        rms = np.sqrt((err ** 2).mean()) / arms
+        if prev_cost is not None:
+            assert cost < prev_cost and rms > prev_err
+        prev_cost, prev_err = cost, rms
+    assert l0.sum() > 0 and l2.sum() > 0                   # a mix of orders at the loosest tolerance
+    a, p, l0, l2, l4, lpp = T.forces_tol(1e-4 * arms, w.eps)
+    assert l2.sum() > 0 and l4.sum() > 0
