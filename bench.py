@@ -32,11 +32,22 @@ if ROOT not in sys.path:
 #   P-C order 4: 10 add + 68 mul + 96 fma + rsqrt          = 271   (as compiled: FADD2 / FMUL2 / FFMA2 per sink pair in SASS)
 FLOPS_PP = 20
 FLOPS_PC = {0: 21, 2: 58, 4: 271}
-# DRAM bytes of one forces_kernel launch from the ncu --set full capture of the default workload
-# (profiles/r01_forces_walk_kernels_c2_2p24.md: dram__bytes_read.sum 14.563 GB + dram__bytes_write.sum 1.201 GB;
-# the lists alone are 4 B x 0.88e9 entries = 3.5 GB of compulsory reads, acc + pot 0.27 GB of writes), at the
-# default bucket sizes NLEAF 16 / NCRIT 256; other workloads: null
-NCU_TRAFFIC_BYTES = {("c2", 24, 0.6, 2, 16, 256): 15.764e9}
+# roofline.traffic: DRAM bytes of one forces_kernel launch (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum),
+# looked up in profiles/forces_traffic.csv by workload; null where no capture was taken
+def ncu_traffic(config, n, theta, order, nleaf, ncrit):
+    import csv
+
+    try:
+        with open(os.path.join(ROOT, "profiles", "forces_traffic.csv")) as f:
+            for r in csv.DictReader(l for l in f if not l.startswith("#")):
+                if (int(r["config"]), int(r["n"]), float(r["theta"]), int(r["order"]), int(r["nleaf"]), int(r["ncrit"])) == \
+                        (config, n, theta, order, nleaf, ncrit):
+                    return float(r["dram_bytes"])
+    except (OSError, KeyError, ValueError):
+        pass
+    return None
+
+
 # FP32 peak derived from unit counts and clocks (B200_PROFILING.md: 148 SMs, clocks.max.sm 1965 MHz;
 # 128 FP32 lanes per SM, FMA = 2 flops): 148 * 128 * 2 * 1.965e9
 FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
@@ -44,6 +55,13 @@ SORT_BYTES_PER_BODY = 8 * 24 - 4      # 8 passes x (12 B read + 12 B write); pas
 SORT_BYTES_SURVEY = 8 + 8 * 24        # SURVEY 8(d) count for d = 8 (with a histogram pre-pass over the keys; here keygen counts)
 KEYGEN_BYTES_PER_BODY = 40          # 12 B pos + 4 B mass read; 8 B key + 16 B float4 body written (+ digit histograms)
 GATHER_BYTES_PER_BODY = 36          # 4 B permutation + 16 B float4 gathered, 16 B written
+# tree + hash + groups: the sorted keys twice (levels, emit) and the per-body level word written and read,
+# per cell the SoA record (key 8, first, count, mask, child, parent 4 each), the 16-byte walk record, the leaf list
+# entry or hash slot (4): 24 B per body + 48 B per cell
+TREE_BYTES = (24, 48)
+# upward pass: 16 B per body read once; per cell the three 32-byte records written (centre/mass/b_max, raw and staged
+# quadrupole) and, for the internal eighth, its children's 64 B read: 16 B per body + 104 B per cell (order 2)
+MOMENTS_BYTES = (16, 104)
 
 
 def parse():
@@ -134,36 +152,59 @@ class ClockSampler:
                 "reasons": sorted(reasons)}
 
 
-def cpu_oracle_sample(args, w_full, budget_s=15.0):
-    """The oracle as it stands, whole path, on a smaller replica of the same workload."""
-    import numpy as np
+_ORACLE_TREES = {}
 
+
+def _oracle_tree(args, w_full):
+    """The oracle's tree of the bench workload itself where its build takes well under a minute (n <= 2^24: keys, stable
+    sort, tree, groups and the moments of every cell); a replica made by the same generator for the 2^27-body config,
+    whose build alone takes many minutes.  Returns (tree, workload it was built on, build seconds)."""
     from oracle import oracle as O
     from paper_1310_4502_b200 import workloads as W
 
-    scale = {0: 14, 1: 18, 2: 18, 3: 32, 4: 32}[args.config]
-    if args.scale is not None:
-        scale = min(scale, args.scale)
-    w = W.config(args.config, scale)
-    t0 = time.perf_counter()
-    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic, nleaf=args.nleaf, ncrit=args.ncrit)
-    t_build = time.perf_counter() - t0
+    key = (args.config, args.scale, args.nleaf, args.ncrit)
+    if key not in _ORACLE_TREES:
+        w = w_full
+        if w_full.n > (1 << 24):
+            w = W.config(args.config, 64)  # a 64^3 lattice made by the same recipe
+        t0 = time.perf_counter()
+        T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=w.periodic, nleaf=args.nleaf, ncrit=args.ncrit)
+        _ORACLE_TREES[key] = (T, w, time.perf_counter() - t0)
+    return _ORACLE_TREES[key]
+
+
+def cpu_oracle_sample(args, w_full, budget_s=12.0, threads=None):
+    """The oracle as it stands on a bounded sample: its whole path on the bench workload, the walk + evaluation on
+    random sink groups until the budget is spent, the build charged pro rata."""
+    import numpy as np
+
+    from oracle import oracle as O
+
+    T, w, t_build = _oracle_tree(args, w_full)
+    O.set_num_threads(threads or os.cpu_count() or 1)
+    nthreads = O.num_threads()
     counts = T.cells()["count"][T.groups()]
     order = np.random.default_rng(0).permutation(T.ngroups)
-    done, inter, t_eval, chunk = 0, 0, 0.0, max(8, O.num_threads() * 4)
+    done, inter, t_eval, chunk = 0, 0, 0.0, max(8, nthreads * 2)
     while done < T.ngroups and t_eval < budget_s:
         sel = order[done:done + chunk]
         t1 = time.perf_counter()
-        _, _, lpc, lpp = T.forces(w_full.theta, w.eps, w_full.order, groups=sel)
+        if args.tol is not None:
+            _, _, l0, l2, l4, lpp = T.forces_tol(args.tol, w.eps, groups=sel)
+            lpc = l0 + l2 + l4
+        else:
+            _, _, lpc, lpp = T.forces(w_full.theta, w.eps, w_full.order, groups=sel)
         t_eval += time.perf_counter() - t1
         inter += int((counts[sel] * (lpc + lpp)).sum())
         done += len(sel)
     frac = done / T.ngroups
     t = t_eval + t_build * frac
-    return {"value": inter / t / 1e9, "unit": "Ginteractions/s", "cores": O.num_threads(), "kind": "oracle",
-            "sample": (f"{w.name}: same generator at n={w.n}; oracle keys+sort+tree+moments in full "
-                       f"({t_build:.1f} s, charged pro rata) and walk+evaluation of {done}/{T.ngroups} "
-                       f"random sink groups ({t_eval:.1f} s), theta={w_full.theta}, order={w_full.order}"),
+    nbodies = int(counts[order[:done]].sum())
+    return {"value": inter / t / 1e9, "unit": "Ginteractions/s", "cores": nthreads, "kind": "oracle",
+            "n": w.n, "same_workload_as_gpu": w.n == w_full.n, "interactions_per_particle": inter / max(nbodies, 1),
+            "sample": (f"{w.name}, n={w.n}: oracle keys+sort+tree+groups+moments in full ({t_build:.1f} s, charged pro rata), "
+                       f"walk + evaluation of {done}/{T.ngroups} random sink groups "
+                       f"({nbodies} bodies, {t_eval:.1f} s on {nthreads} threads), theta={w_full.theta}, order={w_full.order}, double precision"),
             "seconds": t, "interactions": inter}
 
 
@@ -184,12 +225,17 @@ def run_reference(args):
     secs = sum(v["seconds"] for v in vals)
     value = inter / secs / 1e9
     base = vals[-1]
+    one = cpu_oracle_sample(args, w, budget_s=4.0, threads=1)
+    cfg = config_dict(args, w)
+    cfg["cpu_sample_n"] = base["n"]
     out = {"impl": "reference", "metric": "interactions_per_second", "value": value, "unit": "Ginteractions/s",
            "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * wall / args.steps,
            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": config_dict(args, w), "gpu_launches": 0,
+           "config": cfg, "gpu_launches": 0,
            "cpu_baseline": {"value": value, "unit": "Ginteractions/s", "cores": base["cores"], "kind": "oracle",
-                            "sample": base["sample"]},
+                            "sample": base["sample"], "n": base["n"], "same_workload_as_gpu": base["same_workload_as_gpu"],
+                            "interactions_per_particle": base["interactions_per_particle"],
+                            "value_1_thread": one["value"]},
            "e2e": {"value": value, "unit": "Ginteractions/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out))
 
@@ -306,7 +352,7 @@ def main():
     kern_s = stage["ms_eval"] * 1e-3
     achieved = flops / kern_s / 1e12
     tf_scalar, tf_packed = hot.hot_measure_fp32()  # register-only FMA chains on this device, after the timed region
-    traffic = NCU_TRAFFIC_BYTES.get(("c%d" % args.config, int(round(np.log2(w.n))), w.theta, w.order, args.nleaf, args.ncrit))
+    traffic = None if args.tol is not None else ncu_traffic(args.config, w.n, w.theta, w.order, args.nleaf, args.ncrit)
     out = {
         "metric": "interactions_per_second", "value": inter_all / (ms_max * 1e-3) / 1e9, "unit": "Ginteractions/s",
         "n_gpus": world, "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_max,
@@ -325,6 +371,8 @@ def main():
             "sort_GBps": SORT_BYTES_PER_BODY * w.n / (stage["ms_sort"] * 1e-3) / 1e9,
             "sort_GBps_survey_count": SORT_BYTES_SURVEY * w.n / (stage["ms_sort"] * 1e-3) / 1e9,
             "gather_GBps": GATHER_BYTES_PER_BODY * w.n / (stage["ms_gather"] * 1e-3) / 1e9,
+            "tree_GBps": (TREE_BYTES[0] * w.n + TREE_BYTES[1] * st["n_cells"]) / (stage["ms_tree"] * 1e-3) / 1e9,
+            "moments_GBps": (MOMENTS_BYTES[0] * w.n + MOMENTS_BYTES[1] * st["n_cells"]) / (max(stage["ms_moments"], 1e-6) * 1e-3) / 1e9,
             "walk_list_GBps": 2 * 4 * st["list_entries"] / (stage["ms_walk"] * 1e-3) / 1e9,
             "walk_Gcells_per_s": st["cells_visited"] / (stage["ms_walk"] * 1e-3) / 1e9},
         "gpu_launches": int((st["launches_build"] + st["launches_forces"]) * args.steps),
@@ -344,11 +392,19 @@ def main():
         out["hbm_stages"]["peak_GBps"] = peaks.get("hbm_gbs")
     except (OSError, ValueError):
         out["hbm_stages"]["peak_GBps"] = 6650.0
+    pk = out["hbm_stages"]["peak_GBps"]
+    out["hbm_stages"]["frac_of_peak"] = {k[:-5]: out["hbm_stages"][k] / pk for k in ("keygen_GBps", "sort_GBps", "gather_GBps", "tree_GBps", "moments_GBps")}
+    build_bytes = (KEYGEN_BYTES_PER_BODY + SORT_BYTES_PER_BODY + GATHER_BYTES_PER_BODY + TREE_BYTES[0]) * w.n + TREE_BYTES[1] * st["n_cells"]
+    out["hbm_stages"]["build_GBps"] = build_bytes / (stage["ms_build_total"] * 1e-3) / 1e9
+    out["hbm_stages"]["frac_of_peak"]["build"] = out["hbm_stages"]["build_GBps"] / pk
     if e2e:
         out["e2e"] = e2e
     if not args.no_cpu_baseline and world == 1:
         cb = cpu_oracle_sample(args, w)
-        out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample")}
+        out["cpu_baseline"] = {k: cb[k] for k in ("value", "unit", "cores", "kind", "sample", "n", "same_workload_as_gpu",
+                                                  "interactions_per_particle")}
+        out["cpu_baseline"]["value_1_thread"] = cpu_oracle_sample(args, w, budget_s=4.0, threads=1)["value"]
+        out["config"]["cpu_sample_n"] = cb["n"]
     print(json.dumps(out))
     if dist is not None:
         dist.destroy_process_group()

@@ -883,6 +883,14 @@ void orc_tree_forces_tol(orc_t *t, double tol, double eps, const int64_t *groups
         free(a); free(p);
     }
 }
+/* thread count of the OpenMP loops (bench.py times the oracle with 1 thread and with all cores) */
+void orc_set_num_threads(int n) {
+#ifdef _OPENMP
+    if (n > 0) omp_set_num_threads(n);
+#else
+    (void)n;
+#endif
+}
 int orc_num_threads(void) {
 #ifdef _OPENMP
     return omp_get_max_threads();

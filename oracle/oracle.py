@@ -148,6 +148,10 @@ def mac_bound(mom35, b, R, p):
     return lib().orc_mac_bound(_p(mom35), C.c_double(b), C.c_double(R), int(p))
 
 
+def set_num_threads(n):
+    lib().orc_set_num_threads(int(n))
+
+
 def num_threads():
     return lib().orc_num_threads()
 

@@ -311,6 +311,11 @@ def test_host_buffer_entry_point_matches_device_path(hot):
     acc, pot = hot.hot_forces(w.theta, w.eps, w.order)
     ha, hp = hot.hot_step_host(w.pos, w.mass, w.lo, w.size, w.periodic, w.theta, w.eps, w.order)
     assert (acc.cpu().numpy() == ha).all() and (pot.cpu().numpy() == hp).all()
+    # page-locked arrays (what bench.py's e2e leg passes): same bits
+    import torch
+    pa = torch.zeros((w.n, 3), dtype=torch.float32).pin_memory(); pp = torch.zeros(w.n, dtype=torch.float32).pin_memory()
+    hot.hot_step_host(w.pos, w.mass, w.lo, w.size, w.periodic, w.theta, w.eps, w.order, pa.numpy(), pp.numpy())
+    assert (pa.numpy() == ha).all() and (pp.numpy() == hp).all()
 
 
 def test_runs_on_a_user_stream(hot):
