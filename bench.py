@@ -352,6 +352,7 @@ def main():
     kern_s = stage["ms_eval"] * 1e-3
     achieved = flops / kern_s / 1e12
     tf_scalar, tf_packed = hot.hot_measure_fp32()  # register-only FMA chains on this device, after the timed region
+    tf_2reg, tf_3reg, tf_s3reg = hot.hot_measure_fp32_operands()  # the same pipe fed from the register file
     traffic = None if args.tol is not None else ncu_traffic(args.config, w.n, w.theta, w.order, args.nleaf, args.ncrit)
     out = {
         "metric": "interactions_per_second", "value": inter_all / (ms_max * 1e-3) / 1e9, "unit": "Ginteractions/s",
@@ -382,7 +383,9 @@ def main():
                      "traffic": traffic,
                      "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md Roofline); "
                                     "MEASURED_PEAKS.json holds no FP32 figure",
-                     "peak_measured_ffma_TFLOPs": {"scalar": tf_scalar, "packed_f32x2": tf_packed},
+                     "peak_measured_ffma_TFLOPs": {"scalar": tf_scalar, "packed_f32x2": tf_packed,
+                                                   "packed_2_register_sources": tf_2reg, "packed_3_register_sources": tf_3reg,
+                                                   "scalar_3_register_sources": tf_s3reg},
                      "frac_of_measured_ffma": achieved / max(tf_scalar, tf_packed),
                      "flops_per_interaction": {"pp": FLOPS_PP, "pc": FLOPS_PC[w.order]},
                      "kernel_ms": stage["ms_eval"], "kernel_share_of_step": stage["ms_eval"] / ms_max},

@@ -137,6 +137,11 @@ const char* hot_last_error(void);
  * register-only fused-multiply-add chain, scalar (FFMA) and packed pairs (FFMA2); FMA = 2 flops.
  * ~10 ms of device time on the library's stream.  Outputs: host. */
 int hot_measure_fp32(double* tflops_scalar, double* tflops_packed);
+/* The same pipe fed from the register file, which delivers 64 bits per lane and clock: TFLOP/s of fused multiply-adds
+ * whose sources are [0] packed pairs, two different registers (a*a+d), [1] packed pairs, three different registers
+ * (a*b+d), [2] scalar, three different registers.  [1] and [2] fall to 2/3 of the peak: the ceiling of the inner loops
+ * of the interaction kernels, most of whose operands are per-sink registers.  tflops3: host, [3]. */
+int hot_measure_fp32_operands(double* tflops3);
 
 /* Host-only, needs no GPU: the 165 Taylor coefficients c_abc (a+b+c <= 8, degree-major, x exponent
  * descending then y; odd ones are zero) of psi_sm(r) = psi(r) - sum_{|n|_inf<=2} 1/|r-n| about r = 0, in

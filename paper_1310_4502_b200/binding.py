@@ -64,6 +64,7 @@ def _load():
         lib.hot_set_list_arena.argtypes = [C.c_int64]
         lib.hot_far_coefficients.argtypes = [C.c_void_p]
         lib.hot_measure_fp32.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        lib.hot_measure_fp32_operands.argtypes = [C.POINTER(C.c_double)]
         lib.hot_free.restype = None
         lib.hot_export_keys.argtypes = [C.c_void_p, C.c_void_p]
         lib.hot_export_cells.argtypes = [C.c_void_p] * 6 + [C.c_int64, C.POINTER(C.c_int64)]
@@ -103,6 +104,13 @@ def hot_measure_fp32():
     a, b = C.c_double(), C.c_double()
     _check(_load().hot_measure_fp32(C.byref(a), C.byref(b)))
     return a.value, b.value
+
+
+def hot_measure_fp32_operands():
+    """TFLOP/s of FMAs reading (packed, 2 registers), (packed, 3 registers), (scalar, 3 registers) per instruction."""
+    out = (C.c_double * 3)()
+    _check(_load().hot_measure_fp32_operands(out))
+    return tuple(out)
 
 
 def hot_far_coefficients() -> np.ndarray:

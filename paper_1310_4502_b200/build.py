@@ -28,16 +28,11 @@ def _newest_dep() -> float:
     return max(os.path.getmtime(p) for p in deps)
 
 
-def _extra_flags():
-    """extra nvcc flags for tuning sweeps (e.g. HOT_NVCC_EXTRA="-DHOT_SMAX=6"); empty in normal builds"""
-    return os.environ.get("HOT_NVCC_EXTRA", "").split()
-
-
 def _compile(src: str) -> str:
     obj = os.path.join(OBJ, src.replace(".cu", ".o"))
     if os.path.exists(obj) and os.path.getmtime(obj) >= _newest_dep():
         return obj
-    cmd = ["nvcc", *NVCC_FLAGS, *_extra_flags(), "-c", os.path.join(CSRC, src), "-o", obj]
+    cmd = ["nvcc", *NVCC_FLAGS, "-c", os.path.join(CSRC, src), "-o", obj]
     r = subprocess.run(cmd, capture_output=True, text=True)
     if r.returncode != 0:
         raise RuntimeError(f"nvcc failed for {src}:\n{r.stdout}\n{r.stderr}")

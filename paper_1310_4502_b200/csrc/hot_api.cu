@@ -9,8 +9,6 @@
 #include "hot_internal.h"
 
 long long g_hot_launches = 0;
-unsigned long long g_hot_dbg_mask = ~0ull;
-int g_hot_sb_shift = 16; // groups per superblock of the interaction kernel's work-item order (hot_forces.cu), log2
 
 namespace {
 
@@ -140,9 +138,6 @@ float ms_between(cudaEvent_t a, cudaEvent_t b) {
 
 extern "C" {
 
-int hot_debug_set_mask(unsigned long long m) { g_hot_dbg_mask = m; return HOT_OK; }
-int hot_debug_set_sb_shift(int s) { if (s < 8 || s > 30) return HOT_EINVAL; g_hot_sb_shift = s; return HOT_OK; } // TEMP sweep hook
-
 const char* hot_last_error(void) { return g.err; }
 
 int hot_set_stream(void* s) {
@@ -153,6 +148,12 @@ int hot_set_stream(void* s) {
 int hot_measure_fp32(double* tflops_scalar, double* tflops_packed) {
     if (!tflops_scalar || !tflops_packed) return fail(HOT_EINVAL, "hot_measure_fp32: NULL output");
     CUDA_TRY(measure_fp32(tflops_scalar, tflops_packed, g.stream));
+    return HOT_OK;
+}
+
+int hot_measure_fp32_operands(double* tflops3) {
+    if (!tflops3) return fail(HOT_EINVAL, "hot_measure_fp32_operands: NULL output");
+    CUDA_TRY(measure_fp32_operands(tflops3, g.stream));
     return HOT_OK;
 }
 
@@ -404,7 +405,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     a.far = t.periodic ? t.far : nullptr;
     a.seg = -1; a.lpc0 = t.glpc0; a.lpc2 = t.glpc2; a.do_pp = 1; a.accumulate = 0;
     a.acc = acc; a.pot = pot; a.counter = g.d_counter + 1;
-    a.sb_shift = g_hot_sb_shift; a.dbg_mask = g_hot_dbg_mask;
+    a.sb_shift = 16; // 2^16 sink groups per superblock of the work-item order (hot_forces.cu; 2^13 ... whole set measured equal, smaller slower)
     CUDA_TRY(tree_alloc(&g.d_cls, plan_cls_elems(ng, a.sb_shift)));
     a.cls = g.d_cls;
     CUDA_TRY(tree_alloc(&g.d_items, (size_t)(HOT_MAX_NCRIT / 64 + 2) * (size_t)ng)); // passes per group: full ones of >= 64 sinks, one split in two

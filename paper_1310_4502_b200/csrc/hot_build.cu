@@ -122,9 +122,7 @@ cudaError_t launch_keygen(const float* pos, const float* mass, int64_t n, float 
 // then two look-back state arrays of 256 words per tile (a pass uses one and clears the other).
 // ------------------------------------------------------------------------------------------
 #define SORT_THREADS 256
-#ifndef SORT_ITEMS
 #define SORT_ITEMS 16
-#endif
 #define SORT_TILE (SORT_THREADS * SORT_ITEMS)
 #define SORT_WARPS (SORT_THREADS / 32)
 #define SORT_STATE0 4352
@@ -191,12 +189,8 @@ __global__ void __launch_bounds__(1024) scan_rows_kernel(uint32_t* __restrict__ 
 // Stable scatter of one tile.  PASS is a template parameter so that a digit is one byte of one key half (PRMT);
 // FULLT marks a full tile (every tile but the last): no per-key bounds predicates.
 // Shared memory: the digit-ordered tile (keys 32 KB + values 16 KB, dynamic) and 10.5 KB of counters.
-#ifndef SORT_MINBLK
-#define SORT_MINBLK 3
-#endif
-#ifndef SORT_LOOK
-#define SORT_LOOK 4
-#endif
+#define SORT_MINBLK 3  // resident tiles per SM (tile-size sweep in DESIGN.md)
+#define SORT_LOOK 4    // earlier tiles read per look-back round trip
 #define SORT_SMEM_BYTES (SORT_TILE * 12)
 template <int PASS> __device__ __forceinline__ uint32_t sort_digit(uint64_t k) {
     const uint32_t h = PASS < 4 ? (uint32_t)k : (uint32_t)(k >> 32);

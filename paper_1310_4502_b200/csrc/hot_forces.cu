@@ -21,27 +21,11 @@
 
 #define FULL 0xffffffffu
 #define BATCH 32               // sources per staged batch
-#ifndef WARPS_PER_BLOCK
-#define WARPS_PER_BLOCK 4
-#endif
-#ifndef HOT_FLUSH_N
-#define HOT_FLUSH_N 64     // sources a lane sums in fp32 before the partial sums go to the fp64 running sums
-#endif
-#ifndef HOT_SMAX
-#define HOT_SMAX 6             // sinks per lane (tunable 2..8; 6 at 3 blocks/SM measured best with NCRIT >= 128)
-#endif
-#define SMAX HOT_SMAX
-#ifndef HOT_PP_UNROLL
-#define HOT_PP_UNROLL 2
-#endif
-#define HOT_STR(x) #x
-#define HOT_UNROLL(n) _Pragma(HOT_STR(unroll n))
-#ifndef HOT_UNROLL2_S
-#define HOT_UNROLL2_S 6
-#endif
-#ifndef HOT_MINBLK
-#define HOT_MINBLK 3           // resident blocks per SM the order 0/2 kernels are compiled for
-#endif
+#define WARPS_PER_BLOCK 4      // 3 blocks per SM at 166 registers (5 warps at 128 registers measured slower)
+#define FLUSH_N 64             // sources a lane sums in fp32 before the partial sums go to the fp64 running sums
+#define SMAX 6                 // sinks per lane (measured: 6 at 3 blocks/SM beats 4 at 4 and 8 at 2, NCRIT >= 128)
+#define UNROLL2_S 6            // two sources per loop trip for this many sinks per lane and more (more variants unrolled: slower, instruction cache)
+#define MINBLK 3               // resident blocks per SM the kernels are compiled for
 
 template <int ORDER> struct PCQ { static constexpr int v = ORDER >= 4 ? 12 : (ORDER >= 2 ? 3 : 1); }; // float4 per staged cell
 
@@ -67,15 +51,10 @@ struct f2 { unsigned long long v; };
 __device__ __forceinline__ f2 mk2(float lo, float hi) { f2 r; asm("mov.b64 %0, {%1, %2};" : "=l"(r.v) : "f"(lo), "f"(hi)); return r; }
 __device__ __forceinline__ float lo2(f2 a) { float x; asm("{ .reg .f32 t; mov.b64 {%0, t}, %1; }" : "=f"(x) : "l"(a.v)); return x; }
 __device__ __forceinline__ float hi2(f2 a) { float y; asm("{ .reg .f32 t; mov.b64 {t, %0}, %1; }" : "=f"(y) : "l"(a.v)); return y; }
-#ifdef HOT_ASM_VOLATILE
-#define HOT_ASM asm volatile
-#else
-#define HOT_ASM asm
-#endif
-__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; HOT_ASM("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; HOT_ASM("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; HOT_ASM("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
-__device__ __forceinline__ f2 vfma(f2 a, f2 b, f2 c) { f2 r; HOT_ASM("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
+__device__ __forceinline__ f2 operator+(f2 a, f2 b) { f2 r; asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ f2 operator-(f2 a, f2 b) { f2 r; asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ f2 operator*(f2 a, f2 b) { f2 r; asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r.v) : "l"(a.v), "l"(b.v)); return r; }
+__device__ __forceinline__ f2 vfma(f2 a, f2 b, f2 c) { f2 r; asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r.v) : "l"(a.v), "l"(b.v), "l"(c.v)); return r; }
 __device__ __forceinline__ float vfma(float a, float b, float c) { return fmaf(a, b, c); }
 __device__ __forceinline__ f2 vrsqrt(f2 a) { return mk2(rsqrt_approx(lo2(a)), rsqrt_approx(hi2(a))); }
 __device__ __forceinline__ float vrsqrt(float a) { return rsqrt_approx(a); }
@@ -200,134 +179,6 @@ __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const f
     a[3] = a[3] + ph;
 }
 
-// ---- all NP sink pairs of a lane against one source, instruction order chosen for the operand-reuse cache ----------
-// A packed instruction that reads three different registers occupies the FP32 pipe for three cycles instead of two
-// (measured).  An operand that the previous instruction used in the same position comes
-// from the reuse cache instead.  The same arithmetic as pp_one / pc_one per pair, written so that consecutive
-// instructions share either the source's scalar (across the pairs) or a per-pair quantity (across the components).
-#ifdef HOT_BLOCK_ORDER
-template <int NP>
-__device__ __forceinline__ void pp_block(const float4 ns, const f2 (&x)[NP][3], const float eps2, f2 (&a)[NP][4]) {
-    f2 d[NP][3], r2[NP], ri[NP], nmr[NP], nmr3[NP];
-    const f2 sx = splat<f2>(ns.x), sy = splat<f2>(ns.y), sz = splat<f2>(ns.z), sw = splat<f2>(ns.w), e2 = splat<f2>(eps2);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) d[p][2] = x[p][2] + sz;
-#pragma unroll
-    for (int p = 0; p < NP; ++p) d[p][1] = x[p][1] + sy;
-#pragma unroll
-    for (int p = 0; p < NP; ++p) d[p][0] = x[p][0] + sx;
-#pragma unroll
-    for (int p = 0; p < NP; ++p) r2[p] = vfma(d[p][2], d[p][2], e2);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) r2[p] = vfma(d[p][1], d[p][1], r2[p]);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) r2[p] = vfma(d[p][0], d[p][0], r2[p]);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) ri[p] = vrsqrt(r2[p]);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) nmr[p] = sw * ri[p];
-#pragma unroll
-    for (int p = 0; p < NP; ++p) { const f2 ri2 = ri[p] * ri[p]; nmr3[p] = nmr[p] * ri2; }
-#pragma unroll
-    for (int p = 0; p < NP; ++p) {
-        a[p][0] = vfma(nmr3[p], d[p][0], a[p][0]);
-        a[p][1] = vfma(nmr3[p], d[p][1], a[p][1]);
-        a[p][2] = vfma(nmr3[p], d[p][2], a[p][2]);
-        a[p][3] = a[p][3] + nmr[p];
-    }
-}
-template <int ORDER, int NP>
-__device__ __forceinline__ void pc_block(const float4 q0, const float4 q1, const float4 q2, const f2 (&x)[NP][3], const float eps2, f2 (&a)[NP][4]) {
-    static_assert(ORDER <= 2, "orders 0 and 2");
-    f2 R[NP][3], u[NP], ri[NP], ri2[NP], ri3[NP];
-    const f2 e2 = splat<f2>(eps2), nm0 = splat<f2>(q0.w);
-    { const f2 s = splat<f2>(q0.z);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) R[p][2] = x[p][2] + s; }
-    { const f2 s = splat<f2>(q0.y);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) R[p][1] = x[p][1] + s; }
-    { const f2 s = splat<f2>(q0.x);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) R[p][0] = x[p][0] + s; }
-#pragma unroll
-    for (int p = 0; p < NP; ++p) u[p] = vfma(R[p][2], R[p][2], e2);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) u[p] = vfma(R[p][1], R[p][1], u[p]);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) u[p] = vfma(R[p][0], R[p][0], u[p]);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) ri[p] = vrsqrt(u[p]);
-#pragma unroll
-    for (int p = 0; p < NP; ++p) { ri2[p] = ri[p] * ri[p]; ri3[p] = ri[p] * ri2[p]; }
-    if (ORDER < 2) {
-#pragma unroll
-        for (int p = 0; p < NP; ++p) {
-            const f2 c = nm0 * ri3[p];
-            a[p][0] = vfma(c, R[p][0], a[p][0]); a[p][1] = vfma(c, R[p][1], a[p][1]); a[p][2] = vfma(c, R[p][2], a[p][2]);
-        }
-#pragma unroll
-        for (int p = 0; p < NP; ++p) a[p][3] = vfma(nm0, ri[p], a[p][3]);
-        return;
-    }
-    // M = N R with N = 3 M2 (symmetric): column l of N times R_l, the scalar shared by the pairs, snake over (k, p)
-    f2 M[NP][3];
-    { const f2 nxx = splat<f2>(q1.x), nxy = splat<f2>(q1.y), nxz = splat<f2>(q1.z), nyy = splat<f2>(q1.w), nyz = splat<f2>(q2.x), nzz = splat<f2>(q2.y);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) M[p][0] = nxz * R[p][2];
-#pragma unroll
-      for (int p = NP - 1; p >= 0; --p) M[p][1] = nyz * R[p][2];
-#pragma unroll
-      for (int p = 0; p < NP; ++p) M[p][2] = nzz * R[p][2];
-#pragma unroll
-      for (int p = NP - 1; p >= 0; --p) M[p][2] = vfma(nyz, R[p][1], M[p][2]);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) M[p][1] = vfma(nyy, R[p][1], M[p][1]);
-#pragma unroll
-      for (int p = NP - 1; p >= 0; --p) M[p][0] = vfma(nxy, R[p][1], M[p][0]);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) M[p][0] = vfma(nxx, R[p][0], M[p][0]);
-#pragma unroll
-      for (int p = NP - 1; p >= 0; --p) M[p][1] = vfma(nxy, R[p][0], M[p][1]);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) M[p][2] = vfma(nxz, R[p][0], M[p][2]);
-    }
-    f2 ri5[NP], cR[NP], ph[NP];
-#pragma unroll
-    for (int p = 0; p < NP; ++p) ri5[p] = ri3[p] * ri2[p];
-    { const f2 t15 = splat<f2>(q2.z), t05 = splat<f2>(q2.w);
-#pragma unroll
-      for (int p = 0; p < NP; ++p) cR[p] = nm0 * ri3[p];
-#pragma unroll
-      for (int p = NP - 1; p >= 0; --p) ph[p] = nm0 * ri[p];
-#pragma unroll
-      for (int p = 0; p < NP; ++p) ph[p] = vfma(t05, ri3[p], ph[p]);
-#pragma unroll
-      for (int p = NP - 1; p >= 0; --p) cR[p] = vfma(t15, ri5[p], cR[p]);
-    }
-#pragma unroll
-    for (int p = 0; p < NP; ++p) {
-        f2 Q2 = M[p][0] * R[p][0];
-        Q2 = vfma(M[p][1], R[p][1], Q2);
-        Q2 = vfma(M[p][2], R[p][2], Q2);
-        const f2 hQ = ri5[p] * Q2;                       // 3 u^-5/2 (R M2 R)
-        const f2 w7 = splat<f2>(-2.5f) * ri2[p];
-        cR[p] = vfma(hQ, w7, cR[p]);
-        ph[p] = vfma(splat<f2>(-0.5f), hQ, ph[p]);
-    }
-#pragma unroll
-    for (int p = 0; p < NP; ++p) {
-        a[p][0] = vfma(ri5[p], M[p][0], a[p][0]);
-        a[p][1] = vfma(ri5[p], M[p][1], a[p][1]);
-        a[p][2] = vfma(ri5[p], M[p][2], a[p][2]);
-        a[p][0] = vfma(cR[p], R[p][0], a[p][0]);
-        a[p][1] = vfma(cR[p], R[p][1], a[p][1]);
-        a[p][2] = vfma(cR[p], R[p][2], a[p][2]);
-        a[p][3] = a[p][3] + ph[p];
-    }
-}
-#endif
-
 // ---- the sinks of one lane: NP pairs + (S odd) one scalar ------------------------------------------
 template <int S> struct Sinks {
     static constexpr int NP = S / 2, TAIL = S & 1;
@@ -353,12 +204,8 @@ template <int S> struct Sinks {
         return (i & 1) ? hi2(a2[i >> 1][k]) : lo2(a2[i >> 1][k]);
     }
     __device__ __forceinline__ void pp(const float4 ns, float eps2) {
-#ifdef HOT_BLOCK_ORDER
-        if (NP) pp_block<NP ? NP : 1>(ns, x2, eps2, a2);
-#else
 #pragma unroll
         for (int p = 0; p < NP; ++p) pp_one<f2>(ns, x2[p], eps2, a2[p]);
-#endif
         if (TAIL) pp_one<float>(ns, x1, eps2, a1);
     }
     // the group's own bodies: the same packed arithmetic, the j = i slot masked by index through ri = 0 (works for eps = 0)
@@ -377,11 +224,6 @@ template <int S> struct Sinks {
     }
     template <int ORDER>
     __device__ __forceinline__ void pc(const float4 q0, const float4 q1, const float4 q2, const float* m, float eps2) {
-#ifdef HOT_BLOCK_ORDER
-        if (ORDER <= 2) {
-            if (NP) pc_block<(ORDER <= 2 ? ORDER : 2), NP ? NP : 1>(q0, q1, q2, x2, eps2, a2);
-        } else
-#endif
 #pragma unroll
         for (int p = 0; p < NP; ++p) pc_one<ORDER, f2>(q0, q1, q2, m, x2[p], eps2, a2[p]);
         if (TAIL) pc_one<ORDER, float>(q0, q1, q2, m, x1, eps2, a1);
@@ -520,7 +362,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 int j = strm;
                 float4 n0 = st[j < cnt ? j : 0], n1 = n0, n2 = n0;
                 if (ORDER >= 2) { n1 = st[32 + (j < cnt ? j : 0)]; n2 = st[64 + (j < cnt ? j : 0)]; }
-                if (S >= HOT_UNROLL2_S) { // two sources per trip: the sums stay in their registers (no copies at the loop end)
+                if (S >= UNROLL2_S) { // two sources per trip: the sums stay in their registers (no copies at the loop end)
 #pragma unroll 2
                 while (j < cnt) {
                     const float4 q0 = n0, q1 = n1, q2 = n2;
@@ -555,7 +397,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 }
             }
             nacc += (cnt + K - 1) >> lgK;
-            if (nacc >= HOT_FLUSH_N) flush();
+            if (nacc >= FLUSH_N) flush();
         }
         __syncwarp();
     }
@@ -589,7 +431,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
             {
                 int j = strm;
                 float4 nx = st[j < cnt ? j : 0];
-HOT_UNROLL(HOT_PP_UNROLL)
+#pragma unroll 2
                 while (j < cnt) {
                     const float4 sb = nx;
                     j += K;
@@ -598,7 +440,7 @@ HOT_UNROLL(HOT_PP_UNROLL)
                 }
             }
             nacc += (cnt + K - 1) >> lgK;
-            if (nacc >= HOT_FLUSH_N) flush();
+            if (nacc >= FLUSH_N) flush();
         }
         __syncwarp();
     }
@@ -644,29 +486,12 @@ __device__ __forceinline__ void run_chunk(const ForceArgs& P, const int w, const
                                           const uint32_t nc, const int lgL, const int lane) {
     const int S = (int)((nc + (1u << lgL) - 1) >> lgL);
     if (S <= 1) eval_chunk<ORDER, PER, 1>(P, w, g, gi, c0, nc, lgL, lane);
-#if SMAX <= 2
-    else eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
-#elif SMAX <= 3
-    else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
-    else eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
-#else
     else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
     else if (S == 3) eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
-#endif
-#if SMAX <= 3
-#elif SMAX <= 4
-    else eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
-#else
     else if (S == 4) eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
     else if (S == 5) eval_chunk<ORDER, PER, 5>(P, w, g, gi, c0, nc, lgL, lane);
-#if SMAX <= 6
     else eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
-#else
-    else if (S == 6) eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 7) eval_chunk<ORDER, PER, 7>(P, w, g, gi, c0, nc, lgL, lane);
-    else eval_chunk<ORDER, PER, 8>(P, w, g, gi, c0, nc, lgL, lane);
-#endif
-#endif
+    static_assert(SMAX == 6, "one eval_chunk instance per sinks-per-lane count");
 }
 // smallest stream width that holds n sinks with at most SMAX per lane
 __device__ __forceinline__ int fit_lgL(uint32_t n) {
@@ -676,12 +501,10 @@ __device__ __forceinline__ int fit_lgL(uint32_t n) {
 }
 // Relative time of a pass: L lanes per stream each spend (PLAN_A + PLAN_B * S) per source, 32 / L sources at a time;
 // PLAN_C is what a pass costs whatever its sinks (list reads, staging of the sources).
-#ifndef HOT_PLAN_A
-#define HOT_PLAN_A 1
-#define HOT_PLAN_B 3
-#define HOT_PLAN_C 12
-#endif
-__device__ __forceinline__ int pass_cost(int lgL, uint32_t n) { return (HOT_PLAN_A + HOT_PLAN_B * (int)((n + (1u << lgL) - 1) >> lgL)) << lgL; }
+#define PLAN_A 1
+#define PLAN_B 3
+#define PLAN_C 12
+__device__ __forceinline__ int pass_cost(int lgL, uint32_t n) { return (PLAN_A + PLAN_B * (int)((n + (1u << lgL) - 1) >> lgL)) << lgL; }
 
 // The passes of one group.  Sinks in passes of at most 32*SMAX (full passes first: 6 sinks per lane is the most
 // efficient blocking, measured against an even split).  The last nc sinks: one pass with ceil(nc / L) sinks per lane
@@ -700,7 +523,7 @@ __device__ __forceinline__ void plan_group(const uint32_t count, F&& emit) {
             if (sf < 1 || sf > SMAX) continue;
             const uint32_t r = nc - (sf << lg);
             if (r == 0) continue; // an exact fit is the single pass already
-            const int c = pass_cost(lg, sf << lg) + pass_cost(fit_lgL(r), r) + HOT_PLAN_C;
+            const int c = pass_cost(lg, sf << lg) + pass_cost(fit_lgL(r), r) + PLAN_C;
             if (c < best) { best = c; lgL = lg; nmain = sf << lg; }
         }
         emit(c0, nmain, lgL);
@@ -767,7 +590,7 @@ cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st) {
 #endif
 
 template <int ORDER, bool PER>
-__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
+__global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned int total = P.cls[24 * P.nsb];
     while (true) {
@@ -776,9 +599,6 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : HOT_MIN
         q = __shfl_sync(FULL, q, 0);
         if (q >= total) break;
         const uint4 it = P.items[q];
-#ifdef HOT_DEBUG_HOOKS
-        { const int S_ = (int)((it.z + (1u << it.w) - 1) >> it.w); if (!((P.dbg_mask >> (S_ + 8 * (int)it.w)) & 1ull)) continue; }
-#endif
         const int64_t gi = P.g0 + (int64_t)it.x;
         run_chunk<ORDER, PER>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
     }

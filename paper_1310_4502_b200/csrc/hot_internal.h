@@ -11,9 +11,7 @@ extern long long g_hot_launches; // kernels launched by the library since the la
 
 #define HOT_MAXLEVEL 21
 #define HOT_NLEVELS 22        // levels 0..21
-#ifndef HOT_MAX_NCRIT
 #define HOT_MAX_NCRIT 256
-#endif
 #define HOT_MAX_NLEAF 32
 
 // 16-byte record the walk reads per visited cell (S7).
@@ -117,9 +115,7 @@ cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st);
 // Periodic boxes: accepted cells of levels <= HOT_COARSE_LEVEL carry HOT_COARSE_FLAG in the cell list.  They are
 // few (~1250 per group at theta = 0.5) but hold the large, nearly cancelling part of the image sum, so their
 // monopole terms are evaluated in fp64 by coarse_monopole_kernel and left out of the fp32 kernel (R-14).
-#ifndef HOT_COARSE_LEVEL
 #define HOT_COARSE_LEVEL 3
-#endif
 #define HOT_COARSE_FLAG 0x80000000u
 struct WalkArgs {
     const WalkCell* wcell; const GroupRec* group; int64_t g0, g1;
@@ -164,7 +160,6 @@ struct ForceArgs {
     unsigned int* cls;            // plan_cls_elems(g1 - g0, sb_shift) words: per-(superblock, class) counts, starts, cursors, total
     // tolerance mode: one launch per order over its segment of the cell lists (seg = 0, 1, 2; -1: the whole list)
     int seg; const uint32_t *lpc0, *lpc2; int do_pp, accumulate;
-    unsigned long long dbg_mask; // HOT_DEBUG_HOOKS builds only: bit (S + 8 lgL) enables the class
     int sb_shift; unsigned int nsb; // 2^sb_shift groups per superblock (>= 8), number of superblocks of [g0, g1)
 };
 size_t plan_cls_elems(int64_t ngroups, int sb_shift);
@@ -181,3 +176,4 @@ cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, doubl
 
 // ---- FP32 roofline denominator measured on the device (hot_peak.cu) ------------------------------------
 cudaError_t measure_fp32(double* tf_scalar, double* tf_packed, cudaStream_t st);
+cudaError_t measure_fp32_operands(double* tf3, cudaStream_t st); // packed 2 register reads, packed 3, scalar 3
