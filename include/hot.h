@@ -124,6 +124,20 @@ int hot_forces_tol(double tol, double eps, float* acc, float* pot);
 
 int hot_stats(hot_stats_t* out);
 
+/* Softening kernel of the following hot_forces / hot_forces_tol calls ("Plummer or spline [50] kernel").
+ * 0 (default): Plummer, g = (r^2 + eps^2)^(-1/2), also inside the expansions of accepted cells.
+ * 1: the cubic-spline kernel of ref [50] with h = 2.8 eps (same central potential -m/eps): a body is a ball of radius
+ *    h; pairs closer than h use the kernel's closed form, everything else is Newtonian.  An accepted cell must lie
+ *    wholly beyond h from the sink group (integer geometry as in R-7; R-17), so the lists depend on eps.
+ * (The compensating K1 kernel of ref [13], is not built: its formula is not in the paper.) */
+int hot_set_softening(int kind);
+
+/* The "kick" and "drift" operators of the leapfrog around the force call: vel += acc * dt_kick, then
+ * pos += vel * dt_drift, one fp32 fused multiply-add each; periodic != 0 wraps pos into [lo, lo + size).  In a
+ * comoving background the two factors are integrals over the expansion history: the caller's.
+ * pos, vel: device, [n][3] fp32, updated in place; acc: device, [n][3]. */
+int hot_kick_drift(float* pos, float* vel, const float* acc, int64_t n, float dt_kick, float dt_drift, hot_box box, int periodic);
+
 /* Same path with HOST buffers: copies pos/mass to the device, hot_build, hot_forces, copies acc
  * (and pot unless NULL) back; returns after the results are in host memory. */
 int hot_step_host(const float* pos, const float* mass, int64_t n, hot_box box, int periodic,

@@ -83,6 +83,7 @@ static void mi_init(void) {
             }
     MI_READY = 1;
 }
+static int g_soft_kind = 0; /* softening kernel of every routine that takes eps: 0 Plummer, 1 cubic spline (f-4, below) */
 static double factorial(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
 
 /* ------------------------------------------------------------------------------------------
@@ -404,7 +405,7 @@ double orc_dg(int a, int b, int c, const double R[3], double eps) {
 static void cell_on_sink(const double *mo, const double z[3], int order, const double x[3],
                          double eps2, double acc[3], double *pot) {
     double R[3] = {x[0] - z[0], x[1] - z[1], x[2] - z[2]}, D[8];
-    make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + eps2, D, order + 1);
+    make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + (g_soft_kind == 1 ? 0.0 : eps2), D, order + 1);
     for (int k = 0; k < ORC_NMOM; ++k) {
         int a = MI_A[k], b = MI_B[k], c = MI_C[k], n = a + b + c;
         if (n > order) break;
@@ -416,10 +417,39 @@ static void cell_on_sink(const double *mo, const double z[3], int order, const d
         acc[2] += w * dg(a, b, c + 1, R, D);
     }
 }
-/* C-1 summand (eq (2) right-hand side, Plummer-softened): source (y,m) on sink x */
+/* f-4 ("Plummer or spline [50] kernel"): the cubic-spline kernel.  A body is a ball of radius h with
+ * density W(u) = 8/(pi h^3) (1 - 6u^2 + 6u^3) for u = r/h <= 1/2, 16/(pi h^3) (1-u)^3 for u <= 1; its field at
+ * distance r is  m (y - x) fac(r),  phi = m pot(r)  with, from integrating W (enclosed mass and outer shells):
+ *   u <= 1/2: fac h^3 = 32/3 - 192/5 u^2 + 32 u^3,                      pot h = -14/5 + 16/3 u^2 - 48/5 u^4 + 32/5 u^5
+ *   u <= 1  : fac h^3 = 64/3 - 48 u + 192/5 u^2 - 32/3 u^3 - 1/(15 u^3), pot h = -16/5 + 1/(15u) + 32/3 u^2 - 16 u^3 + 48/5 u^4 - 32/15 u^5
+ *   u >  1  : Newtonian.   h = 2.8 eps makes phi(0) = -m/eps as for Plummer softening.
+ * orc_set_softening(1) selects it for every routine that takes eps (direct sum, tree); expansions of accepted cells are
+ * then Newtonian, and a cell is accepted only if its cube is farther than h from the group's cube (R-17). */
+void orc_set_softening(int kind) { g_soft_kind = kind; }
+void orc_spline_kernel(double r, double h, double *fac, double *pot) {
+    double u = r / h;
+    if (u >= 1.0) { *fac = 1.0 / (r * r * r); *pot = -1.0 / r; return; }
+    double u2 = u * u, u3 = u2 * u, h3 = h * h * h;
+    if (u <= 0.5) {
+        *fac = (32.0 / 3.0 - 192.0 / 5.0 * u2 + 32.0 * u3) / h3;
+        *pot = (-14.0 / 5.0 + 16.0 / 3.0 * u2 - 48.0 / 5.0 * u2 * u2 + 32.0 / 5.0 * u2 * u3) / h;
+    } else {
+        *fac = (64.0 / 3.0 - 48.0 * u + 192.0 / 5.0 * u2 - 32.0 / 3.0 * u3 - 1.0 / (15.0 * u3)) / h3;
+        *pot = (-16.0 / 5.0 + 1.0 / (15.0 * u) + 32.0 / 3.0 * u2 - 16.0 * u3 + 48.0 / 5.0 * u2 * u2 - 32.0 / 15.0 * u2 * u3) / h;
+    }
+}
+/* C-1 summand (eq (2) right-hand side, softened): source (y,m) on sink x */
 static void body_on_sink(const double y[3], double m, const double x[3], double eps2,
                          double acc[3], double *pot) {
     double d[3] = {y[0] - x[0], y[1] - x[1], y[2] - x[2]};
+    if (g_soft_kind == 1) {
+        double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]), h = 2.8 * sqrt(eps2), fac, pp;
+        if (r == 0 && h == 0) return; /* coincident, unsoftened: skipped like the self term */
+        orc_spline_kernel(r, h, &fac, &pp);
+        for (int k = 0; k < 3; ++k) acc[k] += m * d[k] * fac;
+        *pot += m * pp;
+        return;
+    }
     double u = d[0] * d[0] + d[1] * d[1] + d[2] * d[2] + eps2;
     double ri = 1.0 / sqrt(u), ri3 = ri / u;
     for (int k = 0; k < 3; ++k) acc[k] += m * d[k] * ri3;
@@ -476,6 +506,8 @@ typedef struct {
     int64_t *pc, *pp; int64_t cap;   /* optional lists: accepted cells / rejected leaves */
     int64_t nleafrej;
     uint8_t *mark;                   /* optional: set to 1 for every accepted cell */
+    double hreal;                    /* spline softening: h = 2.8 eps in the caller's units */
+    double hgrid2;                   /* spline softening: (h / grid spacing)^2; an accepted cell lies beyond h (R-17) */
     int tolmode; double tol; double gc[3], gh; /* error-bound MAC: tolerance, group cube centre and half side */
     int64_t npc_o[3];                /* accepted cells by order: monopole, quadrupole, hexadecapole */
     /* evaluation */
@@ -496,6 +528,7 @@ static int mac_accept(const walk_t *w, int64_t c) {
         if (g < 0) g = 0;
         d2 += (uint64_t)(g * g);
     }
+    if (g_soft_kind == 1 && !((double)d2 > w->hgrid2)) return 0;
     return (double)((uint64_t)(s * s)) < w->theta2 * (double)d2;
 }
 /* ------------------------------------------------------------------------------------------
@@ -529,6 +562,7 @@ static int mac_tol(const walk_t *w, int64_t c) {
         if (g > 0) d2 += g * g;
     }
     double R = sqrt(d2), b = t->bbound[c];
+    if (g_soft_kind == 1 && !(R - b > w->hreal)) return -1; /* every body of the cell beyond h from every sink (R-17) */
     const double *mo = t->mom + (size_t)c * ORC_NMOM;
     if (orc_mac_bound(mo, b, R, 1) <= w->tol) return 0;
     if (orc_mac_bound(mo, b, R, 2) <= w->tol) return 2;
@@ -803,7 +837,7 @@ void orc_tree_forces(orc_t *t, double theta, double eps, int order, const int64_
             for (int ix = -ws; ix <= ws; ++ix) for (int iy = -ws; iy <= ws; ++iy) for (int iz = -ws; iz <= ws; ++iz) {
                 walk_t w; walk_setup(&w, t, theta, groups ? groups[q] : q);
                 w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
-                w.mark = need;
+                w.mark = need; w.hreal = 2.8 * eps; w.hgrid2 = (w.hreal * 2097152.0 / t->size) * (w.hreal * 2097152.0 / t->size);
                 walk_rec(&w, 0);
             }
 #pragma omp parallel for schedule(dynamic, 1)
@@ -822,6 +856,7 @@ void orc_tree_forces(orc_t *t, double theta, double eps, int order, const int64_
             w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
             w.shx[0] = ix * t->size; w.shx[1] = iy * t->size; w.shx[2] = iz * t->size;
             w.eval = 1; w.order = order; w.eps2 = eps * eps; w.acc = a; w.pot = p;
+            w.hreal = 2.8 * eps; w.hgrid2 = (w.hreal * 2097152.0 / t->size) * (w.hreal * 2097152.0 / t->size);
             walk_rec(&w, 0);
             npc += w.npc; npp += w.npp;
         }
@@ -858,6 +893,7 @@ void orc_tree_forces_tol(orc_t *t, double tol, double eps, const int64_t *groups
             w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
             w.shx[0] = ix * t->size; w.shx[1] = iy * t->size; w.shx[2] = iz * t->size;
             w.eval = acc != NULL; w.eps2 = eps * eps; w.acc = a; w.pot = p;
+            w.hreal = 2.8 * eps; w.hgrid2 = (w.hreal * 2097152.0 / t->size) * (w.hreal * 2097152.0 / t->size);
             w.tolmode = 1; w.tol = tol;
             double h = t->size / 2097152.0; /* grid spacing: the group's cube from its integer corner and side */
             w.gh = 0.5 * (double)w.gs * h;
@@ -881,6 +917,25 @@ void orc_tree_forces_tol(orc_t *t, double tol, double eps, const int64_t *groups
                 pot[o] = p[i];
             }
         free(a); free(p);
+    }
+}
+/* f-4 (the "drift" and "kick" operators of the symplectic integrator; their time factors -- in a comoving
+ * background integrals over the expansion history -- are the caller's): v <- v + a dtk, then x <- x + v dtd, in fp32 with
+ * one fused multiply-add each (so that a GPU does the same bits); periodic boxes wrap x back into [lo, lo + size). */
+void orc_kick_drift(float *pos, float *vel, const float *acc, int64_t n, float dtk, float dtd,
+                    const float lo[3], float size, int periodic) {
+    for (int64_t i = 0; i < 3 * n; ++i) {
+        float v = fmaf(acc[i], dtk, vel[i]);
+        float x = fmaf(v, dtd, pos[i]);
+        if (periodic) {
+            float l = lo[i % 3];
+            volatile float t = x - l;
+            volatile float q = floorf(t / size);
+            x = fmaf(-q, size, t) + l;
+            if (x >= l + size) x = l;          /* rounding may land on the upper face */
+            if (x < l) x = l;
+        }
+        vel[i] = v; pos[i] = x;
     }
 }
 /* thread count of the OpenMP loops (bench.py times the oracle with 1 thread and with all cores) */

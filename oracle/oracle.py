@@ -148,6 +148,24 @@ def mac_bound(mom35, b, R, p):
     return lib().orc_mac_bound(_p(mom35), C.c_double(b), C.c_double(R), int(p))
 
 
+def set_softening(kind):
+    """0: Plummer (default); 1: cubic spline with h = 2.8 eps.  Global to the oracle library."""
+    lib().orc_set_softening(int(kind))
+
+
+def spline_kernel(r, h):
+    fac, pot = C.c_double(), C.c_double()
+    lib().orc_spline_kernel(C.c_double(r), C.c_double(h), C.byref(fac), C.byref(pot))
+    return fac.value, pot.value
+
+
+def kick_drift(pos, vel, acc, dtk, dtd, lo, size, periodic):
+    """In place on float32 arrays: v += a dtk; x += v dtd (one fmaf each), periodic wrap."""
+    assert pos.dtype == np.float32 and vel.dtype == np.float32 and pos.flags["C_CONTIGUOUS"] and vel.flags["C_CONTIGUOUS"]
+    acc = _f32(acc); lo = _f32(lo)
+    lib().orc_kick_drift(_p(pos), _p(vel), _p(acc), C.c_int64(pos.shape[0]), C.c_float(dtk), C.c_float(dtd), _p(lo), C.c_float(size), int(bool(periodic)))
+
+
 def set_num_threads(n):
     lib().orc_set_num_threads(int(n))
 

@@ -62,6 +62,8 @@ def _load():
         lib.hot_set_stream.argtypes = [C.c_void_p]
         lib.hot_set_params.argtypes = [C.c_int, C.c_int]
         lib.hot_set_list_arena.argtypes = [C.c_int64]
+        lib.hot_set_softening.argtypes = [C.c_int]
+        lib.hot_kick_drift.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_float, hot_box, C.c_int]
         lib.hot_far_coefficients.argtypes = [C.c_void_p]
         lib.hot_measure_fp32.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
         lib.hot_measure_fp32_operands.argtypes = [C.POINTER(C.c_double)]
@@ -127,6 +129,23 @@ def hot_set_list_arena(max_bytes: int = 0):
 
 def hot_set_params(nleaf: int = 16, ncrit: int = 256):
     _check(_load().hot_set_params(int(nleaf), int(ncrit)))
+
+
+def hot_set_softening(kind: int = 0):
+    """0: Plummer (default); 1: cubic spline with h = 2.8 eps."""
+    _check(_load().hot_set_softening(int(kind)))
+
+
+def hot_kick_drift(pos, vel, acc, dt_kick, dt_drift, lo, size, periodic=False):
+    """In place on contiguous CUDA float32 [n,3] tensors: vel += acc * dt_kick; pos += vel * dt_drift (periodic wrap)."""
+    import torch
+
+    for t_, name in ((pos, "pos"), (vel, "vel"), (acc, "acc")):
+        if not (t_.is_cuda and t_.dtype == torch.float32 and t_.is_contiguous() and t_.dim() == 2 and t_.shape[1] == 3
+                and t_.shape[0] == pos.shape[0] and t_.device.index == torch.cuda.current_device()):
+            raise TypeError(f"hot_kick_drift wants {name} as a contiguous CUDA float32 [n,3] tensor on the current device")
+    _check(_load().hot_kick_drift(pos.data_ptr(), vel.data_ptr(), acc.data_ptr(), pos.shape[0], float(dt_kick), float(dt_drift),
+                                  _box(lo, size), int(bool(periodic))))
 
 
 def hot_free():

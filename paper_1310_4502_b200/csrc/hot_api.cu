@@ -17,6 +17,7 @@ struct Ctx {
     Tree t;
     bool built = false;
     int nleaf = 16, ncrit = 256;
+    int softening = 0; // 0 Plummer, 1 cubic spline (hot_set_softening)
     int last_order = -1, last_tolmode = 0;
     char err[512] = "";
     // scratch owned across calls
@@ -173,6 +174,20 @@ int hot_set_params(int nleaf, int ncrit) {
     if (nleaf < 1 || nleaf > HOT_MAX_NLEAF || ncrit < nleaf || ncrit > HOT_MAX_NCRIT)
         return fail(HOT_EINVAL, "hot_set_params: need 1 <= nleaf <= %d, nleaf <= ncrit <= %d", HOT_MAX_NLEAF, HOT_MAX_NCRIT);
     g.nleaf = nleaf; g.ncrit = ncrit;
+    return HOT_OK;
+}
+
+int hot_set_softening(int kind) {
+    if (kind != 0 && kind != 1) return fail(HOT_EINVAL, "hot_set_softening: kind must be 0 (Plummer) or 1 (cubic spline)");
+    g.softening = kind;
+    return HOT_OK;
+}
+
+int hot_kick_drift(float* pos, float* vel, const float* acc, int64_t n, float dt_kick, float dt_drift, hot_box box, int periodic) {
+    if (!pos || !vel || !acc) return fail(HOT_EINVAL, "hot_kick_drift: NULL argument");
+    if (n < 1) return fail(HOT_EINVAL, "hot_kick_drift: n must be >= 1");
+    if (periodic && !(box.size > 0.0f)) return fail(HOT_EINVAL, "hot_kick_drift: box.size must be positive");
+    CUDA_TRY(launch_kick_drift(pos, vel, acc, n, dt_kick, dt_drift, box.lo[0], box.lo[1], box.lo[2], box.size, periodic ? 1 : 0, g.stream));
     return HOT_OK;
 }
 
@@ -388,6 +403,13 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     WalkArgs wa{};
     wa.wcell = t.wcell; wa.group = t.group; wa.g1 = ng;
     mac_table(theta * theta, wa.mac_t); // theta^2 formed once on the host in double (R-7)
+    const double hreal = g.softening == 1 ? 2.8 * eps : 0.0; // spline softening: support radius of a body (R-17)
+    if (g.softening == 1) { // an accepted cell lies beyond h: d2 > (h / grid spacing)^2, folded into the integer thresholds
+        const double hg = hreal * 2097152.0 / t.size, hgrid2 = hg * hg;
+        const unsigned long long need = hgrid2 < 9.0e18 ? (unsigned long long)std::floor(hgrid2) + 1ull : ~0ull;
+        for (int l = 0; l < HOT_NLEVELS; ++l) if (wa.mac_t[l] < need) wa.mac_t[l] = need;
+    }
+    wa.hreal = hreal;
     wa.tolmode = tolmode; wa.tol = tol; wa.size = t.size; wa.cellA = t.cellA; wa.cellMac = t.cellMac;
     for (int k = 0; k < 3; ++k) wa.lo[k] = t.lo[k];
     if (tolmode) { CUDA_TRY(tree_alloc(&t.glpc0, (size_t)ng)); CUDA_TRY(tree_alloc(&t.glpc2, (size_t)ng)); }
@@ -400,6 +422,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     a.body = t.body; a.perm = t.idx[0]; a.group = t.group;
     a.pcoff = t.pcoff; a.ppoff = t.ppoff; a.lpc = t.glpc; a.lpp = t.glpp;
     a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic;
+    a.spline = g.softening == 1; a.hinv = hreal > 0.0 ? (float)(1.0 / hreal) : INFINITY;
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
     a.far = t.periodic ? t.far : nullptr;

@@ -87,6 +87,44 @@ __device__ __forceinline__ void pp_one_self(const float4 ns, const bool same, co
     a[3] += nmr;
 }
 
+// ---- f-4: cubic-spline softening (R-17) ------------------------------------------------
+// A body is a ball of radius h = 2.8 eps with the spline density; with u = r / h the pair force m (s - x) fac and
+// potential -m npot are  u <= 1/2: fac h^3 = 32/3 - 192/5 u^2 + 32 u^3,            npot h = 14/5 - 16/3 u^2 + 48/5 u^4 - 32/5 u^5
+//                        u <= 1  : fac h^3 = 64/3 - 48u + 192/5 u^2 - 32/3 u^3 - 1/(15 u^3),
+//                                  npot h = 16/5 - 1/(15u) - 32/3 u^2 + 16 u^3 - 48/5 u^4 + 32/15 u^5;   u > 1: Newtonian.
+__device__ __forceinline__ void spline_kernel(const float r2, const float hinv, float& fac, float& npot) {
+    const float ri = rsqrt_approx(fmaxf(r2, 1e-30f)), r = r2 * ri, u = r * hinv, u2 = u * u, hinv3 = hinv * hinv * hinv;
+    const float fi = fmaf(u2, fmaf(32.0f, u, -38.4f), 10.6666667f);
+    const float pi = fmaf(u2, fmaf(u2, fmaf(-6.4f, u, 9.6f), -5.33333333f), 2.8f);
+    const float iu = __fdividef(1.0f, fmaxf(u, 0.25f)), iu3 = iu * iu * iu; // the middle branch is used for u >= 1/2 only
+    const float fm = fmaf(u, fmaf(u, fmaf(-10.6666667f, u, 38.4f), -48.0f), 21.3333333f) - 0.0666666667f * iu3;
+    const float pm = fmaf(u2, fmaf(u, fmaf(u, fmaf(2.13333333f, u, -9.6f), 16.0f), -10.6666667f), 3.2f) - 0.0666666667f * iu;
+    const bool in = u < 0.5f, mid = u < 1.0f;
+    fac = in ? hinv3 * fi : (mid ? hinv3 * fm : ri * ri * ri);
+    npot = in ? hinv * pi : (mid ? hinv * pm : ri);
+}
+__device__ __forceinline__ void pp_one_spline(const float4 ns, const bool skip, const float (&x)[3], const float hinv, float (&a)[4]) {
+    const float dx = x[0] + ns.x, dy = x[1] + ns.y, dz = x[2] + ns.z;
+    float fac, npot;
+    spline_kernel(fmaf(dx, dx, fmaf(dy, dy, dz * dz)), hinv, fac, npot);
+    if (skip) { fac = 0.0f; npot = 0.0f; }
+    const float nmf = ns.w * fac;
+    a[0] = fmaf(nmf, dx, a[0]); a[1] = fmaf(nmf, dy, a[1]); a[2] = fmaf(nmf, dz, a[2]);
+    a[3] = fmaf(ns.w, npot, a[3]);
+}
+__device__ __forceinline__ void pp_pair_spline(const float4 ns, const bool skip0, const bool skip1, const f2 (&x)[3], const float hinv, f2 (&a)[4]) {
+    const f2 dx = x[0] + splat<f2>(ns.x), dy = x[1] + splat<f2>(ns.y), dz = x[2] + splat<f2>(ns.z);
+    const f2 r2 = vfma(dx, dx, vfma(dy, dy, dz * dz));
+    float f0, p0, f1, p1;
+    spline_kernel(lo2(r2), hinv, f0, p0);
+    spline_kernel(hi2(r2), hinv, f1, p1);
+    if (skip0) { f0 = 0.0f; p0 = 0.0f; }
+    if (skip1) { f1 = 0.0f; p1 = 0.0f; }
+    const f2 nm = splat<f2>(ns.w), nmf = nm * mk2(f0, f1);
+    a[0] = vfma(nmf, dx, a[0]); a[1] = vfma(nmf, dy, a[1]); a[2] = vfma(nmf, dz, a[2]);
+    a[3] = vfma(nm, mk2(p0, p1), a[3]);
+}
+
 // ---- S9: one cell on one sink or a pair of sinks, eq (5) with g = (R^2+eps^2)^(-1/2) ----------------
 // (DESIGN.md "P-C formulas").  R = x - z, D_k = (-1)^k (2k-1)!! u^-(2k+1)/2, raw moments, traces.
 // Staged cell j of a batch: float4 slot q of the record sits at st[q*32 + j] (slot-major, so the
@@ -222,6 +260,11 @@ template <int S> struct Sinks {
         }
         if (TAIL) pp_one_self(ns, j == me[S - 1], x1, eps2, a1);
     }
+    __device__ __forceinline__ void pp_spline(const float4 ns, int j, float hinv) { // j: index in the group if ns is one of its own bodies, else -1 (me[] >= 0 or -1 for idle slots: an idle slot never equals j >= 0... nor -1 matters: its result is dropped)
+#pragma unroll
+        for (int p = 0; p < NP; ++p) pp_pair_spline(ns, j >= 0 && j == me[2 * p], j >= 0 && j == me[2 * p + 1], x2[p], hinv, a2[p]);
+        if (TAIL) pp_one_spline(ns, j >= 0 && j == me[S - 1], x1, hinv, a1);
+    }
     template <int ORDER>
     __device__ __forceinline__ void pc(const float4 q0, const float4 q1, const float4 q2, const float* m, float eps2) {
 #pragma unroll
@@ -241,7 +284,7 @@ template <int ORDER> struct WL {
 
 // ---- S8/S9/S10: one chunk (<= 32*SMAX sinks) of one group -----------------------------------------
 // L = 1 << lgL lanes per source stream, S = ceil(nchunk / L) sinks per lane.
-template <int ORDER, bool PER, int S>
+template <int ORDER, bool PER, int S, bool SPL>
 __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const GroupRec g, const int64_t gi, const uint32_t chunk0,
                                         const uint32_t nchunk, const int lgL, const int lane) {
     using Lay = WL<ORDER>;
@@ -278,7 +321,8 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
         for (int k = 0; k < 4; ++k) As[(4 * i + k) * 32] = 0.0;
     }
     sk.zero_partials();
-    const float eps2 = P.eps2;
+    const float eps2 = SPL ? 0.0f : P.eps2; // spline softening: accepted cells lie beyond its support, their expansions are Newtonian
+    const float hinv = P.hinv;
     // fp32 partials are added to the fp64 running sums after at most ~32 sources per lane
     int nacc = 0;
     auto flush = [&]() {
@@ -303,7 +347,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
         }
         __syncwarp();
 #pragma unroll 1
-        for (int j = strm; j < cnt; j += K) sk.pp_self(ppst[j], (int)j0 + j, eps2);
+        for (int j = strm; j < cnt; j += K) { if (SPL) sk.pp_spline(ppst[j], (int)j0 + j, hinv); else sk.pp_self(ppst[j], (int)j0 + j, eps2); }
         __syncwarp();
     }
     flush();
@@ -436,7 +480,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                     const float4 sb = nx;
                     j += K;
                     nx = st[j < cnt ? j : strm];
-                    sk.pp(sb, eps2);
+                    if (SPL) sk.pp_spline(sb, -1, hinv); else sk.pp(sb, eps2);
                 }
             }
             nacc += (cnt + K - 1) >> lgK;
@@ -481,16 +525,16 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
 }
 
 // one pass over the group's lists for sinks [c0, c0 + nc) with L = 1 << lgL lanes per source stream
-template <int ORDER, bool PER>
+template <int ORDER, bool PER, bool SPL>
 __device__ __forceinline__ void run_chunk(const ForceArgs& P, const int w, const GroupRec g, const int64_t gi, const uint32_t c0,
                                           const uint32_t nc, const int lgL, const int lane) {
     const int S = (int)((nc + (1u << lgL) - 1) >> lgL);
-    if (S <= 1) eval_chunk<ORDER, PER, 1>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 2) eval_chunk<ORDER, PER, 2>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 3) eval_chunk<ORDER, PER, 3>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 4) eval_chunk<ORDER, PER, 4>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 5) eval_chunk<ORDER, PER, 5>(P, w, g, gi, c0, nc, lgL, lane);
-    else eval_chunk<ORDER, PER, 6>(P, w, g, gi, c0, nc, lgL, lane);
+    if (S <= 1) eval_chunk<ORDER, PER, 1, SPL>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 2) eval_chunk<ORDER, PER, 2, SPL>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 3) eval_chunk<ORDER, PER, 3, SPL>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 4) eval_chunk<ORDER, PER, 4, SPL>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 5) eval_chunk<ORDER, PER, 5, SPL>(P, w, g, gi, c0, nc, lgL, lane);
+    else eval_chunk<ORDER, PER, 6, SPL>(P, w, g, gi, c0, nc, lgL, lane);
     static_assert(SMAX == 6, "one eval_chunk instance per sinks-per-lane count");
 }
 // smallest stream width that holds n sinks with at most SMAX per lane
@@ -589,7 +633,7 @@ cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st) {
 }
 #endif
 
-template <int ORDER, bool PER>
+template <int ORDER, bool PER, bool SPL>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned int total = P.cls[24 * P.nsb];
@@ -600,39 +644,49 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : MINBLK)
         if (q >= total) break;
         const uint4 it = P.items[q];
         const int64_t gi = P.g0 + (int64_t)it.x;
-        run_chunk<ORDER, PER>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
+        run_chunk<ORDER, PER, SPL>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
     }
 }
 
-template <int ORDER, bool PER> static cudaError_t launch_one(const ForceArgs& a, cudaStream_t st) {
+template <int ORDER, bool PER, bool SPL> static cudaError_t launch_one(const ForceArgs& a, cudaStream_t st) {
     constexpr int smem = WL<ORDER>::bytes * WARPS_PER_BLOCK;
     static int nblocks = 0;
     if (!nblocks) {
-        cudaError_t e = cudaFuncSetAttribute(forces_kernel<ORDER, PER>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(forces_kernel<ORDER, PER, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         int dev = 0, nsm = 0, occ = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, forces_kernel<ORDER, PER>, WARPS_PER_BLOCK * 32, smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, forces_kernel<ORDER, PER, SPL>, WARPS_PER_BLOCK * 32, smem);
         if (e != cudaSuccess) return e;
         nblocks = nsm * (occ < 1 ? 1 : occ);
     }
     HOT_LAUNCHED(1);
-    forces_kernel<ORDER, PER><<<nblocks, WARPS_PER_BLOCK * 32, smem, st>>>(a);
+    forces_kernel<ORDER, PER, SPL><<<nblocks, WARPS_PER_BLOCK * 32, smem, st>>>(a);
     return cudaGetLastError();
 }
 #ifndef HOT_FORCES_PERIODIC_TU
 cudaError_t dispatch_periodic(const ForceArgs& a, cudaStream_t st);
 cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st) {
     if (a.periodic) return dispatch_periodic(a, st);
-    if (a.order >= 4) return launch_one<4, false>(a, st);
-    if (a.order >= 2) return launch_one<2, false>(a, st);
-    return launch_one<0, false>(a, st);
+    if (a.spline) {
+        if (a.order >= 4) return launch_one<4, false, true>(a, st);
+        if (a.order >= 2) return launch_one<2, false, true>(a, st);
+        return launch_one<0, false, true>(a, st);
+    }
+    if (a.order >= 4) return launch_one<4, false, false>(a, st);
+    if (a.order >= 2) return launch_one<2, false, false>(a, st);
+    return launch_one<0, false, false>(a, st);
 }
 #else
 cudaError_t dispatch_periodic(const ForceArgs& a, cudaStream_t st) {
-    if (a.order >= 4) return launch_one<4, true>(a, st);
-    if (a.order >= 2) return launch_one<2, true>(a, st);
-    return launch_one<0, true>(a, st);
+    if (a.spline) {
+        if (a.order >= 4) return launch_one<4, true, true>(a, st);
+        if (a.order >= 2) return launch_one<2, true, true>(a, st);
+        return launch_one<0, true, true>(a, st);
+    }
+    if (a.order >= 4) return launch_one<4, true, false>(a, st);
+    if (a.order >= 2) return launch_one<2, true, false>(a, st);
+    return launch_one<0, true, false>(a, st);
 }
 #endif

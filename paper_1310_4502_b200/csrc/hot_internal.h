@@ -135,6 +135,7 @@ struct WalkArgs {
     int* errflag;                          // bit 2: spill arena exhausted, bit 3: staging too small
     // error-bound criterion (tolmode != 0; R-16): accept at the cheapest order whose bound is <= tol
     int tolmode; double tol; double lo[3], size;
+    double hreal;                          // spline softening: h (an accepted cell lies wholly beyond it), else 0
     const CellA* cellA; const float4* cellMac;   // per cell: centre of mass / (b, 3 B2, 4 sqrt(B2 B4), 6 b B4)
     uint32_t *lpc0, *lpc2;                 // per group: accepted monopoles, quadrupoles (the list is ordered mono | quad | hexa)
 };
@@ -153,6 +154,7 @@ struct ForceArgs {
     const uint32_t* pclist; const uint32_t* pplist; const uint8_t* pcimg; const uint8_t* ppimg;
     const double* far;            // periodic: far field (ax, ay, az, phi) per body in key order, added in fp64; else NULL
     float eps2; int order; int periodic;
+    int spline; float hinv;       // f-4: cubic-spline softening with h = 2.8 eps instead of Plummer; 1 / h
     double lo[3], size;
     float* acc; float* pot;
     unsigned int* counter;        // dynamic scheduler over the work items
@@ -175,5 +177,9 @@ cudaError_t launch_far_eval(const Tree& t, const double* D /*host [165]*/, doubl
 cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, double* farc, double eps2, cudaStream_t st);
 
 // ---- FP32 roofline denominator measured on the device (hot_peak.cu) ------------------------------------
+// ---- f-4: kick and drift (hot_step.cu) -------------------------------------------------------------------
+cudaError_t launch_kick_drift(float* pos, float* vel, const float* acc, int64_t n, float dtk, float dtd, float lox, float loy, float loz,
+                              float size, int periodic, cudaStream_t st);
+
 cudaError_t measure_fp32(double* tf_scalar, double* tf_packed, cudaStream_t st);
 cudaError_t measure_fp32_operands(double* tf3, cudaStream_t st); // packed 2 register reads, packed 3, scalar 3

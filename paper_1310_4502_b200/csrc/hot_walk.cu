@@ -150,7 +150,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
                     if (PER) { zx += (double)(im / 25 - 2) * P.size; zy += (double)((im / 5) % 5 - 2) * P.size; zz += (double)(im % 5 - 2) * P.size; }
                     const double ax = fmax(fabs(zx - gcx) - gh, 0.0), ay = fmax(fabs(zy - gcy) - gh, 0.0), az = fmax(fabs(zz - gcz) - gh, 0.0);
                     const double R2 = ax * ax + ay * ay + az * az, R = sqrt(R2), b = (double)mb.x;
-                    if (R > b) {
+                    if (R > b && R - b > P.hreal) { // (spline softening: every body of the cell beyond the kernel's support)
                         const double t = P.tol * (R - b) * (R - b); // bound_p <= tol  <=>  c_p <= tol (R-b)^2 R^(p+1)
                         if ((double)mb.y <= t * R2) { acc = true; ocode = 0; }
                         else if ((double)mb.z <= t * R2 * R) { acc = true; ocode = 1; }

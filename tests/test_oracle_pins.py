@@ -616,3 +616,89 @@ def test_error_bound_tree_properties():
     assert l0.sum() > 0 and l2.sum() > 0                   # a mix of orders at the loosest tolerance
     a, p, l0, l2, l4, lpp = T.forces_tol(1e-4 * arms, w.eps)
     assert l2.sum() > 0 and l4.sum() > 0
+
+
+# ---------------------------------------------------------------- f-4: spline softening, kick / drift
+def test_spline_kernel_is_the_field_of_the_spline_ball():
+    """PAPER.md:136 (spline kernel of ref [50]).  The force factor and potential are pinned by quadrature of the
+    density they claim to come from: W(u) = 8/(pi h^3) (1 - 6u^2 + 6u^3 | 2 (1-u)^3); enclosed mass / r^3 and
+    -(M(r)/r + 4 pi int_r^h W r' dr'); unit total mass; Newtonian outside; phi(0) = -2.8/h; continuous at the joints."""
+    h = 0.7
+    def W(r):
+        u = r / h
+        return 8 / (np.pi * h ** 3) * np.where(u <= 0.5, 1 - 6 * u ** 2 + 6 * u ** 3, np.where(u <= 1, 2 * (1 - u) ** 3, 0.0))
+    rr = np.linspace(0, h, 400001)
+    dm = 4 * np.pi * W(rr) * rr ** 2
+    M = np.concatenate([[0], np.cumsum(0.5 * (dm[1:] + dm[:-1]) * np.diff(rr))])      # trapezoid
+    sh = 4 * np.pi * W(rr) * rr
+    outer = np.concatenate([np.cumsum((0.5 * (sh[1:] + sh[:-1]) * np.diff(rr))[::-1])[::-1], [0]])
+    assert abs(M[-1] - 1) < 1e-9
+    for r in (0.05 * h, 0.3 * h, 0.5 * h, 0.77 * h, 0.999 * h):
+        i = int(round(r / h * 400000))
+        fac, pot = O.spline_kernel(rr[i], h)
+        assert math.isclose(fac, M[i] / rr[i] ** 3, rel_tol=1e-7), r
+        assert math.isclose(pot, -(M[i] / rr[i] + outer[i]), rel_tol=1e-7), r
+    assert math.isclose(O.spline_kernel(0.0, h)[1], -2.8 / h, rel_tol=1e-15) and math.isclose(O.spline_kernel(0.0, h)[0], 32 / 3 / h ** 3, rel_tol=1e-15)
+    for r in (h, 1.5 * h):
+        fac, pot = O.spline_kernel(r, h)
+        assert math.isclose(fac, r ** -3, rel_tol=1e-15) and math.isclose(pot, -1 / r, rel_tol=1e-15)
+    for r in (0.5 * h, h):
+        a, b = O.spline_kernel(r * (1 - 1e-9), h), O.spline_kernel(r * (1 + 1e-9), h)
+        assert math.isclose(a[0], b[0], rel_tol=1e-7) and math.isclose(a[1], b[1], rel_tol=1e-7)
+
+
+def test_spline_softened_tree_against_direct_sum():
+    w = W.config(2, 11)
+    eps = 2e-3   # h = 5.6e-3: many pairs inside the kernel's support
+    O.set_softening(1)
+    try:
+        ad, pd = O.direct(w.pos, w.mass, eps)
+        T = O.Tree(w.pos, w.mass, w.lo, w.size, nleaf=8, ncrit=32)
+        a0, p0, lpc0, lpp0 = T.forces(0.0, eps, 2)
+        assert np.abs(a0 - ad).max() <= 1e-12 * np.abs(ad).max() and np.abs(p0 - pd).max() <= 1e-12 * np.abs(pd).max()
+        a, p, lpc, lpp = T.forces(0.5, eps, 4)
+        assert np.sqrt(((a - ad) ** 2).sum() / (ad ** 2).sum()) < 1e-4
+    finally:
+        O.set_softening(0)
+    ap, pp = O.direct(w.pos, w.mass, eps)
+    assert not np.allclose(ap, ad) and np.abs(pp - pd).max() > 0     # a different kernel from Plummer's
+    # two bodies: inside the support the pair force is the kernel's, outside Newtonian, always antisymmetric
+    O.set_softening(1)
+    try:
+        for d in (0.3, 0.9, 2.0):
+            pos = np.array([[0.1, 0.2, 0.3], [0.1 + d * 2.8 * 0.01, 0.2, 0.3]], np.float32)
+            m = np.array([1.0, 3.0], np.float32)
+            a2, p2 = O.direct(pos, m, 0.01)
+            r = float(pos[1, 0]) - float(pos[0, 0])
+            fac, pot = O.spline_kernel(r, 0.028)
+            assert math.isclose(a2[0, 0], 3.0 * r * fac, rel_tol=1e-14) and math.isclose(p2[0], 3.0 * pot, rel_tol=1e-14)
+            assert np.allclose(1.0 * a2[0], -(3.0 * a2[1]), rtol=1e-15, atol=0)
+    finally:
+        O.set_softening(0)
+
+
+def test_kick_drift_is_a_second_order_leapfrog():
+    """Kick-drift-kick around the direct sum: a circular two-body orbit closes to O(dt^2) (halving dt quarters the
+    error); the periodic wrap keeps every coordinate inside [lo, lo + size)."""
+    def orbit(nsteps):
+        m = np.array([0.5, 0.5], np.float32)
+        pos = np.array([[0.25, 0.5, 0.5], [0.75, 0.5, 0.5]], np.float32)
+        v = math.sqrt(0.5 / (4 * 0.25))          # circular: v^2 / r = m / (2r)^2, r = 0.25
+        vel = np.array([[0, v, 0], [0, -v, 0]], np.float32)
+        dt = 2 * math.pi * 0.25 / v / nsteps
+        a, _ = O.direct(pos, m, 0.0)
+        for _ in range(nsteps):
+            O.kick_drift(pos, vel, a.astype(np.float32), 0.5 * dt, dt, (0, 0, 0), 1.0, False)
+            a, _ = O.direct(pos, m, 0.0)
+            O.kick_drift(pos, vel, a.astype(np.float32), 0.5 * dt, 0.0, (0, 0, 0), 1.0, False)
+        return float(np.linalg.norm(pos[0].astype(np.float64) - [0.25, 0.5, 0.5]))
+    e1, e2 = orbit(400), orbit(800)
+    assert e1 < 5e-3 and 3.0 < e1 / e2 < 5.0, (e1, e2)
+    rng = np.random.default_rng(9)
+    pos = rng.uniform(0, 1, (1000, 3)).astype(np.float32); vel = rng.normal(0, 3, (1000, 3)).astype(np.float32)
+    p0 = pos.astype(np.float64); v0 = vel.astype(np.float64)
+    O.kick_drift(pos, vel, np.zeros((1000, 3), np.float32), 0.0, 0.7, (0, 0, 0), 1.0, True)
+    assert (pos >= 0).all() and (pos < 1).all()
+    want = (p0 + 0.7 * v0) % 1.0
+    d = np.abs(pos - want); d = np.minimum(d, 1 - d)
+    assert d.max() < 1e-6

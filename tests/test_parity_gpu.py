@@ -621,3 +621,77 @@ def test_error_bound_criterion_with_mixed_orders(hot, cfg, scale, periodic, rtol
     hot.hot_forces_tol(10 * tol, w.eps)
     st2 = hot.hot_stats()
     assert st2["pc_interactions"] + st2["pp_interactions"] < st["pc_interactions"] + st["pp_interactions"]
+
+
+# ---- f-4: spline softening and the kick / drift operators (R-17) --------------------
+@pytest.mark.parametrize("cfg,scale,periodic,order,theta,eps_scale", [(2, 14, False, 2, 0.6, 40.0), (0, 13, False, 4, 0.5, 3.0), (1, 13, False, 0, 0.7, 30.0),
+                                                                  (4, 12, True, 2, 0.5, 4.0)])
+def test_spline_softening_parity(hot, cfg, scale, periodic, order, theta, eps_scale):
+    """Cubic-spline kernel (h = 2.8 eps) against the oracle: list counts bit-exact (the criterion gains "beyond h" in
+    integer geometry), forces to the usual tolerance; eps is enlarged so that many pairs fall inside the support."""
+    w = W.config(cfg, scale)
+    eps = w.eps * eps_scale
+    _build(hot, w, 16, 64)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=periodic, nleaf=16, ncrit=64)
+    hot.hot_set_softening(1)
+    O.set_softening(1)
+    try:
+        acc, pot = hot.hot_forces(theta, eps, order)
+        gg = hot.hot_export_groups()
+        sel = np.sort(np.random.default_rng(4).choice(T.ngroups, min(T.ngroups, 24 if periodic else 128), replace=False))
+        oa, op, lpc, lpp = T.forces(theta, eps, order, groups=sel)
+        # how many pairs the kernel's support holds: the test must exercise all three branches
+        if not periodic:
+            x = w.pos.astype(np.float64)[:2000]
+            d = np.sqrt(((x[:, None, :] - x[None, :, :]) ** 2).sum(-1)); d = d[np.triu_indices(2000, 1)]
+            assert (d < 1.4 * eps).sum() > 20 and ((d >= 1.4 * eps) & (d < 2.8 * eps)).sum() > 20
+    finally:
+        hot.hot_set_softening(0)
+        O.set_softening(0)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]; gp = pot.cpu().numpy().astype(np.float64)[m]
+    an = np.linalg.norm(oa[m], axis=1)
+    if periodic:
+        an = np.maximum(an, np.sqrt((oa[m] ** 2).sum(1).mean()))
+    ea = np.linalg.norm(ga - oa[m], axis=1) / an
+    pscale = 57.18721055 * float(w.mass.astype(np.float64).sum()) / w.size if periodic else 0.0
+    ep = np.abs(gp - op[m]) / (np.abs(op[m]) + pscale)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
+    # back to Plummer: a different answer with different lists (the "beyond h" condition is gone)
+    acc2, _ = hot.hot_forces(theta, eps, order)
+    assert not np.array_equal(acc2.cpu().numpy(), acc.cpu().numpy())
+
+
+def test_kick_drift_bit_exact_and_leapfrog_step(hot):
+    import torch
+
+    rng = np.random.default_rng(12)
+    n = 100003
+    pos = rng.uniform(0, 1, (n, 3)).astype(np.float32); vel = rng.normal(0, 2, (n, 3)).astype(np.float32); acc = rng.normal(0, 5, (n, 3)).astype(np.float32)
+    for periodic in (False, True):
+        p, v = pos.copy(), vel.copy()
+        O.kick_drift(p, v, acc, 0.013, 0.7, (0.0, 0.0, 0.0), 1.0, periodic)
+        dp, dv, da = torch.from_numpy(pos).cuda(), torch.from_numpy(vel).cuda(), torch.from_numpy(acc).cuda()
+        hot.hot_kick_drift(dp, dv, da, 0.013, 0.7, (0.0, 0.0, 0.0), 1.0, periodic)
+        assert np.array_equal(dv.cpu().numpy(), v) and np.array_equal(dp.cpu().numpy(), p)
+        if periodic:
+            assert (p >= 0).all() and (p < 1).all()
+    # an unaligned view takes the scalar path: same bits
+    big = torch.zeros(3 * n + 1, device="cuda")
+    dp = big[1:].view(n, 3); dp.copy_(torch.from_numpy(pos))
+    dv, da = torch.from_numpy(vel).cuda(), torch.from_numpy(acc).cuda()
+    hot.hot_kick_drift(dp, dv, da, 0.013, 0.7, (0.0, 0.0, 0.0), 1.0, True)
+    assert np.array_equal(dp.cpu().numpy(), p)
+    # one kick-drift-kick step of a periodic box through the library alone keeps every body inside and builds again
+    w = W.config(4, 12)
+    dp, dm = torch.from_numpy(w.pos).cuda(), torch.from_numpy(w.mass).cuda()
+    dv = torch.zeros_like(dp)
+    hot.hot_set_params(16, 64)
+    for _ in range(3):
+        hot.hot_build(dp, dm, w.lo, w.size, True)
+        a, _ = hot.hot_forces(0.5, w.eps, 2)
+        hot.hot_kick_drift(dp, dv, a, 0.5e-3, 1e-3, w.lo, w.size, True)
+    hot.hot_build(dp, dm, w.lo, w.size, True)   # HOT_ERANGE would raise
+    assert torch.isfinite(dv).all() and float(dv.abs().max()) > 0
