@@ -492,7 +492,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         CUDA_TRY(launch_plan(a, st));
         if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
             CUDA_TRY(cudaEventRecord(g.evx[4], st));
-            CUDA_TRY(launch_coarse_monopoles(a, t.far, t.farc, eps * eps, st));
+            CUDA_TRY(launch_coarse_monopoles(a, t.far, t.farc, g.softening == 1 ? 0.0 : eps * eps, st)); // spline: accepted cells are Newtonian
             a.far = t.farc;
         }
         CUDA_TRY(cudaEventRecord(g.evx[3], st));

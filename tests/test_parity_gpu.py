@@ -624,7 +624,7 @@ def test_error_bound_criterion_with_mixed_orders(hot, cfg, scale, periodic, rtol
 
 
 # ---- f-4: spline softening and the kick / drift operators (R-17) --------------------
-@pytest.mark.parametrize("cfg,scale,periodic,order,theta,eps_scale", [(2, 14, False, 2, 0.6, 40.0), (0, 13, False, 4, 0.5, 3.0), (1, 13, False, 0, 0.7, 30.0),
+@pytest.mark.parametrize("cfg,scale,periodic,order,theta,eps_scale", [(2, 14, False, 2, 0.6, 40.0), (0, 13, False, 4, 0.5, 15.0), (1, 13, False, 0, 0.7, 60.0),
                                                                   (4, 12, True, 2, 0.5, 4.0)])
 def test_spline_softening_parity(hot, cfg, scale, periodic, order, theta, eps_scale):
     """Cubic-spline kernel (h = 2.8 eps) against the oracle: list counts bit-exact (the criterion gains "beyond h" in
