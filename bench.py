@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 #   P-C order 2:  4 add + 11 mul + 21 fma + rsqrt          = 58    (constant factors folded into the staged moments)
 #   P-C order 4: 10 add + 68 mul + 96 fma + rsqrt          = 271   (as compiled: FADD2 / FMUL2 / FFMA2 per sink pair in SASS)
 FLOPS_PP = 20
-FLOPS_PC = {0: 21, 2: 58, 4: 271}
+FLOPS_PC = {0: 21, 2: 58, 4: 271, 6: 271 + 563, 8: 271 + 1589}  # 6, 8: + the generated terms of degree 5 .. p (fmaf = 2, multiply = 1)
 # roofline.traffic: DRAM bytes of one forces_kernel launch (ncu --set full: dram__bytes_read.sum + dram__bytes_write.sum),
 # looked up in profiles/forces_traffic.csv by workload; null where no capture was taken
 def ncu_traffic(config, n, theta, order, nleaf, ncrit):

@@ -104,7 +104,8 @@ int hot_build(const float* pos, const float* mass, int64_t n, hot_box box, int p
 
 /* theta: opening angle, 0 <= theta < 1 (0: every interaction is particle-particle).
  * eps  : Plummer softening length >= 0 (0 with coincident distinct bodies gives inf/NaN).
- * order: 0 (monopole), 2 (through quadrupole) or 4 (through hexadecapole, octupole included).
+ * order: 0 (monopole), 2 (through quadrupole), 4 (through hexadecapole, octupole included), or 6 / 8: the terms of
+ *        degree 5 .. order come from generated code (csrc/gen_hi_orders.py), an accuracy feature.
  * acc  : device, [n][3] fp32, caller's particle order; overwritten.
  * pot  : device, [n] fp32 or NULL; overwritten.
  * May be called repeatedly on one build with different theta / eps / order. */

@@ -34,7 +34,12 @@
 #endif
 
 #define ORC_MAXLEVEL 21
-#define ORC_NMOM 35 /* multi-indices (a,b,c), a+b+c <= 4 */
+#define ORC_MAXORDER 8
+#define ORC_NMOM_MAX 165 /* multi-indices (a,b,c), a+b+c <= 8 */
+/* moments are kept through degree g_mom_order (4 unless orc_set_moment_order says 6 or 8: f-3, "through p=8") */
+static int g_mom_order = 4;
+static int nmom_of(int order) { return (order + 1) * (order + 2) * (order + 3) / 6; }
+void orc_set_moment_order(int order) { if (order >= 4 && order <= ORC_MAXORDER) g_mom_order = order; }
 
 typedef struct {
     int64_t n;
@@ -58,6 +63,7 @@ typedef struct {
     int64_t ngroups;
     int64_t *gcell;
     /* moments about the centre of mass, eq (6): mom[c][k] = sum m d^alpha_k; com[c][3]; bmax[c] */
+    int nmom;         /* moments per cell: nmom_of(order they were built through) */
     double *mom, *com, *bmax;
     double *bbound;   /* b_max as the upward pass can carry it: see build_bbound */
     int lazy;         /* moments computed on demand, only for the cells a requested group accepts */
@@ -72,11 +78,11 @@ typedef struct {
  * multi-index tables: alpha_k = (a,b,c) ordered by degree, then lexicographic x>y>z:
  * degree 0: 000; degree 1: 100 010 001; degree 2: 200 110 101 020 011 002; ...
  * ---------------------------------------------------------------------------------------- */
-static int MI_A[ORC_NMOM], MI_B[ORC_NMOM], MI_C[ORC_NMOM], MI_READY = 0;
+static int MI_A[ORC_NMOM_MAX], MI_B[ORC_NMOM_MAX], MI_C[ORC_NMOM_MAX], MI_READY = 0;
 static void mi_init(void) {
     if (MI_READY) return;
     int k = 0;
-    for (int d = 0; d <= 4; ++d)
+    for (int d = 0; d <= ORC_MAXORDER; ++d)
         for (int a = d; a >= 0; --a)
             for (int b = d - a; b >= 0; --b) {
                 MI_A[k] = a; MI_B[k] = b; MI_C[k] = d - a - b; ++k;
@@ -236,14 +242,14 @@ static void cell_moments(orc_t *t, int64_t c) {
         for (int k = 0; k < 3; ++k) z[k] += t->m[j] * t->x[3 * j + k];
     }
     for (int k = 0; k < 3; ++k) z[k] /= M0;
-    double *mo = t->mom + (size_t)c * ORC_NMOM, bm = 0;
-    for (int k = 0; k < ORC_NMOM; ++k) mo[k] = 0;
+    double *mo = t->mom + (size_t)c * t->nmom, bm = 0;
+    for (int k = 0; k < t->nmom; ++k) mo[k] = 0;
     for (int64_t j = f; j < e; ++j) {
         double d[3];
         for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - z[k];
         double r = sqrt(d[0] * d[0] + d[1] * d[1] + d[2] * d[2]);
         if (r > bm) bm = r;
-        for (int k = 0; k < ORC_NMOM; ++k)
+        for (int k = 0; k < t->nmom; ++k)
             mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
     }
     for (int k = 0; k < 3; ++k) t->com[3 * c + k] = z[k];
@@ -274,7 +280,8 @@ static void build_bbound(orc_t *t) {
  * (same cell_moments; for the 2^27-body config, where all 2e7 cells would take hours) */
 static void build_moments(orc_t *t, int lazy) {
     mi_init();
-    t->mom = calloc((size_t)t->ncells * ORC_NMOM, sizeof(double));
+    t->nmom = nmom_of(g_mom_order);
+    t->mom = calloc((size_t)t->ncells * t->nmom, sizeof(double));
     t->com = calloc((size_t)t->ncells * 3, sizeof(double));
     t->bmax = calloc((size_t)t->ncells, sizeof(double));
     t->lazy = lazy;
@@ -345,7 +352,7 @@ void orc_get_groups(const orc_t *t, int64_t *gcell) {
 void orc_get_bbound(const orc_t *t, double *bbound) { memcpy(bbound, t->bbound, 8 * (size_t)t->ncells); }
 void orc_get_moments(const orc_t *t, double *mom, double *com, double *bmax) {
     size_t nc = (size_t)t->ncells;
-    if (mom) memcpy(mom, t->mom, 8 * nc * ORC_NMOM);
+    if (mom) memcpy(mom, t->mom, 8 * nc * (size_t)t->nmom);
     if (com) memcpy(com, t->com, 8 * nc * 3);
     if (bmax) memcpy(bmax, t->bmax, 8 * nc);
 }
@@ -367,7 +374,7 @@ static double dg_rec(const int *idx, int nidx, int npairs, int ntot, const doubl
                      const double *D) {
     if (nidx == 0) return D[ntot - npairs];
     double s = R[idx[0]] * dg_rec(idx + 1, nidx - 1, npairs, ntot, R, D);
-    int rest[8];
+    int rest[12];
     for (int j = 1; j < nidx; ++j) {
         if (idx[j] != idx[0]) continue; /* delta_{i0,ij} */
         int q = 0;
@@ -377,7 +384,7 @@ static double dg_rec(const int *idx, int nidx, int npairs, int ntot, const doubl
     return s;
 }
 static double dg(int a, int b, int c, const double R[3], const double *D) {
-    int idx[8], n = 0;
+    int idx[12], n = 0;
     for (int i = 0; i < a; ++i) idx[n++] = 0;
     for (int i = 0; i < b; ++i) idx[n++] = 1;
     for (int i = 0; i < c; ++i) idx[n++] = 2;
@@ -392,7 +399,7 @@ static void make_D(double u, double *D, int kmax) {
 }
 /* exported for the finite-difference pin */
 double orc_dg(int a, int b, int c, const double R[3], double eps) {
-    double D[8]; make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + eps * eps, D, a + b + c);
+    double D[12]; make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + eps * eps, D, a + b + c);
     return dg(a, b, c, R, D);
 }
 
@@ -404,9 +411,9 @@ double orc_dg(int a, int b, int c, const double R[3], double eps) {
  * centre of mass; order 0 -> n=0; order 2 -> n=0,2; order 3 -> n<=3; order 4 -> n<=4.        */
 static void cell_on_sink(const double *mo, const double z[3], int order, const double x[3],
                          double eps2, double acc[3], double *pot) {
-    double R[3] = {x[0] - z[0], x[1] - z[1], x[2] - z[2]}, D[8];
+    double R[3] = {x[0] - z[0], x[1] - z[1], x[2] - z[2]}, D[12];
     make_D(R[0] * R[0] + R[1] * R[1] + R[2] * R[2] + (g_soft_kind == 1 ? 0.0 : eps2), D, order + 1);
-    for (int k = 0; k < ORC_NMOM; ++k) {
+    for (int k = 0; k < nmom_of(order); ++k) {
         int a = MI_A[k], b = MI_B[k], c = MI_C[k], n = a + b + c;
         if (n > order) break;
         if (n == 1) continue; /* dipole about the centre of mass is zero by construction */
@@ -463,7 +470,10 @@ void orc_cell_on_sink(const double *mom35, const double z[3], int order, const d
     cell_on_sink(mom35, z, order, x, eps * eps, acc, pot);
 }
 /* moments of an arbitrary particle set about its centre of mass (same definition as C-5) */
-void orc_moments_of(const double *y, const double *m, int64_t n, double *mom35, double z[3]) {
+void orc_moments_of_order(const double *y, const double *m, int64_t n, int order, double *mom, double z[3]);
+void orc_moments_of(const double *y, const double *m, int64_t n, double *mom35, double z[3]) { orc_moments_of_order(y, m, n, 4, mom35, z); }
+void orc_moments_of_order(const double *y, const double *m, int64_t n, int order, double *mom35, double z[3]) {
+    const int ORC_NMOM = nmom_of(order);
     mi_init();
     double M0 = 0; z[0] = z[1] = z[2] = 0;
     for (int64_t j = 0; j < n; ++j) { M0 += m[j]; for (int k = 0; k < 3; ++k) z[k] += m[j] * y[3 * j + k]; }
@@ -563,7 +573,7 @@ static int mac_tol(const walk_t *w, int64_t c) {
     }
     double R = sqrt(d2), b = t->bbound[c];
     if (g_soft_kind == 1 && !(R - b > w->hreal)) return -1; /* every body of the cell beyond h from every sink (R-17) */
-    const double *mo = t->mom + (size_t)c * ORC_NMOM;
+    const double *mo = t->mom + (size_t)c * t->nmom;
     if (orc_mac_bound(mo, b, R, 1) <= w->tol) return 0;
     if (orc_mac_bound(mo, b, R, 2) <= w->tol) return 2;
     if (orc_mac_bound(mo, b, R, 4) <= w->tol) return 4;
@@ -582,7 +592,7 @@ static void walk_rec(walk_t *w, int64_t c) {
         if (w->eval)
             for (int64_t i = 0; i < w->gcount; ++i) {
                 double z[3] = {t->com[3 * c] + w->shx[0], t->com[3 * c + 1] + w->shx[1], t->com[3 * c + 2] + w->shx[2]};
-                cell_on_sink(t->mom + (size_t)c * ORC_NMOM, z, ord, t->x + 3 * (w->gfirst + i),
+                cell_on_sink(t->mom + (size_t)c * t->nmom, z, ord, t->x + 3 * (w->gfirst + i),
                              w->eps2, w->acc + 3 * i, w->pot + i);
             }
     } else if (t->cchild[c] < 0) {

@@ -56,10 +56,17 @@ def _i64(a):
     return None if a is None else np.ascontiguousarray(a, dtype=np.int64)
 
 
-def multi_indices():
-    """(a,b,c) of the 35 moments, degree-major then x>y>z, as hot_oracle.c orders them."""
+def set_moment_order(order):
+    """Trees created from now on keep moments through this degree (4 by default; 6 or 8 for the high orders of f-3)."""
+    global NMOM
+    lib().orc_set_moment_order(int(order))
+    NMOM = (order + 1) * (order + 2) * (order + 3) // 6
+
+
+def multi_indices(order=4):
+    """(a,b,c) of the moments, degree-major then x>y>z, as hot_oracle.c orders them."""
     out = []
-    for d in range(5):
+    for d in range(order + 1):
         for a in range(d, -1, -1):
             for b in range(d - a, -1, -1):
                 out.append((a, b, d - a - b))
@@ -123,12 +130,12 @@ def dg(a, b, c, R, eps):
     return lib().orc_dg(a, b, c, _p(R), C.c_double(eps))
 
 
-def moments_of(y, m):
+def moments_of(y, m, order=4):
     y = np.ascontiguousarray(y, dtype=np.float64)
     m = np.ascontiguousarray(m, dtype=np.float64)
-    mom = np.empty(NMOM)
+    mom = np.empty((order + 1) * (order + 2) * (order + 3) // 6)
     z = np.empty(3)
-    lib().orc_moments_of(_p(y), _p(m), C.c_int64(y.shape[0]), _p(mom), _p(z))
+    lib().orc_moments_of_order(_p(y), _p(m), C.c_int64(y.shape[0]), int(order), _p(mom), _p(z))
     return mom, z
 
 
@@ -192,6 +199,7 @@ class Tree:
         self._h = C.c_void_p(self._h)
         self.ncells = lib().orc_ncells(self._h)
         self.ngroups = lib().orc_ngroups(self._h)
+        self.nmom = NMOM  # moments per cell of this tree (set_moment_order at creation time)
         self.has_moments = bool(moments)  # moments = 2 ("lazy"): only the cells that forces() needs, on demand
 
     def __del__(self):
@@ -231,7 +239,7 @@ class Tree:
 
     def moments(self):
         nc = self.ncells
-        mom = np.empty((nc, NMOM))
+        mom = np.empty((nc, self.nmom))
         com = np.empty((nc, 3))
         bmax = np.empty(nc)
         lib().orc_get_moments(self._h, _p(mom), _p(com), _p(bmax))

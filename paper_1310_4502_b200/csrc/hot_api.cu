@@ -329,6 +329,11 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         if (!t.cellA) CUDA_TRY(tree_alloc(&t.cellA, (size_t)t.ncells));
         if (order >= 2 && !t.cellM2) { CUDA_TRY(tree_alloc(&t.cellM2, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellE2, (size_t)t.ncells)); }
         if (order >= 4 && !t.cellM34) { CUDA_TRY(tree_alloc(&t.cellM34, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellMac, (size_t)t.ncells)); }
+        if (order >= 6) { // f-3: raw moments of degree 5 .. order and their trace record (gen_hi_orders.py), in units of the cell side
+            CUDA_TRY(tree_alloc(&t.cellHiRaw, (size_t)t.ncells * (size_t)hi_raw_floats(order)));
+            CUDA_TRY(tree_alloc(&t.cellHiT, (size_t)t.ncells * (size_t)hi_record_floats(order)));
+            t.hi_order = order;
+        }
         CUDA_TRY(launch_moments(t, order, st));
         t.mom_order = order;
     }
@@ -421,7 +426,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     a.wcell = t.wcell; a.cellA = t.cellA; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34;
     a.body = t.body; a.perm = t.idx[0]; a.group = t.group;
     a.pcoff = t.pcoff; a.ppoff = t.ppoff; a.lpc = t.glpc; a.lpp = t.glpp;
-    a.eps2 = (float)(eps * eps); a.order = order; a.periodic = t.periodic;
+    a.eps2 = (float)(eps * eps); a.order = order > 4 ? 4 : order; a.periodic = t.periodic; // orders 6, 8: the kernels of hot_forces.cu through 4, hot_hi.cu adds the rest
     a.spline = g.softening == 1; a.hinv = hreal > 0.0 ? (float)(1.0 / hreal) : INFINITY;
     for (int k = 0; k < 3; ++k) a.lo[k] = t.lo[k];
     a.size = t.size;
@@ -496,7 +501,10 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
             a.far = t.farc;
         }
         CUDA_TRY(cudaEventRecord(g.evx[3], st));
-        if (!tolmode) CUDA_TRY(launch_forces(a, st));
+        if (!tolmode) {
+            CUDA_TRY(launch_forces(a, st));
+            if (order > 4) CUDA_TRY(launch_forces_hi(a, order, t.cellHiT, hi_record_floats(t.hi_order), st));
+        }
         else { // one launch per order over its part of the cell lists; the first also takes the bodies and the far field
             ForceArgs b = a;
             b.seg = 0; b.order = 0; CUDA_TRY(launch_forces(b, st));
@@ -556,7 +564,7 @@ int hot_forces(double theta, double eps, int order, float* acc, float* pot) {
     if (!acc) return fail(HOT_EINVAL, "hot_forces: NULL acc");
     if (!(theta >= 0.0) || !(theta < 1.0)) return fail(HOT_EINVAL, "hot_forces: theta must be in [0, 1)");
     if (!(eps >= 0.0)) return fail(HOT_EINVAL, "hot_forces: eps must be >= 0");
-    if (order != 0 && order != 2 && order != 4) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2 or 4");
+    if (order != 0 && order != 2 && order != 4 && order != 6 && order != 8) return fail(HOT_EINVAL, "hot_forces: order must be 0, 2, 4, 6 or 8");
     return forces_impl(0, theta, 0.0, eps, order, acc, pot);
 }
 int hot_forces_tol(double tol, double eps, float* acc, float* pot) {

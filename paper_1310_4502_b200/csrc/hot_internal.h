@@ -69,6 +69,8 @@ struct Tree {
     CellM2* cellM2 = nullptr;
     CellM2* cellE2 = nullptr; // evaluation form of cellM2 (see CellM2)
     CellM34* cellM34 = nullptr;
+    float *cellHiRaw = nullptr, *cellHiT = nullptr; // orders 6, 8 (f-3): raw moments of degree 5.. and their trace record, per cell, in units of the cell side
+    int hi_order = 0;                        // order those two were built for (their per-cell strides follow from it)
     float4* cellMac = nullptr;               // order 4 only: b, 3 B2, 4 sqrt(B2 B4), 6 b B4 (the error bounds of R-16, numerators)
     uint32_t *glpc0 = nullptr, *glpc2 = nullptr; // per group, tolerance mode: accepted monopoles, quadrupoles
 };
@@ -177,6 +179,10 @@ cudaError_t launch_far_eval(const Tree& t, const double* D /*host [165]*/, doubl
 cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, double* farc, double eps2, cudaStream_t st);
 
 // ---- FP32 roofline denominator measured on the device (hot_peak.cu) ------------------------------------
+// ---- f-3: the terms of degree 5 .. P (P = 6, 8) of every accepted cell, added to acc / pot (hot_hi.cu) ----------
+int hi_record_floats(int order); int hi_raw_floats(int order);
+cudaError_t launch_forces_hi(const ForceArgs& a, int P, const float* hiT, int hi_stride, cudaStream_t st);
+
 // ---- f-4: kick and drift (hot_step.cu) -------------------------------------------------------------------
 cudaError_t launch_kick_drift(float* pos, float* vel, const float* acc, int64_t n, float dtk, float dtd, float lox, float loy, float loz,
                               float size, int periodic, cudaStream_t st);

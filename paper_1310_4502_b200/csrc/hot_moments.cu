@@ -5,18 +5,31 @@
 // Arithmetic is fp64 (the stage is HBM/latency bound); results are stored as the fp32 records the
 // interaction kernels stage, except the centre of mass which stays fp64.
 #include "hot_internal.h"
+#include "hot_hi_generated.inc" // f-3: record layouts and builders of the orders 6 and 8 (gen_hi_orders.py)
 
 // multi-index (a,b,c) -> position, degree-major, x>y>z (same enumeration the moments are exported in)
 __host__ __device__ constexpr int midx(int a, int b, int c) {
     int d = a + b + c;
     return d * (d + 1) * (d + 2) / 6 + (d - a) * (d - a + 1) / 2 + (d - a - b);
 }
-template <int ORDER> struct NMom { static constexpr int v = (ORDER >= 4) ? 35 : (ORDER >= 2 ? 10 : 4); };
+template <int ORDER> struct NMom { static constexpr int v = ORDER >= 2 ? (ORDER + 1) * (ORDER + 2) * (ORDER + 3) / 6 : 4; }; // 10, 35, 84, 165
 
 template <int ORDER>
 __device__ __forceinline__ void add_point(double* M, double m, double dx, double dy, double dz) {
     // M[midx(a,b,c)] += m dx^a dy^b dz^c for 2 <= a+b+c <= ORDER
-    constexpr int P = ORDER >= 4 ? 4 : 2;
+    constexpr int P = ORDER >= 4 ? ORDER : 2;
+    if constexpr (ORDER > 4) { // orders 6, 8 (f-3): plain loops -- 165 moments unrolled would take ptxas many minutes
+        double px[P + 1], py[P + 1], pz[P + 1];
+        px[0] = py[0] = pz[0] = 1.0;
+        for (int k = 1; k <= P; ++k) { px[k] = px[k - 1] * dx; py[k] = py[k - 1] * dy; pz[k] = pz[k - 1] * dz; }
+#pragma unroll 1
+        for (int d = 2; d <= P; ++d)
+#pragma unroll 1
+            for (int a = d; a >= 0; --a)
+#pragma unroll 1
+                for (int b = d - a; b >= 0; --b) M[midx(a, b, d - a - b)] += m * px[a] * py[b] * pz[d - a - b];
+        return;
+    }
     double px[P + 1], py[P + 1], pz[P + 1];
     px[0] = py[0] = pz[0] = 1.0;
 #pragma unroll
@@ -36,7 +49,35 @@ __host__ __device__ constexpr double binom_c(int n, int k) {
 // out += shift of child moments C (about its own centre, dipole = 0) by d
 template <int ORDER>
 __device__ __forceinline__ void add_shifted(double* M, const double* C, double m0, double dx, double dy, double dz) {
-    constexpr int P = ORDER >= 4 ? 4 : 2;
+    constexpr int P = ORDER >= 4 ? ORDER : 2;
+    if constexpr (ORDER > 4) { // plain loops, as in add_point
+        double px[P + 1], py[P + 1], pz[P + 1], bin[P + 1][P + 1];
+        px[0] = py[0] = pz[0] = 1.0;
+        for (int k = 1; k <= P; ++k) { px[k] = px[k - 1] * dx; py[k] = py[k - 1] * dy; pz[k] = pz[k - 1] * dz; }
+        for (int n = 0; n <= P; ++n) { bin[n][0] = 1.0; for (int k = 1; k <= n; ++k) bin[n][k] = bin[n][k - 1] * (double)(n - k + 1) / (double)k; }
+#pragma unroll 1
+        for (int d = 2; d <= P; ++d)
+#pragma unroll 1
+            for (int a = d; a >= 0; --a)
+#pragma unroll 1
+                for (int b = d - a; b >= 0; --b) {
+                    const int c = d - a - b;
+                    double s = 0;
+#pragma unroll 1
+                    for (int i = 0; i <= a; ++i)
+#pragma unroll 1
+                        for (int j = 0; j <= b; ++j)
+#pragma unroll 1
+                            for (int k = 0; k <= c; ++k) {
+                                const int e = i + j + k;
+                                if (e == 1) continue; // dipole about the child's centre of mass
+                                const double mb = e == 0 ? m0 : C[midx(i, j, k)];
+                                s += bin[a][i] * bin[b][j] * bin[c][k] * mb * px[a - i] * py[b - j] * pz[c - k];
+                            }
+                    M[midx(a, b, c)] += s;
+                }
+        return;
+    }
     double px[P + 1], py[P + 1], pz[P + 1];
     px[0] = py[0] = pz[0] = 1.0;
 #pragma unroll
@@ -67,7 +108,8 @@ __device__ __forceinline__ void add_shifted(double* M, const double* C, double m
 
 template <int ORDER>
 __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, double zy, double zz, double bmax, const double* M,
-                                           CellA* cellA, CellM2* cellM2, CellM2* cellE2, CellM34* cellM34, float4* cellMac = nullptr) {
+                                           CellA* cellA, CellM2* cellM2, CellM2* cellE2, CellM34* cellM34, float4* cellMac = nullptr,
+                                           float* hiRaw = nullptr, float* hiT = nullptr, double side = 1.0) {
     CellA A; A.zx = zx; A.zy = zy; A.zz = zz; A.m0 = (float)m0; A.bmax = __double2float_ru(bmax); // rounded up: stays a bound
     if (ORDER >= 2) {
         CellM2 Q;
@@ -101,6 +143,19 @@ __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, doub
         v[34] = v[28] + v[31] + v[33];                 // t4
         v[35] = 0.f;
         cellM34[c] = R;
+        if constexpr (ORDER > 4) { // f-3: degrees 5 .. ORDER, in units of the cell's side (fp32 range), raw and as the trace record
+            constexpr int NRAW = HiOrder<ORDER>::NRAW, NT = HiOrder<ORDER>::NT;
+            const double inv = 1.0 / side;
+            double sc = inv * inv * inv * inv;
+            int k = 35;
+#pragma unroll 1
+            for (int d = 5; d <= ORDER; ++d) {
+                sc *= inv;
+#pragma unroll 1
+                for (int q = 0; q < (d + 1) * (d + 2) / 2; ++q, ++k) hiRaw[(size_t)c * NRAW + (k - 35)] = (float)(M[k] * sc);
+            }
+            hi_record<ORDER>(M, inv, hiT + (size_t)c * NT);
+        }
         if (cellMac) { // numerators of the error bounds of DESIGN.md R-16, rounded up: b, 3 B2, 4 sqrt(B2 B4), 6 b B4
             const double B2 = M[midx(2, 0, 0)] + M[midx(0, 2, 0)] + M[midx(0, 0, 2)];
             const double B4 = M[midx(4, 0, 0)] + M[midx(0, 4, 0)] + M[midx(0, 0, 4)] + 2.0 * (M[midx(2, 2, 0)] + M[midx(2, 0, 2)] + M[midx(0, 2, 2)]);
@@ -109,7 +164,7 @@ __device__ __forceinline__ void store_cell(int64_t c, double m0, double zx, doub
     }
 }
 template <int ORDER>
-__device__ __forceinline__ void load_child(int64_t c, const CellM2* cellM2, const CellM34* cellM34, double* C) {
+__device__ __forceinline__ void load_child(int64_t c, const CellM2* cellM2, const CellM34* cellM34, double* C, const float* hiRaw = nullptr, double side = 1.0) {
     if (ORDER >= 2) {
         const float4 q0 = reinterpret_cast<const float4*>(cellM2 + c)[0], q1 = reinterpret_cast<const float4*>(cellM2 + c)[1];
         C[midx(2, 0, 0)] = q0.x; C[midx(1, 1, 0)] = q0.y; C[midx(1, 0, 1)] = q0.z;
@@ -124,6 +179,17 @@ __device__ __forceinline__ void load_child(int64_t c, const CellM2* cellM2, cons
         }
         C[34] = reinterpret_cast<const float*>(cellM34 + c)[24];
     }
+    if constexpr (ORDER > 4) {
+        constexpr int NRAW = HiOrder<ORDER>::NRAW;
+        double sc = side * side * side * side;
+        int k = 35;
+#pragma unroll 1
+        for (int d = 5; d <= ORDER; ++d) {
+            sc *= side;
+#pragma unroll 1
+            for (int q = 0; q < (d + 1) * (d + 2) / 2; ++q, ++k) C[k] = (double)hiRaw[(size_t)c * NRAW + (k - 35)] * sc;
+        }
+    }
 }
 
 // Leaves, one thread each, in BODY order (leafcell, written by tree_emit): neighbouring threads read neighbouring
@@ -132,7 +198,9 @@ struct MomArgs {
     const int32_t* leafcell; int64_t nleaves;
     const uint32_t *cfirst, *ccount, *cmask; const int32_t* cchild; const float4* body;
     CellA* cellA; CellM2* cellM2; CellM2* cellE2; CellM34* cellM34; float4* cellMac;
+    float *hiRaw, *hiT; const WalkCell* wcell; double size; // orders 6, 8: raw and trace records in units of the cell side (side = size / 2^level)
 };
+__device__ __forceinline__ double cell_side(const MomArgs& P, int64_t c) { return ldexp(P.size, -(int)(P.wcell[c].w >> 27)); }
 template <int ORDER>
 __global__ void __launch_bounds__(128) moments_leaves_kernel(const __grid_constant__ MomArgs P) {
     constexpr int NM = NMom<ORDER>::v;
@@ -156,7 +224,7 @@ __global__ void __launch_bounds__(128) moments_leaves_kernel(const __grid_consta
         bmax = fmax(bmax, dx * dx + dy * dy + dz * dz);
         if (ORDER >= 2) add_point<ORDER>(M, (double)b.w, dx, dy, dz);
     }
-    store_cell<ORDER>(c0, m0, zx, zy, zz, sqrt(bmax), M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac);
+    store_cell<ORDER>(c0, m0, zx, zy, zz, sqrt(bmax), M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac, P.hiRaw, P.hiT, ORDER > 4 ? cell_side(P, c0) : 1.0);
 }
 // an internal cell from its children (one level down, already done): parallel-axis shift, fixed child order
 template <int ORDER>
@@ -180,11 +248,11 @@ __device__ __forceinline__ void combine_children(const MomArgs& P, int64_t c) {
         bmax = fmax(bmax, sqrt(dx * dx + dy * dy + dz * dz) + (double)A.bmax);
         if (ORDER >= 2) {
             double C[NM];
-            load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C);
+            load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C, P.hiRaw, ORDER > 4 ? cell_side(P, ch + q) : 1.0);
             add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
         }
     }
-    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac);
+    store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac, P.hiRaw, P.hiT, ORDER > 4 ? cell_side(P, c) : 1.0);
 }
 // One level of internal cells.  A warp looks at 32 consecutive cells of the level, keeps the internal ones (one in eight
 // on average) and hands each to an OCTET of lanes: lane q of the octet loads child q (all children of the warp's cells in
@@ -226,7 +294,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constan
             bmax = sqrt(dx * dx + dy * dy + dz * dz) + (double)A.bmax;
             if (ORDER >= 2) {
                 double C[NM];
-                load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C);
+                load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C, P.hiRaw, ORDER > 4 ? cell_side(P, ch + q) : 1.0);
                 add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
             }
         }
@@ -238,7 +306,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constan
                 for (int k = 4; k < NM; ++k) M[k] += __shfl_xor_sync(0xffffffffu, M[k], o);
             }
         }
-        if (have && q == 0) store_cell<ORDER>(cell, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac);
+        if (have && q == 0) store_cell<ORDER>(cell, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac, P.hiRaw, P.hiT, ORDER > 4 ? cell_side(P, cell) : 1.0);
         // drop the four cells just done
         for (int i = 0; i < 4 && todo; ++i) todo &= todo - 1;
     }
@@ -257,7 +325,7 @@ template <int ORDER> static cudaError_t moments_run(const Tree& t, const MomArgs
     HOT_LAUNCHED(1);
     moments_leaves_kernel<ORDER><<<(unsigned)((t.nleaves + 127) / 128), 128, 0, st>>>(a);
     // deepest level such that levels 0 .. ltop are cheap enough for ONE block (the order-4 shift is ~2000 fp64 operations per child)
-    const int64_t top_cells = ORDER >= 4 ? 128 : 640;
+    const int64_t top_cells = ORDER >= 6 ? 16 : ORDER >= 4 ? 128 : 640;
     int ltop = -1;
     while (ltop + 1 <= t.max_level && t.level_base[ltop + 2] <= top_cells) ++ltop;
     for (int l = t.max_level - 1; l > ltop; --l) { // the deepest level holds leaves only
@@ -278,6 +346,9 @@ cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
     MomArgs a;
     a.leafcell = t.leafcell; a.nleaves = t.nleaves; a.cfirst = t.cfirst; a.ccount = t.ccount; a.cmask = t.cmask; a.cchild = t.cchild;
     a.body = t.body; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34; a.cellMac = order >= 4 ? t.cellMac : nullptr;
+    a.hiRaw = t.cellHiRaw; a.hiT = t.cellHiT; a.wcell = t.wcell; a.size = t.size;
+    if (order >= 8) return moments_run<8>(t, a, st);
+    if (order >= 6) return moments_run<6>(t, a, st);
     if (order >= 4) return moments_run<4>(t, a, st);
     if (order >= 2) return moments_run<2>(t, a, st);
     return moments_run<0>(t, a, st);

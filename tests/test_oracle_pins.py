@@ -702,3 +702,43 @@ def test_kick_drift_is_a_second_order_leapfrog():
     want = (p0 + 0.7 * v0) % 1.0
     d = np.abs(pos - want); d = np.minimum(d, 1 - d)
     assert d.max() < 1e-6
+
+
+# ---------------------------------------------------------------- f-3: orders 6 and 8
+def test_order_law_and_fig6_claim_for_high_orders():
+    """PAPER.md:267 (Fig 6): "A single p=8 multipole is more accurate than direct summation in single precision at
+    r=4" for 512 particles randomly distributed in a unit cube; and the (b/r)^(p+1) law for p = 5 .. 8."""
+    x = np.array([2.0, 1.5, -1.0])
+    for order, ratio in ((5, 64.0), (6, 128.0), (7, 256.0), (8, 512.0)):
+        errs = []
+        for b in (0.2, 0.1):
+            y, m = _cluster(b)
+            mom, z = O.moments_of(y, m, order=8)
+            a, p = O.cell_on_sink(mom, z, order, x, 0.0)
+            ad, pd = _direct_on(x, y, m, 0.0)
+            errs.append(np.linalg.norm(a - ad) / np.linalg.norm(ad))
+        assert abs(errs[0] / errs[1] / ratio - 1) < 0.2, (order, errs[0] / errs[1])
+    rng = np.random.default_rng(6)
+    y = rng.uniform(-0.5, 0.5, (512, 3)); m = np.full(512, 1 / 512)
+    xs = 4.0 * np.array([0.6, 0.64, 0.48])
+    ad, _ = _direct_on(xs, y, m, 0.0)
+    y32, x32, m32 = y.astype(np.float32), xs.astype(np.float32), m.astype(np.float32)
+    a32 = np.zeros(3, np.float32)
+    for j in range(512):  # the direct sum as a single-precision code does it
+        d = y32[j] - x32
+        u = np.float32((d * d).sum())
+        a32 += m32[j] * d / np.float32(u * np.sqrt(u))
+    e32 = np.linalg.norm(a32.astype(np.float64) - ad) / np.linalg.norm(ad)
+    mom, z = O.moments_of(y, m, order=8)
+    e = {o: np.linalg.norm(O.cell_on_sink(mom, z, o, xs, 0.0)[0] - ad) / np.linalg.norm(ad) for o in (2, 4, 6, 8)}
+    assert e[8] < e32 < e[4], (e, e32)
+    assert e[2] > e[4] > e[6] > e[8]
+
+
+def test_generated_high_order_code_is_what_the_generator_writes():
+    import importlib.util
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    path = os.path.join(root, "paper_1310_4502_b200", "csrc", "gen_hi_orders.py")
+    spec = importlib.util.spec_from_file_location("gen_hi_orders", path)
+    g = importlib.util.module_from_spec(spec); spec.loader.exec_module(g)
+    assert g.generate() == open(os.path.join(root, "paper_1310_4502_b200", "csrc", "hot_hi_generated.inc")).read()

@@ -695,3 +695,39 @@ def test_kick_drift_bit_exact_and_leapfrog_step(hot):
         hot.hot_kick_drift(dp, dv, a, 0.5e-3, 1e-3, w.lo, w.size, True)
     hot.hot_build(dp, dm, w.lo, w.size, True)   # HOT_ERANGE would raise
     assert torch.isfinite(dv).all() and float(dv.abs().max()) > 0
+
+
+# ---- f-3: expansion orders 6 and 8 from the generator ------------------------------------------
+@pytest.mark.parametrize("cfg,scale,periodic,order,theta", [(2, 13, False, 6, 0.6), (2, 13, False, 8, 0.7), (0, 12, False, 8, 0.5), (4, 10, True, 6, 0.5)])
+def test_high_order_parity(hot, cfg, scale, periodic, order, theta):
+    """Orders 6 and 8: the hand-written kernels through order 4 plus the generated terms of degree 5 .. p, against the
+    oracle's general multi-index recursion at the same order; same lists as at any order (bit-exact counts)."""
+    w = W.config(cfg, scale)
+    _build(hot, w, 16, 64)
+    O.set_moment_order(order)
+    try:
+        T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=periodic, nleaf=16, ncrit=64)
+    finally:
+        O.set_moment_order(4)
+    acc, pot = hot.hot_forces(theta, w.eps, order)
+    gg = hot.hot_export_groups()
+    sel = np.sort(np.random.default_rng(8).choice(T.ngroups, min(T.ngroups, 12 if periodic else 48), replace=False))
+    oa, op, lpc, lpp = T.forces(theta, w.eps, order, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]; gp = pot.cpu().numpy().astype(np.float64)[m]
+    an = np.linalg.norm(oa[m], axis=1)
+    if periodic:
+        an = np.maximum(an, np.sqrt((oa[m] ** 2).sum(1).mean()))
+    ea = np.linalg.norm(ga - oa[m], axis=1) / an
+    pscale = 57.18721055 * float(w.mass.astype(np.float64).sum()) / w.size if periodic else 0.0
+    ep = np.abs(gp - op[m]) / (np.abs(op[m]) + pscale)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    assert np.median(ep) <= 1e-5 and np.quantile(ep, 0.999) <= 1e-4, (np.median(ep), np.quantile(ep, 0.999))
+    if not periodic:  # the point of the high orders: the error against the definition keeps falling (fp32 floor ~1e-7)
+        ad, _ = O.direct(w.pos, w.mass, w.eps)
+        e = {}
+        for o in (4, order):
+            a, _ = hot.hot_forces(theta, w.eps, o)
+            e[o] = float(np.sqrt(((a.cpu().numpy().astype(np.float64) - ad) ** 2).sum() / (ad ** 2).sum()))
+        assert e[order] < 0.5 * e[4], e
