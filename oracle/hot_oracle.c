@@ -66,6 +66,7 @@ typedef struct {
     int nmom;         /* moments per cell: nmom_of(order they were built through) */
     double *mom, *com, *bmax;
     double *bbound;   /* b_max as the upward pass can carry it: see build_bbound */
+    double *bgmom;    /* f-1: moments about the cell CENTRE minus those of the uniform cube (build_bg_moments), [ncells][35] */
     int lazy;         /* moments computed on demand, only for the cells a requested group accepts */
     uint8_t *momdone; /* lazy: 1 where mom/com/bmax of the cell are filled */
     /* periodic far field (C-9 step 2), built on demand */
@@ -89,6 +90,8 @@ static void mi_init(void) {
             }
     MI_READY = 1;
 }
+static int g_with_dipole = 0; /* set while background-subtracted cells (expanded about cell centres, f-1) are evaluated */
+#pragma omp threadprivate(g_with_dipole)
 static int g_soft_kind = 0; /* softening kernel of every routine that takes eps: 0 Plummer, 1 cubic spline (f-4, below) */
 static double factorial(int n) { double f = 1; for (int i = 2; i <= n; ++i) f *= i; return f; }
 
@@ -299,7 +302,7 @@ void orc_destroy(orc_t *t) {
     free(t->key); free(t->skey); free(t->perm); free(t->x); free(t->m);
     free(t->ckey); free(t->clevel); free(t->cfirst); free(t->ccount); free(t->cmask);
     free(t->cchild); free(t->cparent); free(t->gcell); free(t->mom); free(t->com); free(t->bmax);
-    free(t->bbound); free(t->momdone);
+    free(t->bbound); free(t->momdone); free(t->bgmom);
     free(t);
 }
 orc_t *orc_create(const float *pos, const float *mass, int64_t n, const float lo[3], float size,
@@ -416,7 +419,7 @@ static void cell_on_sink(const double *mo, const double z[3], int order, const d
     for (int k = 0; k < nmom_of(order); ++k) {
         int a = MI_A[k], b = MI_B[k], c = MI_C[k], n = a + b + c;
         if (n > order) break;
-        if (n == 1) continue; /* dipole about the centre of mass is zero by construction */
+        if (n == 1 && !g_with_dipole) continue; /* dipole about the centre of mass is zero by construction */
         double w = ((n & 1) ? -1.0 : 1.0) / (factorial(a) * factorial(b) * factorial(c)) * mo[k];
         *pot -= w * dg(a, b, c, R, D);
         acc[0] += w * dg(a + 1, b, c, R, D);
@@ -518,6 +521,9 @@ typedef struct {
     uint8_t *mark;                   /* optional: set to 1 for every accepted cell */
     double hreal;                    /* spline softening: h = 2.8 eps in the caller's units */
     double hgrid2;                   /* spline softening: (h / grid spacing)^2; an accepted cell lies beyond h (R-17) */
+    int bgmode; int64_t klo[3], khi[3]; double rhobar; /* f-1: near cube K_G on the integer grid, mean density */
+    int64_t nbg, nvirt;              /* f-1: background-subtracted accepted cells, accepted virtual (empty) cubes */
+    double bgvol;                    /* f-1: volume of all subtracted cubes, in grid cells */
     int tolmode; double tol; double gc[3], gh; /* error-bound MAC: tolerance, group cube centre and half side */
     int64_t npc_o[3];                /* accepted cells by order: monopole, quadrupole, hexadecapole */
     /* evaluation */
@@ -885,6 +891,216 @@ void orc_tree_forces(orc_t *t, double theta, double eps, int order, const int64_
         free(a); free(p);
     }
 }
+
+/* ------------------------------------------------------------------------------------------
+ * f-1: per-cell background subtraction (Fig 2; reading DESIGN.md R-18).  Periodic
+ * boxes only: rhobar = total mass / size^3.
+ *  - For sink group G the NEAR CUBE K_G is the 5 x 5 x 5 block of cells of G's level centred on G.
+ *    Inside it the walk is the usual one ("the bodies inside cell a interact with the bodies and cells
+ *    inside the gray shaded area as usual").
+ *  - A cell outside K_G that the criterion accepts interacts through its moments about the cell CENTRE
+ *    minus those of a cube of density rhobar, through the same order p ("we only want to subtract the
+ *    uniform background expansion up to the same order as the multipole expansion of the matter"); the
+ *    dipole is present.  Empty octants of opened cells and the cubes of rejected leaves outside K_G
+ *    ("empty cell c ... must have its background contribution subtracted as well") become VIRTUAL cubes
+ *    carrying only the negative background; one that the criterion rejects is subdivided.  Cells that
+ *    straddle K_G are opened (a straddling leaf: its bodies directly, its cube as a virtual cube whose
+ *    parts inside K_G are dropped).  So the subtracted cubes tile exactly (5 size)^3 minus K_G.
+ *  - "The background contribution of the gray shaded area ... is removed analytically": what was
+ *    subtracted is added back in closed form, rhobar x [field of the homogeneous (5 size)^3 cube - field
+ *    of the homogeneous cube K_G] (orc_cube_field: "the analytic expression for the force inside a
+ *    uniform cube").
+ * ---------------------------------------------------------------------------------------- */
+static double cube_moment_1d(int a, double s) { return (a & 1) ? 0.0 : 2.0 * pow(0.5 * s, a + 1) / (a + 1); } /* int_{-s/2}^{s/2} x^a dx */
+void orc_cube_moments(double side, double *mom35) { /* raw moments of a unit-density cube about its centre */
+    mi_init();
+    for (int k = 0; k < 35; ++k) mom35[k] = cube_moment_1d(MI_A[k], side) * cube_moment_1d(MI_B[k], side) * cube_moment_1d(MI_C[k], side);
+}
+static void build_bg_moments(orc_t *t) {
+    if (t->bgmom) return;
+    mi_init();
+    t->bgmom = calloc((size_t)t->ncells * 35, sizeof(double));
+    double M = 0; for (int64_t j = 0; j < t->n; ++j) M += t->m[j];
+    double rhobar = M / (t->size * t->size * t->size), h = t->size / 2097152.0;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int64_t c = 0; c < t->ncells; ++c) {
+        int64_t o[3]; key_corner(t->ckey[c], t->clevel[c], o);
+        double side = (double)((int64_t)1 << (ORC_MAXLEVEL - t->clevel[c])) * h, ctr[3], cube[35];
+        for (int k = 0; k < 3; ++k) ctr[k] = t->lo[k] + (double)o[k] * h + 0.5 * side;
+        orc_cube_moments(side, cube);
+        double *mo = t->bgmom + (size_t)c * 35;
+        for (int64_t j = t->cfirst[c]; j < t->cfirst[c] + t->ccount[c]; ++j) {
+            double d[3]; for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - ctr[k];
+            for (int k = 0; k < 35; ++k) mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
+        }
+        for (int k = 0; k < 35; ++k) mo[k] -= rhobar * cube[k];
+    }
+}
+/* potential (= -int dy / |x - y|) and acceleration (towards the mass) at x of the homogeneous unit-density cube
+ * [lo, lo + side)^3, inside or outside: sum over the corners (X,Y,Z) = corner - x with sign (-1)^(i+j+k) of
+ *   F  = XY ln(Z+r) + YZ ln(X+r) + ZX ln(Y+r) - (X^2 atan(YZ/(Xr)) + Y^2 atan(ZX/(Yr)) + Z^2 atan(XY/(Zr))) / 2,
+ *   dF = Y ln(Z+r) + Z ln(Y+r) - X atan(YZ/(Xr))     (x component; cyclic for y, z)
+ * (refs [59, 46] of the paper; pinned by quadrature in tests/test_oracle_pins.py). */
+static double cube_F_l(double a, double b, double c, double r) { return a * b == 0 ? 0.0 : a * b * log(c + r); }
+static double cube_F_t(double a, double b, double c, double r) { return a == 0 ? 0.0 : 0.5 * a * a * atan(b * c / (a * r)); }
+static double cube_dF(double X, double Y, double Z, double r) {
+    return (Y == 0 ? 0.0 : Y * log(Z + r)) + (Z == 0 ? 0.0 : Z * log(Y + r)) - (X == 0 ? 0.0 : X * atan(Y * Z / (X * r)));
+}
+void orc_cube_field(const double x[3], const double lo[3], double side, double *phi, double acc[3]) {
+    double f = 0, g[3] = {0, 0, 0};
+    for (int i = 0; i < 2; ++i) for (int j = 0; j < 2; ++j) for (int k = 0; k < 2; ++k) {
+        double X = lo[0] + i * side - x[0], Y = lo[1] + j * side - x[1], Z = lo[2] + k * side - x[2];
+        double r = sqrt(X * X + Y * Y + Z * Z), sg = ((i + j + k) & 1) ? -1.0 : 1.0;
+        f += sg * (cube_F_l(X, Y, Z, r) + cube_F_l(Y, Z, X, r) + cube_F_l(Z, X, Y, r) - cube_F_t(X, Y, Z, r) - cube_F_t(Y, Z, X, r) - cube_F_t(Z, X, Y, r));
+        g[0] += sg * cube_dF(X, Y, Z, r); g[1] += sg * cube_dF(Y, Z, X, r); g[2] += sg * cube_dF(Z, X, Y, r);
+    }
+    *phi = f; acc[0] = g[0]; acc[1] = g[1]; acc[2] = g[2];
+}
+/* where a cube [o, o+s)^3 of the integer grid lies relative to K_G: 0 inside, 1 outside, 2 straddling */
+static int bg_where(const walk_t *w, const int64_t o[3], int64_t s) {
+    int inside = 1;
+    for (int k = 0; k < 3; ++k) {
+        if (o[k] + s <= w->klo[k] || o[k] >= w->khi[k]) return 1;
+        if (o[k] < w->klo[k] || o[k] + s > w->khi[k]) inside = 0;
+    }
+    return inside ? 0 : 2;
+}
+static int bg_mac(const walk_t *w, const int64_t oc[3], int64_t s) { /* the criterion of R-7 on a cube given by corner (image shift applied) and side */
+    uint64_t d2 = 0;
+    for (int k = 0; k < 3; ++k) {
+        int64_t g1 = oc[k] - (w->go[k] + w->gs), g2 = w->go[k] - (oc[k] + s);
+        int64_t g = g1 > g2 ? g1 : g2;
+        if (g < 0) g = 0;
+        d2 += (uint64_t)(g * g);
+    }
+    return (double)((uint64_t)(s * s)) < w->theta2 * (double)d2;
+}
+/* a virtual cube: only the negative background.  level, corner o (unshifted; the image shift is w->sh) */
+static void bg_virtual(walk_t *w, int level, const int64_t o[3]) {
+    const orc_t *t = w->t;
+    int64_t s = (int64_t)1 << (ORC_MAXLEVEL - level), oc[3] = {o[0] + w->sh[0], o[1] + w->sh[1], o[2] + w->sh[2]};
+    int where = bg_where(w, oc, s);
+    if (where == 0) return;
+    if (where == 1 && (bg_mac(w, oc, s) || level == ORC_MAXLEVEL)) {
+        w->nvirt++; w->bgvol += (double)s * (double)s * (double)s;
+        if (w->eval) {
+            double h = t->size / 2097152.0, side = (double)s * h, cube[35], ctr[3];
+            orc_cube_moments(side, cube);
+            for (int k = 0; k < 35; ++k) cube[k] *= -w->rhobar;
+            for (int k = 0; k < 3; ++k) ctr[k] = t->lo[k] + (double)oc[k] * h + 0.5 * side;
+            g_with_dipole = 1;
+            for (int64_t i = 0; i < w->gcount; ++i)
+                cell_on_sink(cube, ctr, w->order, t->x + 3 * (w->gfirst + i), w->eps2, w->acc + 3 * i, w->pot + i);
+            g_with_dipole = 0;
+        }
+        return;
+    }
+    for (int q = 0; q < 8; ++q) {
+        int64_t oo[3] = {o[0] + ((q >> 2) & 1) * (s / 2), o[1] + ((q >> 1) & 1) * (s / 2), o[2] + (q & 1) * (s / 2)};
+        bg_virtual(w, level + 1, oo);
+    }
+}
+static void walk_bg(walk_t *w, int64_t c) {
+    const orc_t *t = w->t;
+    int level = t->clevel[c];
+    int64_t o[3], s = (int64_t)1 << (ORC_MAXLEVEL - level), oc[3];
+    key_corner(t->ckey[c], level, o);
+    for (int k = 0; k < 3; ++k) oc[k] = o[k] + w->sh[k];
+    int where = bg_where(w, oc, s);
+    int accept = where != 2 && mac_accept(w, c);
+    if (accept) {
+        w->npc++;
+        if (where == 1) { w->nbg++; w->bgvol += (double)s * (double)s * (double)s; }
+        if (w->eval) {
+            if (where == 1) { /* background-subtracted, about the cell centre, dipole included */
+                double h = t->size / 2097152.0, side = (double)s * h, ctr[3];
+                for (int k = 0; k < 3; ++k) ctr[k] = t->lo[k] + (double)oc[k] * h + 0.5 * side;
+                g_with_dipole = 1;
+                for (int64_t i = 0; i < w->gcount; ++i)
+                    cell_on_sink(t->bgmom + (size_t)c * 35, ctr, w->order < 1 ? 1 : w->order, t->x + 3 * (w->gfirst + i), w->eps2, w->acc + 3 * i, w->pot + i); /* about the centre the dipole is the leading correction: order 0 keeps it */
+                g_with_dipole = 0;
+            } else
+                for (int64_t i = 0; i < w->gcount; ++i) {
+                    double z[3] = {t->com[3 * c] + w->shx[0], t->com[3 * c + 1] + w->shx[1], t->com[3 * c + 2] + w->shx[2]};
+                    cell_on_sink(t->mom + (size_t)c * t->nmom, z, w->order, t->x + 3 * (w->gfirst + i), w->eps2, w->acc + 3 * i, w->pot + i);
+                }
+        }
+        return;
+    }
+    if (t->cchild[c] < 0) { /* a rejected leaf: its bodies directly; outside K_G its cube's background separately */
+        w->npp += t->ccount[c];
+        if (w->eval)
+            for (int64_t i = 0; i < w->gcount; ++i)
+                for (int64_t j = t->cfirst[c]; j < t->cfirst[c] + t->ccount[c]; ++j) {
+                    if (j == w->gfirst + i && w->sh[0] == 0 && w->sh[1] == 0 && w->sh[2] == 0) continue;
+                    double y[3] = {t->x[3 * j] + w->shx[0], t->x[3 * j + 1] + w->shx[1], t->x[3 * j + 2] + w->shx[2]};
+                    body_on_sink(y, t->m[j], t->x + 3 * (w->gfirst + i), w->eps2, w->acc + 3 * i, w->pot + i);
+                }
+        if (where != 0) bg_virtual(w, level, o);
+        return;
+    }
+    int k = 0;
+    for (int q = 0; q < 8; ++q) {
+        if ((t->cmask[c] >> q) & 1) { walk_bg(w, t->cchild[c] + k); ++k; }
+        else if (where != 0) { /* an empty octant outside (or across) K_G */
+            int64_t oo[3] = {o[0] + ((q >> 2) & 1) * (s / 2), o[1] + ((q >> 1) & 1) * (s / 2), o[2] + (q & 1) * (s / 2)};
+            bg_virtual(w, level + 1, oo);
+        }
+    }
+}
+void orc_tree_forces_bg(orc_t *t, double theta, double eps, int order, const int64_t *groups, int64_t ng,
+                        double *acc, double *pot, int64_t *Lpc, int64_t *Lbg, int64_t *Lvirt, int64_t *Lpp, double *Vol) {
+    mi_init();
+    if (!t->periodic || order > 4) return;
+    far_prepare(t);
+    build_bg_moments(t);
+    if (!groups) ng = t->ngroups;
+    double M = 0; for (int64_t j = 0; j < t->n; ++j) M += t->m[j];
+    const double rhobar = M / (t->size * t->size * t->size), h = t->size / 2097152.0;
+#pragma omp parallel for schedule(dynamic, 4)
+    for (int64_t q = 0; q < ng; ++q) {
+        int64_t g = groups ? groups[q] : q;
+        walk_t w; walk_setup(&w, t, theta, g);
+        int64_t nG = w.gcount, npc = 0, nbg = 0, nv = 0, npp = 0;
+        double vol = 0;
+        double *a = calloc((size_t)nG * 3, sizeof(double)), *p = calloc((size_t)nG, sizeof(double));
+        for (int ix = -2; ix <= 2; ++ix) for (int iy = -2; iy <= 2; ++iy) for (int iz = -2; iz <= 2; ++iz) {
+            walk_setup(&w, t, theta, g);
+            w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
+            w.shx[0] = ix * t->size; w.shx[1] = iy * t->size; w.shx[2] = iz * t->size;
+            w.eval = acc != NULL; w.order = order; w.eps2 = eps * eps; w.acc = a; w.pot = p;
+            w.bgmode = 1; w.rhobar = rhobar;
+            for (int k = 0; k < 3; ++k) { w.klo[k] = w.go[k] - 2 * w.gs; w.khi[k] = w.go[k] + 3 * w.gs; }
+            walk_bg(&w, 0);
+            npc += w.npc; nbg += w.nbg; nv += w.nvirt; npp += w.npp; vol += w.bgvol;
+        }
+        if (Vol) Vol[q] = vol / (2097152.0 * 2097152.0 * 2097152.0); /* in units of the box volume */
+        if (Lpc) Lpc[q] = npc;
+        if (Lbg) Lbg[q] = nbg;
+        if (Lvirt) Lvirt[q] = nv;
+        if (Lpp) Lpp[q] = npp;
+        if (acc) {
+            double big_lo[3], k_lo[3], kside = 5.0 * (double)w.gs * h;
+            for (int k = 0; k < 3; ++k) { big_lo[k] = t->lo[k] - 2.0 * t->size; k_lo[k] = t->lo[k] + (double)(w.go[k] - 2 * w.gs) * h; }
+            for (int64_t i = 0; i < nG; ++i) {
+                int64_t sidx = w.gfirst + i, o = (int64_t)t->perm[sidx];
+                double v, gr[3]; far_on_sink(t, t->x + 3 * sidx, &v, gr);
+                p[i] -= v / t->size;
+                for (int k = 0; k < 3; ++k) a[3 * i + k] += gr[k] / (t->size * t->size);
+                /* what was subtracted, added back in closed form: rhobar x (homogeneous (5 size)^3 cube - homogeneous K_G) */
+                double pb, ab[3], pk, ak[3];
+                orc_cube_field(t->x + 3 * sidx, big_lo, 5.0 * t->size, &pb, ab);
+                orc_cube_field(t->x + 3 * sidx, k_lo, kside, &pk, ak);
+                p[i] += rhobar * (pb - pk);
+                for (int k = 0; k < 3; ++k) a[3 * i + k] += rhobar * (ab[k] - ak[k]);
+                for (int k = 0; k < 3; ++k) acc[3 * o + k] = a[3 * i + k];
+                pot[o] = p[i];
+            }
+        }
+        free(a); free(p);
+    }
+}
+
 /* f-2: the same evaluation with the error-bound MAC; list counts per order (summed over images) */
 void orc_tree_forces_tol(orc_t *t, double tol, double eps, const int64_t *groups, int64_t ng,
                          double *acc, double *pot, int64_t *Lpc0, int64_t *Lpc2, int64_t *Lpc4, int64_t *Lpp) {

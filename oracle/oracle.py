@@ -177,6 +177,20 @@ def set_num_threads(n):
     lib().orc_set_num_threads(int(n))
 
 
+def cube_field(x, lo, side):
+    """Potential and acceleration at x of the homogeneous unit-density cube [lo, lo+side)^3 (closed form)."""
+    x = np.ascontiguousarray(x, dtype=np.float64); lo = np.ascontiguousarray(lo, dtype=np.float64)
+    phi = C.c_double(); a = np.empty(3)
+    lib().orc_cube_field(_p(x), _p(lo), C.c_double(side), C.byref(phi), _p(a))
+    return phi.value, a
+
+
+def cube_moments(side):
+    mom = np.empty(35)
+    lib().orc_cube_moments(C.c_double(side), _p(mom))
+    return mom
+
+
 def num_threads():
     return lib().orc_num_threads()
 
@@ -295,6 +309,19 @@ class Tree:
         lib().orc_tree_forces_tol(self._h, C.c_double(tol), C.c_double(eps), _p(groups), C.c_int64(ng),
                                   _p(acc), _p(pot), _p(l0), _p(l2), _p(l4), _p(lpp))
         return acc, pot, l0, l2, l4, lpp
+
+    def forces_bg(self, theta, eps, order, groups=None):
+        """Periodic boxes with per-cell background subtraction (R-18): acc, pot, and per listed group the accepted
+        cells (all), the background-subtracted ones among them, the accepted virtual cubes, and L_pp."""
+        groups = _i64(groups)
+        ng = self.ngroups if groups is None else groups.shape[0]
+        acc = np.full((self.n, 3), np.nan); pot = np.full(self.n, np.nan)
+        lpc, lbg, lv, lpp = (np.empty(ng, np.int64) for _ in range(4))
+        vol = np.empty(ng)
+        lib().orc_tree_forces_bg(self._h, C.c_double(theta), C.c_double(eps), int(order), _p(groups), C.c_int64(ng),
+                                 _p(acc), _p(pot), _p(lpc), _p(lbg), _p(lv), _p(lpp), _p(vol))
+        self.bg_volume = vol  # subtracted volume per group in units of the box: 125 - (5 s_G / size)^3 exactly
+        return acc, pot, lpc, lbg, lv, lpp
 
     def far_table(self):
         co = np.empty(165)

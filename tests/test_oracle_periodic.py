@@ -117,3 +117,93 @@ def test_translation_invariance():
     a1, p1 = O.ewald_direct(pos1.astype(np.float32), w.mass, 1.0, w.eps)
     a2, p2 = O.ewald_direct(pos2.astype(np.float32), w.mass, 1.0, w.eps)
     assert np.abs(a1 - a2).max() < 1e-9 * np.abs(a1).max() and np.abs(p1 - p2).max() < 1e-9
+
+
+# ---------------------------------------------------------------- f-1: per-cell background subtraction (R-18)
+def test_cube_moments_and_closed_form_field():
+    """PAPER.md:76-84.  Moments of the uniform cube (rho s^3, rho s^5/12, rho s^7/80, rho s^7/144), by the
+    closed 1-D integrals and by quadrature; the closed-form potential and force of the homogeneous cube (refs [59, 46])
+    against numerical integration, outside, inside, on a face and on the plane of a face."""
+    s = 0.37
+    mom = O.cube_moments(s)
+    mi = O.multi_indices()
+    want = {(0, 0, 0): s ** 3, (2, 0, 0): s ** 5 / 12, (0, 2, 0): s ** 5 / 12, (4, 0, 0): s ** 7 / 80, (2, 2, 0): s ** 7 / 144, (0, 2, 2): s ** 7 / 144}
+    for k, ab in enumerate(mi):
+        if ab in want:
+            assert math.isclose(mom[k], want[ab], rel_tol=1e-14), ab
+        elif any(e % 2 for e in ab):
+            assert mom[k] == 0.0, ab
+    n = 200
+    q = ((np.arange(n) + 0.5) / n - 0.5) * s
+    X, Y, Z = np.meshgrid(q, q, q, indexing="ij")
+    wq = (s / n) ** 3
+    assert math.isclose(mom[mi.index((2, 2, 0))], (X ** 2 * Y ** 2).sum() * wq, rel_tol=1e-4)
+    assert math.isclose(mom[mi.index((4, 0, 0))], (X ** 4).sum() * wq, rel_tol=1e-4)
+    lo = np.array([0.1, -0.2, 0.3]); side = 0.8
+    n = 96
+    q = (np.arange(n) + 0.5) / n * side
+    X, Y, Z = np.meshgrid(lo[0] + q, lo[1] + q, lo[2] + q, indexing="ij")
+    for x, tol in (([2.0, 1.0, -1.5], 1e-6), ([0.5, 0.1, 0.6], 3e-4), ([0.95, 0.3, 0.7], 1e-4), ([0.9, 0.2, 0.7], 3e-4), ([0.3, 0.6, 0.9], 3e-4)):
+        x = np.array(x)
+        d = np.stack([X - x[0], Y - x[1], Z - x[2]], -1)
+        r = np.sqrt((d * d).sum(-1))
+        pq = -((side / n) ** 3 / r).sum()
+        aq = ((side / n) ** 3 * d / r[..., None] ** 3).sum((0, 1, 2))
+        p, a = O.cube_field(x, lo, side)
+        assert abs(p - pq) <= tol * abs(pq) * 10, (x, p, pq)
+        assert np.abs(a - aq).max() <= max(tol * 200 * np.abs(aq).max(), 2e-3), (x, a, aq)
+    # far away the cube is a point mass; inside, the Laplacian of the potential is 4 pi (finite differences)
+    p, a = O.cube_field([30.0, -20.0, 10.0], lo, side)
+    R = np.array([30.0, -20.0, 10.0]) - (lo + side / 2)
+    assert math.isclose(p, -side ** 3 / np.linalg.norm(R), rel_tol=1e-4)
+    x0 = lo + np.array([0.31, 0.42, 0.55]) * side
+    hh = 1e-3
+    lap = sum(O.cube_field(x0 + hh * e, lo, side)[0] + O.cube_field(x0 - hh * e, lo, side)[0] for e in np.eye(3)) - 6 * O.cube_field(x0, lo, side)[0]
+    assert math.isclose(lap / hh ** 2, 4 * math.pi, rel_tol=1e-4)
+    for k, e in enumerate(np.eye(3)):  # acceleration = -grad phi
+        fd = -(O.cube_field(x0 + hh * e, lo, side)[0] - O.cube_field(x0 - hh * e, lo, side)[0]) / (2 * hh)
+        assert math.isclose(O.cube_field(x0, lo, side)[1][k], fd, rel_tol=1e-5, abs_tol=1e-8)
+
+
+@pytest.mark.parametrize("cfg,side,order,theta", [(3, 10, 2, 0.5), (4, 12, 4, 0.5), (4, 10, 0, 0.6)])
+def test_background_subtraction_is_consistent_with_the_plain_periodic_tree(cfg, side, order, theta):
+    """The background-subtracted walk computes the same periodic field as the plain one and as the direct Ewald sum
+    (the subtracted cubes are added back in closed form): differences at the level of the truncation error; the
+    subtracted cubes tile exactly (5 L)^3 minus the near cube; on a perfect lattice every subtracted monopole is 0."""
+    w = W.config(cfg, side)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=True, nleaf=8, ncrit=32)
+    sel = np.arange(0, T.ngroups, max(1, T.ngroups // 12))
+    a0, p0, lpc0, lpp0 = T.forces(theta, w.eps, order, groups=sel)
+    a1, p1, lpc1, lbg, lv, lpp1 = T.forces_bg(theta, w.eps, order, groups=sel)
+    m = ~np.isnan(p0)
+    sinks = np.nonzero(m)[0]
+    ae, pe = O.ewald_direct(w.pos, w.mass, w.size, w.eps, sinks=sinks)
+    arms = np.sqrt((ae ** 2).sum(1).mean())
+    e0 = np.sqrt(((a0[m] - ae) ** 2).sum(1).mean()) / arms
+    e1 = np.sqrt(((a1[m] - ae) ** 2).sum(1).mean()) / arms
+    assert e1 < max(3 * e0, 2e-3) and e1 < 0.05, (e0, e1)
+    prms = np.sqrt(((pe - pe.mean()) ** 2).mean())
+    assert np.abs(p1[m] - pe).max() < max(3 * np.abs(p0[m] - pe).max(), 1e-3 * prms), (np.abs(p1[m] - pe).max(), np.abs(p0[m] - pe).max())
+    assert (lbg > 0).all() and (lbg <= lpc1).all() and (lpp1 <= lpp0).all()
+    c = T.cells()
+    gs = w.size * np.ldexp(1.0, -c["level"][T.groups()[sel]].astype(np.int64))
+    assert np.allclose(T.bg_volume, 125.0 - (5 * gs / w.size) ** 3, rtol=1e-12)
+    # smaller theta: both converge to the Ewald sum
+    a2, p2, *_ = T.forces_bg(0.3, w.eps, order, groups=sel)
+    e2 = np.sqrt(((a2[m] - ae) ** 2).sum(1).mean()) / arms
+    assert e2 < e1 or e2 < 1e-5
+
+
+def test_background_subtracted_moments_vanish_on_a_perfect_lattice():
+    K = 8
+    q = (np.arange(K) + 0.5) / K
+    pos = np.stack(np.meshgrid(q, q, q, indexing="ij"), -1).reshape(-1, 3).astype(np.float32)
+    mass = np.full(K ** 3, 1.0 / K ** 3, np.float32)
+    T = O.Tree(pos, mass, (0, 0, 0), 1.0, periodic=True, nleaf=1, ncrit=8)
+    a, p, lpc, lbg, lv, lpp = T.forces_bg(0.5, 1e-3, 4, groups=np.array([0, T.ngroups // 2, T.ngroups - 1]))
+    m = ~np.isnan(p)
+    a0, p0, *_ = T.forces(0.5, 1e-3, 4, groups=np.array([0, T.ngroups // 2, T.ngroups - 1]))
+    # zero force on a lattice: what is left is the truncation error of the near region, no worse than without subtraction
+    assert np.abs(a[m]).max() < 5e-6 and np.abs(a[m]).max() <= 1.5 * np.abs(a0[m]).max()
+    assert np.allclose(p[m], 2.8372974794806 / K ** 2, rtol=1e-3)
+    assert (lv == 0).all()   # a full lattice has no empty octants outside the near cube
