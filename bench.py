@@ -77,6 +77,7 @@ def parse():
     ap.add_argument("--tol", type=float, default=None, help="error-bound criterion (hot_forces_tol): absolute acceleration tolerance per interaction; not the BASELINE workload")
     ap.add_argument("--nleaf", type=int, default=16)
     ap.add_argument("--ncrit", type=int, default=256)
+    ap.add_argument("--background", action="store_true", help="periodic configs: per-cell background subtraction (hot_set_background)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -284,6 +285,7 @@ def main():
     torch.cuda.set_device(local)
     w = workload(args, rank)
     hot.hot_set_params(args.nleaf, args.ncrit)
+    hot.hot_set_background(bool(args.background))
     pos = torch.from_numpy(w.pos).cuda()
     mass = torch.from_numpy(w.mass).cuda()
     acc = torch.empty((w.n, 3), dtype=torch.float32, device="cuda")

@@ -133,6 +133,16 @@ int hot_stats(hot_stats_t* out);
  * (The compensating K1 kernel of ref [13], is not built: its formula is not in the paper.) */
 int hot_set_softening(int kind);
 
+/* Per-cell background subtraction for periodic boxes (Fig 2; R-18), 0 (default) or 1; applies to
+ * the following hot_forces calls (orders 0, 2, 4; not hot_forces_tol).  Around each sink group a near cube (5 x 5 x 5
+ * cells of the group's level) is walked as usual; a cell accepted outside it interacts through its moments about the
+ * cell centre minus those of a cube of the mean density (same order, dipole included); empty octants and the cubes of
+ * rejected leaves out there count as negative-background cubes; what was subtracted is added back in closed form (the
+ * field of a homogeneous cube).  Same field as without it to the truncation error, without the cancellation of large
+ * terms in fp32; L_pc of hot_export_groups then counts plain and background-subtracted cells together and
+ * hot_export_group_orders returns (plain cells, background-subtracted cells, accepted negative-background cubes). */
+int hot_set_background(int on);
+
 /* The "kick" and "drift" operators of the leapfrog around the force call: vel += acc * dt_kick, then
  * pos += vel * dt_drift, one fp32 fused multiply-add each; periodic != 0 wraps pos into [lo, lo + size).  In a
  * comoving background the two factors are integrals over the expansion history: the caller's.

@@ -66,6 +66,7 @@ typedef struct {
     int nmom;         /* moments per cell: nmom_of(order they were built through) */
     double *mom, *com, *bmax;
     double *bbound;   /* b_max as the upward pass can carry it: see build_bbound */
+    uint8_t *bgdone;  /* lazy trees: 1 where bgmom of the cell is filled */
     double *bgmom;    /* f-1: moments about the cell CENTRE minus those of the uniform cube (build_bg_moments), [ncells][35] */
     int lazy;         /* moments computed on demand, only for the cells a requested group accepts */
     uint8_t *momdone; /* lazy: 1 where mom/com/bmax of the cell are filled */
@@ -302,7 +303,7 @@ void orc_destroy(orc_t *t) {
     free(t->key); free(t->skey); free(t->perm); free(t->x); free(t->m);
     free(t->ckey); free(t->clevel); free(t->cfirst); free(t->ccount); free(t->cmask);
     free(t->cchild); free(t->cparent); free(t->gcell); free(t->mom); free(t->com); free(t->bmax);
-    free(t->bbound); free(t->momdone); free(t->bgmom);
+    free(t->bbound); free(t->momdone); free(t->bgmom); free(t->bgdone);
     free(t);
 }
 orc_t *orc_create(const float *pos, const float *mass, int64_t n, const float lo[3], float size,
@@ -524,6 +525,7 @@ typedef struct {
     int bgmode; int64_t klo[3], khi[3]; double rhobar; /* f-1: near cube K_G on the integer grid, mean density */
     int64_t nbg, nvirt;              /* f-1: background-subtracted accepted cells, accepted virtual (empty) cubes */
     double bgvol;                    /* f-1: volume of all subtracted cubes, in grid cells */
+    uint8_t *markbg;                 /* optional: set to 1 for every accepted background-subtracted cell */
     int tolmode; double tol; double gc[3], gh; /* error-bound MAC: tolerance, group cube centre and half side */
     int64_t npc_o[3];                /* accepted cells by order: monopole, quadrupole, hexadecapole */
     /* evaluation */
@@ -916,25 +918,29 @@ void orc_cube_moments(double side, double *mom35) { /* raw moments of a unit-den
     mi_init();
     for (int k = 0; k < 35; ++k) mom35[k] = cube_moment_1d(MI_A[k], side) * cube_moment_1d(MI_B[k], side) * cube_moment_1d(MI_C[k], side);
 }
-static void build_bg_moments(orc_t *t) {
+static void bg_cell_moments(orc_t *t, int64_t c, double rhobar) {
+    const double h = t->size / 2097152.0;
+    int64_t o[3]; key_corner(t->ckey[c], t->clevel[c], o);
+    double side = (double)((int64_t)1 << (ORC_MAXLEVEL - t->clevel[c])) * h, ctr[3], cube[35];
+    for (int k = 0; k < 3; ++k) ctr[k] = t->lo[k] + (double)o[k] * h + 0.5 * side;
+    orc_cube_moments(side, cube);
+    double *mo = t->bgmom + (size_t)c * 35;
+    for (int k = 0; k < 35; ++k) mo[k] = 0;
+    for (int64_t j = t->cfirst[c]; j < t->cfirst[c] + t->ccount[c]; ++j) {
+        double d[3]; for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - ctr[k];
+        for (int k = 0; k < 35; ++k) mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
+    }
+    for (int k = 0; k < 35; ++k) mo[k] -= rhobar * cube[k];
+}
+static double total_mass(const orc_t *t) { double M = 0; for (int64_t j = 0; j < t->n; ++j) M += t->m[j]; return M; }
+static void build_bg_moments(orc_t *t) { /* every cell, or (lazy trees) none now: orc_tree_forces_bg fills in what its groups accept */
     if (t->bgmom) return;
     mi_init();
     t->bgmom = calloc((size_t)t->ncells * 35, sizeof(double));
-    double M = 0; for (int64_t j = 0; j < t->n; ++j) M += t->m[j];
-    double rhobar = M / (t->size * t->size * t->size), h = t->size / 2097152.0;
+    if (t->lazy) { t->bgdone = calloc((size_t)t->ncells, 1); return; }
+    double rhobar = total_mass(t) / (t->size * t->size * t->size);
 #pragma omp parallel for schedule(dynamic, 64)
-    for (int64_t c = 0; c < t->ncells; ++c) {
-        int64_t o[3]; key_corner(t->ckey[c], t->clevel[c], o);
-        double side = (double)((int64_t)1 << (ORC_MAXLEVEL - t->clevel[c])) * h, ctr[3], cube[35];
-        for (int k = 0; k < 3; ++k) ctr[k] = t->lo[k] + (double)o[k] * h + 0.5 * side;
-        orc_cube_moments(side, cube);
-        double *mo = t->bgmom + (size_t)c * 35;
-        for (int64_t j = t->cfirst[c]; j < t->cfirst[c] + t->ccount[c]; ++j) {
-            double d[3]; for (int k = 0; k < 3; ++k) d[k] = t->x[3 * j + k] - ctr[k];
-            for (int k = 0; k < 35; ++k) mo[k] += t->m[j] * pow(d[0], MI_A[k]) * pow(d[1], MI_B[k]) * pow(d[2], MI_C[k]);
-        }
-        for (int k = 0; k < 35; ++k) mo[k] -= rhobar * cube[k];
-    }
+    for (int64_t c = 0; c < t->ncells; ++c) bg_cell_moments(t, c, rhobar);
 }
 /* potential (= -int dy / |x - y|) and acceleration (towards the mass) at x of the homogeneous unit-density cube
  * [lo, lo + side)^3, inside or outside: sum over the corners (X,Y,Z) = corner - x with sign (-1)^(i+j+k) of
@@ -1010,7 +1016,8 @@ static void walk_bg(walk_t *w, int64_t c) {
     int accept = where != 2 && mac_accept(w, c);
     if (accept) {
         w->npc++;
-        if (where == 1) { w->nbg++; w->bgvol += (double)s * (double)s * (double)s; }
+        if (where == 1) { w->nbg++; w->bgvol += (double)s * (double)s * (double)s; if (w->markbg) w->markbg[c] = 1; }
+        else if (w->mark) w->mark[c] = 1;
         if (w->eval) {
             if (where == 1) { /* background-subtracted, about the cell centre, dipole included */
                 double h = t->size / 2097152.0, side = (double)s * h, ctr[3];
@@ -1055,8 +1062,25 @@ void orc_tree_forces_bg(orc_t *t, double theta, double eps, int order, const int
     far_prepare(t);
     build_bg_moments(t);
     if (!groups) ng = t->ngroups;
-    double M = 0; for (int64_t j = 0; j < t->n; ++j) M += t->m[j];
-    const double rhobar = M / (t->size * t->size * t->size), h = t->size / 2097152.0;
+    const double rhobar = total_mass(t) / (t->size * t->size * t->size), h = t->size / 2097152.0;
+    if (t->lazy) { /* the moments (both kinds) of the cells these groups accept: mark them (walk only), then fill them in */
+        uint8_t *need = calloc((size_t)t->ncells, 1), *needbg = calloc((size_t)t->ncells, 1);
+#pragma omp parallel for schedule(dynamic, 4)
+        for (int64_t q = 0; q < ng; ++q)
+            for (int ix = -2; ix <= 2; ++ix) for (int iy = -2; iy <= 2; ++iy) for (int iz = -2; iz <= 2; ++iz) {
+                walk_t w; walk_setup(&w, t, theta, groups ? groups[q] : q);
+                w.sh[0] = (int64_t)ix << ORC_MAXLEVEL; w.sh[1] = (int64_t)iy << ORC_MAXLEVEL; w.sh[2] = (int64_t)iz << ORC_MAXLEVEL;
+                w.bgmode = 1; w.mark = need; w.markbg = needbg;
+                for (int k = 0; k < 3; ++k) { w.klo[k] = w.go[k] - 2 * w.gs; w.khi[k] = w.go[k] + 3 * w.gs; }
+                walk_bg(&w, 0);
+            }
+#pragma omp parallel for schedule(dynamic, 1)
+        for (int64_t c = 0; c < t->ncells; ++c) {
+            if (need[c] && !t->momdone[c]) { cell_moments(t, c); t->momdone[c] = 1; }
+            if (needbg[c] && !t->bgdone[c]) { bg_cell_moments(t, c, rhobar); t->bgdone[c] = 1; }
+        }
+        free(need); free(needbg);
+    }
 #pragma omp parallel for schedule(dynamic, 4)
     for (int64_t q = 0; q < ng; ++q) {
         int64_t g = groups ? groups[q] : q;

@@ -63,6 +63,7 @@ def _load():
         lib.hot_set_params.argtypes = [C.c_int, C.c_int]
         lib.hot_set_list_arena.argtypes = [C.c_int64]
         lib.hot_set_softening.argtypes = [C.c_int]
+        lib.hot_set_background.argtypes = [C.c_int]
         lib.hot_kick_drift.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_float, hot_box, C.c_int]
         lib.hot_far_coefficients.argtypes = [C.c_void_p]
         lib.hot_measure_fp32.argtypes = [C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -134,6 +135,11 @@ def hot_set_params(nleaf: int = 16, ncrit: int = 256):
 def hot_set_softening(kind: int = 0):
     """0: Plummer (default); 1: cubic spline with h = 2.8 eps."""
     _check(_load().hot_set_softening(int(kind)))
+
+
+def hot_set_background(on: bool = False):
+    """Per-cell background subtraction in periodic boxes for the following hot_forces calls."""
+    _check(_load().hot_set_background(int(bool(on))))
 
 
 def hot_kick_drift(pos, vel, acc, dt_kick, dt_drift, lo, size, periodic=False):

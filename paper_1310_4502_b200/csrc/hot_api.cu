@@ -18,7 +18,9 @@ struct Ctx {
     bool built = false;
     int nleaf = 16, ncrit = 256;
     int softening = 0; // 0 Plummer, 1 cubic spline (hot_set_softening)
-    int last_order = -1, last_tolmode = 0;
+    int background = 0; // 1: per-cell background subtraction in periodic boxes (hot_set_background)
+    uint4 *d_vstack = nullptr, *d_vstage = nullptr, *d_pvlist = nullptr; // virtual cubes of the background-subtracted walk
+    int last_order = -1, last_tolmode = 0, last_bgmode = 0;
     char err[512] = "";
     // scratch owned across calls
     int* d_flags = nullptr;               // [0] build error bits, [1] hash max probe, [2] forces error bits
@@ -180,6 +182,12 @@ int hot_set_params(int nleaf, int ncrit) {
 int hot_set_softening(int kind) {
     if (kind != 0 && kind != 1) return fail(HOT_EINVAL, "hot_set_softening: kind must be 0 (Plummer) or 1 (cubic spline)");
     g.softening = kind;
+    return HOT_OK;
+}
+
+int hot_set_background(int on) {
+    if (on != 0 && on != 1) return fail(HOT_EINVAL, "hot_set_background: 0 or 1");
+    g.background = on;
     return HOT_OK;
 }
 
@@ -351,9 +359,19 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
             CUDA_TRY(cudaMemcpyAsync(S, g.d_farS, sizeof(S), cudaMemcpyDeviceToHost, st));
             CUDA_TRY(cudaStreamSynchronize(st));
             far_sink_polynomial(S, t.farD);
+            t.total_mass = S[0];
             CUDA_TRY(launch_far_eval(t, t.farD, t.far, st)); // depends on the bodies only: kept for every hot_forces on this build
             t.far_ready = true;
         }
+    }
+    const int bgmode = t.periodic && g.background && !tolmode && order <= 4; // f-1 (R-18)
+    const double rhobar = t.total_mass / (t.size * t.size * t.size);
+    if (bgmode && t.bg_order != order) { // moments about the cell centres minus the uniform cube's, through the same order
+        CUDA_TRY(tree_alloc(&t.bgA, (size_t)t.ncells));
+        if (order >= 2) CUDA_TRY(tree_alloc(&t.bgE2, (size_t)t.ncells));
+        if (order >= 4) CUDA_TRY(tree_alloc(&t.bgM34, (size_t)t.ncells));
+        CUDA_TRY(launch_bg_moments(t, order, rhobar, st));
+        t.bg_order = order;
     }
     CUDA_TRY(cudaEventRecord(g.ev[8], st));
     // S7: the walk writes every group's lists into the arena; S8/S9/S10 evaluate them.  The arena is
@@ -371,7 +389,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     CUDA_TRY(tree_alloc(&t.glvis, (size_t)ng));
     CUDA_TRY(tree_alloc(&t.pcoff, (size_t)ng));
     CUDA_TRY(tree_alloc(&t.ppoff, (size_t)ng));
-    CUDA_TRY(tree_alloc(&g.d_tops, 2));
+    CUDA_TRY(tree_alloc(&g.d_tops, 3));
     const size_t esz = t.periodic ? 5 : 4; // bytes per list entry: u32 (+ u8 image id)
     if (g.stage_cap < 1024) g.stage_cap = 16384;
     // arena capacity in entries: what the last call needed plus 12%, else a first guess
@@ -417,7 +435,20 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     wa.hreal = hreal;
     wa.tolmode = tolmode; wa.tol = tol; wa.size = t.size; wa.cellA = t.cellA; wa.cellMac = t.cellMac;
     for (int k = 0; k < 3; ++k) wa.lo[k] = t.lo[k];
-    if (tolmode) { CUDA_TRY(tree_alloc(&t.glpc0, (size_t)ng)); CUDA_TRY(tree_alloc(&t.glpc2, (size_t)ng)); }
+    if (tolmode || bgmode) { CUDA_TRY(tree_alloc(&t.glpc0, (size_t)ng)); CUDA_TRY(tree_alloc(&t.glpc2, (size_t)ng)); }
+    wa.bgmode = bgmode; wa.cmask = t.cmask;
+    const int64_t vstack_cap = 4096, vstage_cap = 4096;
+    unsigned long long cappv = 0;
+    if (bgmode) {
+        CUDA_TRY(tree_alloc(&g.d_vstack, (size_t)nwarps * (size_t)vstack_cap));
+        CUDA_TRY(tree_alloc(&g.d_vstage, (size_t)nwarps * (size_t)vstage_cap));
+        cappv = (unsigned long long)ng * 192ull + 65536ull;
+        CUDA_TRY(tree_alloc(&g.d_pvlist, (size_t)cappv));
+        CUDA_TRY(tree_alloc(&t.glpv, (size_t)ng));
+        CUDA_TRY(tree_alloc(&t.gpvoff, (size_t)ng));
+    }
+    wa.vstack = g.d_vstack; wa.vstack_cap = vstack_cap; wa.vstage = g.d_vstage; wa.vstage_cap = vstage_cap;
+    wa.pvlist = g.d_pvlist; wa.cappv = cappv; wa.lpv = t.glpv; wa.pvoff = t.gpvoff;
     wa.lpc0 = t.glpc0; wa.lpc2 = t.glpc2;
     wa.periodic = t.periodic; wa.lpc = t.glpc; wa.lpp = t.glpp; wa.lvis = t.glvis; wa.pcoff = t.pcoff; wa.ppoff = t.ppoff;
     wa.tops = g.d_tops; wa.first_fail = g.d_flags + 3;
@@ -455,7 +486,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     while (g0 < ng) {
         const int ff0 = INT_MAX;
         CUDA_TRY(cudaMemsetAsync(g.d_counter, 0, 2 * sizeof(unsigned int), st));
-        CUDA_TRY(cudaMemsetAsync(g.d_tops, 0, 2 * sizeof(unsigned long long), st));
+        CUDA_TRY(cudaMemsetAsync(g.d_tops, 0, 3 * sizeof(unsigned long long), st));
         CUDA_TRY(cudaMemcpyAsync(g.d_flags + 3, &ff0, sizeof(int), cudaMemcpyHostToDevice, st));
         wa.g0 = g0; wa.g1 = g0 + budget < ng ? g0 + budget : ng;
         wa.pclist = g.d_pclist; wa.pplist = g.d_pplist; wa.pcimg = g.d_pcimg; wa.ppimg = g.d_ppimg; wa.cappc = cappc; wa.cappp = cappp;
@@ -470,6 +501,8 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         CUDA_TRY(cudaStreamSynchronize(st));
         ms_walk += ms_between(g.evx[0], g.evx[1]);
         if (fl[0] & 4) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted");
+        if (fl[0] & 16) return fail(HOT_EINTERNAL, "hot_forces: virtual-cube scratch of the background-subtracted walk exhausted");
+        if (fl[0] & 32) return fail(HOT_ENOMEM, "hot_forces: the virtual-cube list of the background-subtracted walk does not fit its arena");
         if (fl[0] & 8) { // a group's lists outgrew the per-warp staging area: enlarge it and walk this range again
             if (g.stage_cap >= ((int64_t)1 << 26)) return fail(HOT_ENOMEM, "hot_forces: one sink group's interaction list exceeds 2^26 entries");
             g.stage_cap *= 4;
@@ -495,7 +528,12 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         a.nsb = (unsigned int)((F - g0 + ((int64_t)1 << a.sb_shift) - 1) >> a.sb_shift);
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
         CUDA_TRY(launch_plan(a, st));
-        if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
+        if (bgmode) { // far field + background added back + flagged cells + virtual cubes -> farc, in fp64 (hot_bg.cu)
+            CUDA_TRY(cudaEventRecord(g.evx[4], st));
+            a.lpc0 = t.glpc0; a.lpc2 = t.glpc2;
+            CUDA_TRY(launch_forces_bg(a, t, t.far, t.farc, g.d_pvlist, t.glpv, t.gpvoff, rhobar, st));
+            a.far = t.farc; a.seg = 0; // the interaction kernel takes the plain cells (inside the near cube) and the bodies
+        } else if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
             CUDA_TRY(cudaEventRecord(g.evx[4], st));
             CUDA_TRY(launch_coarse_monopoles(a, t.far, t.farc, g.softening == 1 ? 0.0 : eps * eps, st)); // spline: accepted cells are Newtonian
             a.far = t.farc;
@@ -543,7 +581,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     s.pc_monopole = s.pc_quadrupole = s.pc_hexadecapole = 0;
     if (tolmode) { s.pc_monopole = stat[4]; s.pc_quadrupole = stat[5]; s.pc_hexadecapole = stat[3] - stat[4] - stat[5]; }
     else (order == 0 ? s.pc_monopole : order == 2 ? s.pc_quadrupole : s.pc_hexadecapole) = stat[3];
-    g.last_tolmode = tolmode;
+    g.last_tolmode = tolmode; g.last_bgmode = bgmode;
     s.ms_moments = ms_between(g.ev[5], g.ev[6]);
     s.ms_walk = ms_walk;
     s.ms_eval = ms_eval;
@@ -583,9 +621,19 @@ int hot_export_group_orders(uint64_t* lmono, uint64_t* lquad, uint64_t* lhexa, i
     const size_t ng = (size_t)t.ngroups;
     std::vector<uint32_t> tot(ng), a0(ng, 0), a2(ng, 0);
     CUDA_TRY(cudaMemcpy(tot.data(), t.glpc, 4 * ng, cudaMemcpyDeviceToHost));
-    if (g.last_tolmode) {
+    if (g.last_tolmode || g.last_bgmode) {
         CUDA_TRY(cudaMemcpy(a0.data(), t.glpc0, 4 * ng, cudaMemcpyDeviceToHost));
         CUDA_TRY(cudaMemcpy(a2.data(), t.glpc2, 4 * ng, cudaMemcpyDeviceToHost));
+    }
+    if (g.last_bgmode) { // (plain cells, background-subtracted cells, accepted virtual cubes)
+        std::vector<uint32_t> pv(ng);
+        CUDA_TRY(cudaMemcpy(pv.data(), t.glpv, 4 * ng, cudaMemcpyDeviceToHost));
+        for (size_t i = 0; i < ng; ++i) {
+            if (lmono) lmono[i] = a0[i];
+            if (lquad) lquad[i] = a2[i];
+            if (lhexa) lhexa[i] = pv[i];
+        }
+        return HOT_OK;
     } else if (g.last_order == 0) a0 = tot;
     else if (g.last_order == 2) a2 = tot;
     for (size_t i = 0; i < ng; ++i) {

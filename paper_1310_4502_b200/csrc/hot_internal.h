@@ -71,6 +71,10 @@ struct Tree {
     CellM34* cellM34 = nullptr;
     float *cellHiRaw = nullptr, *cellHiT = nullptr; // orders 6, 8 (f-3): raw moments of degree 5.. and their trace record, per cell, in units of the cell side
     int hi_order = 0;                        // order those two were built for (their per-cell strides follow from it)
+    // f-1 (background subtraction, periodic): per cell, moments about the cell centre minus the uniform cube's
+    float4* bgA = nullptr; CellM2* bgE2 = nullptr; CellM34* bgM34 = nullptr; int bg_order = -1;
+    double total_mass = 0.0;                 // sum of the masses in fp64 (the far field's zeroth moment)
+    uint32_t* glpv = nullptr; unsigned long long* gpvoff = nullptr; // per group: accepted virtual cubes, where they start
     float4* cellMac = nullptr;               // order 4 only: b, 3 B2, 4 sqrt(B2 B4), 6 b B4 (the error bounds of R-16, numerators)
     uint32_t *glpc0 = nullptr, *glpc2 = nullptr; // per group, tolerance mode: accepted monopoles, quadrupoles
 };
@@ -140,6 +144,12 @@ struct WalkArgs {
     double hreal;                          // spline softening: h (an accepted cell lies wholly beyond it), else 0
     const CellA* cellA; const float4* cellMac;   // per cell: centre of mass / (b, 3 B2, 4 sqrt(B2 B4), 6 b B4)
     uint32_t *lpc0, *lpc2;                 // per group: accepted monopoles, quadrupoles (the list is ordered mono | quad | hexa)
+    // background subtraction (bgmode != 0, periodic; R-18): lpc0 / lpc2 = plain / background-subtracted cells
+    int bgmode; const uint32_t* cmask;
+    uint4* vstack; int64_t vstack_cap;     // per warp: virtual cubes still to look at
+    uint4* vstage; int64_t vstage_cap;     // per warp: accepted virtual cubes of the group being walked
+    uint4* pvlist; unsigned long long cappv; // arena of the accepted virtual cubes (tops[2]); per group lpv, pvoff
+    uint32_t* lpv; unsigned long long* pvoff;
 };
 int walk_grid_warps();
 cudaError_t launch_walk(const WalkArgs& a, cudaStream_t st);
@@ -179,6 +189,12 @@ cudaError_t launch_far_eval(const Tree& t, const double* D /*host [165]*/, doubl
 cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, double* farc, double eps2, cudaStream_t st);
 
 // ---- FP32 roofline denominator measured on the device (hot_peak.cu) ------------------------------------
+// ---- f-1: per-cell background subtraction (hot_bg.cu) ---------------------------------------------------------
+cudaError_t launch_bg_moments(const Tree& t, int order, double rhobar, cudaStream_t st);
+// farc[body] = far[body] + background added back in closed form + flagged cells + virtual cubes, groups [a.g0, a.g1)
+cudaError_t launch_forces_bg(const ForceArgs& a, const Tree& t, const double* far, double* farc, const uint4* pvlist, const uint32_t* lpv,
+                             const unsigned long long* pvoff, double rhobar, cudaStream_t st);
+
 // ---- f-3: the terms of degree 5 .. P (P = 6, 8) of every accepted cell, added to acc / pot (hot_hi.cu) ----------
 int hi_record_floats(int order); int hi_raw_floats(int order);
 cudaError_t launch_forces_hi(const ForceArgs& a, int P, const float* hiT, int hi_stride, cudaStream_t st);

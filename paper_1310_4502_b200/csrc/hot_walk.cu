@@ -34,7 +34,12 @@
 // monopole / quadrupole / hexadecapole whose bound at the distance to the group's cube is below the tolerance; the
 // order rides in bits 29-30 of the staged entry and the list is laid out monopoles | quadrupoles | hexadecapoles.
 #define HOT_ORDER_SHIFT 29
-template <bool PER, bool TOL>
+// BG (periodic boxes, with the opening angle): per-cell background subtraction (R-18; Fig 2).
+// K_G = the 5 x 5 x 5 block of cells of the group's level around the group.  A cell across K_G's boundary is opened;
+// an accepted cell outside K_G is flagged (bit 29: it is evaluated about its centre minus the uniform cube; the list is
+// laid out plain | flagged); empty octants of opened cells and the cubes of rejected leaves outside K_G go to a stack of
+// VIRTUAL cubes (only the negative background), which are accepted by the same criterion or subdivided.
+template <bool PER, bool TOL, bool BG>
 __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_constant__ WalkArgs P) {
     __shared__ uint32_t s_ring[WALK_WARPS][RING];
     __shared__ uint8_t s_img[PER ? WALK_WARPS : 1][PER ? RING : 1];
@@ -48,6 +53,8 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
     uint32_t* const spp = spc + P.stage_cap;                 // staged run list
     uint8_t* const ipc = PER ? P.stage_img + gwarp * 2 * P.stage_cap : nullptr;
     uint8_t* const ipp = PER ? ipc + P.stage_cap : nullptr;
+    uint4* const vstack = BG ? P.vstack + gwarp * P.vstack_cap : nullptr;   // virtual cubes to look at: (x | y<<21, y>>11 | z<<10, level, image)
+    uint4* const vstage = BG ? P.vstage + gwarp * P.vstage_cap : nullptr;   // accepted virtual cubes of the group
     const uint32_t lt = (1u << lane) - 1u;
     constexpr int M = RING - 1, DEQ_DFS = RING / 4, NIMG = PER ? 125 : 1;
     unsigned long long nspill = 0;
@@ -70,7 +77,9 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
             gcx = P.lo[0] + ((double)gox + 0.5 * gs) * h; gcy = P.lo[1] + ((double)goy + 0.5 * gs) * h; gcz = P.lo[2] + ((double)goz + 0.5 * gs) * h;
             gh = 0.5 * (double)gs * h;
         }
-        uint32_t n0 = 0, n2 = 0; // TOL: accepted monopoles, quadrupoles
+        uint32_t n0 = 0, n2 = 0; // TOL: accepted monopoles, quadrupoles; BG: plain, background-subtracted cells
+        const int klx = gox - 2 * gs, kly = goy - 2 * gs, klz = goz - 2 * gs, khx = gox + 3 * gs, khy = goy + 3 * gs, khz = goz + 3 * gs; // BG: K_G
+        uint32_t vtop = 0, npv = 0; // BG: virtual cubes on the stack / accepted
         uint32_t npc = 0, nrun = 0, nbody = 0, nvis = 0; // list lengths, bodies in the runs, cells visited
         int head = 0, top = 0, gtop = 0, next_img = 0;
         while (true) {
@@ -139,8 +148,13 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
             const uint32_t gy = (uint32_t)max(0, max(cy - ghy, goy - (cy + s)));
             const uint32_t gz = (uint32_t)max(0, max(cz - ghz, goz - (cz + s)));
             const unsigned long long d2 = (unsigned long long)gx * gx + (unsigned long long)gy * gy + (unsigned long long)gz * gz;
-            bool acc; int ocode = 0;
-            if (!TOL) acc = v && d2 >= P.mac_t[lev]; // == (double)(s*s) < theta^2 * (double)d2, see mac_table()
+            bool acc; int ocode = 0, where = 0; // BG: 0 inside K_G, 1 outside, 2 across its boundary
+            if (BG && v) {
+                const bool out = cx + s <= klx || cx >= khx || cy + s <= kly || cy >= khy || cz + s <= klz || cz >= khz;
+                const bool in = cx >= klx && cx + s <= khx && cy >= kly && cy + s <= khy && cz >= klz && cz + s <= khz;
+                where = out ? 1 : (in ? 0 : 2);
+            }
+            if (!TOL) { acc = v && d2 >= P.mac_t[lev] && (!BG || where != 2); if (BG) ocode = where == 1; } // == (double)(s*s) < theta^2 * (double)d2, see mac_table()
             else {
                 acc = false;
                 if (v) {
@@ -166,10 +180,10 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
             if (acc) {
                 const uint32_t p = npc + __popc(macc & lt);
                 // periodic: cells of the coarsest levels are marked; their monopoles are summed in fp64 (hot_periodic.cu)
-                if (p < scap) { spc[p] = ((PER && lev <= HOT_COARSE_LEVEL) ? (c | HOT_COARSE_FLAG) : c) | (TOL ? (uint32_t)ocode << HOT_ORDER_SHIFT : 0u); if (PER) ipc[p] = (uint8_t)im; }
+                if (p < scap) { spc[p] = ((PER && !BG && lev <= HOT_COARSE_LEVEL) ? (c | HOT_COARSE_FLAG) : c) | ((TOL || BG) ? (uint32_t)ocode << HOT_ORDER_SHIFT : 0u); if (PER) ipc[p] = (uint8_t)im; }
             }
             npc += __popc(macc);
-            if (TOL) { n0 += __popc(__ballot_sync(FULL, acc && ocode == 0)); n2 += __popc(__ballot_sync(FULL, acc && ocode == 1)); }
+            if (TOL || BG) { n0 += __popc(__ballot_sync(FULL, acc && ocode == 0)); n2 += __popc(__ballot_sync(FULL, acc && ocode == 1)); }
             // rejected leaves -> one body run each (a leaf holds <= 32 bodies except at the finest level)
             if (mrej) {
                 uint32_t nb = rej_leaf ? cnt : 0u;
@@ -204,7 +218,69 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
                 if (PER) rimg[p] = (uint8_t)im;
             }
             top += __popc(mopen);
+            if (BG) { // virtual cubes: the cube of a rejected leaf, the empty octants of an opened cell -- outside or across K_G only
+                uint32_t miss = 0;
+                if (open && where != 0) miss = ~P.cmask[c] & 0xffu;
+                const int nv = (rej_leaf && where != 0) ? 1 : __popc(miss);
+                int incl = nv;
+#pragma unroll
+                for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULL, incl, o); if (lane >= o) incl += y; }
+                const int tot = __shfl_sync(FULL, incl, 31);
+                if (tot) {
+                    if ((int64_t)vtop + tot > P.vstack_cap) { if (lane == 0) atomicOr(P.errflag, 16); }
+                    else {
+                        uint32_t at = vtop + (uint32_t)(incl - nv);
+                        const int ux = cx - ((im / 25 - 2) << HOT_MAXLEVEL), uy = cy - (((im / 5) % 5 - 2) << HOT_MAXLEVEL), uz = cz - ((im % 5 - 2) << HOT_MAXLEVEL); // unshifted corner
+                        if (rej_leaf && where != 0) vstack[at] = make_uint4((uint32_t)ux | ((uint32_t)uy << 21), ((uint32_t)uy >> 11) | ((uint32_t)uz << 10), (uint32_t)lev, (uint32_t)im);
+                        else
+                            for (uint32_t mm = miss; mm; mm &= mm - 1) {
+                                const int q8 = __ffs((int)mm) - 1, hs = s >> 1;
+                                const uint32_t qx = (uint32_t)(ux + ((q8 >> 2) & 1) * hs), qy = (uint32_t)(uy + ((q8 >> 1) & 1) * hs), qz = (uint32_t)(uz + (q8 & 1) * hs);
+                                vstack[at++] = make_uint4(qx | (qy << 21), (qy >> 11) | (qz << 10), (uint32_t)lev + 1u, (uint32_t)im);
+                            }
+                        vtop += (uint32_t)tot;
+                    }
+                }
+            }
             __syncwarp();
+        }
+        if (BG) { // the virtual cubes: inside K_G dropped; outside accepted by the criterion (or at the finest level); else subdivided
+            while (vtop > 0) {
+                const uint32_t take = min(32u, vtop);
+                vtop -= take;
+                __syncwarp();
+                uint4 e = make_uint4(0, 0, 0, 0);
+                const bool have = (uint32_t)lane < take;
+                if (have) e = vstack[vtop + lane];
+                const int lev = (int)e.z, im = (int)e.w, s = 1 << (HOT_MAXLEVEL - lev);
+                const int ux = (int)(e.x & 0x1fffffu), uy = (int)((e.x >> 21) | ((e.y & 0x3ffu) << 11)), uz = (int)((e.y >> 10) & 0x1fffffu);
+                const int cx = ux + ((im / 25 - 2) << HOT_MAXLEVEL), cy = uy + (((im / 5) % 5 - 2) << HOT_MAXLEVEL), cz = uz + ((im % 5 - 2) << HOT_MAXLEVEL);
+                const bool out = cx + s <= klx || cx >= khx || cy + s <= kly || cy >= khy || cz + s <= klz || cz >= khz;
+                const bool in = cx >= klx && cx + s <= khx && cy >= kly && cy + s <= khy && cz >= klz && cz + s <= khz;
+                const uint32_t gx = (uint32_t)max(0, max(cx - ghx, gox - (cx + s)));
+                const uint32_t gy = (uint32_t)max(0, max(cy - ghy, goy - (cy + s)));
+                const uint32_t gz = (uint32_t)max(0, max(cz - ghz, goz - (cz + s)));
+                const unsigned long long d2 = (unsigned long long)gx * gx + (unsigned long long)gy * gy + (unsigned long long)gz * gz;
+                const bool accv = have && out && (d2 >= P.mac_t[lev] || lev == HOT_MAXLEVEL);
+                const bool sub = have && !in && !accv;
+                const uint32_t macc = __ballot_sync(FULL, accv), msub = __ballot_sync(FULL, sub);
+                if (accv) { const uint32_t q = npv + __popc(macc & lt); if (q < (uint32_t)P.vstage_cap) vstage[q] = e; }
+                npv += __popc(macc);
+                if (msub) {
+                    const uint32_t tot = 8u * __popc(msub);
+                    if ((int64_t)vtop + tot > P.vstack_cap) { if (lane == 0) atomicOr(P.errflag, 16); break; }
+                    if (sub) {
+                        uint32_t at = vtop + 8u * __popc(msub & lt);
+                        const int hs = s >> 1;
+                        for (int q8 = 0; q8 < 8; ++q8) {
+                            const uint32_t qx = (uint32_t)(ux + ((q8 >> 2) & 1) * hs), qy = (uint32_t)(uy + ((q8 >> 1) & 1) * hs), qz = (uint32_t)(uz + (q8 & 1) * hs);
+                            vstack[at++] = make_uint4(qx | (qy << 21), (qy >> 11) | (qz << 10), (uint32_t)lev + 1u, (uint32_t)im);
+                        }
+                    }
+                    vtop += tot;
+                }
+            }
+            if (npv > (uint32_t)P.vstage_cap) { if (lane == 0) atomicOr(P.errflag, 16); continue; }
         }
         // the group's lists are complete: take a slice of the arena and move them there; the body
         // runs are expanded to one body index per entry on the way (32 entries per step)
@@ -221,7 +297,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
         if (!ok) continue;
         pcb = __shfl_sync(FULL, pcb, 0); ppb = __shfl_sync(FULL, ppb, 0);
         __syncwarp();
-        if (!TOL) {
+        if (!TOL && !BG) {
             for (uint32_t j = lane; j < npc; j += 32) { P.pclist[pcb + j] = spc[j]; if (PER) P.pcimg[pcb + j] = ipc[j]; }
         } else { // three stable passes: monopoles, quadrupoles, hexadecapoles; the order bits are dropped
             uint32_t base = 0;
@@ -263,9 +339,20 @@ __global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_cons
                 else { roff = 0u; r += (uint32_t)ne; }
             }
         }
+        if (BG) { // the accepted virtual cubes: their own arena
+            unsigned long long pvb = 0;
+            if (lane == 0) {
+                pvb = atomicAdd(P.tops + 2, (unsigned long long)npv);
+                if (pvb + npv > P.cappv) { atomicOr(P.errflag, 32); pvb = ~0ull; }
+            }
+            pvb = __shfl_sync(FULL, pvb, 0);
+            __syncwarp();
+            if (pvb != ~0ull) for (uint32_t j = lane; j < npv; j += 32) P.pvlist[pvb + j] = vstage[j];
+            if (lane == 0) { P.lpv[gi] = npv; P.pvoff[gi] = pvb == ~0ull ? 0ull : pvb; }
+        }
         if (lane == 0) {
             P.lpc[gi] = npc; P.lpp[gi] = nbody; P.lvis[gi] = nvis;
-            if (TOL) { P.lpc0[gi] = n0; P.lpc2[gi] = n2; }
+            if (TOL || BG) { P.lpc0[gi] = n0; P.lpc2[gi] = n2; }
             P.pcoff[gi] = pcb; P.ppoff[gi] = ppb;
         }
         __syncwarp();
@@ -279,10 +366,11 @@ int walk_grid_warps() { // resident warps of the walk grid: blocks/SM of the var
         int dev = 0, nsm = 0, occ = 1 << 20, o = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false, true>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, true>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false, false, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, false, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<false, true, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, true, false>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&o, walk_kernel<true, false, true>, WALK_WARPS * 32, 0) == cudaSuccess && o > 0 && o < occ) occ = o;
         if (occ == 1 << 20) occ = 1;
         cudaGetLastError();
         nw = nsm * occ * WALK_WARPS;
@@ -293,10 +381,11 @@ cudaError_t launch_walk(const WalkArgs& a, cudaStream_t st) {
     const int nb = walk_grid_warps() / WALK_WARPS;
     HOT_LAUNCHED(1);
     if (a.tolmode) {
-        if (a.periodic) walk_kernel<true, true><<<nb, WALK_WARPS * 32, 0, st>>>(a);
-        else walk_kernel<false, true><<<nb, WALK_WARPS * 32, 0, st>>>(a);
-    } else if (a.periodic) walk_kernel<true, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
-    else walk_kernel<false, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+        if (a.periodic) walk_kernel<true, true, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+        else walk_kernel<false, true, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+    } else if (a.periodic && a.bgmode) walk_kernel<true, false, true><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+    else if (a.periodic) walk_kernel<true, false, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
+    else walk_kernel<false, false, false><<<nb, WALK_WARPS * 32, 0, st>>>(a);
     return cudaGetLastError();
 }
 

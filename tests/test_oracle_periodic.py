@@ -188,6 +188,10 @@ def test_background_subtraction_is_consistent_with_the_plain_periodic_tree(cfg, 
     c = T.cells()
     gs = w.size * np.ldexp(1.0, -c["level"][T.groups()[sel]].astype(np.int64))
     assert np.allclose(T.bg_volume, 125.0 - (5 * gs / w.size) ** 3, rtol=1e-12)
+    # a lazy tree (moments of the accepted cells only, as the 2^27-body test uses) does the same arithmetic
+    T2 = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=True, nleaf=8, ncrit=32, moments=2)
+    a3, p3, *_ = T2.forces_bg(theta, w.eps, order, groups=sel)
+    assert np.array_equal(a3, a1, equal_nan=True) and np.array_equal(p3, p1, equal_nan=True)
     # smaller theta: both converge to the Ewald sum
     a2, p2, *_ = T.forces_bg(0.3, w.eps, order, groups=sel)
     e2 = np.sqrt(((a2[m] - ae) ** 2).sum(1).mean()) / arms

@@ -476,6 +476,34 @@ def test_full_size_parity_on_sampled_groups(hot, cfg, order, theta, nsel):
     assert checked >= 1
     assert st["n"] == w.n and st["pp_interactions"] > 0 and st["pc_interactions"] > 0
     assert np.isfinite(acc.cpu().numpy()).all() and np.isfinite(pot.cpu().numpy()).all()
+    if w.periodic:
+        # f-1 at full size: with the per-cell background subtraction (R-18) the counts are bit-exact and the PLAIN
+        # tolerance holds for the acceleration and for the potential (no 57.19 M/L in the denominator, no fp64
+        # monopole stage); the potential's tail is taken against max(|phi|, rms phi): its box mean is zero (R-11)
+        del acc, pot
+        sub = sel[: max(8, nsel // 2)]
+        hot.hot_set_background(True)
+        try:
+            acc, pot = hot.hot_forces(theta, w.eps, order)
+            gg = hot.hot_export_groups()
+            go = hot.hot_export_group_orders()
+            stb = hot.hot_stats()
+        finally:
+            hot.hot_set_background(False)
+        oa, op, lpc, lbg, lv, lpp = T.forces_bg(theta, w.eps, order, groups=sub)
+        assert (gg["lpc"][sub] == lpc.astype(np.uint64)).all() and (gg["lpp"][sub] == lpp.astype(np.uint64)).all()
+        assert (go["quad"][sub] == lbg.astype(np.uint64)).all() and (go["hexa"][sub] == lv.astype(np.uint64)).all()
+        m = ~np.isnan(op)
+        ga = acc.cpu().numpy().astype(np.float64)[m]
+        gp = pot.cpu().numpy().astype(np.float64)[m]
+        ea = np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)
+        ep = np.abs(gp - op[m]) / np.abs(op[m])
+        ept = np.abs(gp - op[m]) / np.maximum(np.abs(op[m]), np.sqrt((op[m] ** 2).mean()))
+        print("full-size parity with background subtraction", cfg, "acc median", np.median(ea), "p99.9", np.quantile(ea, 0.999),
+              "pot median", np.median(ep), "p99.9 vs max(|phi|, rms)", np.quantile(ept, 0.999),
+              "ms eval", stb["ms_eval"], "ms bg", stb["ms_coarse"], "ms walk", stb["ms_walk"])
+        assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+        assert np.median(ep) <= 1e-5 and np.quantile(ept, 0.999) <= 1e-4, (np.median(ep), np.quantile(ept, 0.999))
 
 
 @pytest.mark.slow
@@ -731,3 +759,45 @@ def test_high_order_parity(hot, cfg, scale, periodic, order, theta):
             a, _ = hot.hot_forces(theta, w.eps, o)
             e[o] = float(np.sqrt(((a.cpu().numpy().astype(np.float64) - ad) ** 2).sum() / (ad ** 2).sum()))
         assert e[order] < 0.5 * e[4], e
+
+
+# ---- f-1: per-cell background subtraction in periodic boxes (R-18) ------------------------
+@pytest.mark.parametrize("cfg,side,order,theta,ncrit", [(3, 16, 4, 0.5, 64), (4, 16, 2, 0.5, 64), (4, 12, 0, 0.6, 32), (3, 24, 2, 0.5, 64)])
+def test_background_subtraction_parity(hot, cfg, side, order, theta, ncrit):
+    """Against the oracle's forces_bg: the walk's counts bit-exact (plain cells, background-subtracted cells, negative-
+    background cubes, bodies -- integer geometry throughout), forces AND potentials at the plain tolerance: with the
+    background subtracted the potential no longer is a small difference of two O(60 M/L) fp32 sums (R-13 is not needed)."""
+    w = W.config(cfg, side)
+    _build(hot, w, 16, ncrit)
+    T = O.Tree(w.pos, w.mass, w.lo, w.size, periodic=True, nleaf=16, ncrit=ncrit)
+    hot.hot_set_background(True)
+    try:
+        acc, pot = hot.hot_forces(theta, w.eps, order)
+        gg = hot.hot_export_groups()
+        go = hot.hot_export_group_orders()
+        st = hot.hot_stats()
+    finally:
+        hot.hot_set_background(False)
+    sel = np.sort(np.random.default_rng(3).choice(T.ngroups, min(T.ngroups, 32), replace=False))
+    oa, op, lpc, lbg, lv, lpp = T.forces_bg(theta, w.eps, order, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    assert (go["quad"][sel] == lbg.astype(np.uint64)).all() and (go["mono"][sel] == (lpc - lbg).astype(np.uint64)).all()
+    assert (go["hexa"][sel] == lv.astype(np.uint64)).all(), "accepted negative-background cubes"
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]; gp = pot.cpu().numpy().astype(np.float64)[m]
+    arms = np.sqrt((oa[m] ** 2).sum(axis=1).mean())
+    ea = np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)
+    ep = np.abs(gp - op[m]) / np.abs(op[m])
+    # the periodic potential has zero box mean (R-11): a body can sit where it crosses zero, so the tail of the relative
+    # error is taken against max(|phi_i|, rms of phi over the set); the median is the plain per-body relative error
+    prms = np.sqrt((op[m] ** 2).mean())
+    ept = np.abs(gp - op[m]) / np.maximum(np.abs(op[m]), prms)
+    print("bg parity", cfg, side, "acc median", np.median(ea), "p99.9", np.quantile(ea, 0.999), "pot median", np.median(ep), "p99.9", np.quantile(ep, 0.999),
+          "p99.9 vs max(|phi|, rms)", np.quantile(ept, 0.999), "phi rms", prms, "x 57.19 M/L:", prms / (57.18721055 * float(w.mass.astype(np.float64).sum()) / w.size))
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    assert np.median(ep) <= 1e-5 and np.quantile(ept, 0.999) <= 1e-4, (np.median(ep), np.quantile(ept, 0.999))
+    assert st["ms_coarse"] > 0 and np.isfinite(ga).all()
+    # the same field as without subtraction, to the truncation error of the expansions
+    acc0, pot0 = hot.hot_forces(theta, w.eps, order)
+    d = np.linalg.norm(acc.cpu().numpy().astype(np.float64) - acc0.cpu().numpy().astype(np.float64), axis=1)
+    assert np.sqrt((d ** 2).mean()) < (0.05 if order == 0 else 5e-3) * arms
