@@ -20,6 +20,7 @@ struct Ctx {
     int softening = 0; // 0 Plummer, 1 cubic spline (hot_set_softening)
     int background = 0; // 1: per-cell background subtraction in periodic boxes (hot_set_background)
     uint4 *d_vstack = nullptr, *d_vstage = nullptr, *d_pvlist = nullptr; // virtual cubes of the background-subtracted walk
+    int64_t pv_per_group = 192; // their arena is sized for this many per group; grown fourfold when a walk overflows it
     int last_order = -1, last_tolmode = 0, last_bgmode = 0;
     char err[512] = "";
     // scratch owned across calls
@@ -442,7 +443,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     if (bgmode) {
         CUDA_TRY(tree_alloc(&g.d_vstack, (size_t)nwarps * (size_t)vstack_cap));
         CUDA_TRY(tree_alloc(&g.d_vstage, (size_t)nwarps * (size_t)vstage_cap));
-        cappv = (unsigned long long)ng * 192ull + 65536ull;
+        cappv = (unsigned long long)ng * (unsigned long long)g.pv_per_group + 65536ull;
         CUDA_TRY(tree_alloc(&g.d_pvlist, (size_t)cappv));
         CUDA_TRY(tree_alloc(&t.glpv, (size_t)ng));
         CUDA_TRY(tree_alloc(&t.gpvoff, (size_t)ng));
@@ -502,7 +503,15 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         ms_walk += ms_between(g.evx[0], g.evx[1]);
         if (fl[0] & 4) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted");
         if (fl[0] & 16) return fail(HOT_EINTERNAL, "hot_forces: virtual-cube scratch of the background-subtracted walk exhausted");
-        if (fl[0] & 32) return fail(HOT_ENOMEM, "hot_forces: the virtual-cube list of the background-subtracted walk does not fit its arena");
+        if (fl[0] & 32) { // the accepted virtual cubes outgrew their arena: enlarge it and walk this range again
+            if (g.pv_per_group >= (1 << 16)) return fail(HOT_ENOMEM, "hot_forces: the virtual-cube list of the background-subtracted walk does not fit its arena");
+            g.pv_per_group *= 4;
+            cappv = (unsigned long long)ng * (unsigned long long)g.pv_per_group + 65536ull;
+            CUDA_TRY(tree_alloc(&g.d_pvlist, (size_t)cappv));
+            wa.pvlist = g.d_pvlist; wa.cappv = cappv;
+            CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
+            continue;
+        }
         if (fl[0] & 8) { // a group's lists outgrew the per-warp staging area: enlarge it and walk this range again
             if (g.stage_cap >= ((int64_t)1 << 26)) return fail(HOT_ENOMEM, "hot_forces: one sink group's interaction list exceeds 2^26 entries");
             g.stage_cap *= 4;
@@ -528,11 +537,17 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         a.nsb = (unsigned int)((F - g0 + ((int64_t)1 << a.sb_shift) - 1) >> a.sb_shift);
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
         CUDA_TRY(launch_plan(a, st));
-        if (bgmode) { // far field + background added back + flagged cells + virtual cubes -> farc, in fp64 (hot_bg.cu)
+        if (bgmode) { // hot_bg.cu: far field + background added back + virtual cubes -> farc (fp64); then the flagged cells about
+                      // their centres through the blocked kernel, added to farc; the launch below takes the plain near field
             CUDA_TRY(cudaEventRecord(g.evx[4], st));
             a.lpc0 = t.glpc0; a.lpc2 = t.glpc2;
-            CUDA_TRY(launch_forces_bg(a, t, t.far, t.farc, g.d_pvlist, t.glpv, t.gpvoff, rhobar, st));
-            a.far = t.farc; a.seg = 0; // the interaction kernel takes the plain cells (inside the near cube) and the bodies
+            CUDA_TRY(launch_forces_bg(a, t, t.far, t.farc, g.d_pvlist, t.glpv, t.gpvoff, rhobar, 0, st));
+            ForceArgs b = a;
+            b.seg = 1; b.do_pp = 0; b.bgv = 1; b.bgA = t.bgA; b.bgE2 = t.bgE2; b.bgM34 = t.bgM34; b.out_farc = t.farc; b.far = nullptr;
+            if (g.softening == 1) b.eps2 = 0.0f; // spline: accepted cells are Newtonian
+            CUDA_TRY(launch_forces(b, st));
+            CUDA_TRY(cudaMemsetAsync(g.d_counter + 1, 0, sizeof(unsigned int), st)); // the work-item scheduler starts over
+            a.far = t.farc; a.seg = 0; // the plain cells (inside the near cube) and the bodies
         } else if (t.periodic) { // fp64 monopoles of the coarsest accepted cells + far field -> farc (hot_periodic.cu)
             CUDA_TRY(cudaEventRecord(g.evx[4], st));
             CUDA_TRY(launch_coarse_monopoles(a, t.far, t.farc, g.softening == 1 ? 0.0 : eps * eps, st)); // spline: accepted cells are Newtonian

@@ -5,12 +5,14 @@
 //                       (PAPER.md:86); the dipole is present.  fp64 arithmetic, fp32 records.
 //   forces_bg_kernel  : per sink, in fp64: the far field of hot_periodic.cu + the background added back in closed form,
 //                       rhobar x [homogeneous (5 L)^3 cube - homogeneous near cube K_G] ("removed analytically", Fig 2;
-//                       refs [59, 46]) + the flagged cells of the walk about their centres (fp32 terms, now small) + the
-//                       virtual cubes (empty octants, cubes of rejected leaves: only the negative background).
-//                       The result goes to farc[], which the interaction kernel of hot_forces.cu adds to its fp64 sums
-//                       of the plain near field before the one rounding to fp32.
-// One warp per sink group, sinks one per lane, cells one at a time through shared memory: a plain kernel; the far cells
-// it evaluates are ~2/3 of a periodic run's interactions, so tuning it like hot_forces.cu is the next step.
+//                       refs [59, 46]) + the virtual cubes (empty octants, cubes of rejected leaves: only the negative
+//                       background; few) -> farc[].  The flagged cells of the walk (most of a periodic run's
+//                       interactions) are evaluated about their centres, with the dipole, by the blocked kernel of
+//                       hot_forces.cu (its BGV variant), which adds its fp64 sums to farc[]; the launch over the plain near
+//                       field then adds farc[] to its own fp64 sums before the one rounding to fp32.
+//                       (with_cells = 1 makes this kernel evaluate the flagged cells too: the plain form the blocked one was
+//                       checked against, 2.4 x slower.)
+// One warp per sink group, sinks one per lane, entries one at a time through shared memory.
 #include "hot_interact.cuh"
 
 __host__ __device__ constexpr int bidx(int a, int b, int c) {
@@ -127,7 +129,7 @@ template <int ORDER>
 __global__ void __launch_bounds__(BG_WARPS * 32) forces_bg_kernel(const __grid_constant__ ForceArgs A, const double* __restrict__ far, double* __restrict__ farc,
                                                                   const float4* __restrict__ bgA, const CellM2* __restrict__ bgE2, const CellM34* __restrict__ bgM34,
                                                                   const uint4* __restrict__ pvlist, const uint32_t* __restrict__ lpv, const unsigned long long* __restrict__ pvoff,
-                                                                  double rhobar) {
+                                                                  double rhobar, int with_cells) {
     __shared__ __align__(16) float s_rec[BG_WARPS][4 + 4 + 8 + 36];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     float* const rec = s_rec[w];
@@ -139,7 +141,7 @@ __global__ void __launch_bounds__(BG_WARPS * 32) forces_bg_kernel(const __grid_c
         const int gox = (int)(gw.x & 0x1fffffu), goy = (int)((gw.x >> 21) | ((gw.y & 0x3ffu) << 11)), goz = (int)((gw.y >> 10) & 0x1fffffu);
         const double ox = A.lo[0] + ((double)gox + 0.5 * gs) * h, oy = A.lo[1] + ((double)goy + 0.5 * gs) * h, oz = A.lo[2] + ((double)goz + 0.5 * gs) * h;
         const unsigned long long o0 = A.pcoff[gi] + A.lpc0[gi]; // the flagged cells follow the plain ones
-        const int n = (int)A.lpc2[gi], nv = (int)lpv[gi];
+        const int n = with_cells ? (int)A.lpc2[gi] : 0, nv = (int)lpv[gi]; // with_cells = 0: the flagged cells go through hot_forces.cu's kernel
         const unsigned long long v0 = pvoff[gi];
         for (uint32_t s0 = 0; s0 < g.count; s0 += 32) {
             const uint32_t loc = s0 + lane;
@@ -223,14 +225,14 @@ cudaError_t launch_bg_moments(const Tree& t, int order, double rhobar, cudaStrea
     return cudaGetLastError();
 }
 cudaError_t launch_forces_bg(const ForceArgs& a, const Tree& t, const double* far, double* farc, const uint4* pvlist, const uint32_t* lpv,
-                             const unsigned long long* pvoff, double rhobar, cudaStream_t st) {
+                             const unsigned long long* pvoff, double rhobar, int with_cells, cudaStream_t st) {
     const int64_t ng = a.g1 - a.g0;
     if (ng <= 0) return cudaSuccess;
     int64_t nb = (ng + BG_WARPS - 1) / BG_WARPS;
     if (nb > 148 * 32) nb = 148 * 32;
     HOT_LAUNCHED(1);
-    if (a.order >= 4) forces_bg_kernel<4><<<(unsigned)nb, BG_WARPS * 32, 0, st>>>(a, far, farc, t.bgA, t.bgE2, t.bgM34, pvlist, lpv, pvoff, rhobar);
-    else if (a.order >= 2) forces_bg_kernel<2><<<(unsigned)nb, BG_WARPS * 32, 0, st>>>(a, far, farc, t.bgA, t.bgE2, t.bgM34, pvlist, lpv, pvoff, rhobar);
-    else forces_bg_kernel<0><<<(unsigned)nb, BG_WARPS * 32, 0, st>>>(a, far, farc, t.bgA, t.bgE2, t.bgM34, pvlist, lpv, pvoff, rhobar);
+    if (a.order >= 4) forces_bg_kernel<4><<<(unsigned)nb, BG_WARPS * 32, 0, st>>>(a, far, farc, t.bgA, t.bgE2, t.bgM34, pvlist, lpv, pvoff, rhobar, with_cells);
+    else if (a.order >= 2) forces_bg_kernel<2><<<(unsigned)nb, BG_WARPS * 32, 0, st>>>(a, far, farc, t.bgA, t.bgE2, t.bgM34, pvlist, lpv, pvoff, rhobar, with_cells);
+    else forces_bg_kernel<0><<<(unsigned)nb, BG_WARPS * 32, 0, st>>>(a, far, farc, t.bgA, t.bgE2, t.bgM34, pvlist, lpv, pvoff, rhobar, with_cells);
     return cudaGetLastError();
 }

@@ -86,17 +86,17 @@ template <int S> struct Sinks {
         for (int p = 0; p < NP; ++p) pp_pair_spline(ns, j >= 0 && j == me[2 * p], j >= 0 && j == me[2 * p + 1], x2[p], hinv, a2[p]);
         if (TAIL) pp_one_spline(ns, j >= 0 && j == me[S - 1], x1, hinv, a1);
     }
-    template <int ORDER>
-    __device__ __forceinline__ void pc(const float4 q0, const float4 q1, const float4 q2, const float* m, float eps2) {
+    template <int ORDER, bool DIP = false>
+    __device__ __forceinline__ void pc(const float4 q0, const float4 q1, const float4 q2, const float* m, float eps2, const float4 qd = make_float4(0.f, 0.f, 0.f, 0.f)) {
 #pragma unroll
-        for (int p = 0; p < NP; ++p) pc_one<ORDER, f2>(q0, q1, q2, m, x2[p], eps2, a2[p]);
-        if (TAIL) pc_one<ORDER, float>(q0, q1, q2, m, x1, eps2, a1);
+        for (int p = 0; p < NP; ++p) pc_one<ORDER, f2, DIP>(q0, q1, q2, m, x2[p], eps2, a2[p], qd);
+        if (TAIL) pc_one<ORDER, float, DIP>(q0, q1, q2, m, x1, eps2, a1, qd);
     }
 };
 
 // ---- per-warp shared-memory layout (byte offsets from the warp's base) -------------------------
-template <int ORDER> struct WL {
-    static constexpr int NQ = PCQ<ORDER>::v;
+template <int ORDER, bool BGV = false> struct WL {
+    static constexpr int NQ = PCQ<ORDER>::v + (BGV ? 1 : 0); // background-subtracted cells: one more slot, the dipole
     static constexpr int pcst = 0;                               // 2 x [NQ][32] float4  staged cells
     static constexpr int ppst = pcst + 2 * NQ * 32 * 16;         // 2 x [32] float4      staged bodies
     static constexpr int accum = ppst + 2 * 32 * 16;             // [SMAX*4][32] double  running sums (acc, pot) per lane
@@ -105,11 +105,11 @@ template <int ORDER> struct WL {
 
 // ---- S8/S9/S10: one chunk (<= 32*SMAX sinks) of one group -----------------------------------------
 // L = 1 << lgL lanes per source stream, S = ceil(nchunk / L) sinks per lane.
-template <int ORDER, bool PER, int S, bool SPL>
+template <int ORDER, bool PER, int S, bool SPL, bool BGV>
 __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const GroupRec g, const int64_t gi, const uint32_t chunk0,
                                         const uint32_t nchunk, const int lgL, const int lane) {
-    using Lay = WL<ORDER>;
-    constexpr int NQ = Lay::NQ;
+    using Lay = WL<ORDER, BGV>;
+    constexpr int NQ = Lay::NQ, QD = PCQ<ORDER>::v; // QD: slot of the dipole (BGV)
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned char* const base = smem_raw + (size_t)w * Lay::bytes;
     float4* const pcst = reinterpret_cast<float4*>(base + Lay::pcst);
@@ -188,6 +188,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
         const int nb = (n + BATCH - 1) / BATCH;
         CellA cA;
         cA.zx = cA.zy = cA.zz = 0.0; cA.m0 = 0.f; cA.bmax = 0.f;
+        float4 dipv = make_float4(0.f, 0.f, 0.f, 0.f); // BGV: (mass - cube, dipole) of the cell being gathered
         uint32_t cnext = 0; int inext = 62, pim = 62;
         auto fetch_idx = [&](int b) { // list entries of batch b
             if (b * BATCH + lane < n) { cnext = pl[b * BATCH + lane]; if (PER) inext = pi[b * BATCH + lane]; }
@@ -196,16 +197,26 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
             if (b * BATCH + lane < n) {
                 const uint32_t c = PER ? (cnext & ~HOT_COARSE_FLAG) : cnext;
                 pim = inext;
-                cA = P.cellA[c];
-                if (PER && (cnext & HOT_COARSE_FLAG)) cA.m0 = 0.f; // its monopole is summed in fp64 elsewhere (hot_periodic.cu)
+                if (BGV) { // a background-subtracted cell: expansion centre = the cell's centre, mass and dipole from bgA
+                    const WalkCell wc = P.wcell[c];
+                    const double hh = P.size * (1.0 / 2097152.0), half = 0.5 * ldexp(P.size, -(int)(wc.w >> 27));
+                    cA.zx = P.lo[0] + (double)(wc.x & 0x1fffffu) * hh + half;
+                    cA.zy = P.lo[1] + (double)((wc.x >> 21) | ((wc.y & 0x3ffu) << 11)) * hh + half;
+                    cA.zz = P.lo[2] + (double)((wc.y >> 10) & 0x1fffffu) * hh + half;
+                    dipv = P.bgA[c];
+                    cA.m0 = dipv.x;
+                } else {
+                    cA = P.cellA[c];
+                    if (PER && (cnext & HOT_COARSE_FLAG)) cA.m0 = 0.f; // its monopole is summed in fp64 elsewhere (hot_periodic.cu)
+                }
                 float4* const dst = pcst + (b & 1) * NQ * BATCH + lane;
                 if (ORDER >= 2) {
-                    const float4* src = reinterpret_cast<const float4*>(P.cellE2 + c);
+                    const float4* src = reinterpret_cast<const float4*>((BGV ? P.bgE2 : P.cellE2) + c);
                     cp_async16(dst + 1 * BATCH, src);
                     cp_async16(dst + 2 * BATCH, src + 1);
                 }
                 if (ORDER >= 4) {
-                    const float4* src = reinterpret_cast<const float4*>(P.cellM34 + c);
+                    const float4* src = reinterpret_cast<const float4*>((BGV ? P.bgM34 : P.cellM34) + c);
 #pragma unroll
                     for (int k = 0; k < 9; ++k) cp_async16(dst + (3 + k) * BATCH, src + k);
                 }
@@ -219,33 +230,37 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                 double shx = 0, shy = 0, shz = 0;
                 if (PER) shift_of(pim, shx, shy, shz);
                 st[lane] = make_float4((float)(ox - (cA.zx + shx)), (float)(oy - (cA.zy + shy)), (float)(oz - (cA.zz + shz)), -cA.m0);
+                if (BGV) st[QD * 32 + lane] = make_float4(dipv.y, dipv.z, dipv.w, 0.f);
             }
             if (ORDER >= 2) cp_async_wait_all();
             __syncwarp();
             if (b + 1 < nb) { issue(b + 1); fetch_idx(b + 2); } // in flight during the arithmetic below
             if (ORDER < 4) { // the next source's record is read while the current one is evaluated
                 int j = strm;
-                float4 n0 = st[j < cnt ? j : 0], n1 = n0, n2 = n0;
+                float4 n0 = st[j < cnt ? j : 0], n1 = n0, n2 = n0, nd = n0;
                 if (ORDER >= 2) { n1 = st[32 + (j < cnt ? j : 0)]; n2 = st[64 + (j < cnt ? j : 0)]; }
+                if (BGV) nd = st[QD * 32 + (j < cnt ? j : 0)];
                 if (S >= UNROLL2_S) { // two sources per trip: the sums stay in their registers (no copies at the loop end)
 #pragma unroll 2
                 while (j < cnt) {
-                    const float4 q0 = n0, q1 = n1, q2 = n2;
+                    const float4 q0 = n0, q1 = n1, q2 = n2, qd = nd;
                     j += K;
                     const int jn = j < cnt ? j : strm;
                     n0 = st[jn];
                     if (ORDER >= 2) { n1 = st[32 + jn]; n2 = st[64 + jn]; }
-                    sk.template pc<ORDER>(q0, q1, q2, nullptr, eps2);
+                    if (BGV) nd = st[QD * 32 + jn];
+                    sk.template pc<ORDER, BGV>(q0, q1, q2, nullptr, eps2, qd);
                 }
                 } else {
 #pragma unroll 1
                 while (j < cnt) {
-                    const float4 q0 = n0, q1 = n1, q2 = n2;
+                    const float4 q0 = n0, q1 = n1, q2 = n2, qd = nd;
                     j += K;
                     const int jn = j < cnt ? j : strm;
                     n0 = st[jn];
                     if (ORDER >= 2) { n1 = st[32 + jn]; n2 = st[64 + jn]; }
-                    sk.template pc<ORDER>(q0, q1, q2, nullptr, eps2);
+                    if (BGV) nd = st[QD * 32 + jn];
+                    sk.template pc<ORDER, BGV>(q0, q1, q2, nullptr, eps2, qd);
                 }
                 }
             } else {
@@ -258,7 +273,7 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
                         const float4 t = st[(3 + k) * 32 + j];
                         m[4 * k] = t.x; m[4 * k + 1] = t.y; m[4 * k + 2] = t.z; m[4 * k + 3] = t.w;
                     }
-                    sk.template pc<ORDER>(q0, q1, q2, m, eps2);
+                    sk.template pc<ORDER, BGV>(q0, q1, q2, m, eps2, BGV ? st[QD * 32 + j] : make_float4(0.f, 0.f, 0.f, 0.f));
                 }
             }
             nacc += (cnt + K - 1) >> lgK;
@@ -326,7 +341,15 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
     if (strm == 0) {
 #pragma unroll
         for (int i = 0; i < S; ++i) {
-            if (sk.me[i] >= 0) {
+            if (BGV) { // the background-subtracted cells' share goes to farc (fp64, key order): the launch over the plain
+                       // near field adds it to its own fp64 sums and rounds once
+                if (sk.me[i] >= 0) {
+                    double4* const f = reinterpret_cast<double4*>(P.out_farc) + (g.first + sk.me[i]);
+                    double4 r = *f;
+                    r.x += A[i][0]; r.y += A[i][1]; r.z += A[i][2]; r.w += A[i][3];
+                    *f = r;
+                }
+            } else if (sk.me[i] >= 0) {
                 const uint32_t o = P.perm[g.first + sk.me[i]];
                 if (PER && P.far) {
                     const double4 f = reinterpret_cast<const double4*>(P.far)[g.first + sk.me[i]];
@@ -346,16 +369,16 @@ __device__ __noinline__ void eval_chunk(const ForceArgs& P, const int w, const G
 }
 
 // one pass over the group's lists for sinks [c0, c0 + nc) with L = 1 << lgL lanes per source stream
-template <int ORDER, bool PER, bool SPL>
+template <int ORDER, bool PER, bool SPL, bool BGV>
 __device__ __forceinline__ void run_chunk(const ForceArgs& P, const int w, const GroupRec g, const int64_t gi, const uint32_t c0,
                                           const uint32_t nc, const int lgL, const int lane) {
     const int S = (int)((nc + (1u << lgL) - 1) >> lgL);
-    if (S <= 1) eval_chunk<ORDER, PER, 1, SPL>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 2) eval_chunk<ORDER, PER, 2, SPL>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 3) eval_chunk<ORDER, PER, 3, SPL>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 4) eval_chunk<ORDER, PER, 4, SPL>(P, w, g, gi, c0, nc, lgL, lane);
-    else if (S == 5) eval_chunk<ORDER, PER, 5, SPL>(P, w, g, gi, c0, nc, lgL, lane);
-    else eval_chunk<ORDER, PER, 6, SPL>(P, w, g, gi, c0, nc, lgL, lane);
+    if (S <= 1) eval_chunk<ORDER, PER, 1, SPL, BGV>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 2) eval_chunk<ORDER, PER, 2, SPL, BGV>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 3) eval_chunk<ORDER, PER, 3, SPL, BGV>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 4) eval_chunk<ORDER, PER, 4, SPL, BGV>(P, w, g, gi, c0, nc, lgL, lane);
+    else if (S == 5) eval_chunk<ORDER, PER, 5, SPL, BGV>(P, w, g, gi, c0, nc, lgL, lane);
+    else eval_chunk<ORDER, PER, 6, SPL, BGV>(P, w, g, gi, c0, nc, lgL, lane);
     static_assert(SMAX == 6, "one eval_chunk instance per sinks-per-lane count");
 }
 // smallest stream width that holds n sinks with at most SMAX per lane
@@ -454,7 +477,7 @@ cudaError_t launch_plan(const ForceArgs& a, cudaStream_t st) {
 }
 #endif
 
-template <int ORDER, bool PER, bool SPL>
+template <int ORDER, bool PER, bool SPL, bool BGV>
 __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : MINBLK) forces_kernel(const __grid_constant__ ForceArgs P) {
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     const unsigned int total = P.cls[24 * P.nsb];
@@ -465,25 +488,25 @@ __global__ void __launch_bounds__(WARPS_PER_BLOCK * 32, ORDER >= 4 ? 3 : MINBLK)
         if (q >= total) break;
         const uint4 it = P.items[q];
         const int64_t gi = P.g0 + (int64_t)it.x;
-        run_chunk<ORDER, PER, SPL>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
+        run_chunk<ORDER, PER, SPL, BGV>(P, w, P.group[gi], gi, it.y, it.z, (int)it.w, lane);
     }
 }
 
-template <int ORDER, bool PER, bool SPL> static cudaError_t launch_one(const ForceArgs& a, cudaStream_t st) {
-    constexpr int smem = WL<ORDER>::bytes * WARPS_PER_BLOCK;
+template <int ORDER, bool PER, bool SPL, bool BGV = false> static cudaError_t launch_one(const ForceArgs& a, cudaStream_t st) {
+    constexpr int smem = WL<ORDER, BGV>::bytes * WARPS_PER_BLOCK;
     static int nblocks = 0;
     if (!nblocks) {
-        cudaError_t e = cudaFuncSetAttribute(forces_kernel<ORDER, PER, SPL>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+        cudaError_t e = cudaFuncSetAttribute(forces_kernel<ORDER, PER, SPL, BGV>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
         if (e != cudaSuccess) return e;
         int dev = 0, nsm = 0, occ = 0;
         cudaGetDevice(&dev);
         cudaDeviceGetAttribute(&nsm, cudaDevAttrMultiProcessorCount, dev);
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, forces_kernel<ORDER, PER, SPL>, WARPS_PER_BLOCK * 32, smem);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, forces_kernel<ORDER, PER, SPL, BGV>, WARPS_PER_BLOCK * 32, smem);
         if (e != cudaSuccess) return e;
         nblocks = nsm * (occ < 1 ? 1 : occ);
     }
     HOT_LAUNCHED(1);
-    forces_kernel<ORDER, PER, SPL><<<nblocks, WARPS_PER_BLOCK * 32, smem, st>>>(a);
+    forces_kernel<ORDER, PER, SPL, BGV><<<nblocks, WARPS_PER_BLOCK * 32, smem, st>>>(a);
     return cudaGetLastError();
 }
 #ifndef HOT_FORCES_PERIODIC_TU
@@ -501,6 +524,11 @@ cudaError_t launch_forces(const ForceArgs& a, cudaStream_t st) {
 }
 #else
 cudaError_t dispatch_periodic(const ForceArgs& a, cudaStream_t st) {
+    if (a.bgv) { // the flagged cells of a background-subtracted walk (hot_bg.cu): about their centres, with the dipole
+        if (a.order >= 4) return launch_one<4, true, false, true>(a, st);
+        if (a.order >= 2) return launch_one<2, true, false, true>(a, st);
+        return launch_one<0, true, false, true>(a, st);
+    }
     if (a.spline) {
         if (a.order >= 4) return launch_one<4, true, true>(a, st);
         if (a.order >= 2) return launch_one<2, true, true>(a, st);

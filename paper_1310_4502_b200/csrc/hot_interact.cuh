@@ -98,16 +98,24 @@ __device__ __forceinline__ void pp_pair_spline(const float4 ns, const bool skip0
 //   slot 0: (-zx, -zy, -zz, -M0)  NEGATED centre of mass relative to the group origin, negated mass
 //   slot 1: 3 (xx, xy, xz, yy)  slot 2: (3 yz, 3 zz, 1.5 t2, 0.5 t2)          ORDER >= 2  (the cellE2 record)
 //   slots 3..11: M3 (10) M4 (15) t3 (3) T4 (6: xx xy xz yy yz zz) t4 (1) pad   ORDER >= 4
-template <int ORDER, class T>
+// DIP (background-subtracted cells, expanded about the cell centre: hot_bg.cu, R-18): qd = (M1x, M1y, M1z, -) adds
+//   phi_1 = D1 (M1 . R) = -ri^3 (M1 . R),   a_1 = -[D2 (M1 . R) R + D1 M1] = -3 ri^5 (M1 . R) R + ri^3 M1.
+template <int ORDER, class T, bool DIP = false>
 __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const float4 q2, const float* __restrict__ m,
-                                       const T (&x)[3], const float eps2, T (&a)[4]) {
+                                       const T (&x)[3], const float eps2, T (&a)[4], const float4 qd = make_float4(0.f, 0.f, 0.f, 0.f)) {
     const T Rx = x[0] + splat<T>(q0.x), Ry = x[1] + splat<T>(q0.y), Rz = x[2] + splat<T>(q0.z);
     const T u = vfma(Rx, Rx, vfma(Ry, Ry, vfma(Rz, Rz, splat<T>(eps2))));
     const T ri = vrsqrt(u);
     const T ri2 = ri * ri, ri3 = ri * ri2;
     const T nm0 = splat<T>(q0.w);
     if (ORDER < 2) {
-        const T c = nm0 * ri3;
+        T c = nm0 * ri3;
+        if (DIP) {
+            const T dR = vfma(splat<T>(qd.x), Rx, vfma(splat<T>(qd.y), Ry, splat<T>(qd.z) * Rz)), w = ri3 * dR;
+            c = vfma(splat<T>(-3.0f) * ri2, w, c);
+            a[0] = vfma(ri3, splat<T>(qd.x), a[0]); a[1] = vfma(ri3, splat<T>(qd.y), a[1]); a[2] = vfma(ri3, splat<T>(qd.z), a[2]);
+            a[3] = a[3] - w;
+        }
         a[0] = vfma(c, Rx, a[0]); a[1] = vfma(c, Ry, a[1]); a[2] = vfma(c, Rz, a[2]);
         a[3] = vfma(nm0, ri, a[3]);
         return;
@@ -122,6 +130,12 @@ __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const f
     const T hQ = ri5 * Q2;                                          // 3 u^-5/2 (R M2 R)
     T cR = vfma(hQ, w7, vfma(splat<T>(q2.z), ri5, nm0 * ri3));      // -7.5 u^-7/2 Q2 + 1.5 t2 u^-5/2 - M0 u^-3/2
     T ph = vfma(splat<T>(-0.5f), hQ, vfma(splat<T>(q2.w), ri3, nm0 * ri));
+    if (DIP) {
+        const T dR = vfma(splat<T>(qd.x), Rx, vfma(splat<T>(qd.y), Ry, splat<T>(qd.z) * Rz));
+        cR = vfma(splat<T>(-3.0f) * ri5, dR, cR);
+        ph = ph - ri3 * dR;
+        a[0] = vfma(ri3, splat<T>(qd.x), a[0]); a[1] = vfma(ri3, splat<T>(qd.y), a[1]); a[2] = vfma(ri3, splat<T>(qd.z), a[2]);
+    }
     const T D2 = ri5;                                               // multiplies N R = 3 M2 R
     if (ORDER < 4) { // accumulate straight into the partial sums
         a[0] = vfma(cR, Rx, vfma(D2, Mx, a[0]));

@@ -174,6 +174,8 @@ struct ForceArgs {
     unsigned int* cls;            // plan_cls_elems(g1 - g0, sb_shift) words: per-(superblock, class) counts, starts, cursors, total
     // tolerance mode: one launch per order over its segment of the cell lists (seg = 0, 1, 2; -1: the whole list)
     int seg; const uint32_t *lpc0, *lpc2; int do_pp, accumulate;
+    // background subtraction: bgv = 1 evaluates the flagged cells (seg 1) from these records into out_farc[body][4] (fp64)
+    int bgv; const float4* bgA; const CellM2* bgE2; const CellM34* bgM34; double* out_farc;
     int sb_shift; unsigned int nsb; // 2^sb_shift groups per superblock (>= 8), number of superblocks of [g0, g1)
 };
 size_t plan_cls_elems(int64_t ngroups, int sb_shift);
@@ -193,7 +195,7 @@ cudaError_t launch_coarse_monopoles(const ForceArgs& a, const double* far, doubl
 cudaError_t launch_bg_moments(const Tree& t, int order, double rhobar, cudaStream_t st);
 // farc[body] = far[body] + background added back in closed form + flagged cells + virtual cubes, groups [a.g0, a.g1)
 cudaError_t launch_forces_bg(const ForceArgs& a, const Tree& t, const double* far, double* farc, const uint4* pvlist, const uint32_t* lpv,
-                             const unsigned long long* pvoff, double rhobar, cudaStream_t st);
+                             const unsigned long long* pvoff, double rhobar, int with_cells, cudaStream_t st);
 
 // ---- f-3: the terms of degree 5 .. P (P = 6, 8) of every accepted cell, added to acc / pot (hot_hi.cu) ----------
 int hi_record_floats(int order); int hi_raw_floats(int order);
