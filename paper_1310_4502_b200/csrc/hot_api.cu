@@ -336,6 +336,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     // S6: moments, cached per build at the highest order asked so far
     if (t.mom_order < order) {
         if (!t.cellA) CUDA_TRY(tree_alloc(&t.cellA, (size_t)t.ncells));
+        if (t.periodic && !t.cellM0d) CUDA_TRY(tree_alloc(&t.cellM0d, (size_t)t.ncells));
         if (order >= 2 && !t.cellM2) { CUDA_TRY(tree_alloc(&t.cellM2, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellE2, (size_t)t.ncells)); }
         if (order >= 4 && !t.cellM34) { CUDA_TRY(tree_alloc(&t.cellM34, (size_t)t.ncells)); CUDA_TRY(tree_alloc(&t.cellMac, (size_t)t.ncells)); }
         if (order >= 6) { // f-3: raw moments of degree 5 .. order and their trace record (gen_hi_orders.py), in units of the cell side

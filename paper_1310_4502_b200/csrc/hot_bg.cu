@@ -29,7 +29,7 @@ __device__ __forceinline__ double cube1d(int a, double s) { // int_{-s/2}^{s/2} 
 struct BgRec { float m0, d1x, d1y, d1z; CellM2 E2; CellM34 M34; };
 
 template <int ORDER>
-__global__ void __launch_bounds__(128) bg_moments_kernel(const WalkCell* __restrict__ wcell, const CellA* __restrict__ cellA,
+__global__ void __launch_bounds__(128) bg_moments_kernel(const WalkCell* __restrict__ wcell, const CellA* __restrict__ cellA, const double* __restrict__ m0d,
                                                          const CellM2* __restrict__ cellM2, const CellM34* __restrict__ cellM34,
                                                          int64_t ncells, double lox, double loy, double loz, double size, double rhobar,
                                                          float4* __restrict__ bgA, CellM2* __restrict__ bgE2, CellM34* __restrict__ bgM34) {
@@ -42,7 +42,8 @@ __global__ void __launch_bounds__(128) bg_moments_kernel(const WalkCell* __restr
     const double cy = loy + (double)((wc.x >> 21) | ((wc.y & 0x3ffu) << 11)) * h + 0.5 * side;
     const double cz = loz + (double)((wc.y >> 10) & 0x1fffffu) * h + 0.5 * side;
     const CellA A = cellA[c];
-    const double m0 = (double)A.m0, dx = A.zx - cx, dy = A.zy - cy, dz = A.zz - cz; // centre of mass relative to the cell centre
+    const double m0 = m0d[c], dx = A.zx - cx, // the fp64 mass: mass - rhobar s^3 is a small difference for the coarse cells
+                  dy = A.zy - cy, dz = A.zz - cz; // centre of mass relative to the cell centre
     constexpr int P = ORDER >= 4 ? 4 : (ORDER >= 2 ? 2 : 1);
     constexpr int NM = (P + 1) * (P + 2) * (P + 3) / 6;
     double C[NM], M[NM];
@@ -219,9 +220,9 @@ __global__ void __launch_bounds__(BG_WARPS * 32) forces_bg_kernel(const __grid_c
 cudaError_t launch_bg_moments(const Tree& t, int order, double rhobar, cudaStream_t st) {
     const unsigned nb = (unsigned)((t.ncells + 127) / 128);
     HOT_LAUNCHED(1);
-    if (order >= 4) bg_moments_kernel<4><<<nb, 128, 0, st>>>(t.wcell, t.cellA, t.cellM2, t.cellM34, t.ncells, t.lo[0], t.lo[1], t.lo[2], t.size, rhobar, t.bgA, t.bgE2, t.bgM34);
-    else if (order >= 2) bg_moments_kernel<2><<<nb, 128, 0, st>>>(t.wcell, t.cellA, t.cellM2, t.cellM34, t.ncells, t.lo[0], t.lo[1], t.lo[2], t.size, rhobar, t.bgA, t.bgE2, t.bgM34);
-    else bg_moments_kernel<0><<<nb, 128, 0, st>>>(t.wcell, t.cellA, t.cellM2, t.cellM34, t.ncells, t.lo[0], t.lo[1], t.lo[2], t.size, rhobar, t.bgA, t.bgE2, t.bgM34);
+    if (order >= 4) bg_moments_kernel<4><<<nb, 128, 0, st>>>(t.wcell, t.cellA, t.cellM0d, t.cellM2, t.cellM34, t.ncells, t.lo[0], t.lo[1], t.lo[2], t.size, rhobar, t.bgA, t.bgE2, t.bgM34);
+    else if (order >= 2) bg_moments_kernel<2><<<nb, 128, 0, st>>>(t.wcell, t.cellA, t.cellM0d, t.cellM2, t.cellM34, t.ncells, t.lo[0], t.lo[1], t.lo[2], t.size, rhobar, t.bgA, t.bgE2, t.bgM34);
+    else bg_moments_kernel<0><<<nb, 128, 0, st>>>(t.wcell, t.cellA, t.cellM0d, t.cellM2, t.cellM34, t.ncells, t.lo[0], t.lo[1], t.lo[2], t.size, rhobar, t.bgA, t.bgE2, t.bgM34);
     return cudaGetLastError();
 }
 cudaError_t launch_forces_bg(const ForceArgs& a, const Tree& t, const double* far, double* farc, const uint4* pvlist, const uint32_t* lpv,

@@ -72,6 +72,7 @@ struct Tree {
     float *cellHiRaw = nullptr, *cellHiT = nullptr; // orders 6, 8 (f-3): raw moments of degree 5.. and their trace record, per cell, in units of the cell side
     int hi_order = 0;                        // order those two were built for (their per-cell strides follow from it)
     // f-1 (background subtraction, periodic): per cell, moments about the cell centre minus the uniform cube's
+    double* cellM0d = nullptr;               // periodic: cell masses in fp64 (upward pass)
     float4* bgA = nullptr; CellM2* bgE2 = nullptr; CellM34* bgM34 = nullptr; int bg_order = -1;
     double total_mass = 0.0;                 // sum of the masses in fp64 (the far field's zeroth moment)
     uint32_t* glpv = nullptr; unsigned long long* gpvoff = nullptr; // per group: accepted virtual cubes, where they start

@@ -198,6 +198,7 @@ struct MomArgs {
     const int32_t* leafcell; int64_t nleaves;
     const uint32_t *cfirst, *ccount, *cmask; const int32_t* cchild; const float4* body;
     CellA* cellA; CellM2* cellM2; CellM2* cellE2; CellM34* cellM34; float4* cellMac;
+    double* m0d; // periodic boxes: the cell mass in fp64 (the background-subtracted mass of hot_bg.cu is a small difference), else NULL
     float *hiRaw, *hiT; const WalkCell* wcell; double size; // orders 6, 8: raw and trace records in units of the cell side (side = size / 2^level)
 };
 __device__ __forceinline__ double cell_side(const MomArgs& P, int64_t c) { return ldexp(P.size, -(int)(P.wcell[c].w >> 27)); }
@@ -224,6 +225,7 @@ __global__ void __launch_bounds__(128) moments_leaves_kernel(const __grid_consta
         bmax = fmax(bmax, dx * dx + dy * dy + dz * dz);
         if (ORDER >= 2) add_point<ORDER>(M, (double)b.w, dx, dy, dz);
     }
+    if (P.m0d) P.m0d[c0] = m0;
     store_cell<ORDER>(c0, m0, zx, zy, zz, sqrt(bmax), M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac, P.hiRaw, P.hiT, ORDER > 4 ? cell_side(P, c0) : 1.0);
 }
 // an internal cell from its children (one level down, already done): parallel-axis shift, fixed child order
@@ -252,6 +254,7 @@ __device__ __forceinline__ void combine_children(const MomArgs& P, int64_t c) {
             add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
         }
     }
+    if (P.m0d) P.m0d[c] = m0;
     store_cell<ORDER>(c, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac, P.hiRaw, P.hiT, ORDER > 4 ? cell_side(P, c) : 1.0);
 }
 // One level of internal cells.  A warp looks at 32 consecutive cells of the level, keeps the internal ones (one in eight
@@ -306,6 +309,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constan
                 for (int k = 4; k < NM; ++k) M[k] += __shfl_xor_sync(0xffffffffu, M[k], o);
             }
         }
+        if (have && q == 0 && P.m0d) P.m0d[cell] = m0;
         if (have && q == 0) store_cell<ORDER>(cell, m0, zx, zy, zz, bmax, M, P.cellA, P.cellM2, P.cellE2, P.cellM34, P.cellMac, P.hiRaw, P.hiT, ORDER > 4 ? cell_side(P, cell) : 1.0);
         // drop the four cells just done
         for (int i = 0; i < 4 && todo; ++i) todo &= todo - 1;
@@ -346,7 +350,7 @@ cudaError_t launch_moments(const Tree& t, int order, cudaStream_t st) {
     MomArgs a;
     a.leafcell = t.leafcell; a.nleaves = t.nleaves; a.cfirst = t.cfirst; a.ccount = t.ccount; a.cmask = t.cmask; a.cchild = t.cchild;
     a.body = t.body; a.cellA = t.cellA; a.cellM2 = t.cellM2; a.cellE2 = t.cellE2; a.cellM34 = t.cellM34; a.cellMac = order >= 4 ? t.cellMac : nullptr;
-    a.hiRaw = t.cellHiRaw; a.hiT = t.cellHiT; a.wcell = t.wcell; a.size = t.size;
+    a.hiRaw = t.cellHiRaw; a.hiT = t.cellHiT; a.wcell = t.wcell; a.size = t.size; a.m0d = t.cellM0d;
     if (order >= 8) return moments_run<8>(t, a, st);
     if (order >= 6) return moments_run<6>(t, a, st);
     if (order >= 4) return moments_run<4>(t, a, st);
