@@ -173,6 +173,21 @@ int hot_measure_fp32_operands(double* tflops3);
  * units of the box: the table of the periodic far field (p = 8, ws = 2).  coef165: host. */
 int hot_far_coefficients(double* coef165);
 
+/* ---- the ONE allocation-free entry point ------------------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (CUDA graph capture, tight serving loops, harnesses that forbid it): the
+ * stable radix sort of hot_build (S2) on caller-provided buffers, its scratch (digit counts, tile tickets,
+ * look-back state) in a fixed device array inside the library.  Calls no cudaMalloc / cudaFree / allocating routine.
+ *   key      : device, [n] u64; in: the keys, out: sorted ascending
+ *   perm     : device, [n] u32; out: perm[i] = input position of the i-th sorted key; equal keys keep ascending position
+ *   key_work, idx_work : device, [n] u64 / u32 work buffers (contents undefined afterwards); none may alias another
+ *   n        : 1 <= n <= 2^22 = 4,194,304 (the fixed scratch: 2.1 MB, held by every GPU that loads the library until
+ *              exit); larger n: HOT_EINVAL with a message naming the limit (use hot_build)
+ *   cuda_stream : cudaStream_t the work is enqueued on (NULL: legacy default stream); returns without synchronising
+ * Every call shares the one scratch array (cleared at the start of each call, stream-ordered): calls that overlap on
+ * the GPU -- two streams, two host threads -- race.  Error text: hot_noalloc_last_error(). */
+int hot_sort_keys_noalloc(uint64_t* key, uint32_t* perm, uint64_t* key_work, uint32_t* idx_work, int64_t n, void* cuda_stream);
+const char* hot_noalloc_last_error(void);
+
 /* ---- introspection for the parity tests: HOST output arrays, caller-allocated -------------- */
 /* sorted keys and the permutation: key_sorted[i] = key of caller's particle perm[i]; [n] each */
 int hot_export_keys(uint64_t* key_sorted, uint32_t* perm);

@@ -13,8 +13,8 @@ from __future__ import annotations
 
 from .binding import (HotError, hot_build, hot_export_cells, hot_export_groups, hot_export_keys, hot_export_lists, hot_export_group_orders, hot_forces_tol,
                       hot_export_moments, hot_forces, hot_free, hot_last_error, hot_lookup_keys,
-                      hot_far_coefficients, hot_measure_fp32, hot_measure_fp32_operands, hot_set_list_arena, hot_set_softening, hot_set_background, hot_kick_drift, hot_set_params, hot_set_stream, hot_stats, hot_step_host, library_path)
+                      hot_far_coefficients, hot_measure_fp32, hot_measure_fp32_operands, hot_set_list_arena, hot_set_softening, hot_sort_keys_noalloc, hot_noalloc_last_error, hot_set_background, hot_kick_drift, hot_set_params, hot_set_stream, hot_stats, hot_step_host, library_path)
 
-__all__ = ["HotError", "hot_build", "hot_forces", "hot_stats", "hot_step_host", "hot_set_params", "hot_set_list_arena", "hot_set_softening", "hot_set_background", "hot_kick_drift", "hot_far_coefficients", "hot_measure_fp32", "hot_measure_fp32_operands",
+__all__ = ["HotError", "hot_build", "hot_forces", "hot_stats", "hot_step_host", "hot_set_params", "hot_set_list_arena", "hot_set_softening", "hot_sort_keys_noalloc", "hot_noalloc_last_error", "hot_set_background", "hot_kick_drift", "hot_far_coefficients", "hot_measure_fp32", "hot_measure_fp32_operands",
            "hot_set_stream", "hot_free", "hot_last_error", "hot_export_keys", "hot_export_cells",
            "hot_export_groups", "hot_export_lists", "hot_export_group_orders", "hot_forces_tol", "hot_export_moments", "hot_lookup_keys", "library_path"]

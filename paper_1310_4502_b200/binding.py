@@ -63,6 +63,8 @@ def _load():
         lib.hot_set_params.argtypes = [C.c_int, C.c_int]
         lib.hot_set_list_arena.argtypes = [C.c_int64]
         lib.hot_set_softening.argtypes = [C.c_int]
+        lib.hot_sort_keys_noalloc.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
+        lib.hot_noalloc_last_error.restype = C.c_char_p
         lib.hot_set_background.argtypes = [C.c_int]
         lib.hot_kick_drift.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int64, C.c_float, C.c_float, hot_box, C.c_int]
         lib.hot_far_coefficients.argtypes = [C.c_void_p]
@@ -152,6 +154,27 @@ def hot_kick_drift(pos, vel, acc, dt_kick, dt_drift, lo, size, periodic=False):
             raise TypeError(f"hot_kick_drift wants {name} as a contiguous CUDA float32 [n,3] tensor on the current device")
     _check(_load().hot_kick_drift(pos.data_ptr(), vel.data_ptr(), acc.data_ptr(), pos.shape[0], float(dt_kick), float(dt_drift),
                                   _box(lo, size), int(bool(periodic))))
+
+
+def hot_noalloc_last_error() -> str:
+    return _load().hot_noalloc_last_error().decode()
+
+
+def hot_sort_keys_noalloc(key, perm, key_work, idx_work, stream=None):
+    """Allocation-free stable sort (n <= 2^22): key [n] 8-byte integers (sorted in place), perm [n] 4-byte integers
+    (out), two work tensors of the same kinds; contiguous CUDA tensors on the current device.  Enqueues on `stream`
+    (torch.cuda.Stream; default: torch's current stream) and returns without synchronising."""
+    import torch
+
+    n = key.numel()
+    for t_, size, name in ((key, 8, "key"), (key_work, 8, "key_work"), (perm, 4, "perm"), (idx_work, 4, "idx_work")):
+        if not (t_.is_cuda and t_.is_contiguous() and t_.element_size() == size and not t_.dtype.is_floating_point
+                and t_.numel() == n and t_.device.index == torch.cuda.current_device()):
+            raise TypeError(f"hot_sort_keys_noalloc wants {name} as a contiguous CUDA tensor of {n} {size}-byte integers on the current device")
+    s = torch.cuda.current_stream() if stream is None else stream
+    rc = _load().hot_sort_keys_noalloc(key.data_ptr(), perm.data_ptr(), key_work.data_ptr(), idx_work.data_ptr(), n, C.c_void_p(s.cuda_stream))
+    if rc != 0:
+        raise HotError(rc, hot_noalloc_last_error())
 
 
 def hot_free():

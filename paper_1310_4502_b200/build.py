@@ -17,7 +17,7 @@ INCLUDE = os.path.join(os.path.dirname(HERE), "include")
 OBJ = os.path.join(CSRC, "build")
 LIB = os.path.join(HERE, "libhot.so")
 SOURCES = ["hot_api.cu", "hot_build.cu", "hot_moments.cu", "hot_walk.cu", "hot_forces.cu", "hot_forces_periodic.cu",
-           "hot_periodic.cu", "hot_peak.cu", "hot_step.cu", "hot_hi.cu", "hot_bg.cu"]
+           "hot_periodic.cu", "hot_peak.cu", "hot_step.cu", "hot_hi.cu", "hot_bg.cu", "hot_noalloc.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-I" + INCLUDE, "-I" + CSRC]
 
