@@ -241,7 +241,8 @@ __device__ __forceinline__ void combine_children(const MomArgs& P, int64_t c) {
     double m0 = 0, zx = 0, zy = 0, zz = 0, bmax = 0; // bmax: DESIGN.md R-15 (children's radii + centre offsets)
     for (int q = 0; q < nch; ++q) {
         const CellA A = P.cellA[ch + q];
-        m0 += (double)A.m0; zx += (double)A.m0 * A.zx; zy += (double)A.m0 * A.zy; zz += (double)A.m0 * A.zz;
+        const double cm = P.m0d ? P.m0d[ch + q] : (double)A.m0; // periodic boxes carry the masses in fp64 (a 2^24-body cell's mass does not fit fp32's 24 bits)
+        m0 += cm; zx += cm * A.zx; zy += cm * A.zy; zz += cm * A.zz;
     }
     zx /= m0; zy /= m0; zz /= m0;
     for (int q = 0; q < nch; ++q) {
@@ -251,7 +252,7 @@ __device__ __forceinline__ void combine_children(const MomArgs& P, int64_t c) {
         if (ORDER >= 2) {
             double C[NM];
             load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C, P.hiRaw, ORDER > 4 ? cell_side(P, ch + q) : 1.0);
-            add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
+            add_shifted<ORDER>(M, C, P.m0d ? P.m0d[ch + q] : (double)A.m0, dx, dy, dz);
         }
     }
     if (P.m0d) P.m0d[c] = m0;
@@ -281,7 +282,8 @@ __global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constan
         const bool mine = have && q < nch;
         CellA A; A.zx = A.zy = A.zz = 0.0; A.m0 = 0.f; A.bmax = 0.f;
         if (mine) A = P.cellA[ch + q];
-        double m0 = (double)A.m0, zx = m0 * A.zx, zy = m0 * A.zy, zz = m0 * A.zz;
+        const double cm = mine ? (P.m0d ? P.m0d[ch + q] : (double)A.m0) : 0.0;
+        double m0 = cm, zx = m0 * A.zx, zy = m0 * A.zy, zz = m0 * A.zz;
 #pragma unroll
         for (int o = 1; o < 8; o <<= 1) {
             m0 += __shfl_xor_sync(0xffffffffu, m0, o); zx += __shfl_xor_sync(0xffffffffu, zx, o);
@@ -298,7 +300,7 @@ __global__ void __launch_bounds__(128) moments_level_kernel(const __grid_constan
             if (ORDER >= 2) {
                 double C[NM];
                 load_child<ORDER>(ch + q, P.cellM2, P.cellM34, C, P.hiRaw, ORDER > 4 ? cell_side(P, ch + q) : 1.0);
-                add_shifted<ORDER>(M, C, (double)A.m0, dx, dy, dz);
+                add_shifted<ORDER>(M, C, cm, dx, dy, dz);
             }
         }
 #pragma unroll
