@@ -394,6 +394,13 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     CUDA_TRY(tree_alloc(&g.d_tops, 3));
     const size_t esz = t.periodic ? 5 : 4; // bytes per list entry: u32 (+ u8 image id)
     if (g.stage_cap < 1024) g.stage_cap = 16384;
+    // a group's cell list cannot hold more than every cell of every image, nor its run list more than one run per leaf and
+    // per 32 bodies: small problems get a small staging area (it is nwarps x 2 x stage_cap words: 0.8 GB at 16384)
+    int64_t stage_use = g.stage_cap;
+    {
+        const int64_t most = (t.periodic ? 125 : 1) * (t.ncells + t.n / 32 + 1);
+        if (most < stage_use) stage_use = most < 1024 ? 1024 : ((most + 1023) / 1024) * 1024;
+    }
     // arena capacity in entries: what the last call needed plus 12%, else a first guess
     unsigned long long cappc = g.used_pc ? g.used_pc + g.used_pc / 8 + 4096 : (unsigned long long)ng * (t.periodic ? 6000 : 2800) + 65536;
     unsigned long long cappp = g.used_pp ? g.used_pp + g.used_pp / 8 + 4096 : (unsigned long long)ng * (t.periodic ? 3000 : 1400) + 65536;
@@ -417,8 +424,8 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         return HOT_OK;
     };
     auto alloc_stage = [&]() -> int {
-        CUDA_TRY(tree_alloc(&g.d_stage, (size_t)nwarps * 2 * (size_t)g.stage_cap));
-        if (t.periodic) CUDA_TRY(tree_alloc(&g.d_stage_img, (size_t)nwarps * 2 * (size_t)g.stage_cap));
+        CUDA_TRY(tree_alloc(&g.d_stage, (size_t)nwarps * 2 * (size_t)stage_use));
+        if (t.periodic) CUDA_TRY(tree_alloc(&g.d_stage_img, (size_t)nwarps * 2 * (size_t)stage_use));
         return HOT_OK;
     };
     rc = alloc_lists(); if (rc) return rc;
@@ -492,7 +499,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         CUDA_TRY(cudaMemcpyAsync(g.d_flags + 3, &ff0, sizeof(int), cudaMemcpyHostToDevice, st));
         wa.g0 = g0; wa.g1 = g0 + budget < ng ? g0 + budget : ng;
         wa.pclist = g.d_pclist; wa.pplist = g.d_pplist; wa.pcimg = g.d_pcimg; wa.ppimg = g.d_ppimg; wa.cappc = cappc; wa.cappp = cappp;
-        wa.stage = g.d_stage; wa.stage_img = g.d_stage_img; wa.stage_cap = g.stage_cap;
+        wa.stage = g.d_stage; wa.stage_img = g.d_stage_img; wa.stage_cap = stage_use;
         CUDA_TRY(cudaEventRecord(g.evx[0], st));
         CUDA_TRY(launch_walk(wa, st));
         CUDA_TRY(cudaEventRecord(g.evx[1], st));
@@ -515,7 +522,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         }
         if (fl[0] & 8) { // a group's lists outgrew the per-warp staging area: enlarge it and walk this range again
             if (g.stage_cap >= ((int64_t)1 << 26)) return fail(HOT_ENOMEM, "hot_forces: one sink group's interaction list exceeds 2^26 entries");
-            g.stage_cap *= 4;
+            g.stage_cap = stage_use * 4; stage_use = g.stage_cap;
             rc = alloc_stage(); if (rc) return rc;
             CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
             continue;
@@ -533,7 +540,8 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
             rc = alloc_lists(); if (rc) return rc;
             continue;
         }
-        usedpc += tops[0]; usedpp += tops[1];
+        // tops also counts what groups that did not fit asked for: no more than the arena was really written
+        usedpc += tops[0] < cappc ? tops[0] : cappc; usedpp += tops[1] < cappp ? tops[1] : cappp;
         a.g0 = g0; a.g1 = F;
         a.nsb = (unsigned int)((F - g0 + ((int64_t)1 << a.sb_shift) - 1) >> a.sb_shift);
         a.pclist = g.d_pclist; a.pplist = g.d_pplist; a.pcimg = g.d_pcimg; a.ppimg = g.d_ppimg;
