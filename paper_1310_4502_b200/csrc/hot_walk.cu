@@ -23,6 +23,8 @@
 #define FULL 0xffffffffu
 #define WALK_WARPS 8   // warps per block
 #define RING 512       // deque entries per warp (runs of <= 8 sibling cells); a power of two
+#define WALK_MINBLK 6 // resident blocks per SM the kernel is compiled for (40 registers): the walk of one group is a chain of dependent
+                      // cell-record loads, so resident warps are what hides it (3 blocks: 10.4 ms, 5: 6.6, 6: 5.2, 8 with spills: 5.2 at C2)
 
 // Pending work: a ring buffer used as a deque.  An entry is a run of sibling cells
 // (first cell | (count-1) << 28, count <= 8): opening a cell pushes ONE entry.  While the ring is short
@@ -40,7 +42,7 @@
 // laid out plain | flagged); empty octants of opened cells and the cubes of rejected leaves outside K_G go to a stack of
 // VIRTUAL cubes (only the negative background), which are accepted by the same criterion or subdivided.
 template <bool PER, bool TOL, bool BG>
-__global__ void __launch_bounds__(WALK_WARPS * 32) walk_kernel(const __grid_constant__ WalkArgs P) {
+__global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(const __grid_constant__ WalkArgs P) {
     __shared__ uint32_t s_ring[WALK_WARPS][RING];
     __shared__ uint8_t s_img[PER ? WALK_WARPS : 1][PER ? RING : 1];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
