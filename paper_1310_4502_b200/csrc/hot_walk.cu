@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
             if (TOL || BG) { n0 += __popc(__ballot_sync(FULL, acc && ocode == 0)); n2 += __popc(__ballot_sync(FULL, acc && ocode == 1)); }
             // rejected leaves -> one body run each (a leaf holds <= 32 bodies except at the finest level)
             if (mrej) {
-                uint32_t nb = rej_leaf ? cnt : 0u;
+                nbody += rej_leaf ? cnt : 0u; // per lane; summed over the warp when the walk of the group is done
                 const bool small = rej_leaf && cnt <= 32u;
                 const uint32_t msmall = __ballot_sync(FULL, small);
                 uint32_t mbig = mrej & ~msmall;
@@ -203,9 +203,6 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
                     }
                     nrun += nr;
                 }
-#pragma unroll
-                for (int o = 16; o > 0; o >>= 1) nb += __shfl_xor_sync(FULL, nb, o);
-                nbody += nb;
             }
             // opened cells -> their child run into the ring
             if (open) {
@@ -278,6 +275,7 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
             }
             if (npv > (uint32_t)P.vstage_cap) { if (lane == 0) atomicOr(P.errflag, 16); continue; }
         }
+        nbody = __reduce_add_sync(FULL, nbody);
         // the group's lists are complete: take a slice of the arena and move them there; the body
         // runs are expanded to one body index per entry on the way (32 entries per step)
         if (npc > scap || nrun > scap) { if (lane == 0) atomicOr(P.errflag, 8); continue; }
@@ -294,7 +292,22 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
         pcb = __shfl_sync(FULL, pcb, 0); ppb = __shfl_sync(FULL, ppb, 0);
         __syncwarp();
         if (!TOL && !BG) {
-            for (uint32_t j = lane; j < npc; j += 32) { P.pclist[pcb + j] = spc[j]; if (PER) P.pcimg[pcb + j] = ipc[j]; }
+            // four loads in flight per lane: the staged list comes back from L2, and a one-at-a-time copy loop was 20% of the
+            // kernel's warp samples
+            for (uint32_t j0 = lane; j0 < npc; j0 += 128) {
+                uint32_t v[4]; uint8_t vi[4];
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t j = j0 + 32u * k;
+                    v[k] = j < npc ? spc[j] : 0u;
+                    if (PER) vi[k] = j < npc ? ipc[j] : (uint8_t)0;
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const uint32_t j = j0 + 32u * k;
+                    if (j < npc) { P.pclist[pcb + j] = v[k]; if (PER) P.pcimg[pcb + j] = vi[k]; }
+                }
+            }
         } else { // three stable passes: monopoles, quadrupoles, hexadecapoles; the order bits are dropped
             uint32_t base = 0;
             for (uint32_t o = 0; o < 3; ++o)
@@ -312,27 +325,30 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
                 }
         }
         {
-            uint32_t r = 0, roff = 0, out = 0; // next run, bodies of it already written, entries written
-            while (out < nbody) {
+            // The body runs are expanded through the warp's ring buffer, which is empty now: 32 runs per step, one per lane;
+            // an exclusive scan of the run lengths says where each goes; every lane writes its run into the ring (strided
+            // shared-memory stores), then the warp copies the ring out coalesced.  (A warp scan per 32 OUTPUT entries, as in
+            // round 1, was 19% of the kernel's instructions; writing the runs straight to global memory, one run per lane,
+            // was slower still: partial-sector stores.)
+            uint32_t out = 0;
+            for (uint32_t r = 0; r < nrun;) {
                 uint32_t e = 0; int eim = 62, ecnt = 0;
-                if (r + lane < nrun) { e = spp[r + lane]; if (PER) eim = ipp[r + lane]; ecnt = (int)(e >> HOT_RUN_SHIFT) + 1 - (lane == 0 ? (int)roff : 0); }
+                if (r + lane < nrun) { e = spp[r + lane]; if (PER) eim = ipp[r + lane]; ecnt = (int)(e >> HOT_RUN_SHIFT) + 1; }
                 int incl = ecnt;
 #pragma unroll
                 for (int o = 1; o < 32; o <<= 1) { const int y = __shfl_up_sync(FULL, incl, o); if (lane >= o) incl += y; }
-                const int excl = incl - ecnt;
-                const bool take = ecnt > 0 && excl < 32; // the run starts inside this step's 32 entries
+                const bool take = ecnt > 0 && incl <= RING; // a run holds <= 32 bodies: at least 16 runs fit
                 const int ne = __popc(__ballot_sync(FULL, take));
-                const int tot = __shfl_sync(FULL, incl, ne - 1), exl = __shfl_sync(FULL, excl, ne - 1);
-                const int nt = min(32, tot);
-                const uint32_t starts = __reduce_or_sync(FULL, take ? (1u << excl) : 0u);
-                const int src = max(0, __popc(starts & ((2u << lane) - 1u)) - 1);
-                const uint32_t eb = __shfl_sync(FULL, (e & ((1u << HOT_RUN_SHIFT) - 1u)) + (lane == 0 ? roff : 0u), src);
-                const int ex = __shfl_sync(FULL, excl, src);
-                const int si = PER ? __shfl_sync(FULL, eim, src) : 0;
-                if (lane < nt) { P.pplist[ppb + out + lane] = eb + (uint32_t)(lane - ex); if (PER) P.ppimg[ppb + out + lane] = (uint8_t)si; }
-                out += (uint32_t)nt;
-                if (tot > 32) { roff = (ne == 1 ? roff : 0u) + (uint32_t)(32 - exl); r += (uint32_t)(ne - 1); } // last run only partly written
-                else { roff = 0u; r += (uint32_t)ne; }
+                const int tot = __shfl_sync(FULL, incl, ne - 1);
+                const uint32_t first = e & ((1u << HOT_RUN_SHIFT) - 1u);
+                const int at = incl - ecnt;
+                const int longest = __reduce_max_sync(FULL, take ? ecnt : 0);
+                for (int k = 0; k < longest; ++k)
+                    if (take && k < ecnt) { ring[at + k] = first + (uint32_t)k; if (PER) rimg[at + k] = (uint8_t)eim; }
+                __syncwarp();
+                for (int j = lane; j < tot; j += 32) { P.pplist[ppb + out + j] = ring[j]; if (PER) P.ppimg[ppb + out + j] = rimg[j]; }
+                __syncwarp();
+                out += (uint32_t)tot; r += (uint32_t)ne;
             }
         }
         if (BG) { // the accepted virtual cubes: their own arena
