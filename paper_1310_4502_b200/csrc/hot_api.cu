@@ -20,6 +20,7 @@ struct Ctx {
     int softening = 0; // 0 Plummer, 1 cubic spline (hot_set_softening)
     int background = 0; // 1: per-cell background subtraction in periodic boxes (hot_set_background)
     uint4 *d_vstack = nullptr, *d_vstage = nullptr, *d_pvlist = nullptr; // virtual cubes of the background-subtracted walk
+    int64_t vcap = 4096;        // per-warp capacity of the stack of virtual cubes and of a group's accepted ones; grown fourfold on overflow
     int64_t pv_per_group = 192; // their arena is sized for this many per group; grown fourfold when a walk overflows it
     int last_order = -1, last_tolmode = 0, last_bgmode = 0;
     char err[512] = "";
@@ -446,7 +447,7 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
     for (int k = 0; k < 3; ++k) wa.lo[k] = t.lo[k];
     if (tolmode || bgmode) { CUDA_TRY(tree_alloc(&t.glpc0, (size_t)ng)); CUDA_TRY(tree_alloc(&t.glpc2, (size_t)ng)); }
     wa.bgmode = bgmode; wa.cmask = t.cmask;
-    const int64_t vstack_cap = 4096, vstage_cap = 4096;
+    int64_t vstack_cap = g.vcap, vstage_cap = g.vcap;
     unsigned long long cappv = 0;
     if (bgmode) {
         CUDA_TRY(tree_alloc(&g.d_vstack, (size_t)nwarps * (size_t)vstack_cap));
@@ -510,7 +511,15 @@ int forces_impl(const int tolmode, const double theta, const double tol, const d
         CUDA_TRY(cudaStreamSynchronize(st));
         ms_walk += ms_between(g.evx[0], g.evx[1]);
         if (fl[0] & 4) return fail(HOT_EINTERNAL, "hot_forces: traversal scratch exhausted");
-        if (fl[0] & 16) return fail(HOT_EINTERNAL, "hot_forces: virtual-cube scratch of the background-subtracted walk exhausted");
+        if (fl[0] & 16) { // a group's virtual cubes outgrew the per-warp scratch (sparse sets: much empty space to tile): enlarge it, walk again
+            if (g.vcap >= ((int64_t)1 << 20)) return fail(HOT_EINTERNAL, "hot_forces: virtual-cube scratch of the background-subtracted walk exhausted");
+            g.vcap *= 4; vstack_cap = vstage_cap = g.vcap;
+            CUDA_TRY(tree_alloc(&g.d_vstack, (size_t)nwarps * (size_t)vstack_cap));
+            CUDA_TRY(tree_alloc(&g.d_vstage, (size_t)nwarps * (size_t)vstage_cap));
+            wa.vstack = g.d_vstack; wa.vstack_cap = vstack_cap; wa.vstage = g.d_vstage; wa.vstage_cap = vstage_cap;
+            CUDA_TRY(cudaMemsetAsync(g.d_flags + 2, 0, sizeof(int), st));
+            continue;
+        }
         if (fl[0] & 32) { // the accepted virtual cubes outgrew their arena: enlarge it and walk this range again
             if (g.pv_per_group >= (1 << 16)) return fail(HOT_ENOMEM, "hot_forces: the virtual-cube list of the background-subtracted walk does not fit its arena");
             g.pv_per_group *= 4;

@@ -801,3 +801,125 @@ def test_background_subtraction_parity(hot, cfg, side, order, theta, ncrit):
     acc0, pot0 = hot.hot_forces(theta, w.eps, order)
     d = np.linalg.norm(acc.cpu().numpy().astype(np.float64) - acc0.cpu().numpy().astype(np.float64), axis=1)
     assert np.sqrt((d ** 2).mean()) < (0.05 if order == 0 else 5e-3) * arms
+
+
+def test_seeded_fuzz_of_the_round2_modes(hot):
+    """Seeded random small problems through the round-2 modes: background subtraction (periodic, every theta incl.
+    > 1/sqrt(3) where cells straddle the near cube, tiny and ragged sizes, empty octants), spline softening (open and
+    periodic), orders 6 / 8, and the error-bound criterion.  Counts bit-exact where the criterion is integer, forces at
+    the fuzz tolerance of test_seeded_fuzz_of_sizes_bucket_sizes_orders_and_boundaries."""
+    import torch
+
+    rng = np.random.default_rng(20261105)
+    for trial in range(16):
+        mode = ("bg", "spline", "hi", "tol")[trial % 4]
+        n = int(rng.integers(2, 2500))
+        if mode == "hi":
+            n = min(n, 400)  # the oracle's general tensor recursion is exponential in the order
+        periodic = mode == "bg" or (mode == "spline" and trial % 8 >= 4)
+        nleaf = int(rng.choice([1, 3, 8, 16]))
+        ncrit = int(max(nleaf, rng.choice([4, 32, 64, 256])))
+        order = int(rng.choice([0, 2, 4])) if mode != "hi" else int(rng.choice([6, 8]))
+        theta = float(rng.choice([0.35, 0.5, 0.7, 0.9]))
+        x = rng.uniform(0.0, 1.0, (n, 3))
+        if trial % 3 == 1:  # clumps leave most of the box empty: many virtual cubes
+            c = rng.uniform(0.2, 0.8, (5, 3))
+            x = np.clip(c[rng.integers(0, 5, n)] + 0.02 * rng.standard_normal((n, 3)), 0.0, 0.999)
+        pos = np.minimum(np.ascontiguousarray(x.astype(np.float32)), np.float32(0.9999))
+        mass = (rng.uniform(0.5, 1.5, n) / n).astype(np.float32)
+        eps = 2e-3
+        hot.hot_set_params(nleaf, ncrit)
+        hot.hot_build(torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda(), (0.0, 0.0, 0.0), 1.0, periodic)
+        if mode == "hi":
+            O.set_moment_order(order)
+        try:
+            T = O.Tree(pos, mass, (0.0, 0.0, 0.0), 1.0, periodic=periodic, nleaf=nleaf, ncrit=ncrit)
+        finally:
+            O.set_moment_order(4)
+        nsel = {"bg": 6, "hi": 3}.get(mode, 16)
+        sel = None if T.ngroups <= nsel else np.sort(rng.choice(T.ngroups, nsel, replace=False))
+        idx = np.arange(T.ngroups) if sel is None else sel
+        tag = (trial, mode, n, nleaf, ncrit, order, theta, periodic)
+        if mode == "bg":
+            hot.hot_set_background(True)
+            try:
+                acc, pot = hot.hot_forces(theta, eps, order)
+                gg, go = hot.hot_export_groups(), hot.hot_export_group_orders()
+            finally:
+                hot.hot_set_background(False)
+            oa, op, lpc, lbg, lv, lpp = T.forces_bg(theta, eps, order, groups=sel)
+            assert (gg["lpc"][idx] == lpc.astype(np.uint64)).all() and (gg["lpp"][idx] == lpp.astype(np.uint64)).all(), tag
+            assert (go["quad"][idx] == lbg.astype(np.uint64)).all() and (go["hexa"][idx] == lv.astype(np.uint64)).all(), tag
+        elif mode == "spline":
+            hot.hot_set_softening(1); O.set_softening(1)
+            try:
+                acc, pot = hot.hot_forces(theta, eps * 10, order)
+                gg = hot.hot_export_groups()
+                oa, op, lpc, lpp = T.forces(theta, eps * 10, order, groups=sel)
+            finally:
+                hot.hot_set_softening(0); O.set_softening(0)
+            assert (gg["lpc"][idx] == lpc.astype(np.uint64)).all() and (gg["lpp"][idx] == lpp.astype(np.uint64)).all(), tag
+        elif mode == "hi":
+            acc, pot = hot.hot_forces(theta, eps, order)
+            gg = hot.hot_export_groups()
+            oa, op, lpc, lpp = T.forces(theta, eps, order, groups=sel)
+            assert (gg["lpc"][idx] == lpc.astype(np.uint64)).all() and (gg["lpp"][idx] == lpp.astype(np.uint64)).all(), tag
+        else:
+            ad, _ = O.direct(pos, mass, eps)
+            tol = 1e-3 * float(np.sqrt((ad ** 2).sum(1).mean()))
+            acc, pot = hot.hot_forces_tol(tol, eps)
+            gg, go = hot.hot_export_groups(), hot.hot_export_group_orders()
+            oa, op, l0, l2, l4, lpp = T.forces_tol(tol, eps, groups=sel)
+            same = (go["mono"][idx] == l0.astype(np.uint64)) & (go["quad"][idx] == l2.astype(np.uint64)) & (go["hexa"][idx] == l4.astype(np.uint64))
+            assert same.mean() >= 0.8, tag
+            keep = np.zeros(n, bool)
+            c = T.cells(); perm = T.keys()[2]
+            for g_, ok in zip(idx, same):
+                if ok:
+                    cell = T.groups()[g_]
+                    keep[perm[c["first"][cell]:c["first"][cell] + c["count"][cell]]] = True
+            oa = np.where(keep[:, None], oa, np.nan); op = np.where(keep, op, np.nan)
+        m = ~np.isnan(op)
+        if not m.any():
+            continue
+        ga = acc.cpu().numpy().astype(np.float64)[m]; gpot = pot.cpu().numpy().astype(np.float64)[m]
+        ascale = np.sqrt((oa[m] ** 2).sum(axis=1).mean()) + 1e-300
+        pscale = np.sqrt((op[m] ** 2).mean()) if mode == "bg" else (57.18721055 * float(mass.astype(np.float64).sum()) if periodic else 0.0)
+        ea = np.linalg.norm(ga - oa[m], axis=1) / (np.linalg.norm(oa[m], axis=1) + 1e-3 * ascale)
+        ep = np.abs(gpot - op[m]) / (np.abs(op[m]) + pscale + 1e-300)
+        assert np.median(ea) <= 1e-5 and ea.max() <= 1e-3, tag + (np.median(ea), ea.max())
+        assert np.median(ep) <= 1e-5 and ep.max() <= 1e-3, tag + (np.median(ep), ep.max())
+    hot.hot_set_params(16, 256)
+
+
+def test_background_subtraction_with_many_virtual_cubes(hot):
+    """A clumpy periodic set leaves most of the box empty: a small sink group then has thousands of negative-background
+    cubes (empty octants subdivided down to its own scale), more than the walk's first per-warp scratch holds -- the
+    library enlarges the scratch and walks again."""
+    import torch
+
+    rng = np.random.default_rng(41)
+    n = 1300
+    c = rng.uniform(0.2, 0.8, (5, 3))
+    x = np.clip(c[rng.integers(0, 5, n)] + 0.02 * rng.standard_normal((n, 3)), 0.0, 0.999)
+    pos = np.ascontiguousarray(x.astype(np.float32)); mass = np.full(n, 1.0 / n, np.float32)
+    hot.hot_free()  # start from the default scratch sizes
+    hot.hot_set_params(8, 32)
+    hot.hot_build(torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda(), (0.0, 0.0, 0.0), 1.0, True)
+    hot.hot_set_background(True)
+    try:
+        acc, pot = hot.hot_forces(0.35, 2e-3, 2)
+        gg, go = hot.hot_export_groups(), hot.hot_export_group_orders()
+    finally:
+        hot.hot_set_background(False)
+    assert go["hexa"].max() > 4096, go["hexa"].max()
+    T = O.Tree(pos, mass, (0.0, 0.0, 0.0), 1.0, periodic=True, nleaf=8, ncrit=32)
+    sel = np.unique(np.append(np.arange(0, T.ngroups, max(1, T.ngroups // 6)), int(np.argmax(go["hexa"]))))
+    oa, op, lpc, lbg, lv, lpp = T.forces_bg(0.35, 2e-3, 2, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    assert (go["quad"][sel] == lbg.astype(np.uint64)).all() and (go["hexa"][sel] == lv.astype(np.uint64)).all()
+    m = ~np.isnan(op)
+    ga = acc.cpu().numpy().astype(np.float64)[m]
+    ea = np.linalg.norm(ga - oa[m], axis=1) / np.linalg.norm(oa[m], axis=1)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4, (np.median(ea), np.quantile(ea, 0.999))
+    hot.hot_set_params(16, 256)
