@@ -26,6 +26,15 @@
 #define WALK_MINBLK 6 // resident blocks per SM the kernel is compiled for (40 registers): the walk of one group is a chain of dependent
                       // cell-record loads, so resident warps are what hides it (3 blocks: 10.4 ms, 5: 6.6, 6: 5.2, 8 with spills: 5.2 at C2)
 
+// At 40 registers the kernel is bound by instruction issue (ncu: issue slots 81% busy, 4.2 G warp instructions at C2), and a
+// third of the inner loop was address arithmetic that ptxas re-did every trip -- the warp's number from %ctaid and %tid,
+// 64-bit products with the arena strides -- because nothing of it fitted in registers.  So what a warp needs only now and
+// then lives in SLOTS words behind its ring in shared memory and is RE-READ where it is used (volatile: one LDS.64 and one
+// IMAD.WIDE per staged store instead of eleven instructions): the warp's arena pointers, the number of the group it is
+// walking, its spill count.  4.49 -> 3.78 ms at C2, 1.42 -> 1.22 ms at 128^3 periodic; 1368 -> 1000 instructions.
+enum { SLOT_SPC = 0, SLOT_SPP = 2, SLOT_IPC = 4, SLOT_IPP = 6, SLOT_VSTACK = 8, SLOT_VSTAGE = 10, SLOT_GSTACK = 12, SLOT_GROUP = 14, SLOT_NSPILL = 15, SLOTS = 16 };
+#define WSLOT(T, k) (*reinterpret_cast<T volatile*>(ring + RING + (k)))
+
 // Pending work: a ring buffer used as a deque.  An entry is a run of sibling cells
 // (first cell | (count-1) << 28, count <= 8): opening a cell pushes ONE entry.  While the ring is short
 // the warp pops the four OLDEST entries (breadth-first: keeps the frontier wide and the 32 lanes busy);
@@ -43,28 +52,45 @@
 // VIRTUAL cubes (only the negative background), which are accepted by the same criterion or subdivided.
 template <bool PER, bool TOL, bool BG>
 __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(const __grid_constant__ WalkArgs P) {
-    __shared__ uint32_t s_ring[WALK_WARPS][RING];
+    __shared__ uint32_t s_ring[WALK_WARPS][RING + SLOTS];
     __shared__ uint8_t s_img[PER ? WALK_WARPS : 1][PER ? RING : 1];
     const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
     uint32_t* const ring = s_ring[w];
     uint8_t* const rimg = s_img[PER ? w : 0];
     const int64_t gwarp = (int64_t)blockIdx.x * WALK_WARPS + w;
-    uint32_t* const gstack = P.gstack + gwarp * P.gstack_cap * (PER ? 2 : 1);
     const uint32_t scap = (uint32_t)P.stage_cap;
-    uint32_t* const spc = P.stage + gwarp * 2 * P.stage_cap; // staged cell list
-    uint32_t* const spp = spc + P.stage_cap;                 // staged run list
-    uint8_t* const ipc = PER ? P.stage_img + gwarp * 2 * P.stage_cap : nullptr;
-    uint8_t* const ipp = PER ? ipc + P.stage_cap : nullptr;
-    uint4* const vstack = BG ? P.vstack + gwarp * P.vstack_cap : nullptr;   // virtual cubes to look at: (x | y<<21, y>>11 | z<<10, level, image)
-    uint4* const vstage = BG ? P.vstage + gwarp * P.vstage_cap : nullptr;   // accepted virtual cubes of the group
+    if (lane == 0) {
+        WSLOT(uint32_t*, SLOT_SPC) = P.stage + gwarp * 2 * P.stage_cap;
+        WSLOT(uint32_t*, SLOT_SPP) = P.stage + gwarp * 2 * P.stage_cap + P.stage_cap;
+        WSLOT(uint32_t*, SLOT_GSTACK) = P.gstack + gwarp * P.gstack_cap * (PER ? 2 : 1);
+        if (PER) {
+            WSLOT(uint8_t*, SLOT_IPC) = P.stage_img + gwarp * 2 * P.stage_cap;
+            WSLOT(uint8_t*, SLOT_IPP) = P.stage_img + gwarp * 2 * P.stage_cap + P.stage_cap;
+        }
+        if (BG) {
+            WSLOT(uint4*, SLOT_VSTACK) = P.vstack + gwarp * P.vstack_cap;
+            WSLOT(uint4*, SLOT_VSTAGE) = P.vstage + gwarp * P.vstage_cap;
+        }
+        WSLOT(uint32_t, SLOT_NSPILL) = 0; // touched by lane 0 only
+    }
+    __syncwarp();
+#define spc WSLOT(uint32_t*, SLOT_SPC)       // staged cell list
+#define spp WSLOT(uint32_t*, SLOT_SPP)       // staged run list
+#define ipc WSLOT(uint8_t*, SLOT_IPC)        // their image numbers (periodic)
+#define ipp WSLOT(uint8_t*, SLOT_IPP)
+#define gstack WSLOT(uint32_t*, SLOT_GSTACK) // where the ring spills
+#define vstack WSLOT(uint4*, SLOT_VSTACK)    // BG: virtual cubes to look at: (x | y<<21, y>>11 | z<<10, level, image)
+#define vstage WSLOT(uint4*, SLOT_VSTAGE)    // BG: accepted virtual cubes of the group
     const uint32_t lt = (1u << lane) - 1u;
     constexpr int M = RING - 1, DEQ_DFS = RING / 4, NIMG = PER ? 125 : 1;
-    unsigned long long nspill = 0;
 
     while (true) {
         unsigned int q = 0;
         if (lane == 0) q = atomicAdd(P.counter, 1u);
-        const int64_t gi = P.g0 + (int64_t)__shfl_sync(FULL, q, 0);
+        q = __shfl_sync(FULL, q, 0);
+        if (lane == 0) WSLOT(uint32_t, SLOT_GROUP) = q; // needed again only when the walk of the group is done
+        __syncwarp();
+#define gi (P.g0 + (int64_t)WSLOT(uint32_t, SLOT_GROUP))
         if (gi >= P.g1 || gi > (int64_t)*(volatile int*)P.first_fail) break;
         const GroupRec g = P.group[gi];
         const uint32_t gcell = g.cell;
@@ -106,7 +132,8 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
                     if (PER) gstack[P.gstack_cap + gtop + t] = rimg[(head + t) & M]; // image ids: second half of the arena
                 }
                 __syncwarp();
-                gtop += mv; head = (head + mv) & M; top = keep; ++nspill;
+                gtop += mv; head = (head + mv) & M; top = keep;
+                if (lane == 0) WSLOT(uint32_t, SLOT_NSPILL) = WSLOT(uint32_t, SLOT_NSPILL) + 1u;
             }
             // Up to four entries per step, eight lanes each: lane (sub, ch) = (lane / 8, lane % 8) takes child ch of entry sub.
             // An internal cell of these trees has 7.5 children on average, so the fixed mapping idles few lanes and needs no
@@ -369,7 +396,15 @@ __global__ void __launch_bounds__(WALK_WARPS * 32, WALK_MINBLK) walk_kernel(cons
         }
         __syncwarp();
     }
-    if (lane == 0 && nspill) atomicAdd(&P.stat[1], nspill);
+    if (lane == 0 && WSLOT(uint32_t, SLOT_NSPILL)) atomicAdd(&P.stat[1], (unsigned long long)WSLOT(uint32_t, SLOT_NSPILL));
+#undef gi
+#undef spc
+#undef spp
+#undef ipc
+#undef ipp
+#undef gstack
+#undef vstack
+#undef vstage
 }
 
 int walk_grid_warps() { // resident warps of the walk grid: blocks/SM of the variant that fits fewest
