@@ -14,8 +14,8 @@
 // contiguous slice of the list arena with one atomicAdd per list and copies the lists there.
 // If the arena is full the group is reported (first_fail), the host evaluates what fits and calls
 // the walk again for the rest.
-// The walk is integer- and latency-bound, so it runs at high occupancy (<= 48 registers, ~2.6 KB of
-// shared memory per warp) and leaves the FP32 work to hot_forces.cu.
+// The walk is integer- and latency-bound, so it runs at high occupancy (40 registers, ~2.6 KB of
+// shared memory per warp: 48 warps per SM) and leaves the FP32 work to hot_forces.cu.
 #include <climits>
 
 #include "hot_internal.h"
