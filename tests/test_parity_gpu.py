@@ -550,6 +550,56 @@ def test_long_lists_outgrow_the_walk_staging_and_are_retried(hot):
     hot.hot_free()
 
 
+@pytest.mark.parametrize("periodic,lgn,nsel", [(False, 16, 40), (True, 16, 6)])
+def test_deep_and_broad_tree_spills_the_walks_ring_buffer(hot, periodic, lgn, nsel):
+    """Sixteen nested clumps, each 0.45 of the size of the one around it: a tree 21 levels deep that is broad at every
+    level.  With one-body leaves and theta = 0.3 the depth-first phase of the walk outgrows the warp's 512-entry ring in
+    shared memory: the oldest entries go to the warp's arena in global memory and come back later (hot_stats:
+    walk_spills > 0; no BASELINE configuration gets there).  The lists are the oracle's all the same: counts, the lists
+    of the longest walks as sets, and the sums.  Periodic: the image numbers of the spilled entries travel with them."""
+    import torch
+
+    rng = np.random.default_rng(3)
+    n, nclump = 1 << lgn, 16
+    x = np.zeros((n, 3))
+    scale, per = 0.25, n // nclump
+    for k in range(nclump):
+        x[k * per:(k + 1) * per] = 0.5 + scale * rng.uniform(-1.0, 1.0, (per, 3))
+        scale *= 0.45
+    pos = np.ascontiguousarray(np.clip(x, 0.0, 0.9999).astype(np.float32))
+    mass = rng.uniform(0.5, 1.5, n).astype(np.float32) / np.float32(n)
+    lo, size, theta, eps = (0.0, 0.0, 0.0), 1.0, 0.3, 1e-6
+    hot.hot_set_params(1, 32)
+    hot.hot_build(torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda(), lo, size, periodic)
+    acc, pot = hot.hot_forces(theta, eps, 2)
+    st = hot.hot_stats()
+    assert st["walk_spills"] > 0, "this input is meant to overflow the ring"
+    assert st["max_level"] == 21
+    T = O.Tree(pos, mass, lo, size, periodic=periodic, nleaf=1, ncrit=32)
+    _check_int_artefacts(hot, T)
+    gg = hot.hot_export_groups()
+    longest = np.argsort(gg["lpc"] + gg["lpp"])[-(nsel * 3) // 5:]
+    sel = np.unique(np.append(longest, rng.choice(T.ngroups, nsel, replace=False)))
+    oa, op, lpc, lpp = T.forces(theta, eps, 2, groups=sel)
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    c = T.cells()
+    tail = np.arange(T.ngroups - 200, T.ngroups)  # the lists went through the arena in rounds: it holds the last one's
+    for gi in tail[np.argsort((gg["lpc"] + gg["lpp"])[tail])[-6:]] if not periodic else []:
+        L = hot.hot_export_lists(int(gi))
+        gf, gk = int(gg["first"][gi]), int(gg["count"][gi])
+        pc, lv = T.walk_lists(theta, int(gi))
+        bodies = np.concatenate([np.arange(c["first"][l], c["first"][l] + c["count"][l]) for l in lv])
+        bodies = bodies[(bodies < gf) | (bodies >= gf + gk)]
+        assert np.array_equal(np.sort(L["pc_cell"]), np.sort(pc)), (gi, "accepted cells")
+        assert np.array_equal(np.sort(L["pp_body"]), np.sort(bodies)), (gi, "listed bodies")
+    ea, ep = _rel_errors(acc, pot, oa, op)
+    if periodic:  # the potential against the scale of the explicit image sum (DESIGN.md R-13)
+        m = ~np.isnan(op)
+        ep = np.abs(pot.cpu().numpy().astype(np.float64)[m] - op[m]) / (np.abs(op[m]) + 57.18721055 * float(mass.astype(np.float64).sum()))
+    assert np.median(ea) <= 1e-5 and np.median(ep) <= 1e-5, (np.median(ea), np.median(ep))
+    hot.hot_free()
+
+
 def test_seeded_fuzz_of_sizes_bucket_sizes_orders_and_boundaries(hot):
     """Seeded random small problems: every sink-blocking variant (1-6 sinks per lane, 1-32 source
     streams, multi-pass groups), odd sizes, clustered and coincident bodies, open and periodic."""
