@@ -145,55 +145,63 @@ __device__ __forceinline__ void pc_one(const float4 q0, const float4 q1, const f
         return;
     }
     T vx = D2 * Mx, vy = D2 * My, vz = D2 * Mz;
+    T cP; // coefficient of P = R / u in the acceleration (degrees 3 and 4)
+    T Px, Py, Pz;
     {
-        const T ri5 = ri3 * ri2, ri7 = ri5 * ri2, ri9 = ri7 * ri2, ri11 = ri9 * ri2;
-        const T D2f = splat<T>(3.0f) * ri5, D3 = splat<T>(-15.0f) * ri7, D4 = splat<T>(105.0f) * ri9, D5 = splat<T>(-945.0f) * ri11;
+        // Degrees 3 and 4 in P = R u^-1 instead of R: every contraction of an n-th moment with k copies of R carries u^-k with it, so
+        // the coefficients left are ri, ri3 and ri5 only.  With R itself they are ri7 ... ri11, and ri11 overflows fp32 for
+        // |R| < 5.8e-4 length units although the term it multiplies is tiny there -- the error-bound criterion accepts small
+        // cells that close (inf accelerations at N >= 2^22 in tolerance mode before this), an opening angle at level >= 12.
+        //   S3 = M3 PPP, V3 = M3 PP, T3 = t3 P, S4 = M4 PPPP, W4 = M4 PPP, Q4 = T4 PP, U = T4 P;
+        //   phi3 = (-15 ri S3 + 9 ri3 T3)/6          phi4 = -(105 ri S4 - 90 ri3 Q4 + 9 ri5 t4)/24
+        //   a3 = -[105 ri S3 P - 45 ri3 V3 - 45 ri3 T3 P + 9 ri5 t3]/6
+        //   a4 = [-945 ri S4 P + 420 ri3 W4 + 630 ri3 Q4 P - 180 ri5 U - 45 ri5 t4 P]/24
+        Px = Rx * ri2; Py = Ry * ri2; Pz = Rz * ri2;
         const float* m3 = m;          // 10
         const float* m4 = m + 10;     // 15
         const float* t3 = m + 25;     // 3
         const float* T4 = m + 28;     // 6: xx xy xz yy yz zz
         const T t4 = splat<T>(m[34]);
 #define SP(v) splat<T>(v)
-        const T xx = Rx * Rx, yy = Ry * Ry, zz = Rz * Rz, xy = Rx * Ry, xz = Rx * Rz, yz = Ry * Rz;
+        const T xx = Px * Px, yy = Py * Py, zz = Pz * Pz, xy = Px * Py, xz = Px * Pz, yz = Py * Pz;
         const T xy2 = xy + xy, xz2 = xz + xz, yz2 = yz + yz;
-        // V3_k = M3_ijk R_i R_j
+        // V3_k = M3_ijk P_i P_j
         const T V3x = vfma(SP(m3[0]), xx, vfma(SP(m3[1]), xy2, vfma(SP(m3[2]), xz2, vfma(SP(m3[3]), yy, vfma(SP(m3[4]), yz2, SP(m3[5]) * zz)))));
         const T V3y = vfma(SP(m3[1]), xx, vfma(SP(m3[3]), xy2, vfma(SP(m3[4]), xz2, vfma(SP(m3[6]), yy, vfma(SP(m3[7]), yz2, SP(m3[8]) * zz)))));
         const T V3z = vfma(SP(m3[2]), xx, vfma(SP(m3[4]), xy2, vfma(SP(m3[5]), xz2, vfma(SP(m3[7]), yy, vfma(SP(m3[8]), yz2, SP(m3[9]) * zz)))));
-        const T S3 = vfma(V3x, Rx, vfma(V3y, Ry, V3z * Rz));
-        const T T3 = vfma(SP(t3[0]), Rx, vfma(SP(t3[1]), Ry, SP(t3[2]) * Rz));
-        // cubic monomials with multiplicities: W4_k = M4_ijlk R_i R_j R_l
+        const T S3 = vfma(V3x, Px, vfma(V3y, Py, V3z * Pz));
+        const T T3 = vfma(SP(t3[0]), Px, vfma(SP(t3[1]), Py, SP(t3[2]) * Pz));
+        // cubic monomials with multiplicities: W4_k = M4_ijlk P_i P_j P_l
         const T c3 = SP(3.0f);
-        const T cxxx = xx * Rx, cyyy = yy * Ry, czzz = zz * Rz;
-        const T cxxy = c3 * xx * Ry, cxxz = c3 * xx * Rz, cxyy = c3 * Rx * yy, cxzz = c3 * Rx * zz;
-        const T cyyz = c3 * yy * Rz, cyzz = c3 * Ry * zz, cxyz = SP(6.0f) * xy * Rz;
+        const T cxxx = xx * Px, cyyy = yy * Py, czzz = zz * Pz;
+        const T cxxy = c3 * xx * Py, cxxz = c3 * xx * Pz, cxyy = c3 * Px * yy, cxzz = c3 * Px * zz;
+        const T cyyz = c3 * yy * Pz, cyzz = c3 * Py * zz, cxyz = SP(6.0f) * xy * Pz;
         const T W4x = vfma(SP(m4[0]), cxxx, vfma(SP(m4[1]), cxxy, vfma(SP(m4[2]), cxxz, vfma(SP(m4[3]), cxyy, vfma(SP(m4[4]), cxyz,
                       vfma(SP(m4[5]), cxzz, vfma(SP(m4[6]), cyyy, vfma(SP(m4[7]), cyyz, vfma(SP(m4[8]), cyzz, SP(m4[9]) * czzz)))))))));
         const T W4y = vfma(SP(m4[1]), cxxx, vfma(SP(m4[3]), cxxy, vfma(SP(m4[4]), cxxz, vfma(SP(m4[6]), cxyy, vfma(SP(m4[7]), cxyz,
                       vfma(SP(m4[8]), cxzz, vfma(SP(m4[10]), cyyy, vfma(SP(m4[11]), cyyz, vfma(SP(m4[12]), cyzz, SP(m4[13]) * czzz)))))))));
         const T W4z = vfma(SP(m4[2]), cxxx, vfma(SP(m4[4]), cxxy, vfma(SP(m4[5]), cxxz, vfma(SP(m4[7]), cxyy, vfma(SP(m4[8]), cxyz,
                       vfma(SP(m4[9]), cxzz, vfma(SP(m4[11]), cyyy, vfma(SP(m4[12]), cyyz, vfma(SP(m4[13]), cyzz, SP(m4[14]) * czzz)))))))));
-        const T S4 = vfma(W4x, Rx, vfma(W4y, Ry, W4z * Rz));
-        const T Ux = vfma(SP(T4[0]), Rx, vfma(SP(T4[1]), Ry, SP(T4[2]) * Rz));
-        const T Uy = vfma(SP(T4[1]), Rx, vfma(SP(T4[3]), Ry, SP(T4[4]) * Rz));
-        const T Uz = vfma(SP(T4[2]), Rx, vfma(SP(T4[4]), Ry, SP(T4[5]) * Rz));
-        const T Q4 = vfma(Ux, Rx, vfma(Uy, Ry, Uz * Rz));
-        // phi3 = (D3 S3 + 3 D2 T3)/6 ; phi4 = -(D4 S4 + 6 D3 Q4 + 3 D2 t4)/24
-        ph = vfma(D3 * SP(1.0f / 6.0f), S3, vfma(SP(0.5f) * D2f, T3, ph));
-        ph = vfma(D4 * SP(-1.0f / 24.0f), S4, vfma(SP(-0.25f) * D3, Q4, vfma(SP(-0.125f) * D2f, t4, ph)));
-        // a3 = -[D4 S3 R + 3 D3 V3 + 3 D3 T3 R + 3 D2 t3]/6
-        // a4 = [D5 S4 R + 4 D4 W4 + 6 D4 Q4 R + 12 D3 U + 3 D3 t4 R]/24
-        cR = vfma(D4 * SP(-1.0f / 6.0f), S3, vfma(SP(-0.5f) * D3, T3, cR));
-        cR = vfma(D5 * SP(1.0f / 24.0f), S4, vfma(SP(0.25f) * D4, Q4, vfma(SP(0.125f) * D3, t4, cR)));
-        const T hD3n = SP(-0.5f) * D3, hD2n = SP(-0.5f) * D2f, sD4 = D4 * SP(1.0f / 6.0f), hD3p = SP(0.5f) * D3;
-        vx = vfma(hD3n, V3x, vfma(hD2n, SP(t3[0]), vfma(sD4, W4x, vfma(hD3p, Ux, vx))));
-        vy = vfma(hD3n, V3y, vfma(hD2n, SP(t3[1]), vfma(sD4, W4y, vfma(hD3p, Uy, vy))));
-        vz = vfma(hD3n, V3z, vfma(hD2n, SP(t3[2]), vfma(sD4, W4z, vfma(hD3p, Uz, vz))));
+        const T S4 = vfma(W4x, Px, vfma(W4y, Py, W4z * Pz));
+        const T Ux = vfma(SP(T4[0]), Px, vfma(SP(T4[1]), Py, SP(T4[2]) * Pz));
+        const T Uy = vfma(SP(T4[1]), Px, vfma(SP(T4[3]), Py, SP(T4[4]) * Pz));
+        const T Uz = vfma(SP(T4[2]), Px, vfma(SP(T4[4]), Py, SP(T4[5]) * Pz));
+        const T Q4 = vfma(Ux, Px, vfma(Uy, Py, Uz * Pz));
+        const T r1a = SP(-2.5f) * ri, r1b = SP(-4.375f) * ri, r3a = SP(1.5f) * ri3, r3b = SP(3.75f) * ri3, r5a = SP(-0.375f) * ri5;
+        ph = vfma(r1a, S3, vfma(r3a, T3, ph));                               // -15/6 ri S3 + 9/6 ri3 T3
+        ph = vfma(r1b, S4, vfma(r3b, Q4, vfma(r5a, t4, ph)));                // -105/24 ri S4 + 90/24 ri3 Q4 - 9/24 ri5 t4
+        const T r1c = SP(-17.5f) * ri, r3c = SP(7.5f) * ri3, r1d = SP(-39.375f) * ri, r3d = SP(26.25f) * ri3, r5d = SP(-1.875f) * ri5;
+        cP = vfma(r1c, S3, r3c * T3);                                        // -105/6 ri S3 + 45/6 ri3 T3
+        cP = vfma(r1d, S4, vfma(r3d, Q4, vfma(r5d, t4, cP)));                // -945/24 ri S4 + 630/24 ri3 Q4 - 45/24 ri5 t4
+        const T r5e = SP(-1.5f) * ri5, r3e = SP(17.5f) * ri3, r5f = SP(-7.5f) * ri5;
+        vx = vfma(r3c, V3x, vfma(r5e, SP(t3[0]), vfma(r3e, W4x, vfma(r5f, Ux, vx)))); // 45/6 ri3 V3 - 9/6 ri5 t3 + 420/24 ri3 W4 - 180/24 ri5 U
+        vy = vfma(r3c, V3y, vfma(r5e, SP(t3[1]), vfma(r3e, W4y, vfma(r5f, Uy, vy))));
+        vz = vfma(r3c, V3z, vfma(r5e, SP(t3[2]), vfma(r3e, W4z, vfma(r5f, Uz, vz))));
 #undef SP
     }
-    a[0] = a[0] + vfma(cR, Rx, vx);
-    a[1] = a[1] + vfma(cR, Ry, vy);
-    a[2] = a[2] + vfma(cR, Rz, vz);
+    a[0] = a[0] + vfma(cR, Rx, vfma(cP, Px, vx));
+    a[1] = a[1] + vfma(cR, Ry, vfma(cP, Py, vy));
+    a[2] = a[2] + vfma(cR, Rz, vfma(cP, Pz, vz));
     a[3] = a[3] + ph;
 }
 

@@ -702,6 +702,41 @@ def test_error_bound_criterion_with_mixed_orders(hot, cfg, scale, periodic, rtol
 
 
 # ---- f-4: spline softening and the kick / drift operators (R-17) --------------------
+def test_close_small_cells_do_not_overflow_the_hexadecapole_terms(hot):
+    """The error-bound criterion accepts a small cell (tiny b_max) a few softening lengths from a sink, at order 4 too.
+    The degree-3/4 terms are evaluated in P = R / u so that no inverse power above u^-5/2 appears: with R itself the
+    coefficient u^-11/2 overflowed fp32 for |R| < 5.8e-4 box units (inf accelerations on 10 bodies of this set, 899 at
+    N = 2^24).  All outputs finite, and the bodies that used to overflow agree with the oracle like the rest."""
+    import torch
+
+    w = W.config(2, 22)
+    _build(hot, w, 16, 256)
+    acc, pot = hot.hot_forces(0.6, w.eps, 2)
+    arms = float(acc.double().pow(2).sum(1).mean().sqrt())
+    for rel in (1e-2, 1e-4):
+        a2, p2 = hot.hot_forces_tol(rel * arms, w.eps)
+        assert bool(torch.isfinite(a2).all()) and bool(torch.isfinite(p2).all()), rel
+    st = hot.hot_stats()
+    assert st["pc_hexadecapole"] > 0
+    # plain order 4 on a set with cells at level >= 12 inside the old overflow radius: a dense clump, theta 0.9
+    rng = np.random.default_rng(12)
+    n = 1 << 14
+    pos = (0.5 + 2e-4 * rng.standard_normal((n, 3))).astype(np.float32)
+    mass = np.full(n, 1.0 / n, np.float32)
+    hot.hot_set_params(2, 16)
+    hot.hot_build(torch.from_numpy(pos).cuda(), torch.from_numpy(mass).cuda(), (0.0, 0.0, 0.0), 1.0, False)
+    acc, pot = hot.hot_forces(0.9, 1e-7, 4)
+    assert bool(torch.isfinite(acc).all()) and bool(torch.isfinite(pot).all())
+    T = O.Tree(pos, mass, (0.0, 0.0, 0.0), 1.0, periodic=False, nleaf=2, ncrit=16)
+    sel = np.sort(rng.choice(T.ngroups, 64, replace=False))
+    oa, op, lpc, lpp = T.forces(0.9, 1e-7, 4, groups=sel)
+    gg = hot.hot_export_groups()
+    assert (gg["lpc"][sel] == lpc.astype(np.uint64)).all() and (gg["lpp"][sel] == lpp.astype(np.uint64)).all()
+    ea, ep = _rel_errors(acc, pot, oa, op)
+    assert np.median(ea) <= 1e-5 and np.quantile(ea, 0.999) <= 1e-4 and np.median(ep) <= 1e-5, (np.median(ea), np.quantile(ea, 0.999), np.median(ep))
+    hot.hot_free()
+
+
 @pytest.mark.parametrize("cfg,scale,periodic,order,theta,eps_scale", [(2, 14, False, 2, 0.6, 40.0), (0, 13, False, 4, 0.5, 15.0), (1, 13, False, 0, 0.7, 60.0),
                                                                   (4, 12, True, 2, 0.5, 4.0)])
 def test_spline_softening_parity(hot, cfg, scale, periodic, order, theta, eps_scale):
